@@ -1,0 +1,574 @@
+// oracle/mps_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, single-threaded C++17 CPU implementation of the MPS time-step
+// particle-interaction path of arXiv 2105.01677 ("A Fluid Simulation System
+// Based on the MPS Method"), written from the paper text only.  It is the
+// oracle the CUDA path (paper_2105_01677_b200/csrc) is compared against and
+// shares no code, header, table or helper with it.  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+// may load it.  Build: g++ -O2 -ffp-contract=off -shared -fPIC (oracle/build.py).
+//
+// Citations: "P:n" = /root/reference/PAPER.md line n.  "Qk" = reading k listed
+// in DESIGN.md section 3 (where the paper is silent, ambiguous or garbled).
+//
+// Every function follows the paper's order and notation step by step; there is
+// no blocking, fusion or reordering.  Particles stay in the caller's original
+// order; the cell grid is used only to find neighbours (and to report the
+// sort), and `brute` replaces it by the O(N^2) double loop that *defines* the
+// fixed-radius neighbour set.
+//
+// Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force neighbour sets,
+// hand-computed n0 / lambda shells, lattice densities, free-surface counts,
+// Laplacian of a quadratic, gradient of a linear field, Eq. 7 value, operator
+// symmetry / row sums, CG vs dense Cholesky, momentum conservation, hydrostatic
+// rho*g*h.  Whole-step trajectories in a moving fluid: the paper prints no
+// values => "parity unpinned" against the paper for those (pinned on the parts).
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+enum { FLUID = 0, WALL = 1, DUMMY = 2, GHOST = 3 };
+
+struct Prm {
+  int dim;
+  double l0, re_n, re_lap, dt, g[3];
+  int n_phases;
+  double rho[2], nu[2], c0, gamma, beta, compress, ppe_relax, cg_rtol;
+  int cg_maxit;
+  double cs;
+  int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean, cell_div;
+  double dmin[3], dmax[3];
+  int max_neighbours;
+  double n0_n, n0_lap, lam;
+};
+
+// I2 (Eq.5 on the initial lattice; "weighted average of
+// r_ij^2"): sums over the ideal cubic lattice, o in Z^dim \ {0}, |o| l0 < re.
+void lattice_constants(int dim, double l0, double re, double* n0, double* lam, int* count) {
+  int R = (int)std::ceil(re / l0) + 1;
+  double sw = 0.0, sr2w = 0.0;
+  int cnt = 0;
+  for (int oz = (dim == 3 ? -R : 0); oz <= (dim == 3 ? R : 0); ++oz)
+    for (int oy = -R; oy <= R; ++oy)
+      for (int ox = -R; ox <= R; ++ox) {
+        if (ox == 0 && oy == 0 && oz == 0) continue;
+        double dx = ox * l0, dy = oy * l0, dz = oz * l0;
+        double r2 = (dx * dx + dy * dy) + dz * dz;
+        if (r2 < re * re) {
+          double r = std::sqrt(r2);
+          double w = re / r - 1.0;  // P:123 Eq.3
+          sw += w;
+          sr2w += r2 * w;
+          ++cnt;
+        }
+      }
+  *n0 = sw;
+  *lam = sr2w / sw;
+  *count = cnt;
+}
+
+struct Orc {
+  Prm prm;
+  int n = 0;
+  std::vector<double> f[18];  // x y z u v w n p ax ay az nut b phat gx gy gz xcg
+  std::vector<int> type, phase, bc, key, perm, cell_start;
+  double h = 0, inv_h = 0;
+  int nc[3] = {0, 0, 0};
+  int ncells = 0;
+  bool brute = false;
+  bool binned = false;
+  double n0_n = 0, n0_lap = 0, lam = 0, A_lap = 0;
+  int cg_iters = 0;
+  double cg_relres = 0;
+  int n_ghost = 0, n_surface = 0, max_nb = 0;
+
+  std::vector<double>&X() { return f[0]; }
+  std::vector<double>&Y() { return f[1]; }
+  std::vector<double>&Z() { return f[2]; }
+
+  void init_constants() {
+    int c;
+    double lam_n;
+    // I1-I3
+    if (prm.n0_n > 0) n0_n = prm.n0_n; else lattice_constants(prm.dim, prm.l0, prm.re_n, &n0_n, &lam_n, &c);
+    double n0l, lm;
+    lattice_constants(prm.dim, prm.l0, prm.re_lap, &n0l, &lm, &c);
+    n0_lap = prm.n0_lap > 0 ? prm.n0_lap : n0l;
+    lam = prm.lam > 0 ? prm.lam : lm;
+    A_lap = 2.0 * prm.dim / (n0_lap * lam);  // P:170 Eq.10
+    // I4 (cells "have sides equal to r_e"; cell_div = 1)
+    h = std::max(prm.re_n, prm.re_lap) / prm.cell_div;
+    inv_h = 1.0 / h;
+    ncells = 1;
+    for (int a = 0; a < 3; ++a) {
+      nc[a] = (int)std::ceil((prm.dmax[a] - prm.dmin[a]) * inv_h);
+      if (nc[a] < 1) nc[a] = 1;
+      ncells *= nc[a];
+    }
+  }
+
+  // BIN: B1-B4.
+  void bin() {
+    key.assign(n, 0);
+    n_ghost = 0;
+    for (int i = 0; i < n; ++i) {
+      const double pos[3] = {f[0][i], f[1][i], f[2][i]};
+      int c[3];
+      bool out = (type[i] == GHOST);
+      for (int a = 0; a < 3; ++a) {
+        double fl = std::floor((pos[a] - prm.dmin[a]) * inv_h);
+        if (!(fl >= 0.0 && fl < (double)nc[a])) { out = true; c[a] = 0; }
+        else c[a] = (int)fl;
+      }
+      if (out) { type[i] = GHOST; key[i] = ncells; ++n_ghost; }  // B1, B2
+      else key[i] = c[0] + nc[0] * (c[1] + nc[1] * c[2]);
+    }
+    // B3: stable sort by key, ties by ascending original index.
+    perm.resize(n);
+    for (int i = 0; i < n; ++i) perm[i] = i;
+    std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return key[a] < key[b]; });
+    // B4: cell_start[c] = #{k : key[perm[k]] < c}, c = 0..ncells
+    cell_start.assign(ncells + 1, 0);
+    {
+      int k = 0;
+      for (int c = 0; c <= ncells; ++c) {
+        while (k < n && key[perm[k]] < c) ++k;
+        cell_start[c] = k;
+      }
+    }
+    binned = true;
+  }
+  void ensure_binned() { if (!binned) bin(); }
+
+  // NEIGHBOURS(i, re) (Eq.3, strict r < re; Q2 rounding of the test).
+  template <class F>
+  void for_neighbours(int i, double re, F&& fn) {
+    const double re2 = re * re;
+    const double xi = f[0][i], yi = f[1][i], zi = f[2][i];
+    auto test = [&](int j) {
+      if (j == i || type[j] == GHOST) return;
+      double dx = f[0][j] - xi, dy = f[1][j] - yi, dz = f[2][j] - zi;
+      double r2 = (dx * dx + dy * dy) + dz * dz;
+      if (r2 < re2) fn(j, dx, dy, dz, r2);
+    };
+    if (type[i] == GHOST) return;
+    if (brute) {
+      for (int j = 0; j < n; ++j) test(j);
+      return;
+    }
+    int R = (int)std::ceil(re * inv_h);
+    int k = key[i];
+    int cx = k % nc[0], cy = (k / nc[0]) % nc[1], cz = k / (nc[0] * nc[1]);
+    for (int dz = -R; dz <= R; ++dz) {
+      int z2 = cz + dz;
+      if (z2 < 0 || z2 >= nc[2]) continue;
+      for (int dy = -R; dy <= R; ++dy) {
+        int y2 = cy + dy;
+        if (y2 < 0 || y2 >= nc[1]) continue;
+        for (int dx = -R; dx <= R; ++dx) {
+          int x2 = cx + dx;
+          if (x2 < 0 || x2 >= nc[0]) continue;
+          int c = x2 + nc[0] * (y2 + nc[1] * z2);
+          for (int s = cell_start[c]; s < cell_start[c + 1]; ++s) test(perm[s]);
+        }
+      }
+    }
+  }
+
+  double w_of(double re, double r2) const { return re / std::sqrt(r2) - 1.0; }  // P:123 Eq.3
+
+  // step 6 (Eq.5): all non-ghost i; all non-ghost j count.
+  void density() {
+    ensure_binned();
+    const double re = prm.re_n;
+    max_nb = 0;
+    for (int i = 0; i < n; ++i) {
+      double s = 0.0;
+      int cnt = 0;
+      for_neighbours(i, re, [&](int, double, double, double, double r2) { s += w_of(re, r2); ++cnt; });
+      f[6][i] = s;
+      max_nb = std::max(max_nb, cnt);
+    }
+  }
+
+  double nu_of(int i) const { return prm.nu[phase[i]] + f[11][i]; }
+
+  // step 2 (Eq.13, [51]; Q10): Smagorinsky eddy viscosity.
+  void smagorinsky() {
+    ensure_binned();
+    const double re = prm.re_n, d = prm.dim;
+    for (int i = 0; i < n; ++i) {
+      f[11][i] = 0.0;
+      if (prm.cs <= 0.0 || type[i] != FLUID) continue;
+      double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};  // G[a][b] = d u_b / d x_a
+      const double ui[3] = {f[3][i], f[4][i], f[5][i]};
+      for_neighbours(i, re, [&](int j, double dx, double dy, double dz, double r2) {
+        const bool solid = (type[j] == WALL || type[j] == DUMMY);
+        const double uj[3] = {solid ? 0.0 : f[3][j], solid ? 0.0 : f[4][j], solid ? 0.0 : f[5][j]};
+        const double dr[3] = {dx, dy, dz};
+        const double w = w_of(re, r2);
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b) G[a][b] += (uj[b] - ui[b]) * dr[a] / r2 * w;
+      });
+      double ss = 0.0;
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+          double S = 0.5 * (d / n0_n) * (G[a][b] + G[b][a]);
+          ss += S * S;
+        }
+      f[11][i] = (prm.cs * prm.l0) * (prm.cs * prm.l0) * std::sqrt(2.0 * ss);
+    }
+  }
+
+  // step 3 (Eq.2 viscous + external term, Eq.10; Q9).
+  void viscosity() {
+    ensure_binned();
+    smagorinsky();
+    const double re = prm.re_lap;
+    for (int i = 0; i < n; ++i) {
+      f[8][i] = f[9][i] = f[10][i] = 0.0;
+      if (type[i] != FLUID) continue;
+      const double nui = nu_of(i);
+      const double ui[3] = {f[3][i], f[4][i], f[5][i]};
+      double s[3] = {0, 0, 0};
+      for_neighbours(i, re, [&](int j, double, double, double, double r2) {
+        const bool solid = (type[j] == WALL || type[j] == DUMMY);
+        double nuij;
+        if (solid) nuij = nui;
+        else {
+          const double nuj = nu_of(j);
+          if (prm.nu_pair_mean == 1) nuij = (nui + nuj > 0.0) ? 2.0 * nui * nuj / (nui + nuj) : 0.0;  // Q9 (0/0 -> 0)
+          else nuij = 0.5 * (nui + nuj);
+        }
+        const double w = w_of(re, r2);
+        const double uj[3] = {solid ? 0.0 : f[3][j], solid ? 0.0 : f[4][j], solid ? 0.0 : f[5][j]};
+        for (int a = 0; a < 3; ++a) s[a] += nuij * (uj[a] - ui[a]) * w;
+      });
+      for (int a = 0; a < 3; ++a) f[8 + a][i] = A_lap * s[a] + prm.g[a];
+    }
+  }
+
+  // step 4 (Q8): explicit predictor, fluid only.
+  void predict() {
+    const double dt = prm.dt;
+    for (int i = 0; i < n; ++i) {
+      if (type[i] != FLUID) continue;
+      for (int a = 0; a < 3; ++a) {
+        f[3 + a][i] = f[3 + a][i] + dt * f[8 + a][i];
+        f[a][i] = f[a][i] + dt * f[3 + a][i];
+      }
+    }
+    binned = false;
+  }
+
+  // step 7a (Eq.7; Q4 clamp).
+  static double eos(double rho, double c0, double gamma, double n, double n0) {
+    double q = n / n0, qg;
+    if (gamma == 7.0) { double q2 = q * q, q4 = q2 * q2; qg = q4 * q2 * q; }
+    else qg = std::pow(q, gamma);
+    return rho * c0 * c0 / gamma * (qg - 1.0);
+  }
+  void pressure_explicit() {
+    for (int i = 0; i < n; ++i) {
+      double p = 0.0;
+      if (type[i] == FLUID || type[i] == WALL) {
+        p = eos(prm.rho[phase[i]], prm.c0, prm.gamma, f[6][i], n0_n);
+        if (prm.clamp_negative_p && p < 0.0) p = 0.0;
+      }
+      f[7][i] = p;
+    }
+  }
+
+  // step 7b.1 (Eq.6; Listing 2 comments).
+  void ppe_flags() {
+    n_surface = 0;
+    for (int i = 0; i < n; ++i) {
+      if (type[i] == DUMMY || type[i] == GHOST) bc[i] = -1;
+      else if (f[6][i] < prm.beta * n0_n) { bc[i] = 1; ++n_surface; }
+      else bc[i] = 0;
+    }
+  }
+  // step 7b.2 (Eq.8 divided by -rho; Q5).
+  void ppe_rhs() {
+    for (int i = 0; i < n; ++i)
+      f[12][i] = (bc[i] == 0) ? prm.ppe_relax / (prm.dt * prm.dt) * (f[6][i] - n0_n) / n0_n : 0.0;
+  }
+  double rho_pair(int i, int j) const {
+    const double ri = prm.rho[phase[i]], rj = prm.rho[phase[j]];
+    return prm.rho_pair_mean == 1 ? 2.0 * ri * rj / (ri + rj) : 0.5 * (ri + rj);  // Q6
+  }
+  // step 7b.3 (Listing 2: off-diagonal -val, diagonal += val, diagonal
+  // += 1.00e-7/dt^2, dummy neighbours give 0, rows only where bcon == 0).
+  void ppe_apply(const double* xin, double* yout) {
+    ensure_binned();
+    const double re = prm.re_lap;
+    for (int i = 0; i < n; ++i) {
+      yout[i] = 0.0;
+      if (bc[i] != 0) continue;
+      double s = 0.0;
+      const double xi = xin[i];
+      for_neighbours(i, re, [&](int j, double, double, double, double r2) {
+        if (bc[j] == -1) return;
+        const double c = A_lap * w_of(re, r2) / rho_pair(i, j);
+        s += c * (xi - (bc[j] == 0 ? xin[j] : 0.0));
+      });
+      yout[i] = s + prm.compress / (prm.dt * prm.dt) * xi;
+    }
+  }
+  // step 7b.4 (Eq.9, P:176 CG part; Q15): textbook CG, x0 = 0.
+  int ppe_solve(double rtol, int maxit) {
+    std::vector<double>& x = f[17];
+    std::vector<double> r(n), p(n), Ap(n);
+    const std::vector<double>& b = f[12];
+    double rr = 0.0, bb = 0.0;
+    for (int i = 0; i < n; ++i) { x[i] = 0.0; r[i] = b[i]; p[i] = r[i]; }
+    for (int i = 0; i < n; ++i) if (bc[i] == 0) { rr += r[i] * r[i]; bb += b[i] * b[i]; }
+    cg_iters = 0;
+    cg_relres = 0.0;
+    if (bb == 0.0) return 0;
+    int it;
+    bool conv = false;
+    for (it = 1; it <= maxit; ++it) {
+      ppe_apply(p.data(), Ap.data());
+      double pAp = 0.0;
+      for (int i = 0; i < n; ++i) if (bc[i] == 0) pAp += p[i] * Ap[i];
+      const double alpha = rr / pAp;
+      double rr2 = 0.0;
+      for (int i = 0; i < n; ++i) if (bc[i] == 0) {
+        x[i] += alpha * p[i];
+        r[i] -= alpha * Ap[i];
+        rr2 += r[i] * r[i];
+      }
+      if (rr2 <= rtol * rtol * bb) { rr = rr2; conv = true; break; }
+      const double beta = rr2 / rr;
+      for (int i = 0; i < n; ++i) if (bc[i] == 0) p[i] = r[i] + beta * p[i];
+      rr = rr2;
+    }
+    cg_iters = conv ? it : maxit;
+    cg_relres = std::sqrt(rr / bb);
+    return conv ? cg_iters : -cg_iters;
+  }
+  // step 7b (whole) incl. 7b.5 (Q4 clamp).
+  int pressure_ppe() {
+    ppe_flags();
+    ppe_rhs();
+    int it = ppe_solve(prm.cg_rtol, prm.cg_maxit);
+    for (int i = 0; i < n; ++i) {
+      double p = (bc[i] == 0) ? f[17][i] : 0.0;
+      if (prm.clamp_negative_p && p < 0.0) p = 0.0;
+      f[7][i] = p;
+    }
+    return it;
+  }
+
+  // step 8 (P:215 phi-hat of Eq.14; Q12).
+  void phat() {
+    ensure_binned();
+    const double re = prm.re_n;
+    for (int i = 0; i < n; ++i) {
+      f[13][i] = 0.0;
+      if (type[i] != FLUID && type[i] != WALL) continue;
+      double m = f[7][i];
+      for_neighbours(i, re, [&](int j, double, double, double, double) {
+        if (type[j] == DUMMY) return;
+        if (f[7][j] < m) m = f[7][j];
+      });
+      f[13][i] = m;
+    }
+  }
+  // step 9 (variant 0: cited method [8], BASELINE cfg 2; variant 1: Eq.14
+  // as printed; variant 2: BASELINE cfg 3 wording "(P_i+P_j)/r^2"; Q13).
+  void gradient() {
+    ensure_binned();
+    const double re = prm.re_n, d = prm.dim;
+    for (int i = 0; i < n; ++i) {
+      f[14][i] = f[15][i] = f[16][i] = 0.0;
+      if (type[i] != FLUID) continue;
+      double s[3] = {0, 0, 0};
+      const double pi = f[7][i], phi = f[13][i];
+      for_neighbours(i, re, [&](int j, double dx, double dy, double dz, double r2) {
+        if (type[j] == DUMMY) return;
+        double coef;
+        if (prm.grad_variant == 0) coef = f[7][j] - phi;
+        else if (prm.grad_variant == 1) coef = (pi + f[7][j]) - (phi + f[13][j]);
+        else coef = pi + f[7][j];
+        const double c = coef / r2 * w_of(re, r2);
+        s[0] += c * dx; s[1] += c * dy; s[2] += c * dz;
+      });
+      for (int a = 0; a < 3; ++a) f[14 + a][i] = d / n0_n * s[a];
+    }
+  }
+  // step 10 ("first-order Euler integration"; Q8, Q3, Q11).
+  void correct() {
+    const double dt = prm.dt;
+    for (int i = 0; i < n; ++i) {
+      if (type[i] != FLUID) continue;
+      const double rho = prm.rho[phase[i]];
+      for (int a = 0; a < 3; ++a) {
+        const double us = f[3 + a][i];
+        const double un = us - dt / rho * f[14 + a][i];
+        f[3 + a][i] = un;
+        f[a][i] = f[a][i] + dt * (un - us);
+      }
+    }
+    binned = false;
+  }
+  // STEP k -> k+1 (section 8(c).1 of SURVEY.md / DESIGN.md section 2).
+  int step(int route) {
+    bin();                // 1
+    viscosity();          // 2, 3
+    predict();            // 4
+    bin();                // 5
+    density();            // 6
+    int rc = 0;
+    if (route == 0) pressure_explicit();  // 7a
+    else rc = pressure_ppe();             // 7b
+    phat();               // 8
+    gradient();           // 9
+    correct();            // 10
+    return rc;
+  }
+};
+
+}  // namespace
+
+// ---------------------------------------------------------------------------
+// C interface (loaded with ctypes by oracle/mps_oracle.py).
+// dp / ip: flat parameter arrays, order fixed in oracle/mps_oracle.py.
+// ---------------------------------------------------------------------------
+extern "C" {
+
+void* orc_create(const double* dp, const int* ip, int n, const double* x, const double* y,
+                 const double* z, const double* u, const double* v, const double* w,
+                 const int* type, const int* phase) {
+  Orc* o = new Orc;
+  Prm& p = o->prm;
+  p.l0 = dp[0]; p.re_n = dp[1]; p.re_lap = dp[2]; p.dt = dp[3];
+  p.g[0] = dp[4]; p.g[1] = dp[5]; p.g[2] = dp[6];
+  p.rho[0] = dp[7]; p.rho[1] = dp[8]; p.nu[0] = dp[9]; p.nu[1] = dp[10];
+  p.c0 = dp[11]; p.gamma = dp[12]; p.beta = dp[13]; p.compress = dp[14];
+  p.ppe_relax = dp[15]; p.cg_rtol = dp[16]; p.cs = dp[17];
+  for (int a = 0; a < 3; ++a) { p.dmin[a] = dp[18 + a]; p.dmax[a] = dp[21 + a]; }
+  p.n0_n = dp[24]; p.n0_lap = dp[25]; p.lam = dp[26];
+  p.dim = ip[0]; p.n_phases = ip[1]; p.cg_maxit = ip[2]; p.grad_variant = ip[3];
+  p.clamp_negative_p = ip[4]; p.rho_pair_mean = ip[5]; p.nu_pair_mean = ip[6];
+  p.cell_div = ip[7]; p.max_neighbours = ip[8];
+  o->n = n;
+  for (auto& a : o->f) a.assign(n, 0.0);
+  const double* src[6] = {x, y, z, u, v, w};
+  for (int k = 0; k < 6; ++k) std::copy(src[k], src[k] + n, o->f[k].begin());
+  o->type.assign(type, type + n);
+  o->phase.assign(phase, phase + n);
+  o->bc.assign(n, 0);
+  o->init_constants();
+  return o;
+}
+void orc_destroy(void* h) { delete (Orc*)h; }
+void orc_set_brute(void* h, int b) { ((Orc*)h)->brute = (b != 0); }
+
+int orc_set_f64(void* h, int field, const double* src) {
+  Orc* o = (Orc*)h;
+  if (field < 0 || field >= 18) return -1;
+  std::copy(src, src + o->n, o->f[field].begin());
+  if (field < 3) o->binned = false;
+  return 0;
+}
+int orc_get_f64(void* h, int field, double* dst) {
+  Orc* o = (Orc*)h;
+  if (field < 0 || field >= 18) return -1;
+  std::copy(o->f[field].begin(), o->f[field].end(), dst);
+  return 0;
+}
+static std::vector<int>* ivec(Orc* o, int field) {
+  switch (field) {
+    case 0: return &o->type;
+    case 1: return &o->phase;
+    case 2: return &o->bc;
+    case 3: return &o->key;
+    case 4: return &o->perm;
+  }
+  return nullptr;
+}
+int orc_set_i32(void* h, int field, const int* src) {
+  Orc* o = (Orc*)h;
+  std::vector<int>* v = ivec(o, field);
+  if (!v || field > 2) return -1;
+  v->assign(src, src + o->n);
+  if (field == 0) o->binned = false;
+  return 0;
+}
+int orc_get_i32(void* h, int field, int* dst) {
+  Orc* o = (Orc*)h;
+  std::vector<int>* v = ivec(o, field);
+  if (!v || (int)v->size() != o->n) return -1;
+  std::copy(v->begin(), v->end(), dst);
+  return 0;
+}
+void orc_constants(void* h, double* out) {
+  Orc* o = (Orc*)h;
+  out[0] = o->n0_n; out[1] = o->n0_lap; out[2] = o->lam; out[3] = o->A_lap;
+  out[4] = o->h; out[5] = o->inv_h;
+}
+void orc_grid(void* h, int* out) {
+  Orc* o = (Orc*)h;
+  out[0] = o->nc[0]; out[1] = o->nc[1]; out[2] = o->nc[2]; out[3] = o->ncells;
+}
+void orc_stats(void* h, double* out) {
+  Orc* o = (Orc*)h;
+  out[0] = o->cg_iters; out[1] = o->cg_relres; out[2] = o->n_ghost;
+  out[3] = o->n_surface; out[4] = o->max_nb;
+}
+int orc_bin(void* h) { ((Orc*)h)->bin(); return 0; }
+int orc_get_cell_start(void* h, int* dst) {
+  Orc* o = (Orc*)h;
+  std::copy(o->cell_start.begin(), o->cell_start.end(), dst);
+  return 0;
+}
+// Neighbour sets as CSR in original numbering, each row ascending.  idx may be
+// NULL (count only).  Returns the total number of entries.
+long long orc_neighbours(void* h, double re, int* counts, int* idx, long long cap) {
+  Orc* o = (Orc*)h;
+  o->ensure_binned();
+  long long tot = 0;
+  std::vector<int> row;
+  for (int i = 0; i < o->n; ++i) {
+    row.clear();
+    o->for_neighbours(i, re, [&](int j, double, double, double, double) { row.push_back(j); });
+    std::sort(row.begin(), row.end());
+    counts[i] = (int)row.size();
+    if (idx) for (int j : row) { if (tot < cap) idx[tot] = j; ++tot; }
+    else tot += (long long)row.size();
+  }
+  return tot;
+}
+int orc_density(void* h) { ((Orc*)h)->density(); return 0; }
+int orc_viscosity(void* h) { ((Orc*)h)->viscosity(); return 0; }
+int orc_predict(void* h) { ((Orc*)h)->predict(); return 0; }
+int orc_pressure_explicit(void* h) { ((Orc*)h)->pressure_explicit(); return 0; }
+int orc_ppe_flags(void* h) { ((Orc*)h)->ppe_flags(); return 0; }
+int orc_ppe_rhs(void* h) { ((Orc*)h)->ppe_rhs(); return 0; }
+int orc_ppe_apply(void* h, const double* xin, double* yout) { ((Orc*)h)->ppe_apply(xin, yout); return 0; }
+int orc_ppe_solve(void* h, double rtol, int maxit) { return ((Orc*)h)->ppe_solve(rtol, maxit); }
+int orc_pressure_ppe(void* h) { return ((Orc*)h)->pressure_ppe(); }
+int orc_phat(void* h) { ((Orc*)h)->phat(); return 0; }
+int orc_gradient(void* h) { ((Orc*)h)->gradient(); return 0; }
+int orc_correct(void* h) { ((Orc*)h)->correct(); return 0; }
+int orc_step(void* h, int nsteps, int route) {
+  int rc = 0;
+  for (int s = 0; s < nsteps; ++s) rc = ((Orc*)h)->step(route);
+  return rc;
+}
+void orc_lattice_constants(int dim, double l0, double re, double* out) {
+  double n0, lam; int c;
+  lattice_constants(dim, l0, re, &n0, &lam, &c);
+  out[0] = n0; out[1] = lam; out[2] = c;
+}
+double orc_eos(double rho, double c0, double gamma, double n, double n0) {
+  return Orc::eos(rho, c0, gamma, n, n0);
+}
+
+}  // extern "C"
