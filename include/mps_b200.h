@@ -1,0 +1,237 @@
+/* mps_b200.h -- C-ABI of libmps_b200.so: the MPS time-step particle-interaction
+ * path of arXiv 2105.01677 as hand-written sm_100a CUDA kernels.
+ *
+ * Citations: "P:n" = line n of the paper text; "Qk" = reading k in
+ * DESIGN.md section 3 (where the paper is silent, ambiguous or garbled).
+ *
+ * Conventions for every entry point
+ *  - Returns int: MPS_OK (0) or a negative MPS_ERR_*.  No exception crosses the
+ *    ABI, nothing aborts, nothing prints.  mps_last_error() gives a message.
+ *  - "device pointer" = address in CUDA global memory of the current device,
+ *    owned by the caller (e.g. a torch tensor); "host pointer" = ordinary host
+ *    memory.  The library copies what it needs and never keeps a caller pointer.
+ *  - All floating point data are IEEE fp64.  Particle arrays passed in or out
+ *    with order = MPS_ORDER_ORIGINAL are indexed by the caller's particle index
+ *    (the index at mps_init); with MPS_ORDER_SORTED by the library's current
+ *    cell-sorted slot (see mps_bin).
+ *  - Kernel launches are asynchronous on the ctx's stream.  Device-side error
+ *    flags (neighbour overflow, non-finite position) are read and returned by
+ *    mps_sync, mps_get_stats, mps_pressure_ppe and mps_step.
+ *  - A ctx is not thread-safe.  There is no CPU fallback: every call needs a
+ *    CUDA device of compute capability 10.0 (B200).
+ */
+#ifndef MPS_B200_H
+#define MPS_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mps_ctx mps_ctx;
+
+enum {
+  MPS_OK = 0,
+  MPS_ERR_ARG = -1,                /* null pointer, n <= 0, r_e <= 0, dt <= 0, unsupported option */
+  MPS_ERR_CUDA = -2,               /* CUDA runtime error; string in mps_last_error */
+  MPS_ERR_NEIGHBOUR_OVERFLOW = -3, /* a particle has more than max_neighbours neighbours */
+  MPS_ERR_NOCONV = -4,             /* CG reached cg_maxit; pressures are still written */
+  MPS_ERR_NONFINITE = -5,          /* NaN/Inf position, or two coincident particles (Eq. 3 infinite) */
+  MPS_ERR_ORDER = -6               /* call made before its prerequisite (e.g. density before bin) */
+};
+
+/* particle types ("fluid or boundary p.", "dummy p."; Q3) */
+enum { MPS_FLUID = 0, MPS_WALL = 1, MPS_DUMMY = 2, MPS_GHOST = 3 };
+
+enum { MPS_ORDER_ORIGINAL = 0, MPS_ORDER_SORTED = 1 };
+enum { MPS_ROUTE_EXPLICIT = 0, MPS_ROUTE_PPE = 1 };
+enum { MPS_RADIUS_N = 0, MPS_RADIUS_LAP = 1 };
+
+/* field ids for mps_get_field / mps_set_field.  0..17 are fp64, 32..35 int32. */
+enum {
+  MPS_F_X = 0, MPS_F_Y = 1, MPS_F_Z = 2,       /* position r */
+  MPS_F_U = 3, MPS_F_V = 4, MPS_F_W = 5,       /* velocity u */
+  MPS_F_N = 6,                                 /* particle number density n_i (Eq. 5) */
+  MPS_F_P = 7,                                 /* pressure */
+  MPS_F_AX = 8, MPS_F_AY = 9, MPS_F_AZ = 10,   /* nu lap(u) + g (Eq. 2, Eq. 10) */
+  MPS_F_NUT = 11,                              /* Smagorinsky eddy viscosity (Eq. 13, Q10) */
+  MPS_F_B = 12,                                /* PPE right-hand side (Eq. 8, Q5) */
+  MPS_F_PHAT = 13,                             /* neighbourhood minimum pressure (Eq. 14, Q12) */
+  MPS_F_GX = 14, MPS_F_GY = 15, MPS_F_GZ = 16, /* pressure gradient */
+  MPS_F_XCG = 17,                              /* CG solution before the clamp (Q4) */
+  MPS_I_TYPE = 32, MPS_I_PHASE = 33,
+  MPS_I_BC = 34,                               /* -1 dummy/ghost, 1 free surface, 0 PPE unknown (Eq. 6) */
+  MPS_I_KEY = 35                               /* cell key of the last mps_bin (read only) */
+};
+
+/* Parameters: a POD struct copied at mps_init.  Every reading of DESIGN.md
+ * section 3 is a field here.  Defaults in parentheses are what the tests use. */
+typedef struct mps_params {
+  int32_t dim;              /* 3 (only 3 is supported; P:292 item 1 also offers 2) */
+  int32_t n_phases;         /* 1 or 2 */
+  int32_t cg_maxit;         /* (2000) then MPS_ERR_NOCONV; Q15 */
+  int32_t grad_variant;     /* 0: (p_j - phat_i) standard [8]; 1: Eq. 14 as printed; 2: (p_i + p_j); Q13 */
+  int32_t clamp_negative_p; /* (1) p < 0 -> 0 after either pressure route; Q4 */
+  int32_t rho_pair_mean;    /* 0 arithmetic (default), 1 harmonic; Q6 */
+  int32_t nu_pair_mean;     /* 1 harmonic (default), 0 arithmetic; Q9 */
+  int32_t key_mode;         /* 0: linear x-fastest cell key (the only mode supported) */
+  int32_t cell_div;         /* (1) cell side h = max(re_n, re_lap) / cell_div; 1..3 */
+  int32_t max_neighbours;   /* (300) P:286; capacity of one neighbour row */
+  int32_t reserved_i[2];
+  double l0;                /* initial particle spacing */
+  double re_n;              /* radius for density, p-hat and gradient (2.1 l0) */
+  double re_grad;           /* must equal re_n (one list serves both) */
+  double re_lap;            /* radius for the Laplacian: viscosity and PPE (3.1 l0); >= re_n */
+  double dt;
+  double g[3];
+  double rho[2];            /* density per phase */
+  double nu[2];             /* kinematic viscosity per phase */
+  double c0;                /* speed of sound of Eq. 7; Q14 */
+  double gamma;             /* (7) Eq. 7 */
+  double beta;              /* (0.97) Eq. 6 */
+  double compress;          /* (1e-7) diagonal term compress/dt^2, Listing 2; Q5 */
+  double ppe_relax;         /* (1.0) factor on the PPE source */
+  double cg_rtol;           /* (1e-8) stop at ||r|| <= cg_rtol ||b||; Q15 */
+  double cs;                /* Smagorinsky constant, 0 = off; Q10 */
+  double domain_min[3];     /* particles outside [domain_min, domain_max) become GHOST; Q11 */
+  double domain_max[3];
+  double n0_n;              /* 0 => lattice closed form (Q1) */
+  double n0_lap;            /* 0 => lattice closed form */
+  double lambda;            /* 0 => lattice closed form */
+} mps_params;
+
+typedef struct mps_stats {
+  int32_t cg_iters;         /* iterations of the last mps_pressure_ppe */
+  int32_t cg_converged;
+  double cg_relres;         /* sqrt(r.r / b.b) of the recurrence residual at exit */
+  int32_t max_neighbours;   /* largest r_lap row of the last mps_bin */
+  int32_t n_surface;        /* free-surface particles of the last PPE */
+  int32_t n_ghost;          /* particles currently GHOST */
+  int32_t n_rows;           /* PPE unknowns (bc == 0) of the last PPE */
+  int64_t cg_iters_total;   /* summed over the life of the ctx */
+  int64_t steps_total;
+  int32_t device_error;     /* sticky MPS_ERR_* raised on the device, 0 if none */
+  int32_t reserved;
+} mps_stats;
+
+/* mps_init: create a ctx and copy n particles in (device pointers, caller's
+ * order).  type: MPS_FLUID/WALL/DUMMY/GHOST, phase: 0/1.  Allocates every
+ * buffer any later call needs (nothing is allocated after init).  stream is a
+ * cudaStream_t (may be NULL = default stream).  Computes n0 and lambda on the
+ * ideal cubic lattice unless given (I1-I4 of DESIGN.md section 2; P:134-136,
+ * P:170-174). */
+int mps_init(mps_ctx** out, const mps_params* prm, int64_t n,
+             const double* x, const double* y, const double* z,
+             const double* u, const double* v, const double* w,
+             const int32_t* type, const int32_t* phase, void* stream);
+
+/* Same, from HOST pointers (pageable or pinned); copies are issued on the stream. */
+int mps_init_host(mps_ctx** out, const mps_params* prm, int64_t n,
+                  const double* x, const double* y, const double* z,
+                  const double* u, const double* v, const double* w,
+                  const int32_t* type, const int32_t* phase, void* stream);
+
+int mps_destroy(mps_ctx* ctx);
+
+/* mps_bin: uniform-grid binning (section 4.1).  Cell index
+ * c_a = floor((x_a - domain_min_a) * (1/h)); key = c_x + n_x (c_y + n_y c_z);
+ * out-of-domain or non-finite particles become GHOST with key = n_cells.
+ * Counting sort by key (ties: ascending original index), cell-start table,
+ * physical reorder of the particle arrays, and the per-step neighbour rows at
+ * re_lap (entries within re_n first) that every later sweep streams (Listing 2's
+ * neigh[], without its fixed N x 300 matrix).  Distance test:
+ * r2 = (dx*dx + dy*dy) + dz*dz, each operation rounded, r2 < re*re (Q2). */
+int mps_bin(mps_ctx* ctx);
+
+/* mps_density: n_i = sum_{j != i, r < re_n} (re_n / r - 1) over non-ghost j
+ * (Eq. 5 with P:123 Eq. 3).  Needs mps_bin at the current positions. */
+int mps_density(mps_ctx* ctx);
+
+/* mps_viscosity: a_i = (2 d / (n0 lambda)) sum nu_ij (u_j - u_i) w(r) + g for
+ * fluid i over r < re_lap (Eq. 10, Eq. 2); if cs > 0 first the
+ * Smagorinsky nu_t (Eq. 13; Q9, Q10).  Walls and dummies have u = 0. */
+int mps_viscosity(mps_ctx* ctx);
+
+/* mps_predict: u* = u + dt a; r* = r + dt u* for fluid (Q8).
+ * Invalidates the bin. */
+int mps_predict(mps_ctx* ctx);
+
+/* mps_pressure_explicit: p = rho c0^2 / gamma ((n/n0)^gamma - 1) for fluid and
+ * wall, 0 for dummy (Eq. 7; Q4).  Uses the ctx's n field. */
+int mps_pressure_explicit(mps_ctx* ctx);
+
+/* mps_pressure_ppe: free-surface flags n < beta n0 (Eq. 6), right-hand
+ * side (Eq. 8 divided by -rho; Q5), matrix-free operator with the
+ * structure of Listing 2 and conjugate gradients from x0 = 0 to
+ * ||r|| <= cg_rtol ||b|| (Eq. 9; Q15).  iters_out / relres_out are
+ * HOST pointers (may be NULL), written after a stream synchronisation.
+ * Returns MPS_ERR_NOCONV if cg_maxit was reached (pressures still written). */
+int mps_pressure_ppe(mps_ctx* ctx, int32_t* iters_out, double* relres_out);
+
+/* mps_gradient: p-hat (minimum over i and its non-dummy neighbours within re_n;
+ * P:215, Q12) then the pressure gradient of fluid i, variant grad_variant
+ * (Eq. 14; Q13). */
+int mps_gradient(mps_ctx* ctx);
+
+/* mps_correct: u = u* - (dt / rho_i) G; r = r* + dt (u - u*) for fluid; walls
+ * and dummies do not move (Q8, Q3, Q11).  Invalidates the bin. */
+int mps_correct(mps_ctx* ctx);
+
+/* mps_step: nsteps times { bin, viscosity, predict, bin, density, pressure
+ * (route), gradient, correct }.  No host synchronisation inside except the CG
+ * convergence poll of the PPE route.  Returns the first error met. */
+int mps_step(mps_ctx* ctx, int32_t nsteps, int32_t pressure_route);
+
+/* mps_step_host: the end-to-end call on HOST buffers: init from host arrays,
+ * nsteps steps, copy x,y,z,u,v,w,p (caller's order) back into the same host
+ * arrays (p_out may be NULL), destroy.  All copies are inside the call. */
+int mps_step_host(const mps_params* prm, int64_t n, double* x, double* y, double* z,
+                  double* u, double* v, double* w, const int32_t* type, const int32_t* phase,
+                  double* p_out, int32_t nsteps, int32_t pressure_route, mps_stats* stats_out,
+                  void* stream);
+
+/* Field access for parity tests and checkpoints.  dst/src are DEVICE pointers
+ * to n elements (double for ids < 32, int32_t otherwise). */
+int mps_get_field(mps_ctx* ctx, int32_t field, void* dst, int32_t order);
+int mps_set_field(mps_ctx* ctx, int32_t field, const void* src, int32_t order);
+
+/* perm[k] = caller's original index of sorted slot k (DEVICE, n x uint32). */
+int mps_get_perm(mps_ctx* ctx, uint32_t* dst);
+/* grid[0..2] = cells per axis, grid[3] = n_cells (HOST, 4 x int32). */
+int mps_get_grid(mps_ctx* ctx, int32_t* grid);
+/* cell_start[c] = first sorted slot of cell c, c = 0..n_cells (DEVICE, (n_cells+1) x uint32). */
+int mps_get_cell_start(mps_ctx* ctx, uint32_t* dst);
+/* Neighbour sets of the last mps_bin as CSR in ORIGINAL numbering, each row
+ * ascending: counts[i] (DEVICE, n x uint32) and, if idx != NULL, the first cap
+ * entries of the concatenated rows (DEVICE).  *total (HOST) = number of entries. */
+int mps_get_neighbours(mps_ctx* ctx, int32_t radius_id, uint32_t* counts, uint32_t* idx,
+                       int64_t cap, int64_t* total);
+/* y = A x with the operator and flags of the last mps_pressure_ppe (DEVICE, n doubles each). */
+int mps_ppe_apply(mps_ctx* ctx, const double* x, double* y, int32_t order);
+/* out[0..5] = n0_n, n0_lap, lambda, 2d/(n0_lap lambda), h, 1/h (HOST). */
+int mps_get_constants(mps_ctx* ctx, double* out);
+int mps_get_stats(mps_ctx* ctx, mps_stats* out);
+int mps_sync(mps_ctx* ctx);
+/* Per-kernel CUDA-event timing for bench.py: mps_timers_enable(ctx, mask) with
+ * bit k of mask set times every launch of category k with a CUDA-event pair on
+ * the ctx's stream (mask 0 switches timing off); mps_timers_read returns the
+ * accumulated milliseconds and launch counts (HOST arrays of MPS_NUM_TIMERS). */
+enum {
+  MPS_T_BIN_SORT = 0, MPS_T_BIN_LIST = 1, MPS_T_VISCOSITY = 2, MPS_T_PREDICT = 3,
+  MPS_T_DENSITY = 4, MPS_T_PRESSURE_EXPLICIT = 5, MPS_T_PPE_SETUP = 6, MPS_T_CG_SPMV = 7,
+  MPS_T_CG_UPDATE = 8, MPS_T_GRADIENT = 9, MPS_T_CORRECT = 10, MPS_NUM_TIMERS = 11
+};
+int mps_timers_enable(mps_ctx* ctx, int32_t mask);
+int mps_timers_read(mps_ctx* ctx, double* ms, int64_t* launches);
+/* Kernels launched by this ctx so far (every __global__ launch is counted). */
+int64_t mps_launch_count(mps_ctx* ctx);
+/* Message of the last error of this ctx (owned by the ctx; valid until the
+ * next call).  ctx == NULL returns the message of the last failed mps_init. */
+const char* mps_last_error(mps_ctx* ctx);
+const char* mps_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPS_B200_H */

@@ -1,0 +1,466 @@
+// kernels_bin.cu -- uniform-grid binning (S1-S3 of DESIGN.md): cell key,
+// counting sort with a device-side scan, canonical (stable) order inside each
+// cell, physical reorder, and the per-step neighbour rows.
+// Paper: section 4.1 (cell-linked list), P:288, P:273-274 (neigh[] rows).
+#include "mps_internal.h"
+
+namespace {
+
+constexpr int TPB = 256;
+
+// ---------------------------------------------------------------- load / io ---
+__global__ void k_load(int n, const double* __restrict__ x, const double* __restrict__ y,
+                       const double* __restrict__ z, const double* __restrict__ u,
+                       const double* __restrict__ v, const double* __restrict__ w,
+                       const int32_t* __restrict__ type, const int32_t* __restrict__ phase,
+                       double4* __restrict__ pos4, double4* __restrict__ vel4,
+                       uint32_t* __restrict__ tp, uint32_t* __restrict__ oid) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  pos4[i] = make_double4(x[i], y[i], z[i], 0.0);
+  int t = type[i];
+  bool solid = (t == MPS_WALL || t == MPS_DUMMY);
+  vel4[i] = make_double4(solid ? 0.0 : u[i], solid ? 0.0 : v[i], solid ? 0.0 : w[i], 0.0);
+  tp[i] = (uint32_t)(t & 0xff) | ((uint32_t)(phase[i] & 1) << 8);
+  oid[i] = (uint32_t)i;
+}
+
+// ---------------------------------------------------------------- S1: keys ---
+// c_a = floor((x_a - min_a) * inv_h); key = c_x + n_x (c_y + n_y c_z); particles
+// outside the grid (or non-finite) become GHOST with key = n_cells.  The rank
+// inside the cell comes from a warp-aggregated atomic on the cell counter; the
+// canonical order (ascending original index) is restored in k_reorder.
+__global__ void k_keys(KConst kc, const double4* __restrict__ pos4, uint32_t* __restrict__ tp,
+                       uint32_t* __restrict__ key_tmp, uint32_t* __restrict__ rank,
+                       uint32_t* __restrict__ cell_count, DevFlags* __restrict__ flags) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool live = i < kc.n;
+  uint32_t key = 0xffffffffu;
+  if (live) {
+    double4 q = pos4[i];
+    uint32_t t = tp[i];
+    bool ghost = (t & 0xff) == MPS_GHOST;
+    // (x - min) * inv_h: a subtraction then a multiplication, each rounded (no FMA possible)
+    double fx = floor(__dmul_rn(__dsub_rn(q.x, kc.dmin[0]), kc.inv_h));
+    double fy = floor(__dmul_rn(__dsub_rn(q.y, kc.dmin[1]), kc.inv_h));
+    double fz = floor(__dmul_rn(__dsub_rn(q.z, kc.dmin[2]), kc.inv_h));
+    bool in = (fx >= 0.0 && fx < (double)kc.nx) && (fy >= 0.0 && fy < (double)kc.ny) &&
+              (fz >= 0.0 && fz < (double)kc.nz);
+    if (!ghost && !(isfinite(q.x) && isfinite(q.y) && isfinite(q.z))) flags->nonfinite = 1;
+    if (ghost || !in) {
+      if (!ghost) tp[i] = (t & ~0xffu) | MPS_GHOST;
+      key = (uint32_t)kc.ncells;
+    } else {
+      key = (uint32_t)((int)fx + kc.nx * ((int)fy + kc.ny * (int)fz));
+    }
+    key_tmp[i] = key;
+  }
+  // warp-aggregated atomic: one atomicAdd per distinct key in the warp
+  unsigned peers = __match_any_sync(0xffffffffu, key);
+  int lane = threadIdx.x & 31;
+  int leader = __ffs(peers) - 1;
+  uint32_t base = 0;
+  if (live && lane == leader) base = atomicAdd(&cell_count[key], (uint32_t)__popc(peers));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (live) rank[i] = base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+}
+
+// ------------------------------------------------- device-side exclusive scan ---
+// Three small kernels (reduce per tile, scan the tile sums in one block, scan
+// each tile with its offset).  Tile = 256 threads x 8 items.
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = TPB * SCAN_ITEMS;
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total) {
+  __shared__ uint32_t warp_sums[TPB / 32];
+  int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) warp_sums[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t s = lane < TPB / 32 ? warp_sums[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < TPB / 32; o <<= 1) {
+      uint32_t t = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += t;
+    }
+    if (lane < TPB / 32) warp_sums[lane] = s;
+  }
+  __syncthreads();
+  uint32_t off = wid ? warp_sums[wid - 1] : 0;
+  *total = warp_sums[TPB / 32 - 1];
+  __syncthreads();
+  return off + inc - v;
+}
+
+__global__ void k_scan_reduce(const uint32_t* __restrict__ in, int64_t n, uint32_t* __restrict__ tile_sum) {
+  int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
+  uint32_t s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    int64_t i = base + k * TPB + threadIdx.x;
+    if (i < n) s += in[i];
+  }
+  uint32_t tot;
+  block_exclusive_scan(s, &tot);
+  if (threadIdx.x == 0) tile_sum[blockIdx.x] = tot;
+}
+__global__ void k_scan_spine(uint32_t* __restrict__ tile_sum, int ntiles) {
+  uint32_t carry = 0;
+  for (int base = 0; base < ntiles; base += TPB) {
+    int i = base + threadIdx.x;
+    uint32_t v = i < ntiles ? tile_sum[i] : 0;
+    uint32_t tot;
+    uint32_t ex = block_exclusive_scan(v, &tot);
+    if (i < ntiles) tile_sum[i] = carry + ex;
+    carry += tot;
+  }
+}
+__global__ void k_scan_apply(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int64_t n,
+                             const uint32_t* __restrict__ tile_off) {
+  int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS];
+  uint32_t s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    v[k] = (base + k < n) ? in[base + k] : 0;
+    s += v[k];
+  }
+  uint32_t tot;
+  uint32_t ex = block_exclusive_scan(s, &tot) + tile_off[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    if (base + k < n) out[base + k] = ex;
+    ex += v[k];
+  }
+}
+
+// ------------------------------------------------------- S2: scatter + reorder ---
+__global__ void k_scatter(int n, const uint32_t* __restrict__ key_tmp, const uint32_t* __restrict__ rank,
+                          const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ oid,
+                          uint32_t* __restrict__ tmp_src, uint32_t* __restrict__ tmp_oid,
+                          uint32_t* __restrict__ key) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t k = key_tmp[i];
+  uint32_t dst = cell_start[k] + rank[i];
+  tmp_src[dst] = (uint32_t)i;
+  tmp_oid[dst] = oid[i];
+  key[dst] = k;
+}
+
+// Final slot of s inside its cell = number of cell mates with a smaller original
+// index (ties impossible): this makes the sort the unique stable one whatever
+// order the atomics handed out.  Then move the payload.
+__global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
+                          const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ tmp_src,
+                          const uint32_t* __restrict__ tmp_oid, const double4* __restrict__ pos_in,
+                          const double4* __restrict__ vel_in, const uint32_t* __restrict__ tp_in,
+                          double4* __restrict__ pos_out, double4* __restrict__ vel_out,
+                          uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  uint32_t c = key[s];
+  uint32_t lo = cell_start[c];
+  uint32_t hi = (c == (uint32_t)ncells) ? (uint32_t)n : cell_start[c + 1];
+  uint32_t me = tmp_oid[s];
+  uint32_t f = lo;
+  for (uint32_t t = lo; t < hi; ++t) f += (tmp_oid[t] < me) ? 1u : 0u;
+  uint32_t src = tmp_src[s];
+  double4 q = pos_in[src];
+  q.w = 0.0;
+  pos_out[f] = q;
+  vel_out[f] = vel_in[src];
+  tp_out[f] = tp_in[src];
+  oid_out[f] = me;
+}
+
+// ------------------------------------------------ S3: neighbour rows (the sweep) ---
+// One thread per particle i.  For every (dy, dz) row of cells the candidates are
+// one contiguous slot range (x-fastest key).  Decision: r2 = (dx*dx + dy*dy) +
+// dz*dz with every operation rounded separately, r2 < re*re (strict, Eq. 3).
+// Hits inside re_n go to the front of the row, the others to the back.
+__global__ void __launch_bounds__(128)
+k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
+             const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
+             uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
+             DevFlags* __restrict__ flags) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= kc.n) return;
+  uint32_t k = key[i];
+  if (k >= (uint32_t)kc.ncells) {  // ghost
+    cn[i] = 0;
+    co[i] = 0;
+    return;
+  }
+  const double4 pi = pos4[i];
+  const int cx = (int)(k % (uint32_t)kc.nx);
+  const int cy = (int)((k / (uint32_t)kc.nx) % (uint32_t)kc.ny);
+  const int cz = (int)(k / ((uint32_t)kc.nx * (uint32_t)kc.ny));
+  const int R = kc.R_lap;
+  const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
+  uint32_t* row = nbr + ((size_t)(i >> 5) * kc.cap) * 32 + (i & 31);
+  uint32_t nf = 0, nb = 0;
+  const uint32_t cap = (uint32_t)kc.cap;
+  bool coincident = false;
+  for (int dz = -R; dz <= R; ++dz) {
+    int z2 = cz + dz;
+    if (z2 < 0 || z2 >= kc.nz) continue;
+    for (int dy = -R; dy <= R; ++dy) {
+      int y2 = cy + dy;
+      if (y2 < 0 || y2 >= kc.ny) continue;
+      int cbase = kc.nx * (y2 + kc.ny * z2);
+      uint32_t js = cell_start[cbase + x_lo];
+      uint32_t je = cell_start[cbase + x_hi + 1];
+      for (uint32_t j = js; j < je; ++j) {
+        double4 q = pos4[j];
+        double dx = __dsub_rn(q.x, pi.x), dy_ = __dsub_rn(q.y, pi.y), dz_ = __dsub_rn(q.z, pi.z);
+        double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
+        if (r2 < kc.re_lap2 && j != (uint32_t)i) {
+          if (r2 == 0.0) coincident = true;
+          uint32_t t = tp[j];
+          uint32_t e = j | (((t & 0xff) == MPS_DUMMY) ? NB_DUMMY : 0u) | ((t & 0x100) ? NB_PHASE1 : 0u);
+          if (nf + nb < cap) {
+            if (r2 < kc.re_n2) row[(size_t)(nf++) * 32] = e;
+            else row[(size_t)(cap - 1 - (nb++)) * 32] = e;
+          } else {
+            nf++;  // keep counting so that the overflow is visible
+          }
+        }
+      }
+    }
+  }
+  if (nf + nb > cap) {
+    flags->overflow = 1;
+    uint32_t over = nf + nb - cap;
+    nf = nf >= over ? nf - over : 0;  // rows stay within capacity
+  }
+  cn[i] = nf;
+  co[i] = nb;
+  if (coincident) flags->nonfinite = 1;
+  atomicMax(&flags->max_row, (int)(nf + nb));
+}
+
+__global__ void k_count_ghosts(int n, int ncells, const uint32_t* __restrict__ cell_start,
+                               DevFlags* __restrict__ flags) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) flags->n_ghost = n - (int)cell_start[ncells];
+}
+
+// ---------------------------------------------------------- field get / set ---
+__global__ void k_get_f64(int n, int field, int order, const double4* __restrict__ pos4,
+                          const double4* __restrict__ vel4, const double4* __restrict__ acc4,
+                          const double4* __restrict__ grad4, const double* __restrict__ scalar,
+                          const uint32_t* __restrict__ oid, double* __restrict__ dst) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double v;
+  switch (field) {
+    case MPS_F_X: v = pos4[i].x; break;
+    case MPS_F_Y: v = pos4[i].y; break;
+    case MPS_F_Z: v = pos4[i].z; break;
+    case MPS_F_U: v = vel4[i].x; break;
+    case MPS_F_V: v = vel4[i].y; break;
+    case MPS_F_W: v = vel4[i].z; break;
+    case MPS_F_AX: v = acc4[i].x; break;
+    case MPS_F_AY: v = acc4[i].y; break;
+    case MPS_F_AZ: v = acc4[i].z; break;
+    case MPS_F_GX: v = grad4[i].x; break;
+    case MPS_F_GY: v = grad4[i].y; break;
+    case MPS_F_GZ: v = grad4[i].z; break;
+    default: v = scalar[i]; break;
+  }
+  dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = v;
+}
+__global__ void k_set_f64(int n, int field, int order, double4* __restrict__ pos4,
+                          double4* __restrict__ vel4, double4* __restrict__ acc4,
+                          double4* __restrict__ grad4, double* __restrict__ scalar,
+                          const uint32_t* __restrict__ oid, const double* __restrict__ src) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double v = src[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i];
+  switch (field) {
+    case MPS_F_X: pos4[i].x = v; break;
+    case MPS_F_Y: pos4[i].y = v; break;
+    case MPS_F_Z: pos4[i].z = v; break;
+    case MPS_F_U: vel4[i].x = v; break;
+    case MPS_F_V: vel4[i].y = v; break;
+    case MPS_F_W: vel4[i].z = v; break;
+    case MPS_F_AX: acc4[i].x = v; break;
+    case MPS_F_AY: acc4[i].y = v; break;
+    case MPS_F_AZ: acc4[i].z = v; break;
+    case MPS_F_GX: grad4[i].x = v; break;
+    case MPS_F_GY: grad4[i].y = v; break;
+    case MPS_F_GZ: grad4[i].z = v; break;
+    default: scalar[i] = v; break;
+  }
+}
+__global__ void k_get_i32(int n, int field, int order, const uint32_t* __restrict__ tp,
+                          const int8_t* __restrict__ bc, const uint32_t* __restrict__ key,
+                          const uint32_t* __restrict__ oid, int32_t* __restrict__ dst) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int32_t v;
+  switch (field) {
+    case MPS_I_TYPE: v = (int32_t)(tp[i] & 0xff); break;
+    case MPS_I_PHASE: v = (int32_t)((tp[i] >> 8) & 1); break;
+    case MPS_I_BC: v = (int32_t)bc[i]; break;
+    default: v = (int32_t)key[i]; break;
+  }
+  dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = v;
+}
+__global__ void k_set_i32(int n, int field, int order, uint32_t* __restrict__ tp, int8_t* __restrict__ bc,
+                          const uint32_t* __restrict__ oid, const int32_t* __restrict__ src) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int32_t v = src[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i];
+  switch (field) {
+    case MPS_I_TYPE: tp[i] = (tp[i] & ~0xffu) | (uint32_t)(v & 0xff); break;
+    case MPS_I_PHASE: tp[i] = (tp[i] & ~0x100u) | ((uint32_t)(v & 1) << 8); break;
+    case MPS_I_BC: bc[i] = (int8_t)v; break;
+    default: break;
+  }
+}
+
+// ------------------------------------------------ neighbour sets for the tests ---
+__global__ void k_nb_counts(int n, int radius_id, const uint32_t* __restrict__ cn,
+                            const uint32_t* __restrict__ co, const uint32_t* __restrict__ oid,
+                            uint32_t* __restrict__ counts) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  counts[oid[i]] = cn[i] + (radius_id == MPS_RADIUS_LAP ? co[i] : 0u);
+}
+__global__ void k_nb_fill(int n, int cap_row, int radius_id, const uint32_t* __restrict__ nbr,
+                          const uint32_t* __restrict__ cn, const uint32_t* __restrict__ co,
+                          const uint32_t* __restrict__ oid, const uint32_t* __restrict__ offs,
+                          uint32_t* __restrict__ idx, int64_t cap) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t* row = nbr + ((size_t)(i >> 5) * cap_row) * 32 + (i & 31);
+  int64_t base = offs[oid[i]];
+  uint32_t nf = cn[i], nb = (radius_id == MPS_RADIUS_LAP) ? co[i] : 0u;
+  uint32_t m = nf + nb;
+  if (base + m > cap) return;  // caller's buffer too small for this row: skip it
+  // insertion sort by original index while writing
+  for (uint32_t k = 0; k < m; ++k) {
+    uint32_t e = (k < nf) ? row[(size_t)k * 32] : row[(size_t)(cap_row - 1 - (k - nf)) * 32];
+    uint32_t v = oid[e & NB_INDEX];
+    int64_t t = base + k;
+    while (t > base && idx[t - 1] > v) { idx[t] = idx[t - 1]; --t; }
+    idx[t] = v;
+  }
+}
+
+}  // namespace
+
+// ============================================================ host launchers ===
+void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
+                         uint32_t* tmp) {
+  int ntiles = div_up(n, SCAN_TILE);
+  MPS_LAUNCH(c, cat, k_scan_reduce, ntiles, TPB, in, n, tmp);
+  MPS_LAUNCH(c, cat, k_scan_spine, 1, TPB, tmp, ntiles);
+  MPS_LAUNCH(c, cat, k_scan_apply, ntiles, TPB, in, out, n, tmp);
+}
+
+int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const double* z,
+                        const double* u, const double* v, const double* w, const int32_t* type,
+                        const int32_t* phase) {
+  int n = (int)c->n;
+  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_load, div_up(n, TPB), TPB, n, x, y, z, u, v, w, type, phase,
+             c->pos4[c->cur], c->vel4[c->cur], c->tp[c->cur], c->oid[c->cur]);
+  return MPS_OK;
+}
+
+int mpsk_bin(mps_ctx* c) {
+  const int n = (int)c->n;
+  const int nc = c->kc.ncells;
+  const int cur = c->cur, nxt = cur ^ 1;
+  cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * (nc + 2), c->stream);
+  cudaMemsetAsync(&c->flags->max_row, 0, sizeof(int), c->stream);
+  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_keys, div_up(n, TPB), TPB, c->kc, c->pos4[cur], c->tp[cur],
+             c->key_tmp, c->rank, c->cell_count, c->flags);
+  mpsk_exclusive_scan(c, MPS_T_BIN_SORT, c->cell_count, c->cell_start, nc + 2, c->scan_tmp);
+  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_scatter, div_up(n, TPB), TPB, n, c->key_tmp, c->rank,
+             c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key);
+  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_reorder, div_up(n, TPB), TPB, n, nc, c->key, c->cell_start,
+             c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
+             c->vel4[nxt], c->tp[nxt], c->oid[nxt]);
+  c->cur = nxt;
+  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
+  MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, 128), 128, c->kc, c->pos4[nxt], c->tp[nxt],
+             c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags);
+  c->binned = true;
+  c->ppe_ready = false;
+  return MPS_OK;
+}
+
+static const double* scalar_field(mps_ctx* c, int field) {
+  switch (field) {
+    case MPS_F_N: return c->dens;
+    case MPS_F_P: return c->p;
+    case MPS_F_NUT: return c->nut;
+    case MPS_F_B: return c->b;
+    case MPS_F_PHAT: return c->phat;
+    case MPS_F_XCG: return c->cg_x;
+  }
+  return nullptr;
+}
+
+int mpsk_get_field(mps_ctx* c, int field, void* dst, int order) {
+  int n = (int)c->n;
+  int cur = c->cur;
+  if (field >= 0 && field <= MPS_F_XCG) {
+    MPS_LAUNCH(c, MPS_T_BIN_SORT, k_get_f64, div_up(n, TPB), TPB, n, field, order, c->pos4[cur],
+               c->vel4[cur], c->acc4, c->grad4, scalar_field(c, field), c->oid[cur], (double*)dst);
+    return MPS_OK;
+  }
+  if (field >= MPS_I_TYPE && field <= MPS_I_KEY) {
+    MPS_LAUNCH(c, MPS_T_BIN_SORT, k_get_i32, div_up(n, TPB), TPB, n, field, order, c->tp[cur], c->bc,
+               c->key, c->oid[cur], (int32_t*)dst);
+    return MPS_OK;
+  }
+  return MPS_ERR_ARG;
+}
+
+int mpsk_set_field(mps_ctx* c, int field, const void* src, int order) {
+  int n = (int)c->n;
+  int cur = c->cur;
+  if (field >= 0 && field <= MPS_F_XCG) {
+    MPS_LAUNCH(c, MPS_T_BIN_SORT, k_set_f64, div_up(n, TPB), TPB, n, field, order, c->pos4[cur],
+               c->vel4[cur], c->acc4, c->grad4, (double*)scalar_field(c, field), c->oid[cur],
+               (const double*)src);
+    if (field <= MPS_F_Z) { c->binned = false; c->ppe_ready = false; }
+    return MPS_OK;
+  }
+  if (field >= MPS_I_TYPE && field <= MPS_I_BC) {
+    MPS_LAUNCH(c, MPS_T_BIN_SORT, k_set_i32, div_up(n, TPB), TPB, n, field, order, c->tp[cur], c->bc,
+               c->oid[cur], (const int32_t*)src);
+    if (field != MPS_I_BC) { c->binned = false; c->ppe_ready = false; }
+    return MPS_OK;
+  }
+  return MPS_ERR_ARG;
+}
+
+int mpsk_get_neighbours(mps_ctx* c, int radius_id, uint32_t* counts, uint32_t* idx, int64_t cap,
+                        int64_t* total) {
+  int n = (int)c->n;
+  int cur = c->cur;
+  MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_counts, div_up(n, TPB), TPB, n, radius_id, c->cn, c->co,
+             c->oid[cur], counts);
+  // offsets in original order: scan into tmp_src (n entries; free between bins)
+  mpsk_exclusive_scan(c, MPS_T_BIN_LIST, counts, c->tmp_src, n, c->scan_tmp);
+  uint32_t last_off = 0, last_cnt = 0;
+  cudaMemcpyAsync(&last_off, c->tmp_src + (n - 1), 4, cudaMemcpyDeviceToHost, c->stream);
+  cudaMemcpyAsync(&last_cnt, counts + (n - 1), 4, cudaMemcpyDeviceToHost, c->stream);
+  cudaStreamSynchronize(c->stream);
+  if (total) *total = (int64_t)last_off + last_cnt;
+  if (idx) {
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_fill, div_up(n, TPB), TPB, n, c->kc.cap, radius_id, c->nbr,
+               c->cn, c->co, c->oid[cur], c->tmp_src, idx, cap);
+  }
+  return MPS_OK;
+}

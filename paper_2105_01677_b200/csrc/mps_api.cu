@@ -1,0 +1,514 @@
+// mps_api.cu -- the extern "C" boundary of libmps_b200.so (include/mps_b200.h).
+// Host logic only: argument checks, buffer ownership, stage ordering, timers.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "mps_internal.h"
+
+static std::string g_init_error;
+
+#define CK(call)                                                                 \
+  do {                                                                           \
+    cudaError_t e_ = (call);                                                     \
+    if (e_ != cudaSuccess) {                                                     \
+      c->err = std::string(#call) + ": " + cudaGetErrorString(e_);               \
+      return MPS_ERR_CUDA;                                                       \
+    }                                                                            \
+  } while (0)
+
+static int fail(mps_ctx* c, int code, const char* msg) {
+  if (c) c->err = msg;
+  else g_init_error = msg;
+  return code;
+}
+
+// ---- lattice closed forms (I2; Eq. 5) -------------------------
+// n0 = sum over lattice offsets o != 0 with |o| l0 < re of (re / (|o| l0) - 1),
+// lambda = sum |o|^2 l0^2 w / sum w.
+static void lattice_sums(int dim, double l0, double re, double* n0, double* lam) {
+  const int R = (int)ceil(re / l0) + 1;
+  double sw = 0.0, sr2w = 0.0;
+  const int Rz = dim == 3 ? R : 0;
+  for (int a = -Rz; a <= Rz; ++a)
+    for (int b = -R; b <= R; ++b)
+      for (int k = -R; k <= R; ++k) {
+        if (!a && !b && !k) continue;
+        const double ex = k * l0, ey = b * l0, ez = a * l0;
+        const double r2 = (ex * ex + ey * ey) + ez * ez;
+        if (r2 < re * re) {
+          const double w = re / sqrt(r2) - 1.0;
+          sw += w;
+          sr2w += r2 * w;
+        }
+      }
+  *n0 = sw;
+  *lam = sr2w / sw;
+}
+
+template <class T>
+static cudaError_t dalloc(T** p, size_t count) {
+  return cudaMalloc((void**)p, std::max<size_t>(count, 1) * sizeof(T));
+}
+
+static void free_all(mps_ctx* c) {
+  for (int k = 0; k < 2; ++k) {
+    cudaFree(c->pos4[k]); cudaFree(c->vel4[k]); cudaFree(c->tp[k]); cudaFree(c->oid[k]);
+  }
+  cudaFree(c->key); cudaFree(c->key_tmp); cudaFree(c->rank); cudaFree(c->tmp_src);
+  cudaFree(c->tmp_oid); cudaFree(c->cell_count); cudaFree(c->cell_start); cudaFree(c->scan_tmp);
+  cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co);
+  cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
+  cudaFree(c->phat); cudaFree(c->grad4); cudaFree(c->bc);
+  cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
+  cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
+  if (c->cg_host) cudaFreeHost(c->cg_host);
+  if (c->flags_host) cudaFreeHost(c->flags_host);
+  if (c->poll_event) cudaEventDestroy(c->poll_event);
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+}
+
+static int check_params(const mps_params* p, int64_t n) {
+  if (!p) return fail(nullptr, MPS_ERR_ARG, "params is NULL");
+  if (n <= 0 || n > (int64_t)NB_INDEX) return fail(nullptr, MPS_ERR_ARG, "n must be in [1, 2^30)");
+  if (p->dim != 3) return fail(nullptr, MPS_ERR_ARG, "only dim = 3 is supported");
+  if (!(p->l0 > 0) || !(p->re_n > 0) || !(p->re_lap > 0) || !(p->dt > 0))
+    return fail(nullptr, MPS_ERR_ARG, "l0, re_n, re_lap and dt must be positive");
+  if (p->re_grad != p->re_n) return fail(nullptr, MPS_ERR_ARG, "re_grad must equal re_n");
+  if (p->re_lap < p->re_n) return fail(nullptr, MPS_ERR_ARG, "re_lap must be >= re_n");
+  if (p->key_mode != 0) return fail(nullptr, MPS_ERR_ARG, "key_mode 0 (linear) is the only mode");
+  if (p->cell_div < 1 || p->cell_div > 3) return fail(nullptr, MPS_ERR_ARG, "cell_div must be 1..3");
+  if (p->n_phases < 1 || p->n_phases > 2) return fail(nullptr, MPS_ERR_ARG, "n_phases must be 1 or 2");
+  if (p->max_neighbours < 1 || p->max_neighbours > 4096)
+    return fail(nullptr, MPS_ERR_ARG, "max_neighbours must be in [1, 4096]");
+  if (p->grad_variant < 0 || p->grad_variant > 2) return fail(nullptr, MPS_ERR_ARG, "grad_variant must be 0..2");
+  if (!(p->rho[0] > 0) || (p->n_phases == 2 && !(p->rho[1] > 0)))
+    return fail(nullptr, MPS_ERR_ARG, "densities must be positive");
+  if (!(p->gamma > 0) || !(p->cg_rtol > 0) || p->cg_maxit < 1)
+    return fail(nullptr, MPS_ERR_ARG, "gamma, cg_rtol and cg_maxit must be positive");
+  for (int a = 0; a < 3; ++a)
+    if (!(p->domain_max[a] > p->domain_min[a]))
+      return fail(nullptr, MPS_ERR_ARG, "domain_max must exceed domain_min");
+  return MPS_OK;
+}
+
+static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* stream) {
+  if (!out) return fail(nullptr, MPS_ERR_ARG, "out is NULL");
+  *out = nullptr;
+  int rc = check_params(prm, n);
+  if (rc) return rc;
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+    return fail(nullptr, MPS_ERR_CUDA, "no CUDA device: libmps_b200 has no CPU fallback");
+  if (prop.major < 10)
+    return fail(nullptr, MPS_ERR_CUDA, "libmps_b200 is built for sm_100a (B200) only");
+  mps_ctx* c = new (std::nothrow) mps_ctx;
+  if (!c) return fail(nullptr, MPS_ERR_ARG, "out of host memory");
+  c->prm = *prm;
+  c->n = n;
+  c->n_pad = (n + 31) / 32 * 32;
+  c->stream = (cudaStream_t)stream;
+  c->sm_count = prop.multiProcessorCount;
+
+  // constants (I1-I4)
+  KConst& k = c->kc;
+  memset(&k, 0, sizeof(k));
+  double n0n, lam_n, n0l, lam_l;
+  lattice_sums(prm->dim, prm->l0, prm->re_n, &n0n, &lam_n);
+  lattice_sums(prm->dim, prm->l0, prm->re_lap, &n0l, &lam_l);
+  k.n0_n = prm->n0_n > 0 ? prm->n0_n : n0n;
+  k.n0_lap = prm->n0_lap > 0 ? prm->n0_lap : n0l;
+  k.lam = prm->lambda > 0 ? prm->lambda : lam_l;
+  k.A_lap = 2.0 * prm->dim / (k.n0_lap * k.lam);
+  k.re_n = prm->re_n; k.re_n2 = prm->re_n * prm->re_n;
+  k.re_lap = prm->re_lap; k.re_lap2 = prm->re_lap * prm->re_lap;
+  k.dt = prm->dt;
+  for (int a = 0; a < 3; ++a) { k.g[a] = prm->g[a]; k.dmin[a] = prm->domain_min[a]; }
+  k.rho[0] = prm->rho[0]; k.rho[1] = prm->n_phases == 2 ? prm->rho[1] : prm->rho[0];
+  k.nu[0] = prm->nu[0]; k.nu[1] = prm->n_phases == 2 ? prm->nu[1] : prm->nu[0];
+  k.c0 = prm->c0; k.gamma = prm->gamma; k.beta = prm->beta;
+  k.compress_dt2 = prm->compress / (prm->dt * prm->dt);
+  k.relax_dt2 = prm->ppe_relax / (prm->dt * prm->dt);
+  k.cs_l0_sq = (prm->cs * prm->l0) * (prm->cs * prm->l0);
+  k.d_over_n0 = (double)prm->dim / k.n0_n;
+  c->h = std::max(prm->re_n, prm->re_lap) / prm->cell_div;
+  k.inv_h = 1.0 / c->h;
+  int64_t ncells = 1;
+  int nc[3];
+  for (int a = 0; a < 3; ++a) {
+    nc[a] = (int)ceil((prm->domain_max[a] - prm->domain_min[a]) * k.inv_h);
+    if (nc[a] < 1) nc[a] = 1;
+    ncells *= nc[a];
+  }
+  if (ncells > (int64_t)1 << 30) {
+    delete c;
+    return fail(nullptr, MPS_ERR_ARG, "grid has more than 2^30 cells");
+  }
+  k.nx = nc[0]; k.ny = nc[1]; k.nz = nc[2]; k.ncells = (int)ncells;
+  k.R_lap = (int)ceil(prm->re_lap * k.inv_h);
+  k.cap = prm->max_neighbours;
+  k.grad_variant = prm->grad_variant; k.clamp_negative_p = prm->clamp_negative_p;
+  k.rho_pair_mean = prm->rho_pair_mean; k.nu_pair_mean = prm->nu_pair_mean;
+  k.n = (int)n;
+
+  // every buffer any later call needs
+  cudaError_t e = cudaSuccess;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  const size_t N = (size_t)c->n_pad;
+  for (int b = 0; b < 2; ++b) {
+    A(dalloc(&c->pos4[b], N)); A(dalloc(&c->vel4[b], N)); A(dalloc(&c->tp[b], N)); A(dalloc(&c->oid[b], N));
+  }
+  A(dalloc(&c->key, N)); A(dalloc(&c->key_tmp, N)); A(dalloc(&c->rank, N));
+  A(dalloc(&c->tmp_src, N + 1)); A(dalloc(&c->tmp_oid, N));
+  A(dalloc(&c->cell_count, (size_t)ncells + 2)); A(dalloc(&c->cell_start, (size_t)ncells + 2));
+  A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
+  A(dalloc(&c->nbr, N * (size_t)k.cap)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
+  A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
+  A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->grad4, N)); A(dalloc(&c->bc, N));
+  A(dalloc(&c->cg_x, N)); A(dalloc(&c->cg_p, N)); A(dalloc(&c->cg_s, N)); A(dalloc(&c->cg_w, N));
+  A(dalloc(&c->cg_part, (size_t)2 * (c->sm_count * 8 + 8)));
+  A(dalloc(&c->cg, 1)); A(dalloc(&c->flags, 1)); A(dalloc(&c->io_tmp, N));
+  A(cudaMallocHost((void**)&c->cg_host, sizeof(CgScalars)));
+  A(cudaMallocHost((void**)&c->flags_host, sizeof(DevFlags)));
+  A(cudaEventCreateWithFlags(&c->poll_event, cudaEventDisableTiming));
+  if (e != cudaSuccess) {
+    g_init_error = std::string("allocation failed: ") + cudaGetErrorString(e);
+    free_all(c);
+    delete c;
+    return MPS_ERR_CUDA;
+  }
+  memset(c->cg_host, 0, sizeof(CgScalars));
+  memset(c->flags_host, 0, sizeof(DevFlags));
+  cudaStream_t s = c->stream;
+  cudaMemsetAsync(c->cg, 0, sizeof(CgScalars), s);
+  cudaMemsetAsync(c->flags, 0, sizeof(DevFlags), s);
+  double* zero_d[] = {c->dens, c->p, c->nut, c->b, c->phat, c->cg_x, c->cg_p, c->cg_s, c->cg_w};
+  for (double* z : zero_d) cudaMemsetAsync(z, 0, N * sizeof(double), s);
+  cudaMemsetAsync(c->acc4, 0, N * sizeof(double4), s);
+  cudaMemsetAsync(c->grad4, 0, N * sizeof(double4), s);
+  cudaMemsetAsync(c->bc, 0, N, s);
+  cudaMemsetAsync(c->cn, 0, N * 4, s);
+  cudaMemsetAsync(c->co, 0, N * 4, s);
+  cudaMemsetAsync(c->key, 0, N * 4, s);
+  for (int b = 0; b < 2; ++b) {
+    cudaMemsetAsync(c->pos4[b], 0, N * sizeof(double4), s);
+    cudaMemsetAsync(c->vel4[b], 0, N * sizeof(double4), s);
+    cudaMemsetAsync(c->tp[b], 0, N * 4, s);
+    cudaMemsetAsync(c->oid[b], 0, N * 4, s);
+  }
+  *out = c;
+  return MPS_OK;
+}
+
+// Reads the device-side flags; converts them into a sticky error code.
+static int read_flags(mps_ctx* c) {
+  CK(cudaMemcpyAsync(c->flags_host, c->flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->stats.max_neighbours = c->flags_host->max_row;
+  c->stats.n_ghost = c->flags_host->n_ghost;
+  if (c->flags_host->nonfinite) {
+    c->sticky_error = MPS_ERR_NONFINITE;
+    c->err = "non-finite position or coincident particles";
+  } else if (c->flags_host->overflow) {
+    c->sticky_error = MPS_ERR_NEIGHBOUR_OVERFLOW;
+    c->err = "a particle has more than max_neighbours neighbours";
+  }
+  c->stats.device_error = c->sticky_error;
+  return c->sticky_error;
+}
+
+// ---- timers ---------------------------------------------------------------------
+void mps_timer_begin(mps_ctx* c, int cat) {
+  if (c->ev_used + 2 > c->ev_pool.size()) mps_timer_drain(c);
+  cudaEventRecord(c->ev_pool[c->ev_used], c->stream);
+  c->ev_cat[c->ev_used / 2] = cat;
+}
+void mps_timer_end(mps_ctx* c, int) {
+  cudaEventRecord(c->ev_pool[c->ev_used + 1], c->stream);
+  c->ev_used += 2;
+}
+void mps_timer_drain(mps_ctx* c) {
+  if (c->ev_used == 0) return;
+  cudaStreamSynchronize(c->stream);
+  for (size_t k = 0; k < c->ev_used; k += 2) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->ev_pool[k], c->ev_pool[k + 1]) == cudaSuccess)
+      c->t_ms[c->ev_cat[k / 2]] += ms;
+  }
+  c->ev_used = 0;
+}
+
+extern "C" {
+
+const char* mps_version(void) { return "mps_b200 0.1 (sm_100a)"; }
+
+const char* mps_last_error(mps_ctx* c) { return c ? c->err.c_str() : g_init_error.c_str(); }
+
+int mps_init(mps_ctx** out, const mps_params* prm, int64_t n, const double* x, const double* y,
+             const double* z, const double* u, const double* v, const double* w, const int32_t* type,
+             const int32_t* phase, void* stream) {
+  if (!x || !y || !z || !u || !v || !w || !type || !phase)
+    return fail(nullptr, MPS_ERR_ARG, "a particle array pointer is NULL");
+  int rc = create_ctx(out, prm, n, stream);
+  if (rc) return rc;
+  mps_ctx* c = *out;
+  mpsk_load_particles(c, x, y, z, u, v, w, type, phase);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    g_init_error = std::string("mps_init: ") + cudaGetErrorString(e);
+    free_all(c);
+    delete c;
+    *out = nullptr;
+    return MPS_ERR_CUDA;
+  }
+  return MPS_OK;
+}
+
+int mps_init_host(mps_ctx** out, const mps_params* prm, int64_t n, const double* x, const double* y,
+                  const double* z, const double* u, const double* v, const double* w,
+                  const int32_t* type, const int32_t* phase, void* stream) {
+  if (!x || !y || !z || !u || !v || !w || !type || !phase)
+    return fail(nullptr, MPS_ERR_ARG, "a particle array pointer is NULL");
+  int rc = create_ctx(out, prm, n, stream);
+  if (rc) return rc;
+  mps_ctx* c = *out;
+  // stage through buffers that are free before the first bin
+  double* d[6] = {c->dens, c->p, c->nut, c->b, c->phat, c->cg_x};
+  const double* h[6] = {x, y, z, u, v, w};
+  for (int k = 0; k < 6; ++k)
+    cudaMemcpyAsync(d[k], h[k], n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+  cudaMemcpyAsync(c->key_tmp, type, n * 4, cudaMemcpyHostToDevice, c->stream);
+  cudaMemcpyAsync(c->rank, phase, n * 4, cudaMemcpyHostToDevice, c->stream);
+  mpsk_load_particles(c, d[0], d[1], d[2], d[3], d[4], d[5], (const int32_t*)c->key_tmp,
+                      (const int32_t*)c->rank);
+  for (int k = 0; k < 6; ++k) cudaMemsetAsync(d[k], 0, n * sizeof(double), c->stream);
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) {
+    g_init_error = std::string("mps_init_host: ") + cudaGetErrorString(e);
+    free_all(c);
+    delete c;
+    *out = nullptr;
+    return MPS_ERR_CUDA;
+  }
+  return MPS_OK;
+}
+
+int mps_destroy(mps_ctx* c) {
+  if (!c) return MPS_ERR_ARG;
+  cudaStreamSynchronize(c->stream);
+  free_all(c);
+  delete c;
+  return MPS_OK;
+}
+
+int mps_bin(mps_ctx* c) {
+  if (!c) return MPS_ERR_ARG;
+  mpsk_bin(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+
+#define NEED_BIN(c)                                                                        \
+  do {                                                                                     \
+    if (!(c)) return MPS_ERR_ARG;                                                          \
+    if (!(c)->binned) return fail((c), MPS_ERR_ORDER, "positions changed since the last mps_bin"); \
+  } while (0)
+
+int mps_density(mps_ctx* c) {
+  NEED_BIN(c);
+  mpsk_density(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_viscosity(mps_ctx* c) {
+  NEED_BIN(c);
+  mpsk_viscosity(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_predict(mps_ctx* c) {
+  if (!c) return MPS_ERR_ARG;
+  mpsk_predict(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_pressure_explicit(mps_ctx* c) {
+  if (!c) return MPS_ERR_ARG;
+  mpsk_pressure_explicit(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_pressure_ppe(mps_ctx* c, int32_t* iters_out, double* relres_out) {
+  NEED_BIN(c);
+  int rc = mpsk_pressure_ppe(c);
+  if (iters_out) *iters_out = c->stats.cg_iters;
+  if (relres_out) *relres_out = c->stats.cg_relres;
+  if (rc == MPS_ERR_CUDA) return rc;
+  int fl = read_flags(c);
+  if (fl) return fl;
+  return rc;
+}
+int mps_gradient(mps_ctx* c) {
+  NEED_BIN(c);
+  mpsk_gradient(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_correct(mps_ctx* c) {
+  if (!c) return MPS_ERR_ARG;
+  mpsk_correct(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+
+int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
+  if (!c) return MPS_ERR_ARG;
+  if (nsteps < 0 || (route != MPS_ROUTE_EXPLICIT && route != MPS_ROUTE_PPE))
+    return fail(c, MPS_ERR_ARG, "bad nsteps or pressure_route");
+  int first_err = MPS_OK;
+  for (int s = 0; s < nsteps; ++s) {
+    mpsk_bin(c);
+    mpsk_viscosity(c);
+    mpsk_predict(c);
+    mpsk_bin(c);
+    mpsk_density(c);
+    if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
+    else {
+      int rc = mpsk_pressure_ppe(c);
+      if (rc == MPS_ERR_CUDA) return rc;
+      if (rc && !first_err) first_err = rc;
+    }
+    mpsk_gradient(c);
+    mpsk_correct(c);
+    c->stats.steps_total++;
+  }
+  CK(cudaGetLastError());
+  int fl = read_flags(c);
+  if (fl) return fl;
+  return first_err;
+}
+
+int mps_step_host(const mps_params* prm, int64_t n, double* x, double* y, double* z, double* u,
+                  double* v, double* w, const int32_t* type, const int32_t* phase, double* p_out,
+                  int32_t nsteps, int32_t route, mps_stats* stats_out, void* stream) {
+  mps_ctx* c = nullptr;
+  int rc = mps_init_host(&c, prm, n, x, y, z, u, v, w, type, phase, stream);
+  if (rc) return rc;
+  rc = mps_step(c, nsteps, route);
+  if (rc == MPS_ERR_CUDA || rc == MPS_ERR_ARG) {
+    g_init_error = c->err;
+    mps_destroy(c);
+    return rc;
+  }
+  double* host[7] = {x, y, z, u, v, w, p_out};
+  const int fields[7] = {MPS_F_X, MPS_F_Y, MPS_F_Z, MPS_F_U, MPS_F_V, MPS_F_W, MPS_F_P};
+  for (int k = 0; k < 7; ++k) {
+    if (!host[k]) continue;
+    mpsk_get_field(c, fields[k], c->io_tmp, MPS_ORDER_ORIGINAL);
+    cudaMemcpyAsync(host[k], c->io_tmp, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  }
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (stats_out) *stats_out = c->stats;
+  if (e != cudaSuccess) {
+    g_init_error = std::string("mps_step_host: ") + cudaGetErrorString(e);
+    rc = MPS_ERR_CUDA;
+  } else if (rc) {
+    g_init_error = c->err;
+  }
+  mps_destroy(c);
+  return rc;
+}
+
+int mps_get_field(mps_ctx* c, int32_t field, void* dst, int32_t order) {
+  if (!c || !dst) return MPS_ERR_ARG;
+  if (order != MPS_ORDER_ORIGINAL && order != MPS_ORDER_SORTED) return fail(c, MPS_ERR_ARG, "bad order");
+  int rc = mpsk_get_field(c, field, dst, order);
+  if (rc) return fail(c, rc, "unknown field id");
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_set_field(mps_ctx* c, int32_t field, const void* src, int32_t order) {
+  if (!c || !src) return MPS_ERR_ARG;
+  if (order != MPS_ORDER_ORIGINAL && order != MPS_ORDER_SORTED) return fail(c, MPS_ERR_ARG, "bad order");
+  int rc = mpsk_set_field(c, field, src, order);
+  if (rc) return fail(c, rc, "unknown or read-only field id");
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_get_perm(mps_ctx* c, uint32_t* dst) {
+  if (!c || !dst) return MPS_ERR_ARG;
+  CK(cudaMemcpyAsync(dst, c->oid[c->cur], c->n * 4, cudaMemcpyDeviceToDevice, c->stream));
+  return MPS_OK;
+}
+int mps_get_grid(mps_ctx* c, int32_t* grid) {
+  if (!c || !grid) return MPS_ERR_ARG;
+  grid[0] = c->kc.nx; grid[1] = c->kc.ny; grid[2] = c->kc.nz; grid[3] = c->kc.ncells;
+  return MPS_OK;
+}
+int mps_get_cell_start(mps_ctx* c, uint32_t* dst) {
+  NEED_BIN(c);
+  if (!dst) return MPS_ERR_ARG;
+  CK(cudaMemcpyAsync(dst, c->cell_start, ((size_t)c->kc.ncells + 1) * 4, cudaMemcpyDeviceToDevice, c->stream));
+  return MPS_OK;
+}
+int mps_get_neighbours(mps_ctx* c, int32_t radius_id, uint32_t* counts, uint32_t* idx, int64_t cap,
+                       int64_t* total) {
+  NEED_BIN(c);
+  if (!counts || (radius_id != MPS_RADIUS_N && radius_id != MPS_RADIUS_LAP)) return MPS_ERR_ARG;
+  int rc = mpsk_get_neighbours(c, radius_id, counts, idx, cap, total);
+  CK(cudaGetLastError());
+  return rc;
+}
+int mps_ppe_apply(mps_ctx* c, const double* x, double* y, int32_t order) {
+  NEED_BIN(c);
+  if (!x || !y) return MPS_ERR_ARG;
+  if (!c->ppe_ready) return fail(c, MPS_ERR_ORDER, "mps_ppe_apply needs mps_pressure_ppe first");
+  mpsk_ppe_apply(c, x, y, order);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
+int mps_get_constants(mps_ctx* c, double* out) {
+  if (!c || !out) return MPS_ERR_ARG;
+  out[0] = c->kc.n0_n; out[1] = c->kc.n0_lap; out[2] = c->kc.lam; out[3] = c->kc.A_lap;
+  out[4] = c->h; out[5] = c->kc.inv_h;
+  return MPS_OK;
+}
+int mps_get_stats(mps_ctx* c, mps_stats* out) {
+  if (!c || !out) return MPS_ERR_ARG;
+  int rc = read_flags(c);
+  *out = c->stats;
+  return rc == MPS_ERR_CUDA ? rc : MPS_OK;
+}
+int mps_sync(mps_ctx* c) {
+  if (!c) return MPS_ERR_ARG;
+  return read_flags(c);
+}
+int mps_timers_enable(mps_ctx* c, int32_t on) {  // on = bit mask of categories
+  if (!c) return MPS_ERR_ARG;
+  if (on && c->ev_pool.empty()) {
+    c->ev_pool.resize(8192);
+    c->ev_cat.resize(4096);
+    for (auto& e : c->ev_pool) CK(cudaEventCreate(&e));
+  }
+  if (!on) mps_timer_drain(c);
+  c->timer_mask = (uint32_t)on;
+  if (on) {
+    for (int k = 0; k < MPS_NUM_TIMERS; ++k) { c->t_ms[k] = 0; c->t_launches[k] = 0; }
+  }
+  return MPS_OK;
+}
+int mps_timers_read(mps_ctx* c, double* ms, int64_t* launches) {
+  if (!c) return MPS_ERR_ARG;
+  mps_timer_drain(c);
+  for (int k = 0; k < MPS_NUM_TIMERS; ++k) {
+    if (ms) ms[k] = c->t_ms[k];
+    if (launches) launches[k] = c->t_launches[k];
+  }
+  return MPS_OK;
+}
+int64_t mps_launch_count(mps_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,157 @@
+// mps_internal.h -- internal ctx layout and launch helpers of libmps_b200.so.
+// Not part of the ABI.  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/mps_b200.h"
+
+// ---- data layout in HBM (all arrays in cell-sorted slot order) ---------------
+// pos4[i] = (x, y, z, s): one 32-byte sector per particle, so a neighbour gather
+//           is exactly one sector.  s is the scalar the current sweep gathers
+//           (pressure for the gradient, CG residual for the PPE operator).
+// vel4[i] = (u, v, w, nu_eff): nu_eff < 0 marks WALL/DUMMY (u = 0, nu_ij = nu_i).
+// tp[i]   = type | phase << 8.
+// oid[i]  = caller's original index of slot i (= perm).
+// nbr     = neighbour rows, warp-interleaved ELL: entry k of slot i lives at
+//           ((i >> 5) * cap + k) * 32 + (i & 31).  Entries with r < re_n fill
+//           the row from the front (count cn[i]); entries with re_n <= r < re_lap
+//           fill it from the back (count co[i]).  Entry = slot index of j
+//           | NB_DUMMY if j is a dummy | NB_PHASE1 if j is of phase 1.
+#define NB_DUMMY 0x80000000u
+#define NB_PHASE1 0x40000000u
+#define NB_INDEX 0x3fffffffu
+
+struct CgScalars {
+  double gamma, delta;          // r.r and r.Ar of the current iteration
+  double gamma_old, alpha_old;
+  double alpha, beta;
+  double bb, tol2bb;
+  int iters, done, converged, maxit;
+  unsigned int blocks_done, pad;
+  int n_surface, n_rows;
+};
+
+struct DevFlags {
+  int overflow;       // some row exceeded the capacity
+  int nonfinite;      // NaN/Inf position or coincident pair
+  int max_row;        // largest r_lap row
+  int n_ghost;
+};
+
+struct KConst {  // by-value kernel parameter
+  double re_n, re_n2, re_lap, re_lap2;
+  double n0_n, n0_lap, lam, A_lap;
+  double dt, g[3];
+  double rho[2], nu[2];
+  double c0, gamma, beta, compress_dt2, relax_dt2;
+  double cs_l0_sq, d_over_n0;
+  double dmin[3], inv_h;
+  int nx, ny, nz, ncells;
+  int R_lap;  // cells to each side for re_lap
+  int cap;    // row capacity (max_neighbours)
+  int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean;
+  int n;      // particles
+};
+
+struct mps_ctx {
+  mps_params prm;
+  KConst kc;
+  int64_t n = 0;
+  int64_t n_pad = 0;  // n rounded up to 32
+  cudaStream_t stream = nullptr;
+  double h = 0;
+  // double-buffered sorted particle arrays
+  double4* pos4[2] = {nullptr, nullptr};
+  double4* vel4[2] = {nullptr, nullptr};
+  uint32_t* tp[2] = {nullptr, nullptr};
+  uint32_t* oid[2] = {nullptr, nullptr};
+  int cur = 0;
+  // bin scratch
+  uint32_t* key = nullptr;         // per slot (after bin: key of the slot)
+  uint32_t* key_tmp = nullptr;     // per pre-sort slot
+  uint32_t* rank = nullptr;
+  uint32_t* tmp_src = nullptr;
+  uint32_t* tmp_oid = nullptr;
+  uint32_t* cell_count = nullptr;  // ncells + 2
+  uint32_t* cell_start = nullptr;  // ncells + 2
+  uint32_t* scan_tmp = nullptr;
+  // neighbour rows
+  uint32_t* nbr = nullptr;
+  uint32_t* cn = nullptr;
+  uint32_t* co = nullptr;
+  // per-particle fields
+  double* dens = nullptr;
+  double* p = nullptr;
+  double4* acc4 = nullptr;
+  double* nut = nullptr;
+  double* b = nullptr;
+  double* phat = nullptr;
+  double4* grad4 = nullptr;
+  int8_t* bc = nullptr;
+  // CG vectors
+  double* cg_x = nullptr;
+  double* cg_p = nullptr;
+  double* cg_s = nullptr;
+  double* cg_w = nullptr;
+  double* cg_part = nullptr;  // per-block partial sums
+  CgScalars* cg = nullptr;    // device
+  CgScalars* cg_host = nullptr;  // pinned
+  DevFlags* flags = nullptr;
+  DevFlags* flags_host = nullptr;  // pinned
+  double* io_tmp = nullptr;   // n doubles, staging for get/set
+  cudaEvent_t poll_event = nullptr;
+  // state
+  bool binned = false;
+  bool ppe_ready = false;
+  int sticky_error = 0;
+  mps_stats stats{};
+  std::string err;
+  int64_t launches = 0;
+  // timers
+  uint32_t timer_mask = 0;  // bit k: time category k with CUDA events
+  double t_ms[MPS_NUM_TIMERS] = {0};
+  int64_t t_launches[MPS_NUM_TIMERS] = {0};
+  std::vector<cudaEvent_t> ev_pool;
+  std::vector<int> ev_cat;
+  size_t ev_used = 0;
+  int sm_count = 148;
+};
+
+// ---- launch helper: counts launches, optional CUDA-event timing ------------------
+void mps_timer_begin(mps_ctx* c, int cat);
+void mps_timer_end(mps_ctx* c, int cat);
+void mps_timer_drain(mps_ctx* c);
+
+#define MPS_LAUNCH(c, cat, kern, grid, block, ...)                         \
+  do {                                                                     \
+    if (((c)->timer_mask >> (cat)) & 1u) mps_timer_begin((c), (cat));                       \
+    kern<<<(grid), (block), 0, (c)->stream>>>(__VA_ARGS__);                \
+    (c)->launches++;                                                       \
+    (c)->t_launches[(cat)]++;                                              \
+    if (((c)->timer_mask >> (cat)) & 1u) mps_timer_end((c), (cat));                         \
+  } while (0)
+
+static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ---- stage launchers (defined in the .cu files) -----------------------------------
+int mpsk_bin(mps_ctx* c);                 // keys, counting sort, reorder, neighbour rows
+void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
+                         uint32_t* tmp);
+int mpsk_density(mps_ctx* c);
+int mpsk_viscosity(mps_ctx* c);
+int mpsk_predict(mps_ctx* c);
+int mpsk_pressure_explicit(mps_ctx* c);
+int mpsk_pressure_ppe(mps_ctx* c);
+int mpsk_ppe_apply(mps_ctx* c, const double* x, double* y, int order);
+int mpsk_gradient(mps_ctx* c);
+int mpsk_correct(mps_ctx* c);
+int mpsk_get_field(mps_ctx* c, int field, void* dst, int order);
+int mpsk_set_field(mps_ctx* c, int field, const void* src, int order);
+int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const double* z,
+                        const double* u, const double* v, const double* w, const int32_t* type,
+                        const int32_t* phase);
+int mpsk_get_neighbours(mps_ctx* c, int radius_id, uint32_t* counts, uint32_t* idx, int64_t cap,
+                        int64_t* total);

@@ -1,0 +1,415 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element
+by element on the same seeded inputs.  Bars (north_star / DESIGN.md section 5):
+bit-exact keys, sort, cell table and neighbour sets; single-step fp64 fields
+within 1e-10 (max-norm, relative to the field's scale); PPE pressure: true
+relative residual under the ORACLE's operator <= 2e-8; 20-step trajectories
+within 1e-7 of the longest tank side."""
+import numpy as np
+import pytest
+
+from paper_2105_01677_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2105_01677_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import mps_oracle
+    return mps_oracle
+
+
+def relerr(a, b, floor):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), floor))
+
+
+def vec_relerr(ga, oa, floor):
+    d = np.sqrt(sum((g - o) ** 2 for g, o in zip(ga, oa)))
+    s = np.sqrt(sum(o ** 2 for o in oa))
+    return float(d.max() / max(s.max(), floor))
+
+
+def moved_state(O, s, nsteps=2, **over):
+    """Oracle state after a few explicit steps (off-lattice, non-zero velocities)."""
+    o = O.Oracle(s, **over)
+    o.step(nsteps, 0)
+    return o
+
+
+def inject(g, o, names):
+    for k in names:
+        g.set(k, o.get(k))
+
+
+# ---------------------------------------------------------------- S1, S2: bin ---
+@pytest.mark.parametrize("cell_div", [1, 2, 3])
+@pytest.mark.parametrize("scene", ["tank", "config1"])
+def test_bin_is_bit_exact(B, O, scene, cell_div):
+    s = scenes.small_tank(shuffle=True) if scene == "tank" else scenes.make_scene(1, shuffle=True)
+    s.x[5] = 10.0            # outside the domain -> GHOST
+    s.y[17] = float("nan")   # non-finite -> GHOST + error flag
+    s.z[40] = -1.0
+    o = O.Oracle(s, cell_div=cell_div)
+    key, perm, cs = o.bin()
+    g = B.Mps(s, cell_div=cell_div)
+    g.bin()
+    assert g.grid() == o.grid()
+    assert np.array_equal(g.get("key"), key)
+    assert np.array_equal(g.perm(), perm)
+    assert np.array_equal(g.cell_start(), cs)
+    assert np.array_equal(g.get("type"), o.get("type"))
+    # sorted-order view is consistent with perm
+    assert np.array_equal(g.get("x", B.ORDER_SORTED)[:-3], s.x[perm][:-3])
+    with pytest.raises(B.MpsError) as ei:
+        g.sync()
+    assert ei.value.code == B.MPS_ERR_NONFINITE
+    assert g.stats()["n_ghost"] == 3 == o.stats()["n_ghost"]
+    # a second bin of the already sorted state gives the same answer
+    g.bin()
+    assert np.array_equal(g.perm(), perm) and np.array_equal(g.cell_start(), cs)
+
+
+def test_bin_after_motion_matches_oracle(B, O):
+    s = scenes.small_tank(shuffle=True)
+    o = moved_state(O, s, 3)
+    g = B.Mps(s)
+    g.bin()
+    inject(g, o, ("x", "y", "z"))
+    key, perm, cs = o.bin()
+    g.bin()
+    assert np.array_equal(g.get("key"), key)
+    assert np.array_equal(g.perm(), perm)
+    assert np.array_equal(g.cell_start(), cs)
+
+
+# ----------------------------------------------------------- S3: neighbour sets ---
+@pytest.mark.parametrize("cell_div", [1, 2])
+@pytest.mark.parametrize("scene", ["tank_moved", "config1", "cloud"])
+def test_neighbour_sets_are_bit_exact(B, O, scene, cell_div):
+    if scene == "cloud":
+        s = scenes.random_cloud(3000, 10 * 0.031, seed=3)
+        s.params.update(l0=0.01, re_n=0.021, re_lap=0.031)
+        o = O.Oracle(s, cell_div=cell_div)
+        g = B.Mps(s, cell_div=cell_div)
+    else:
+        s = scenes.small_tank(shuffle=True) if scene == "tank_moved" else scenes.make_scene(1, shuffle=True)
+        o = moved_state(O, s, 2, cell_div=cell_div)
+        g = B.Mps(s, cell_div=cell_div)
+        inject(g, o, ("x", "y", "z"))
+    g.bin()
+    for rid, re in ((B.RADIUS_N, s.params["re_n"]), (B.RADIUS_LAP, s.params["re_lap"])):
+        co, io = o.neighbours(re)
+        cg, ig = g.neighbours(rid)
+        assert np.array_equal(cg, co)
+        assert np.array_equal(ig, io)
+        assert cg.max() <= 300
+    assert g.stats()["max_neighbours"] == o.neighbours(s.params["re_lap"])[0].max()
+
+
+# ------------------------------------------------------ S4-S11: single stages ---
+def _pair(B, O, s, **over):
+    o = moved_state(O, s, 2, **over)
+    g = B.Mps(s, **over)
+    inject(g, o, ("x", "y", "z", "u", "v", "w"))
+    g.bin()
+    return g, o
+
+
+@pytest.mark.parametrize("scene", ["tank", "config1"])
+def test_density(B, O, scene):
+    s = scenes.small_tank(shuffle=True) if scene == "tank" else scenes.make_scene(1)
+    g, o = _pair(B, O, s)
+    g.density(); o.density()
+    n0 = o.constants()["n0_n"]
+    assert relerr(g.get("n"), o.get("n"), n0) <= TOL
+    assert g.constants()["n0_n"] == pytest.approx(n0, rel=1e-15)
+    assert g.constants()["lam"] == pytest.approx(o.constants()["lam"], rel=1e-15)
+    assert g.constants()["A_lap"] == pytest.approx(o.constants()["A_lap"], rel=1e-15)
+
+
+@pytest.mark.parametrize("over", [dict(), dict(cs=0.12), dict(nu=(1e-3, 5e-3), n_phases=2, cs=0.12),
+                                  dict(nu=(1e-3, 5e-3), n_phases=2, nu_pair_mean=0)])
+def test_viscosity_and_smagorinsky(B, O, over):
+    s = scenes.small_tank(shuffle=True)
+    s.phase[s.z > 0.03] = 1
+    g, o = _pair(B, O, s, **over)
+    g.viscosity(); o.viscosity()
+    assert vec_relerr([g.get(k) for k in ("ax", "ay", "az")], [o.get(k) for k in ("ax", "ay", "az")], 9.81) <= TOL
+    nut_o = o.get("nut")
+    assert relerr(g.get("nut"), nut_o, 1e-12) <= 1e-9 if over.get("cs") else (g.get("nut") == 0).all()
+    if over.get("cs"):
+        assert nut_o.max() > 0
+    # viscous part alone (g = 0) so that the comparison is not dominated by gravity
+    over2 = dict(over, g=(0.0, 0.0, 0.0), nu=(0.7, 1.3), n_phases=2)
+    g2, o2 = _pair(B, O, s, **over2)
+    g2.viscosity(); o2.viscosity()
+    ao = [o2.get(k) for k in ("ax", "ay", "az")]
+    assert np.sqrt(sum(a ** 2 for a in ao)).max() > 1.0
+    assert vec_relerr([g2.get(k) for k in ("ax", "ay", "az")], ao, 1e-6) <= TOL
+
+
+def test_predict_and_correct(B, O):
+    s = scenes.small_tank(shuffle=True)
+    g, o = _pair(B, O, s)
+    g.viscosity(); o.viscosity()
+    g.predict(); o.predict()
+    for k in ("x", "y", "z", "u", "v", "w"):
+        assert np.array_equal(g.get(k), o.get(k)) or relerr(g.get(k), o.get(k), 1e-3) <= 1e-14, k
+    with pytest.raises(B.MpsError) as ei:
+        g.density()
+    assert ei.value.code == B.MPS_ERR_ORDER
+    g.bin()
+    g.density(); o.density()
+    g.pressure_explicit(); o.pressure_explicit()
+    g.gradient(); o.phat(); o.gradient()
+    g.correct(); o.correct()
+    L = 0.12
+    for k in ("x", "y", "z"):
+        assert relerr(g.get(k), o.get(k), L) <= 1e-13, k
+    assert vec_relerr([g.get(k) for k in "uvw"], [o.get(k) for k in "uvw"], 1e-3) <= TOL
+    fixed = s.type != scenes.FLUID
+    assert np.array_equal(g.get("x")[fixed], s.x[fixed]) and (g.get("u")[fixed] == 0).all()
+
+
+@pytest.mark.parametrize("over", [dict(), dict(clamp_negative_p=0), dict(gamma=5.5),
+                                  dict(n_phases=2, rho=(1000.0, 800.0))])
+def test_pressure_explicit(B, O, over):
+    s = scenes.small_tank(shuffle=True)
+    s.phase[s.z > 0.03] = 1
+    g, o = _pair(B, O, s, **over)
+    g.density(); o.density()
+    g.set("n", o.get("n"))
+    g.pressure_explicit(); o.pressure_explicit()
+    po = o.get("p")
+    assert relerr(g.get("p"), po, 1000.0 * 100.0 * 1e-6) <= TOL
+    if over.get("clamp_negative_p", 1) == 0:
+        assert po.min() < 0
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("route", [0, 1])
+def test_phat_and_gradient(B, O, variant, route):
+    s = scenes.small_tank(shuffle=True)
+    g, o = _pair(B, O, s, grad_variant=variant)
+    if route == 1:
+        # the PPE gives p > 0 only once gravity has compressed the column (a few PPE
+        # steps), and at the predicted positions r*
+        o.step(4, 1)
+        o.viscosity(); o.predict()
+        inject(g, o, ("x", "y", "z", "u", "v", "w"))
+        g.bin()
+    o.density()
+    if route == 0:
+        o.pressure_explicit()
+    else:
+        assert o.pressure_ppe() > 0
+    g.set("p", o.get("p"))
+    g.gradient(); o.phat(); o.gradient()
+    assert relerr(g.get("phat"), o.get("phat"), 1.0) <= 1e-15
+    Go = [o.get(k) for k in ("gx", "gy", "gz")]
+    assert np.sqrt(sum(a ** 2 for a in Go)).max() > 10.0
+    assert vec_relerr([g.get(k) for k in ("gx", "gy", "gz")], Go, 1000.0 * 9.81 * 0.01) <= TOL
+
+
+# ------------------------------------------------------------------- S8b: PPE ---
+@pytest.mark.parametrize("over", [dict(), dict(compress=0.0), dict(n_phases=2, rho=(1000.0, 800.0)),
+                                  dict(n_phases=2, rho=(1000.0, 800.0), rho_pair_mean=1),
+                                  dict(clamp_negative_p=0), dict(cell_div=2)])
+def test_ppe_flags_rhs_operator_and_solution(B, O, over):
+    s = scenes.small_tank(shuffle=True)
+    s.phase[s.z > 0.03] = 1
+    g, o = _pair(B, O, s, **over)
+    o.viscosity(); o.predict()
+    inject(g, o, ("x", "y", "z", "u", "v", "w"))
+    g.bin()
+    g.density(); o.density()
+    n0 = o.constants()["n0_n"]
+    assert relerr(g.get("n"), o.get("n"), n0) <= TOL
+    g.set("n", o.get("n"))  # same n on both sides: flags decided on identical numbers
+    it_g, relres_g = g.pressure_ppe()
+    o.ppe_flags(); o.ppe_rhs()
+    bc = o.get("bc")
+    assert np.array_equal(g.get("bc"), bc)
+    assert relerr(g.get("b"), o.get("b"), 1.0) <= 1e-14
+    st = g.stats()
+    assert st["n_surface"] == o.stats()["n_surface"] and st["n_rows"] == int((bc == 0).sum())
+    # operator parity on a random vector
+    rows = bc == 0
+    v = np.where(rows, np.random.default_rng(0).standard_normal(s.n), 0.0)
+    Ao = o.ppe_apply(v)
+    assert relerr(g.ppe_apply(v), Ao, 1e-30) <= TOL
+    # solution: true residual under the oracle's operator, and distance to a tight solve
+    x = g.get("xcg")
+    b = o.get("b")
+    assert (x[~rows] == 0).all()
+    true_rel = np.linalg.norm(b - o.ppe_apply(x)) / np.linalg.norm(b)
+    assert true_rel <= 2e-8
+    assert relres_g <= 1e-8 and st["cg_converged"] == 1
+    it_o = o.ppe_solve(o.params["cg_rtol"], 5000)
+    assert abs(it_g - it_o) <= 3
+    it_t = o.ppe_solve(1e-13, 5000)
+    xt = o.get("xcg")
+    kappa_est = 4.0 * (it_o / np.log(2.0 / 1e-8)) ** 2
+    dist = np.linalg.norm(x - xt) / np.linalg.norm(xt)
+    assert dist <= 1e-8 * kappa_est
+    print(f"PPE {over}: iters gpu {it_g} oracle {it_o}, true relres {true_rel:.2e}, "
+          f"|x - x_tight|/|x_tight| {dist:.2e} (bound {1e-8 * kappa_est:.1e})")
+    # pressures (after the clamp) against the oracle's own solve at the same tolerance
+    o.pressure_ppe()
+    assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-8 * kappa_est
+
+
+def test_ppe_noconv_and_zero_rhs(B, O):
+    s = scenes.small_tank(shuffle=True)
+    g = B.Mps(s, cg_maxit=3)
+    g.bin(); g.density()
+    with pytest.raises(B.MpsError) as ei:
+        g.pressure_ppe()
+    assert ei.value.code == B.MPS_ERR_NOCONV
+    it, _ = g.pressure_ppe(allow_noconv=True)
+    assert it == 3 and g.stats()["cg_converged"] == 0
+    # b = 0 (n = n0 everywhere): zero iterations, zero pressure
+    g2 = B.Mps(s)
+    g2.bin()
+    g2.set("n", np.full(s.n, g2.constants()["n0_n"]))
+    it, rr = g2.pressure_ppe()
+    assert it == 0 and rr == 0.0 and (g2.get("p") == 0).all()
+
+
+# --------------------------------------------------------------- whole steps ---
+def _trajectory(B, O, s, nsteps, route, **over):
+    g = B.Mps(s, **over)
+    o = O.Oracle(s, **over)
+    g.step(nsteps, route)
+    o.step(nsteps, route)
+    L = max(hi - lo for lo, hi in zip(s.params["domain_min"], s.params["domain_max"]))
+    d = np.sqrt(sum((g.get(k) - o.get(k)) ** 2 for k in "xyz"))
+    moved = np.sqrt(sum((o.get(k) - getattr(s, k)) ** 2 for k in "xyz")).max()
+    assert np.array_equal(g.get("type"), o.get("type"))
+    return d.max() / L, d.max() / s.params["l0"], moved / s.params["l0"], g, o
+
+
+def test_trajectory_config1_explicit_20_steps(B, O):
+    s = scenes.make_scene(1)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, 0)
+    print(f"config 1, 20 explicit steps: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}; max displacement {moved:.2f} l0")
+    assert moved > 0.05
+    assert eL <= 1e-7
+    assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-6
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_trajectory_small_tank_ppe_20_steps(B, O, variant):
+    s = scenes.small_tank(shuffle=True)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, 1, grad_variant=variant)
+    print(f"small tank, 20 PPE steps, variant {variant}: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}; moved {moved:.2f} l0")
+    assert eL <= 1e-7
+    assert g.stats()["cg_iters_total"] > 0
+
+
+def test_two_phase_smagorinsky_ppe_steps(B, O):
+    # config 4 in miniature: two layers, Cs = 0.12, density-weighted PPE operator
+    l0 = 0.01
+    s = scenes._lattice_scene("mini4", l0, (10, 8, 14), [((0, 0, 0), (10, 8, 5), 0), ((0, 0, 5), (10, 8, 10), 1)],
+                              seed=4, wall_phase_split_z=5)
+    over = dict(n_phases=2, rho=(1000.0, 800.0), nu=(1e-6, 5e-6), cs=0.12)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 10, 1, **over)
+    print(f"two-phase mini config 4, 10 PPE steps: max |dr|/L = {eL:.2e}")
+    assert eL <= 1e-7
+
+
+def test_config2_ppe_two_steps(B, O):
+    s = scenes.make_scene(2)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 2, 1)
+    print(f"config 2 (N={s.n}), 2 PPE steps: max |dr|/L = {eL:.2e}; cg iters {g.stats()['cg_iters']} vs {o.stats()['cg_iters']}")
+    assert eL <= 1e-7
+
+
+def test_step_host_equals_ctx_path(B, O):
+    s = scenes.small_tank(shuffle=True)
+    g = B.Mps(s)
+    g.step(3, 1)
+    arrays = {k: getattr(s, k).copy() for k in ("x", "y", "z", "u", "v", "w", "type", "phase")}
+    rc, st, p = B.step_host(s, arrays, 3, 1)
+    assert rc == 0 and st["steps_total"] == 3
+    for k in ("x", "y", "z", "u", "v", "w"):
+        assert np.array_equal(arrays[k], g.get(k)), k
+    assert np.array_equal(p, g.get("p"))
+
+
+# ------------------------------------------------------------------ edge cases ---
+def test_edge_single_particle_and_isolated(B, O):
+    s = scenes.random_cloud(1, 1.0, seed=1)
+    g = B.Mps(s)
+    g.step(2, 0)
+    assert g.get("n")[0] == 0 and g.stats()["max_neighbours"] == 0
+    # far apart particles: no neighbours, free fall
+    s = scenes.random_cloud(50, 100.0, seed=2)
+    s.params.update(l0=0.01, re_n=0.021, re_lap=0.031, cell_div=1, domain_max=(100.0, 100.0, 100.0))
+    s.z += 10.0
+    s.params["domain_max"] = (100.0, 100.0, 120.0)
+    g = B.Mps(s); o = O.Oracle(s)
+    g.step(3, 1); o.step(3, 1)
+    assert np.array_equal(g.get("z"), o.get("z")) and (g.get("p") == 0).all()
+
+
+def test_edge_overflow_and_coincident(B, O):
+    s = scenes.small_tank()
+    g = B.Mps(s, max_neighbours=64)
+    g.bin()
+    with pytest.raises(B.MpsError) as ei:
+        g.sync()
+    assert ei.value.code == B.MPS_ERR_NEIGHBOUR_OVERFLOW
+    s2 = scenes.small_tank()
+    s2.x[1], s2.y[1], s2.z[1] = s2.x[0], s2.y[0], s2.z[0]
+    g2 = B.Mps(s2)
+    g2.bin()
+    with pytest.raises(B.MpsError) as ei:
+        g2.sync()
+    assert ei.value.code == B.MPS_ERR_NONFINITE
+
+
+def test_edge_all_particles_leave_domain(B, O):
+    s = scenes.small_tank()
+    s.params["domain_max"] = (0.05, 0.05, 0.05)
+    g = B.Mps(s); o = O.Oracle(s)
+    key, perm, cs = o.bin()
+    g.bin()
+    assert np.array_equal(g.perm(), perm) and np.array_equal(g.cell_start(), cs)
+    assert g.stats()["n_ghost"] == o.stats()["n_ghost"] > 0
+    g.step(1, 0); o.step(1, 0)
+    assert np.array_equal(g.get("type"), o.get("type"))
+
+
+def test_full_size_sampled_config3(B, O):
+    """Config 3 (N = 438,208) in the launch configuration bench.py times: bin + density
+    + neighbour rows checked on sampled particles against the brute-force definition."""
+    s = scenes.make_scene(3)
+    g = B.Mps(s)
+    g.bin(); g.density()
+    n = g.get("n")
+    cnt_n, _ = g.neighbours(B.RADIUS_N)
+    rng = np.random.default_rng(5)
+    sample = rng.choice(s.n, 200, replace=False)
+    re = s.params["re_n"]
+    for i in sample:
+        dx, dy, dz = s.x - s.x[i], s.y - s.y[i], s.z - s.z[i]
+        r2 = (dx * dx + dy * dy) + dz * dz
+        m = r2 < re * re
+        m[i] = False
+        assert cnt_n[i] == m.sum()
+        ni = (re / np.sqrt(r2[m]) - 1.0).sum()
+        assert abs(n[i] - ni) <= 1e-10 * 14.4
+    key = g.get("key"); perm = g.perm()
+    assert (np.diff(key[perm].astype(np.int64)) >= 0).all()
+    same = np.diff(key[perm].astype(np.int64)) == 0
+    assert (np.diff(perm.astype(np.int64))[same] > 0).all()
