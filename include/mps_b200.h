@@ -191,6 +191,17 @@ int mps_step_host(const mps_params* prm, int64_t n, double* x, double* y, double
                   double* p_out, int32_t nsteps, int32_t pressure_route, mps_stats* stats_out,
                   void* stream);
 
+/* mps_upload_host / mps_download_host: the per-step host boundary of an existing
+ * ctx (no allocation).  upload replaces all n particles from HOST arrays in the
+ * caller's order (as mps_init_host does; invalidates the bin); download writes
+ * x,y,z,u,v,w and p (caller's order; any pointer may be NULL) to HOST arrays and
+ * synchronises the stream.  Pinned buffers make the copies asynchronous. */
+int mps_upload_host(mps_ctx* ctx, const double* x, const double* y, const double* z,
+                    const double* u, const double* v, const double* w,
+                    const int32_t* type, const int32_t* phase);
+int mps_download_host(mps_ctx* ctx, double* x, double* y, double* z,
+                      double* u, double* v, double* w, double* p);
+
 /* Field access for parity tests and checkpoints.  dst/src are DEVICE pointers
  * to n elements (double for ids < 32, int32_t otherwise). */
 int mps_get_field(mps_ctx* ctx, int32_t field, void* dst, int32_t order);

@@ -31,7 +31,8 @@ TIMERS = ["bin_sort", "bin_list", "viscosity", "predict", "density", "pressure_e
 # Names the header declares (checked by tests/test_abi.py against include/mps_b200.h).
 SYMBOLS = ["mps_init", "mps_init_host", "mps_destroy", "mps_bin", "mps_density", "mps_viscosity",
            "mps_predict", "mps_pressure_explicit", "mps_pressure_ppe", "mps_gradient",
-           "mps_correct", "mps_step", "mps_step_host", "mps_get_field", "mps_set_field",
+           "mps_correct", "mps_step", "mps_step_host", "mps_upload_host", "mps_download_host",
+           "mps_get_field", "mps_set_field",
            "mps_get_perm", "mps_get_grid", "mps_get_cell_start", "mps_get_neighbours",
            "mps_ppe_apply", "mps_get_constants", "mps_get_stats", "mps_sync",
            "mps_timers_enable", "mps_timers_read", "mps_launch_count", "mps_last_error",
@@ -108,6 +109,8 @@ def _load():
     L.mps_step.argtypes = [vp, i32, i32]
     L.mps_step_host.argtypes = [C.POINTER(MpsParams), i64] + [vp] * 6 + [vp, vp, vp, i32, i32,
                                                                       C.POINTER(MpsStats), vp]
+    L.mps_upload_host.argtypes = [vp] + [vp] * 8
+    L.mps_download_host.argtypes = [vp] + [vp] * 7
     L.mps_get_field.argtypes = [vp, i32, vp, i32]
     L.mps_set_field.argtypes = [vp, i32, vp, i32]
     L.mps_get_perm.argtypes = [vp, vp]
@@ -211,6 +214,14 @@ class Mps:
 
     def sync(self): self._ck(lib.mps_sync(self.h))
 
+    def upload_host(self, ptrs) -> None:
+        """ptrs: 8 host addresses (x, y, z, u, v, w, type, phase), n elements each."""
+        self._ck(lib.mps_upload_host(self.h, *ptrs))
+
+    def download_host(self, ptrs) -> None:
+        """ptrs: 7 host addresses (x, y, z, u, v, w, p) or None; synchronises."""
+        self._ck(lib.mps_download_host(self.h, *ptrs))
+
     # ---- fields -------------------------------------------------------------------
     def get_dev(self, name: str, order: int = ORDER_ORIGINAL):
         fid = FIELDS[name]
@@ -259,6 +270,13 @@ class Mps:
                                         tot.value, C.byref(tot)))
         self.stream.synchronize()
         return counts.cpu().numpy(), idx.cpu().numpy()[: tot.value]
+
+    def neighbour_counts(self, radius_id: int) -> np.ndarray:
+        counts = self.torch.empty(self.n, dtype=self.torch.int32, device=self.device)
+        tot = C.c_int64(0)
+        self._ck(lib.mps_get_neighbours(self.h, radius_id, counts.data_ptr(), None, 0, C.byref(tot)))
+        self.stream.synchronize()
+        return counts.cpu().numpy()
 
     def ppe_apply(self, x, order: int = ORDER_ORIGINAL) -> np.ndarray:
         xt = self.torch.as_tensor(np.ascontiguousarray(x, np.float64)).to(self.device)

@@ -422,6 +422,42 @@ int mps_step_host(const mps_params* prm, int64_t n, double* x, double* y, double
   return rc;
 }
 
+int mps_upload_host(mps_ctx* c, const double* x, const double* y, const double* z, const double* u,
+                    const double* v, const double* w, const int32_t* type, const int32_t* phase) {
+  if (!c) return MPS_ERR_ARG;
+  if (!x || !y || !z || !u || !v || !w || !type || !phase)
+    return fail(c, MPS_ERR_ARG, "a particle array pointer is NULL");
+  const int64_t n = c->n;
+  // stage through per-particle fields that every step recomputes before reading
+  double* d[6] = {c->dens, c->p, c->nut, c->b, c->phat, c->cg_x};
+  const double* h[6] = {x, y, z, u, v, w};
+  for (int k = 0; k < 6; ++k)
+    CK(cudaMemcpyAsync(d[k], h[k], n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->key_tmp, type, n * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->rank, phase, n * 4, cudaMemcpyHostToDevice, c->stream));
+  mpsk_load_particles(c, d[0], d[1], d[2], d[3], d[4], d[5], (const int32_t*)c->key_tmp,
+                      (const int32_t*)c->rank);
+  for (int k = 0; k < 6; ++k) cudaMemsetAsync(d[k], 0, n * sizeof(double), c->stream);
+  CK(cudaGetLastError());
+  c->binned = false;
+  c->ppe_ready = false;
+  return MPS_OK;
+}
+
+int mps_download_host(mps_ctx* c, double* x, double* y, double* z, double* u, double* v, double* w,
+                      double* p) {
+  if (!c) return MPS_ERR_ARG;
+  double* host[7] = {x, y, z, u, v, w, p};
+  const int fields[7] = {MPS_F_X, MPS_F_Y, MPS_F_Z, MPS_F_U, MPS_F_V, MPS_F_W, MPS_F_P};
+  for (int k = 0; k < 7; ++k) {
+    if (!host[k]) continue;
+    mpsk_get_field(c, fields[k], c->io_tmp, MPS_ORDER_ORIGINAL);
+    CK(cudaMemcpyAsync(host[k], c->io_tmp, c->n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  return MPS_OK;
+}
+
 int mps_get_field(mps_ctx* c, int32_t field, void* dst, int32_t order) {
   if (!c || !dst) return MPS_ERR_ARG;
   if (order != MPS_ORDER_ORIGINAL && order != MPS_ORDER_SORTED) return fail(c, MPS_ERR_ARG, "bad order");

@@ -353,10 +353,10 @@ def test_edge_single_particle_and_isolated(B, O):
     g.step(2, 0)
     assert g.get("n")[0] == 0 and g.stats()["max_neighbours"] == 0
     # far apart particles: no neighbours, free fall
-    s = scenes.random_cloud(50, 100.0, seed=2)
-    s.params.update(l0=0.01, re_n=0.021, re_lap=0.031, cell_div=1, domain_max=(100.0, 100.0, 100.0))
-    s.z += 10.0
-    s.params["domain_max"] = (100.0, 100.0, 120.0)
+    s = scenes.random_cloud(50, 2.0, seed=2)
+    s.params.update(l0=0.01, re_n=0.021, re_lap=0.031, cell_div=1)
+    s.z += 1.0
+    s.params["domain_max"] = (2.0, 2.0, 3.5)  # 65 x 65 x 113 cells of side 0.031
     g = B.Mps(s); o = O.Oracle(s)
     g.step(3, 1); o.step(3, 1)
     assert np.array_equal(g.get("z"), o.get("z")) and (g.get("p") == 0).all()
