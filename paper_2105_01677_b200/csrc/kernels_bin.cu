@@ -181,69 +181,104 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
 }
 
 // ------------------------------------------------ S3: neighbour rows (the sweep) ---
-// One thread per particle i.  For every (dy, dz) row of cells the candidates are
-// one contiguous slot range (x-fastest key).  Decision: r2 = (dx*dx + dy*dy) +
-// dz*dz with every operation rounded separately, r2 < re*re (strict, Eq. 3).
-// Hits inside re_n go to the front of the row, the others to the back.
-__global__ void __launch_bounds__(128)
+// One warp per particle i, the 32 lanes test 32 candidates j at a time.  For every
+// (dy, dz) row of cells the candidates are one contiguous slot range (x-fastest
+// key), read as coalesced 32-byte records.  Decision: r2 = (dx*dx + dy*dy) + dz*dz
+// with every operation rounded separately, r2 < re*re (strict, Eq. 3; Q2).  Hits
+// are compacted with a ballot and written as contiguous runs: inside re_n to the
+// front of the row, the others to the back; entries come out in ascending slot
+// order, so every later sum has a fixed order.
+constexpr int ROWS_TPB = 256;
+constexpr int ROWS_PPW = 4;  // particles per warp (consecutive slots: same candidate cells)
+
+__global__ void __launch_bounds__(ROWS_TPB)
 k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
              const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
              uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
              DevFlags* __restrict__ flags) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= kc.n) return;
-  uint32_t k = key[i];
-  if (k >= (uint32_t)kc.ncells) {  // ghost
-    cn[i] = 0;
-    co[i] = 0;
-    return;
-  }
-  const double4 pi = pos4[i];
-  const int cx = (int)(k % (uint32_t)kc.nx);
-  const int cy = (int)((k / (uint32_t)kc.nx) % (uint32_t)kc.ny);
-  const int cz = (int)(k / ((uint32_t)kc.nx * (uint32_t)kc.ny));
+  const int lane = threadIdx.x & 31;
+  const int warp = (blockIdx.x * ROWS_TPB + threadIdx.x) >> 5;
+  const uint32_t lt_mask = (1u << lane) - 1u;
   const int R = kc.R_lap;
-  const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
-  uint32_t* row = nbr + ((size_t)(i >> 5) * kc.cap) * 32 + (i & 31);
-  uint32_t nf = 0, nb = 0;
   const uint32_t cap = (uint32_t)kc.cap;
-  bool coincident = false;
-  for (int dz = -R; dz <= R; ++dz) {
-    int z2 = cz + dz;
-    if (z2 < 0 || z2 >= kc.nz) continue;
-    for (int dy = -R; dy <= R; ++dy) {
-      int y2 = cy + dy;
-      if (y2 < 0 || y2 >= kc.ny) continue;
-      int cbase = kc.nx * (y2 + kc.ny * z2);
-      uint32_t js = cell_start[cbase + x_lo];
-      uint32_t je = cell_start[cbase + x_hi + 1];
-      for (uint32_t j = js; j < je; ++j) {
-        double4 q = pos4[j];
-        double dx = __dsub_rn(q.x, pi.x), dy_ = __dsub_rn(q.y, pi.y), dz_ = __dsub_rn(q.z, pi.z);
-        double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
-        if (r2 < kc.re_lap2 && j != (uint32_t)i) {
-          if (r2 == 0.0) coincident = true;
-          uint32_t t = tp[j];
-          uint32_t e = j | (((t & 0xff) == MPS_DUMMY) ? NB_DUMMY : 0u) | ((t & 0x100) ? NB_PHASE1 : 0u);
-          if (nf + nb < cap) {
-            if (r2 < kc.re_n2) row[(size_t)(nf++) * 32] = e;
-            else row[(size_t)(cap - 1 - (nb++)) * 32] = e;
+  int warp_max = 0;
+  bool coincident = false, overflow = false;
+  for (int t = 0; t < ROWS_PPW; ++t) {
+    const int i = warp * ROWS_PPW + t;
+    if (i >= kc.n) break;
+    const uint32_t k = key[i];
+    if (k >= (uint32_t)kc.ncells) {  // ghost
+      if (lane == 0) { cn[i] = 0; co[i] = 0; }
+      continue;
+    }
+    const double4 pi = pos4[i];
+    const int cx = (int)(k % (uint32_t)kc.nx);
+    const int cy = (int)((k / (uint32_t)kc.nx) % (uint32_t)kc.ny);
+    const int cz = (int)(k / ((uint32_t)kc.nx * (uint32_t)kc.ny));
+    const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
+    uint32_t* row = nbr + (size_t)i * (size_t)kc.stride;
+    uint32_t nf = 0, nb = 0;  // warp-uniform
+    for (int dz = -R; dz <= R; ++dz) {
+      const int z2 = cz + dz;
+      if (z2 < 0 || z2 >= kc.nz) continue;
+      for (int dy = -R; dy <= R; ++dy) {
+        const int y2 = cy + dy;
+        if (y2 < 0 || y2 >= kc.ny) continue;
+        const int cbase = kc.nx * (y2 + kc.ny * z2);
+        const uint32_t js = cell_start[cbase + x_lo];
+        const uint32_t je = cell_start[cbase + x_hi + 1];
+        for (uint32_t j0 = js; j0 < je; j0 += 32) {
+          const uint32_t j = j0 + (uint32_t)lane;
+          bool in_lap = false, in_n = false;
+          uint32_t e = 0;
+          if (j < je) {
+            const double4 q = pos4[j];
+            const double dx = __dsub_rn(q.x, pi.x), dy_ = __dsub_rn(q.y, pi.y), dz_ = __dsub_rn(q.z, pi.z);
+            const double r2 =
+                __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
+            in_lap = (r2 < kc.re_lap2) && (j != (uint32_t)i);
+            if (in_lap) {
+              in_n = r2 < kc.re_n2;
+              if (r2 == 0.0) coincident = true;
+              const uint32_t tj = tp[j];
+              const uint32_t ty = tj & 0xff;
+              e = j | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
+                  ((tj & 0x100) ? NB_PHASE1 : 0u);
+            }
+          }
+          const uint32_t m_n = __ballot_sync(0xffffffffu, in_n);
+          const uint32_t m_o = __ballot_sync(0xffffffffu, in_lap && !in_n);
+          const uint32_t add_n = (uint32_t)__popc(m_n), add_o = (uint32_t)__popc(m_o);
+          if (nf + nb + add_n + add_o <= cap) {
+            if (in_n) row[nf + (uint32_t)__popc(m_n & lt_mask)] = e;
+            else if (in_lap) row[(uint32_t)kc.stride - 1u - (nb + (uint32_t)__popc(m_o & lt_mask))] = e;
+            nf += add_n;
+            nb += add_o;
           } else {
-            nf++;  // keep counting so that the overflow is visible
+            // keep what fits (front entries first, in order), then stop storing
+            overflow = true;
+            const uint32_t room = cap - (nf + nb);
+            const uint32_t pn = (uint32_t)__popc(m_n & lt_mask);
+            if (in_n && pn < room) row[nf + pn] = e;
+            const uint32_t took_n = add_n < room ? add_n : room;
+            const uint32_t room_o = room - took_n;
+            const uint32_t po = (uint32_t)__popc(m_o & lt_mask);
+            if (in_lap && !in_n && po < room_o) row[(uint32_t)kc.stride - 1u - (nb + po)] = e;
+            nf += took_n;
+            nb += add_o < room_o ? add_o : room_o;
           }
         }
       }
     }
+    if (lane == 0) { cn[i] = nf; co[i] = nb; }
+    warp_max = max(warp_max, (int)(nf + nb));
   }
-  if (nf + nb > cap) {
-    flags->overflow = 1;
-    uint32_t over = nf + nb - cap;
-    nf = nf >= over ? nf - over : 0;  // rows stay within capacity
+  coincident = __any_sync(0xffffffffu, coincident);
+  if (lane == 0) {
+    if (overflow) flags->overflow = 1;
+    if (coincident) flags->nonfinite = 1;
+    if (warp_max > 0) atomicMax(&flags->max_row, warp_max);
   }
-  cn[i] = nf;
-  co[i] = nb;
-  if (coincident) flags->nonfinite = 1;
-  atomicMax(&flags->max_row, (int)(nf + nb));
 }
 
 __global__ void k_count_ghosts(int n, int ncells, const uint32_t* __restrict__ cell_start,
@@ -340,14 +375,14 @@ __global__ void k_nb_fill(int n, int cap_row, int radius_id, const uint32_t* __r
                           uint32_t* __restrict__ idx, int64_t cap) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const uint32_t* row = nbr + ((size_t)(i >> 5) * cap_row) * 32 + (i & 31);
+  const uint32_t* row = nbr + (size_t)i * (size_t)cap_row;
   int64_t base = offs[oid[i]];
   uint32_t nf = cn[i], nb = (radius_id == MPS_RADIUS_LAP) ? co[i] : 0u;
   uint32_t m = nf + nb;
   if (base + m > cap) return;  // caller's buffer too small for this row: skip it
   // insertion sort by original index while writing
   for (uint32_t k = 0; k < m; ++k) {
-    uint32_t e = (k < nf) ? row[(size_t)k * 32] : row[(size_t)(cap_row - 1 - (k - nf)) * 32];
+    uint32_t e = (k < nf) ? row[k] : row[cap_row - 1 - (k - nf)];
     uint32_t v = oid[e & NB_INDEX];
     int64_t t = base + k;
     while (t > base && idx[t - 1] > v) { idx[t] = idx[t - 1]; --t; }
@@ -391,10 +426,11 @@ int mpsk_bin(mps_ctx* c) {
              c->vel4[nxt], c->tp[nxt], c->oid[nxt]);
   c->cur = nxt;
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
-  MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, 128), 128, c->kc, c->pos4[nxt], c->tp[nxt],
+  MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc, c->pos4[nxt], c->tp[nxt],
              c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags);
   c->binned = true;
   c->ppe_ready = false;
+  c->posw_is_p = false;
   return MPS_OK;
 }
 
@@ -434,6 +470,7 @@ int mpsk_set_field(mps_ctx* c, int field, const void* src, int order) {
                c->vel4[cur], c->acc4, c->grad4, (double*)scalar_field(c, field), c->oid[cur],
                (const double*)src);
     if (field <= MPS_F_Z) { c->binned = false; c->ppe_ready = false; }
+    if (field == MPS_F_P) c->posw_is_p = false;
     return MPS_OK;
   }
   if (field >= MPS_I_TYPE && field <= MPS_I_BC) {
@@ -459,7 +496,7 @@ int mpsk_get_neighbours(mps_ctx* c, int radius_id, uint32_t* counts, uint32_t* i
   cudaStreamSynchronize(c->stream);
   if (total) *total = (int64_t)last_off + last_cnt;
   if (idx) {
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_fill, div_up(n, TPB), TPB, n, c->kc.cap, radius_id, c->nbr,
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_fill, div_up(n, TPB), TPB, n, c->kc.stride, radius_id, c->nbr,
                c->cn, c->co, c->oid[cur], c->tmp_src, idx, cap);
   }
   return MPS_OK;

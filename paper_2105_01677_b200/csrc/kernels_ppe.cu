@@ -3,232 +3,341 @@
 // matrix-free operator with the structure of Listing 2, and the
 // conjugate-gradient solve (Eq. 9; Q15).
 //
-// CG is run in the single-reduction (Chronopoulos-Gear) form: one operator
-// kernel per iteration computes w = A r fused with the two dot products r.r and
-// r.w (warp shuffles, one partial per block, the last block to finish reduces
-// them in a fixed order and derives alpha and beta); one update kernel then
-// advances p, s = A p, x and r.  All scalars stay on the device; the host only
-// polls a done flag every few iterations.  In exact arithmetic the iterates are
-// those of textbook CG; the matrix is never stored.
-#include "mps_internal.h"
+// The whole solve is ONE persistent cooperative kernel (k_ppe_cg): flags and
+// right-hand side, ordered compaction of the unknown rows, then the CG loop in its
+// single-reduction (Chronopoulos-Gear) form with two grid barriers per iteration:
+//   phase A  w = A r fused with the dot products r.r and r.w (L lanes per row,
+//            shuffles inside the row group, one partial per block)
+//   barrier  every block adds the partials in index order -> identical alpha, beta
+//   phase B  p = r + beta p; s = w + beta s; x += alpha p; r -= alpha s
+//   barrier  r (kept in pos4.w, so a neighbour gather is one 32-byte sector) is visible
+// All scalars stay on the device and the convergence test is taken by every block
+// from the same numbers, so there is no host poll.  In exact arithmetic the
+// iterates are those of textbook CG; the matrix is never stored.
+#include <algorithm>
+
+#include "sweep_common.cuh"
 
 namespace {
 
-constexpr int TPB = 128;
+constexpr int CG_TPB = 512;
 
-__device__ __forceinline__ const uint32_t* row_of(const uint32_t* nbr, int cap, int i) {
-  return nbr + ((size_t)(i >> 5) * cap) * 32 + (i & 31);
-}
+struct PpeArgs {
+  double4* pos4;  // .w: CG residual r during the solve, pressure at exit
+  const uint32_t* tp;
+  const double* dens;
+  int8_t* bc;
+  double* b;
+  double* x;
+  double* pv;
+  double* sv;
+  double* wv;
+  double* p;
+  const uint32_t* nbr;
+  const uint32_t* cn;
+  const uint32_t* co;
+  uint32_t* rows;
+  uint32_t* bcount;  // 2 per block: rows, surface
+  double* part;      // 2 per block
+  CgScalars* cg;
+  GridBar* bar;
+  double tol2;
+  int maxit;
+};
 
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
-
-// Block-wide sum of two values; result valid in thread 0.
+// ---- block-wide sum of two values, result broadcast to every thread ---------------
+template <int NT>
 __device__ __forceinline__ void block_sum2(double& a, double& b) {
-  __shared__ double sh[2][TPB / 32];
+  __shared__ double sh[2][NT / 32];
   a = warp_sum(a);
   b = warp_sum(b);
-  int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __syncthreads();  // sh may still be read from the previous call
   if (lane == 0) { sh[0][wid] = a; sh[1][wid] = b; }
   __syncthreads();
-  if (threadIdx.x == 0) {
-    double sa = 0.0, sb = 0.0;
-#pragma unroll
-    for (int k = 0; k < TPB / 32; ++k) { sa += sh[0][k]; sb += sh[1][k]; }
-    a = sa;
-    b = sb;
-  }
-  __syncthreads();
-}
-
-// Publishes this block's partial sums; the last block to arrive adds all
-// partials in index order (deterministic) and returns true in its thread 0.
-__device__ __forceinline__ bool grid_sum2(double& a, double& b, double* part, unsigned int* counter) {
-  __shared__ bool last;
-  block_sum2(a, b);
-  if (threadIdx.x == 0) {
-    part[2 * blockIdx.x] = a;
-    part[2 * blockIdx.x + 1] = b;
-    __threadfence();
-    unsigned int t = atomicAdd(counter, 1u);
-    last = (t == gridDim.x - 1);
-  }
-  __syncthreads();
-  if (!last) return false;
-  __threadfence();
   double sa = 0.0, sb = 0.0;
-  for (int k = threadIdx.x; k < (int)gridDim.x; k += TPB) {
-    sa += __ldcg(&part[2 * k]);
-    sb += __ldcg(&part[2 * k + 1]);
-  }
-  block_sum2(sa, sb);
+#pragma unroll
+  for (int k = 0; k < NT / 32; ++k) { sa += sh[0][k]; sb += sh[1][k]; }
   a = sa;
   b = sb;
-  if (threadIdx.x == 0) *counter = 0;
-  return threadIdx.x == 0;
 }
 
-// -------------------------------------------------- S8b-1, S8b-2: flags + rhs ---
-__global__ void __launch_bounds__(TPB)
-k_ppe_setup(KConst kc, double tol2, int maxit, double4* __restrict__ pos4,
-            const uint32_t* __restrict__ tp, const double* __restrict__ dens, int8_t* __restrict__ bc,
-            double* __restrict__ b, double* __restrict__ x, double* __restrict__ pv,
-            double* __restrict__ sv, double* __restrict__ part, CgScalars* __restrict__ cg) {
-  double bb = 0.0, cnt = 0.0;
-  int n_surf = 0, n_rows = 0;
-  for (int i = blockIdx.x * TPB + threadIdx.x; i < kc.n; i += gridDim.x * TPB) {
-    uint32_t ty = tp[i] & 0xff;
-    int8_t f;
-    double bi = 0.0;
-    if (ty == MPS_DUMMY || ty == MPS_GHOST) f = -1;
-    else if (dens[i] < kc.beta * kc.n0_n) { f = 1; ++n_surf; }
-    else {
-      f = 0;
-      ++n_rows;
-      bi = kc.relax_dt2 * (dens[i] - kc.n0_n) / kc.n0_n;
-    }
-    bc[i] = f;
-    b[i] = bi;
-    x[i] = 0.0;
-    pv[i] = 0.0;
-    sv[i] = 0.0;
-    pos4[i].w = bi;  // r0 = b
-    bb += bi * bi;
-  }
-  cnt = (double)(n_surf) + 67108864.0 * (double)n_rows;  // two counters in one exact double
-  if (grid_sum2(bb, cnt, part, &cg->blocks_done)) {
-    double rows = floor(cnt / 67108864.0);
-    cg->n_rows = (int)rows;
-    cg->n_surface = (int)(cnt - rows * 67108864.0);
-    cg->bb = bb;
-    cg->tol2bb = tol2 * bb;
-    cg->gamma = bb;
-    cg->delta = 0.0;
-    cg->gamma_old = 1.0;
-    cg->alpha_old = 1.0;
-    cg->alpha = 0.0;
-    cg->beta = 0.0;
-    cg->iters = 0;
-    cg->maxit = maxit;
-    cg->done = (bb == 0.0) ? 1 : 0;
-    cg->converged = (bb == 0.0) ? 1 : 0;
-  }
+// ---- grid barrier (all blocks are co-resident: cooperative launch) ----------------
+// One thread per block arrives with a release fence and spins on the generation
+// word; the fence after the spin makes every later plain load of the block see the
+// other blocks' writes (it invalidates the SM's L1).  A spin that lasts longer than
+// about two seconds raises barrier_timeout and lets the kernel drain instead of hanging.
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
 }
-
-// ------------------------------------------------------ S8b-3: y = A r (+ dots) ---
-// (A r)_i = sum_{j in N(i, re_lap), j not dummy} c_ij (r_i - r_j) + compress/dt^2 r_i
-// with c_ij = A_lap w(r_ij) / rho_ij, on rows bc_i = 0.  r_j is read from pos4.w,
-// which is 0 on free-surface slots (Dirichlet p = 0) by construction.
-template <bool TWO_PHASE, bool REDUCE>
-__global__ void __launch_bounds__(TPB)
-k_cg_spmv(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
-          const int8_t* __restrict__ bc, const uint32_t* __restrict__ nbr,
-          const uint32_t* __restrict__ cn, const uint32_t* __restrict__ co, double* __restrict__ wv,
-          double* __restrict__ part, CgScalars* __restrict__ cg) {
-  if (REDUCE) {
-    if (cg->done) return;
-  }
-  double gam = 0.0, del = 0.0;
-  const double inv_rho0 = 1.0 / kc.rho[0];
-  for (int i = blockIdx.x * TPB + threadIdx.x; i < kc.n; i += gridDim.x * TPB) {
-    if (bc[i] != 0) {
-      if (!REDUCE) wv[i] = 0.0;
-      continue;
-    }
-    const double4 pi = pos4[i];
-    const uint32_t* row = row_of(nbr, kc.cap, i);
-    const uint32_t nf = cn[i], nb = co[i];
-    const double rho_i = TWO_PHASE ? kc.rho[(tp[i] >> 8) & 1] : kc.rho[0];
-    double s = 0.0;
-    auto term = [&](uint32_t e) {
-      if (e & NB_DUMMY) return;
-      double4 q = pos4[e & NB_INDEX];
-      double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
-      double r2 = dx * dx + dy * dy + dz * dz;
-      double w = kc.re_lap * rsqrt(r2) - 1.0;
-      if (TWO_PHASE) {
-        double rho_j = kc.rho[(e & NB_PHASE1) ? 1 : 0];
-        double rij = kc.rho_pair_mean == 1 ? 2.0 * rho_i * rho_j / (rho_i + rho_j) : 0.5 * (rho_i + rho_j);
-        w = w / rij;
-      }
-      s += w * (pi.w - q.w);
-    };
-    for (uint32_t k = 0; k < nf; ++k) term(row[(size_t)k * 32]);
-    for (uint32_t k = 0; k < nb; ++k) term(row[(size_t)(kc.cap - 1 - k) * 32]);
-    if (!TWO_PHASE) s *= inv_rho0;
-    double wi = kc.A_lap * s + kc.compress_dt2 * pi.w;
-    wv[i] = wi;
-    gam += pi.w * pi.w;
-    del += pi.w * wi;
-  }
-  if (!REDUCE) return;
-  if (grid_sum2(gam, del, part, &cg->blocks_done)) {
-    cg->gamma = gam;
-    cg->delta = del;
-    if (gam <= cg->tol2bb) {
-      cg->done = 1;
-      cg->converged = 1;
-    } else if (cg->iters >= cg->maxit) {
-      cg->done = 1;
-      cg->converged = 0;
+__device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, CgScalars* cg) {
+  __shared__ int dead;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    dead = 0;
+    gen += 1u;
+    __threadfence();
+    const unsigned int prev = atomicAdd(&bar->count, 1u);
+    if (prev == gridDim.x - 1u) {
+      atomicExch(&bar->count, 0u);
+      __threadfence();
+      atomicExch(&bar->gen, gen);
     } else {
-      double beta, alpha;
-      if (cg->iters == 0) {
+      const long long t0 = clock64();
+      while (ld_acquire_u32(&bar->gen) != gen) {
+        if (clock64() - t0 > 4000000000LL) {
+          cg->barrier_timeout = 1;
+          dead = 1;
+          break;
+        }
+      }
+    }
+    __threadfence();
+  }
+  __syncthreads();
+  return dead == 0;
+}
+
+// ---- one row of y = A r ------------------------------------------------------------
+// (A r)_i = sum_{j in N(i, re_lap), j not dummy} c_ij (r_i - r_j) + compress/dt^2 r_i,
+// c_ij = A_lap w(r_ij) / rho_ij (Listing 2; Q5, Q6).  r_j is read from
+// pos4.w, which is 0 on free-surface slots (Dirichlet p = 0).  The L lanes of the
+// group each take every L-th entry; the result is valid in every lane.
+template <bool TWO_PHASE, int L>
+__device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4, const uint32_t* tp,
+                                          const uint32_t* nbr, const uint32_t* cn, const uint32_t* co,
+                                          int i, int sub, bool live, double& ri) {
+  // every lane of the warp must come through here (full-mask shuffles below): a
+  // group without a row passes live = false and any valid i
+  const double4 pi = pos4[i];
+  ri = pi.w;
+  const uint32_t* row = row_ptr(nbr, kc.stride, i);
+  const uint32_t nf = live ? cn[i] : 0u;
+  const uint32_t m = live ? nf + co[i] : 0u;
+  const double rho_i = TWO_PHASE ? kc.rho[(tp[i] >> 8) & 1] : kc.rho[0];
+  double s = 0.0;
+#pragma unroll 2
+  for (uint32_t k = sub; k < m; k += L) {
+    const uint32_t e = row_entry(row, kc.stride, nf, k);
+    if (e & NB_DUMMY) continue;
+    const double4 q = pos4[e & NB_INDEX];
+    const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    double w = fma(kc.re_lap, rsqrt_f64(r2), -1.0);
+    if (TWO_PHASE) {
+      const double rho_j = kc.rho[(e & NB_PHASE1) ? 1 : 0];
+      const double rij =
+          kc.rho_pair_mean == 1 ? 2.0 * rho_i * rho_j / (rho_i + rho_j) : 0.5 * (rho_i + rho_j);
+      w = w / rij;
+    }
+    s = fma(w, pi.w - q.w, s);
+  }
+  s = group_sum<L>(s);
+  if (!TWO_PHASE) s *= 1.0 / kc.rho[0];
+  return fma(kc.A_lap, s, kc.compress_dt2 * pi.w);
+}
+
+// ---- the persistent solve -------------------------------------------------------------
+template <bool TWO_PHASE, int L>
+__global__ void __launch_bounds__(CG_TPB, 2)
+k_ppe_cg(KConst kc, PpeArgs a) {
+  __shared__ uint32_t sh_cnt[2][CG_TPB / 32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int nb = (int)gridDim.x, bid = (int)blockIdx.x;
+  unsigned int gen = 0;
+
+  // -- S8b-1, S8b-2: flags and right-hand side over this block's contiguous chunk --------
+  const int chunk = (kc.n + nb - 1) / nb;
+  const int lo = min(bid * chunk, kc.n), hi = min(lo + chunk, kc.n);
+  {
+    double bb = 0.0, dummy = 0.0;
+    uint32_t n_rows = 0, n_surf = 0;
+    for (int i = lo + tid; i < hi; i += CG_TPB) {
+      const uint32_t ty = a.tp[i] & 0xff;
+      int8_t f;
+      double bi = 0.0;
+      const double ni = a.dens[i];
+      if (ty == MPS_DUMMY || ty == MPS_GHOST) f = -1;
+      else if (ni < kc.beta * kc.n0_n) { f = 1; ++n_surf; }
+      else {
+        f = 0;
+        ++n_rows;
+        bi = kc.relax_dt2 * (ni - kc.n0_n) / kc.n0_n;
+      }
+      a.bc[i] = f;
+      a.b[i] = bi;
+      a.x[i] = 0.0;
+      a.pv[i] = 0.0;
+      a.sv[i] = 0.0;
+      a.pos4[i].w = bi;  // r0 = b
+      bb += bi * bi;
+    }
+    block_sum2<CG_TPB>(bb, dummy);
+    n_rows = __reduce_add_sync(0xffffffffu, n_rows);
+    n_surf = __reduce_add_sync(0xffffffffu, n_surf);
+    if (lane == 0) { sh_cnt[0][wid] = n_rows; sh_cnt[1][wid] = n_surf; }
+    __syncthreads();
+    if (tid == 0) {
+      uint32_t r = 0, s = 0;
+      for (int k = 0; k < CG_TPB / 32; ++k) { r += sh_cnt[0][k]; s += sh_cnt[1][k]; }
+      a.bcount[2 * bid] = r;
+      a.bcount[2 * bid + 1] = s;
+      a.part[2 * bid] = bb;
+      a.part[2 * bid + 1] = 0.0;
+    }
+  }
+  if (!grid_barrier(a.bar, gen, a.cg)) return;
+
+  // -- totals and this block's offset into the compacted row list ------------------------
+  double bb = 0.0;
+  int n_rows = 0, n_surf = 0, row_off = 0;
+  {
+    double v = 0.0, dummy = 0.0;
+    uint32_t r = 0, s = 0, before = 0;
+    for (int k = tid; k < nb; k += CG_TPB) {
+      v += __ldcg(&a.part[2 * k]);
+      const uint32_t rk = __ldcg(&a.bcount[2 * k]);
+      r += rk;
+      s += __ldcg(&a.bcount[2 * k + 1]);
+      if (k < bid) before += rk;
+    }
+    block_sum2<CG_TPB>(v, dummy);
+    bb = v;
+    double fr = (double)r, fs = (double)s;
+    block_sum2<CG_TPB>(fr, fs);
+    double fb = (double)before;
+    block_sum2<CG_TPB>(fb, dummy);
+    n_rows = (int)fr;
+    n_surf = (int)fs;
+    row_off = (int)fb;
+  }
+  // ordered compaction: rows[] ascending in slot index
+  for (int base = lo; base < hi; base += CG_TPB) {
+    const int i = base + tid;
+    const bool is_row = (i < hi) && (a.bc[i] == 0);
+    const uint32_t m = __ballot_sync(0xffffffffu, is_row);
+    __syncthreads();
+    if (lane == 0) sh_cnt[0][wid] = (uint32_t)__popc(m);
+    __syncthreads();
+    uint32_t off = 0, tot = 0;
+#pragma unroll
+    for (int k = 0; k < CG_TPB / 32; ++k) {
+      const uint32_t ck = sh_cnt[0][k];
+      if (k < wid) off += ck;
+      tot += ck;
+    }
+    if (is_row) a.rows[row_off + off + (uint32_t)__popc(m & ((1u << lane) - 1u))] = (uint32_t)i;
+    row_off += (int)tot;
+  }
+  if (!grid_barrier(a.bar, gen, a.cg)) return;
+
+  // -- S8b-3, S8b-4: conjugate gradients ---------------------------------------------------
+  const double tol2bb = a.tol2 * bb;
+  int iters = 0, converged = (bb == 0.0) ? 1 : 0;
+  double gam = bb, gamma_old = 1.0, alpha_old = 1.0;
+  const int gthreads = nb * CG_TPB;
+  const int gtid = bid * CG_TPB + tid;
+  const int sub = tid & (L - 1);
+  if (!converged) {
+    for (;;) {
+      // phase A: w = A r, gamma = r.r, delta = r.w
+      double g_part = 0.0, d_part = 0.0;
+      // warp-uniform trip count: g0 is the warp's first group
+      for (int g0 = (gtid & ~31) / L; g0 < n_rows; g0 += gthreads / L) {
+        const int g = g0 + (lane / L);
+        const bool live = g < n_rows;
+        const int i = live ? (int)a.rows[g] : 0;
+        double ri;
+        const double wi = ppe_row<TWO_PHASE, L>(kc, a.pos4, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+        if (live && sub == 0) {
+          a.wv[i] = wi;
+          g_part = fma(ri, ri, g_part);
+          d_part = fma(ri, wi, d_part);
+        }
+      }
+      block_sum2<CG_TPB>(g_part, d_part);
+      if (tid == 0) {
+        a.part[2 * bid] = g_part;
+        a.part[2 * bid + 1] = d_part;
+      }
+      if (!grid_barrier(a.bar, gen, a.cg)) return;
+      double del = 0.0;
+      gam = 0.0;
+      for (int k = tid; k < nb; k += CG_TPB) {
+        gam += __ldcg(&a.part[2 * k]);
+        del += __ldcg(&a.part[2 * k + 1]);
+      }
+      block_sum2<CG_TPB>(gam, del);
+      if (gam <= tol2bb) { converged = 1; break; }
+      if (iters >= a.maxit) break;
+      double alpha, beta;
+      if (iters == 0) {
         beta = 0.0;
         alpha = gam / del;
       } else {
-        beta = gam / cg->gamma_old;
-        alpha = gam / (del - beta * gam / cg->alpha_old);
+        beta = gam / gamma_old;
+        alpha = gam / (del - beta * gam / alpha_old);
       }
-      cg->alpha = alpha;
-      cg->beta = beta;
-      cg->gamma_old = gam;
-      cg->alpha_old = alpha;
-      cg->iters += 1;
+      gamma_old = gam;
+      alpha_old = alpha;
+      ++iters;
+      // phase B: p = r + beta p; s = w + beta s; x += alpha p; r -= alpha s
+      for (int g = gtid; g < n_rows; g += gthreads) {
+        const int i = (int)a.rows[g];
+        const double r = a.pos4[i].w;
+        const double pn = fma(beta, a.pv[i], r);
+        const double sn = fma(beta, a.sv[i], a.wv[i]);
+        a.pv[i] = pn;
+        a.sv[i] = sn;
+        a.x[i] = fma(alpha, pn, a.x[i]);
+        a.pos4[i].w = fma(-alpha, sn, r);
+      }
+      if (!grid_barrier(a.bar, gen, a.cg)) return;
     }
   }
-}
 
-// ------------------------------------------------------------ S8b-4: CG update ---
-// p = r + beta p; s = w + beta s; x += alpha p; r -= alpha s (rows only).
-__global__ void __launch_bounds__(256)
-k_cg_update(int n, const int8_t* __restrict__ bc, double4* __restrict__ pos4,
-            const double* __restrict__ wv, double* __restrict__ pv, double* __restrict__ sv,
-            double* __restrict__ x, const CgScalars* __restrict__ cg) {
-  if (cg->done) return;
-  const double alpha = cg->alpha, beta = cg->beta;
-  for (int i = blockIdx.x * 256 + threadIdx.x; i < n; i += gridDim.x * 256) {
-    if (bc[i] != 0) continue;
-    double r = pos4[i].w;
-    double p = r + beta * pv[i];
-    double s = wv[i] + beta * sv[i];
-    pv[i] = p;
-    sv[i] = s;
-    x[i] += alpha * p;
-    pos4[i].w = r - alpha * s;
+  // -- S8b-5: pressures from x (Q4), staged into pos4.w for the gradient ------------------
+  for (int i = gtid; i < kc.n; i += gthreads) {
+    double v = (a.bc[i] == 0) ? a.x[i] : 0.0;
+    if (kc.clamp_negative_p && v < 0.0) v = 0.0;
+    a.p[i] = v;
+    a.pos4[i].w = v;
+  }
+  if (bid == 0 && tid == 0) {
+    a.cg->gamma = gam;
+    a.cg->bb = bb;
+    a.cg->tol2bb = tol2bb;
+    a.cg->iters = iters;
+    a.cg->maxit = a.maxit;
+    a.cg->done = 1;
+    a.cg->converged = converged;
+    a.cg->n_rows = n_rows;
+    a.cg->n_surface = n_surf;
   }
 }
 
-// ---------------------------------------------------- S8b-5: pressures from x ---
-__global__ void k_ppe_finish(KConst kc, const int8_t* __restrict__ bc, const double* __restrict__ x,
-                             double* __restrict__ p) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= kc.n) return;
-  double v = (bc[i] == 0) ? x[i] : 0.0;
-  if (kc.clamp_negative_p && v < 0.0) v = 0.0;
-  p[i] = v;
-}
-
-// stage a caller vector into pos4.w (rows only) / read a vector back
+// ---- y = A x for the tests (mps_ppe_apply): stage, apply, read back ---------------------
 __global__ void k_stage_in(int n, int order, const int8_t* __restrict__ bc, const uint32_t* __restrict__ oid,
                            const double* __restrict__ src, double4* __restrict__ pos4) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double v = src[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i];
   pos4[i].w = (bc[i] == 0) ? v : 0.0;
+}
+template <bool TWO_PHASE, int L>
+__global__ void __launch_bounds__(256)
+k_ppe_apply(KConst kc, const double4* pos4, const uint32_t* __restrict__ tp, const int8_t* __restrict__ bc,
+            const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn,
+            const uint32_t* __restrict__ co, double* __restrict__ wv) {
+  const int i = (int)((blockIdx.x * 256u + threadIdx.x) / L);
+  const int sub = threadIdx.x & (L - 1);
+  const bool in = i < kc.n;
+  const bool live = in && bc[i] == 0;
+  double ri;
+  const double wi = ppe_row<TWO_PHASE, L>(kc, pos4, tp, nbr, cn, co, in ? i : 0, sub, live, ri);
+  if (in && sub == 0) wv[i] = live ? wi : 0.0;
 }
 __global__ void k_stage_out(int n, int order, const uint32_t* __restrict__ oid,
                             const double* __restrict__ src, double* __restrict__ dst) {
@@ -237,66 +346,81 @@ __global__ void k_stage_out(int n, int order, const uint32_t* __restrict__ oid,
   dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = src[i];
 }
 
-int spmv_grid(mps_ctx* c) {
-  int need = div_up(c->n, TPB);
-  int cap = c->sm_count * 8;
-  return need < cap ? need : cap;
+template <bool TWO_PHASE, int L>
+cudaError_t launch_cg(mps_ctx* c, PpeArgs& a, int grid) {
+  void* params[] = {(void*)&c->kc, (void*)&a};
+  return cudaLaunchCooperativeKernel((const void*)k_ppe_cg<TWO_PHASE, L>, dim3(grid), dim3(CG_TPB),
+                                     params, 0, c->stream);
+}
+template <bool TWO_PHASE, int L>
+int cg_blocks_per_sm() {
+  int nb = 0;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_ppe_cg<TWO_PHASE, L>, CG_TPB, 0);
+  return nb;
 }
 
-template <bool REDUCE>
-void launch_spmv(mps_ctx* c, int cat) {
-  int cur = c->cur;
-  int grid = spmv_grid(c);
-  if (c->prm.n_phases > 1 && c->prm.rho[0] != c->prm.rho[1]) {
-    MPS_LAUNCH(c, cat, (k_cg_spmv<true, REDUCE>), grid, TPB, c->kc, c->pos4[cur], c->tp[cur], c->bc,
-               c->nbr, c->cn, c->co, c->cg_w, c->cg_part, c->cg);
-  } else {
-    MPS_LAUNCH(c, cat, (k_cg_spmv<false, REDUCE>), grid, TPB, c->kc, c->pos4[cur], c->tp[cur], c->bc,
-               c->nbr, c->cn, c->co, c->cg_w, c->cg_part, c->cg);
-  }
-}
+bool two_phase(const mps_ctx* c) { return c->prm.n_phases > 1 && c->prm.rho[0] != c->prm.rho[1]; }
 
 }  // namespace
 
 // ============================================================ host launchers ===
-int mpsk_pressure_ppe(mps_ctx* c) {
-  const int n = (int)c->n;
-  const int cur = c->cur;
-  const int grid = spmv_grid(c);
-  const double tol2 = c->prm.cg_rtol * c->prm.cg_rtol;
-  MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_ppe_setup, grid, TPB, c->kc, tol2, c->prm.cg_maxit, c->pos4[cur],
-             c->tp[cur], c->dens, c->bc, c->b, c->cg_x, c->cg_p, c->cg_s, c->cg_part, c->cg);
-  c->ppe_ready = true;
-  const int POLL = 8;
-  const int ugrid = std::min(div_up(n, 256), c->sm_count * 8);
-  int batches = 0;
-  bool done = false;
-  // pipelined polling: batch k is enqueued before the host looks at batch k-1
-  while (!done) {
-    for (int it = 0; it < POLL; ++it) {
-      launch_spmv<true>(c, MPS_T_CG_SPMV);
-      MPS_LAUNCH(c, MPS_T_CG_UPDATE, k_cg_update, ugrid, 256, n, c->bc, c->pos4[cur], c->cg_w, c->cg_p,
-                 c->cg_s, c->cg_x, c->cg);
-    }
-    if (batches > 0) {
-      cudaEventSynchronize(c->poll_event);
-      if (c->cg_host->done) done = true;
-    }
-    if (!done) {
-      cudaMemcpyAsync(c->cg_host, c->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream);
-      cudaEventRecord(c->poll_event, c->stream);
-    }
-    ++batches;
-    if ((int64_t)batches * POLL > (int64_t)c->prm.cg_maxit + 4 * POLL) break;  // safety net
+// Number of co-resident blocks of the persistent kernel (called once at init).
+int mpsk_ppe_plan(mps_ctx* c) {
+  int per_sm = 2;
+  const bool tp = two_phase(c);
+  switch (c->cg_lanes) {
+    case 4: per_sm = tp ? cg_blocks_per_sm<true, 4>() : cg_blocks_per_sm<false, 4>(); break;
+    case 16: per_sm = tp ? cg_blocks_per_sm<true, 16>() : cg_blocks_per_sm<false, 16>(); break;
+    default: c->cg_lanes = 8; per_sm = tp ? cg_blocks_per_sm<true, 8>() : cg_blocks_per_sm<false, 8>(); break;
   }
-  MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_ppe_finish, div_up(n, 256), 256, c->kc, c->bc, c->cg_x, c->p);
+  if (per_sm < 1) return MPS_ERR_CUDA;
+  if (per_sm > 2) per_sm = 2;
+  c->cg_grid = per_sm * c->sm_count;
+  return MPS_OK;
+}
+
+int mpsk_pressure_ppe(mps_ctx* c) {
+  const int cur = c->cur;
+  PpeArgs a;
+  a.pos4 = c->pos4[cur]; a.tp = c->tp[cur]; a.dens = c->dens; a.bc = c->bc; a.b = c->b;
+  a.x = c->cg_x; a.pv = c->cg_p; a.sv = c->cg_s; a.wv = c->cg_w; a.p = c->p;
+  a.nbr = c->nbr; a.cn = c->cn; a.co = c->co; a.rows = c->cg_rows; a.bcount = c->cg_bcount;
+  a.part = c->cg_part; a.cg = c->cg; a.bar = c->cg_bar;
+  a.tol2 = c->prm.cg_rtol * c->prm.cg_rtol;
+  a.maxit = c->prm.cg_maxit;
+  // small problems: no more blocks than there is work for (fewer arrivals per barrier)
+  int grid = c->cg_grid;
+  const int want = std::max(c->sm_count, div_up((int64_t)c->n * c->cg_lanes, CG_TPB));
+  if (grid > want) grid = want;
+  cudaMemsetAsync(c->cg_bar, 0, sizeof(GridBar), c->stream);
+  if (((c)->timer_mask >> MPS_T_CG_SPMV) & 1u) mps_timer_begin(c, MPS_T_CG_SPMV);
+  cudaError_t e;
+  const bool tp = two_phase(c);
+  switch (c->cg_lanes) {
+    case 4: e = tp ? launch_cg<true, 4>(c, a, grid) : launch_cg<false, 4>(c, a, grid); break;
+    case 16: e = tp ? launch_cg<true, 16>(c, a, grid) : launch_cg<false, 16>(c, a, grid); break;
+    default: e = tp ? launch_cg<true, 8>(c, a, grid) : launch_cg<false, 8>(c, a, grid); break;
+  }
+  c->launches++;
+  c->t_launches[MPS_T_CG_SPMV]++;
+  if (((c)->timer_mask >> MPS_T_CG_SPMV) & 1u) mps_timer_end(c, MPS_T_CG_SPMV);
+  if (e != cudaSuccess) {
+    c->err = std::string("cooperative launch of k_ppe_cg failed: ") + cudaGetErrorString(e);
+    return MPS_ERR_CUDA;
+  }
+  c->ppe_ready = true;
+  c->posw_is_p = true;
   cudaMemcpyAsync(c->cg_host, c->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream);
-  cudaError_t e = cudaStreamSynchronize(c->stream);
+  e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) {
     c->err = std::string("CUDA error in mps_pressure_ppe: ") + cudaGetErrorString(e);
     return MPS_ERR_CUDA;
   }
   const CgScalars& s = *c->cg_host;
+  if (s.barrier_timeout) {
+    c->err = "grid barrier timed out inside k_ppe_cg";
+    return MPS_ERR_CUDA;
+  }
   c->stats.cg_iters = s.iters;
   c->stats.cg_converged = s.converged;
   c->stats.cg_relres = s.bb > 0.0 ? sqrt(s.gamma / s.bb) : 0.0;
@@ -315,7 +439,15 @@ int mpsk_ppe_apply(mps_ctx* c, const double* x, double* y, int order) {
   const int cur = c->cur;
   MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_stage_in, div_up(n, 256), 256, n, order, c->bc, c->oid[cur], x,
              c->pos4[cur]);
-  launch_spmv<false>(c, MPS_T_PPE_SETUP);
+  c->posw_is_p = false;
+  const int grid = div_up((int64_t)n * 8, 256);
+  if (two_phase(c)) {
+    MPS_LAUNCH(c, MPS_T_PPE_SETUP, (k_ppe_apply<true, 8>), grid, 256, c->kc, c->pos4[cur], c->tp[cur],
+               c->bc, c->nbr, c->cn, c->co, c->cg_w);
+  } else {
+    MPS_LAUNCH(c, MPS_T_PPE_SETUP, (k_ppe_apply<false, 8>), grid, 256, c->kc, c->pos4[cur], c->tp[cur],
+               c->bc, c->nbr, c->cn, c->co, c->cg_w);
+  }
   MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_stage_out, div_up(n, 256), 256, n, order, c->oid[cur], c->cg_w, y);
   return MPS_OK;
 }

@@ -1,6 +1,7 @@
 // mps_api.cu -- the extern "C" boundary of libmps_b200.so (include/mps_b200.h).
 // Host logic only: argument checks, buffer ownership, stage ordering, timers.
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -63,6 +64,7 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
   cudaFree(c->phat); cudaFree(c->grad4); cudaFree(c->bc);
   cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
+  cudaFree(c->cg_rows); cudaFree(c->cg_bcount); cudaFree(c->cg_bar);
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
   if (c->cg_host) cudaFreeHost(c->cg_host);
   if (c->flags_host) cudaFreeHost(c->flags_host);
@@ -72,7 +74,7 @@ static void free_all(mps_ctx* c) {
 
 static int check_params(const mps_params* p, int64_t n) {
   if (!p) return fail(nullptr, MPS_ERR_ARG, "params is NULL");
-  if (n <= 0 || n > (int64_t)NB_INDEX) return fail(nullptr, MPS_ERR_ARG, "n must be in [1, 2^30)");
+  if (n <= 0 || n > (int64_t)NB_INDEX) return fail(nullptr, MPS_ERR_ARG, "n must be in [1, 2^29)");
   if (p->dim != 3) return fail(nullptr, MPS_ERR_ARG, "only dim = 3 is supported");
   if (!(p->l0 > 0) || !(p->re_n > 0) || !(p->re_lap > 0) || !(p->dt > 0))
     return fail(nullptr, MPS_ERR_ARG, "l0, re_n, re_lap and dt must be positive");
@@ -150,6 +152,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.nx = nc[0]; k.ny = nc[1]; k.nz = nc[2]; k.ncells = (int)ncells;
   k.R_lap = (int)ceil(prm->re_lap * k.inv_h);
   k.cap = prm->max_neighbours;
+  k.stride = (k.cap + 7) / 8 * 8;
   k.grad_variant = prm->grad_variant; k.clamp_negative_p = prm->clamp_negative_p;
   k.rho_pair_mean = prm->rho_pair_mean; k.nu_pair_mean = prm->nu_pair_mean;
   k.n = (int)n;
@@ -165,11 +168,13 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->tmp_src, N + 1)); A(dalloc(&c->tmp_oid, N));
   A(dalloc(&c->cell_count, (size_t)ncells + 2)); A(dalloc(&c->cell_start, (size_t)ncells + 2));
   A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
-  A(dalloc(&c->nbr, N * (size_t)k.cap)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
+  A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
   A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
   A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->grad4, N)); A(dalloc(&c->bc, N));
   A(dalloc(&c->cg_x, N)); A(dalloc(&c->cg_p, N)); A(dalloc(&c->cg_s, N)); A(dalloc(&c->cg_w, N));
   A(dalloc(&c->cg_part, (size_t)2 * (c->sm_count * 8 + 8)));
+  A(dalloc(&c->cg_rows, N)); A(dalloc(&c->cg_bcount, (size_t)2 * (c->sm_count * 8 + 8)));
+  A(dalloc(&c->cg_bar, 1));
   A(dalloc(&c->cg, 1)); A(dalloc(&c->flags, 1)); A(dalloc(&c->io_tmp, N));
   A(cudaMallocHost((void**)&c->cg_host, sizeof(CgScalars)));
   A(cudaMallocHost((void**)&c->flags_host, sizeof(DevFlags)));
@@ -180,10 +185,23 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     delete c;
     return MPS_ERR_CUDA;
   }
+  {
+    // lanes per row of the CG operator: 8 by default; MPS_B200_CG_LANES = 4 | 8 | 16 for tuning
+    const char* ev = getenv("MPS_B200_CG_LANES");
+    c->cg_lanes = ev ? atoi(ev) : 8;
+    if (mpsk_ppe_plan(c) != MPS_OK) {
+      g_init_error = "k_ppe_cg cannot be made resident on this device";
+      free_all(c);
+      delete c;
+      return MPS_ERR_CUDA;
+    }
+  }
   memset(c->cg_host, 0, sizeof(CgScalars));
   memset(c->flags_host, 0, sizeof(DevFlags));
   cudaStream_t s = c->stream;
   cudaMemsetAsync(c->cg, 0, sizeof(CgScalars), s);
+  cudaMemsetAsync(c->cg_bar, 0, sizeof(GridBar), s);
+  cudaMemsetAsync(c->cg_rows, 0, N * 4, s);
   cudaMemsetAsync(c->flags, 0, sizeof(DevFlags), s);
   double* zero_d[] = {c->dens, c->p, c->nut, c->b, c->phat, c->cg_x, c->cg_p, c->cg_s, c->cg_w};
   for (double* z : zero_d) cudaMemsetAsync(z, 0, N * sizeof(double), s);

@@ -15,14 +15,18 @@
 // vel4[i] = (u, v, w, nu_eff): nu_eff < 0 marks WALL/DUMMY (u = 0, nu_ij = nu_i).
 // tp[i]   = type | phase << 8.
 // oid[i]  = caller's original index of slot i (= perm).
-// nbr     = neighbour rows, warp-interleaved ELL: entry k of slot i lives at
-//           ((i >> 5) * cap + k) * 32 + (i & 31).  Entries with r < re_n fill
-//           the row from the front (count cn[i]); entries with re_n <= r < re_lap
-//           fill it from the back (count co[i]).  Entry = slot index of j
-//           | NB_DUMMY if j is a dummy | NB_PHASE1 if j is of phase 1.
+// nbr     = neighbour rows, row-major ELL: row of slot i starts at nbr + i * stride
+//           (stride = max_neighbours rounded up to a multiple of 8, so every row
+//           starts on a 32-byte sector).  Entries with r < re_n fill the row from
+//           the front (count cn[i], ascending slot order); entries with
+//           re_n <= r < re_lap fill it from the back (count co[i]).  The L lanes
+//           that share a row read L consecutive entries.  Entry = slot index of j
+//           | NB_DUMMY if j is a dummy | NB_PHASE1 if j is of phase 1 | NB_WALL if
+//           j is a wall particle.
 #define NB_DUMMY 0x80000000u
 #define NB_PHASE1 0x40000000u
-#define NB_INDEX 0x3fffffffu
+#define NB_WALL 0x20000000u
+#define NB_INDEX 0x1fffffffu
 
 struct CgScalars {
   double gamma, delta;          // r.r and r.Ar of the current iteration
@@ -32,6 +36,13 @@ struct CgScalars {
   int iters, done, converged, maxit;
   unsigned int blocks_done, pad;
   int n_surface, n_rows;
+  int barrier_timeout, pad2;
+};
+
+// Grid-wide barrier state of the persistent CG kernel (zeroed at init).
+struct GridBar {
+  unsigned int count;
+  unsigned int gen;
 };
 
 struct DevFlags {
@@ -52,6 +63,7 @@ struct KConst {  // by-value kernel parameter
   int nx, ny, nz, ncells;
   int R_lap;  // cells to each side for re_lap
   int cap;    // row capacity (max_neighbours)
+  int stride; // row stride in entries (cap rounded up to a multiple of 8)
   int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean;
   int n;      // particles
 };
@@ -97,6 +109,12 @@ struct mps_ctx {
   double* cg_s = nullptr;
   double* cg_w = nullptr;
   double* cg_part = nullptr;  // per-block partial sums
+  uint32_t* cg_rows = nullptr;   // compacted slot indices of the PPE unknowns (bc == 0)
+  uint32_t* cg_bcount = nullptr; // per-block row / surface counts of the setup phase
+  GridBar* cg_bar = nullptr;
+  int cg_grid = 0;               // co-resident blocks of the persistent CG kernel
+  int cg_lanes = 8;              // lanes per row of the operator (power of two)
+  bool posw_is_p = false;        // pos4.w currently holds the pressure
   CgScalars* cg = nullptr;    // device
   CgScalars* cg_host = nullptr;  // pinned
   DevFlags* flags = nullptr;
@@ -144,6 +162,7 @@ int mpsk_density(mps_ctx* c);
 int mpsk_viscosity(mps_ctx* c);
 int mpsk_predict(mps_ctx* c);
 int mpsk_pressure_explicit(mps_ctx* c);
+int mpsk_ppe_plan(mps_ctx* c);           // co-resident grid of the persistent CG kernel
 int mpsk_pressure_ppe(mps_ctx* c);
 int mpsk_ppe_apply(mps_ctx* c, const double* x, double* y, int order);
 int mpsk_gradient(mps_ctx* c);

@@ -1,0 +1,56 @@
+// sweep_common.cuh -- device helpers shared by the list-driven sweeps.
+// Not part of the ABI.  Shares nothing with oracle/.
+#pragma once
+#include "mps_internal.h"
+
+// ---- neighbour rows (row-major ELL, see mps_internal.h) ---------------------------
+__device__ __forceinline__ const uint32_t* row_ptr(const uint32_t* nbr, int stride, int i) {
+  return nbr + (size_t)i * (size_t)stride;
+}
+// Entry k of a row with nf front entries: the re_n part grows from the front,
+// the re_n <= r < re_lap part from the back.
+__device__ __forceinline__ uint32_t row_entry(const uint32_t* row, int stride, uint32_t nf, uint32_t k) {
+  return k < nf ? row[k] : row[stride - 1 - (k - nf)];
+}
+
+// ---- 1/sqrt(x) in fp64: hardware seed (about 2^-22) plus one cubically convergent
+// correction y (1 + e/2 + 3e^2/8), e = 1 - x y^2: five fp64 operations, error a
+// few 1e-16 relative.  x must be positive, finite and normal (r^2 of two distinct
+// particles).  No bit-exact quantity depends on it (reading Q2).
+__device__ __forceinline__ double rsqrt_f64(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = x * y;
+  double e = fma(-t, y, 1.0);
+  double q = fma(e, 0.375, 0.5);
+  double c = q * e;
+  return fma(y, c, y);
+}
+
+// ---- 32-byte particle record loads -------------------------------------------------
+// Coherent (ld.global, L1-cached, invalidated by a gpu-scope fence): used inside the
+// persistent CG kernel where pos4.w changes between phases.
+__device__ __forceinline__ double4 ld_pos4(const double4* p) {
+  double4 v;
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%4];\n\t"
+               "ld.global.v2.f64 {%2, %3}, [%4+16];"
+               : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w)
+               : "l"(p)
+               : "memory");
+  return v;
+}
+
+// ---- reductions over the L lanes that share a row (L a power of two <= 32) -----------
+template <int L>
+__device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+  for (int o = L / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+template <int L>
+__device__ __forceinline__ double group_min(double v) {
+#pragma unroll
+  for (int o = L / 2; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ double warp_sum(double v) { return group_sum<32>(v); }
