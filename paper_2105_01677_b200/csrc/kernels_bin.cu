@@ -162,7 +162,8 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
                           const uint32_t* __restrict__ tmp_oid, const double4* __restrict__ pos_in,
                           const double4* __restrict__ vel_in, const uint32_t* __restrict__ tp_in,
                           double4* __restrict__ pos_out, double4* __restrict__ vel_out,
-                          uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out) {
+                          uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out,
+                          uint32_t* __restrict__ ent_out) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   uint32_t c = key[s];
@@ -176,8 +177,13 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
   q.w = 0.0;
   pos_out[f] = q;
   vel_out[f] = vel_in[src];
-  tp_out[f] = tp_in[src];
+  const uint32_t tj = tp_in[src];
+  const uint32_t ty = tj & 0xff;
+  tp_out[f] = tj;
   oid_out[f] = me;
+  // the neighbour-row entry that names this particle (flags of mps_internal.h)
+  ent_out[f] = f | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
+               ((tj & 0x100) ? NB_PHASE1 : 0u);
 }
 
 // ------------------------------------------------ S3: neighbour rows (the sweep) ---
@@ -192,7 +198,7 @@ constexpr int ROWS_TPB = 256;
 constexpr int ROWS_PPW = 4;  // particles per warp (consecutive slots: same candidate cells)
 
 __global__ void __launch_bounds__(ROWS_TPB)
-k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
+k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
              const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
              uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
              DevFlags* __restrict__ flags) {
@@ -251,7 +257,7 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
           const uint32_t add_n = (uint32_t)__popc(m_n), add_o = (uint32_t)__popc(m_o);
           if (nf + nb + add_n + add_o <= cap) {
             if (in_n) row[nf + (uint32_t)__popc(m_n & lt_mask)] = e;
-            else if (in_lap) row[(uint32_t)kc.stride - 1u - (nb + (uint32_t)__popc(m_o & lt_mask))] = e;
+            else if (in_lap) row[back_slot(kc.stride, nb + (uint32_t)__popc(m_o & lt_mask))] = e;
             nf += add_n;
             nb += add_o;
           } else {
@@ -263,7 +269,7 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
             const uint32_t took_n = add_n < room ? add_n : room;
             const uint32_t room_o = room - took_n;
             const uint32_t po = (uint32_t)__popc(m_o & lt_mask);
-            if (in_lap && !in_n && po < room_o) row[(uint32_t)kc.stride - 1u - (nb + po)] = e;
+            if (in_lap && !in_n && po < room_o) row[back_slot(kc.stride, nb + po)] = e;
             nf += took_n;
             nb += add_o < room_o ? add_o : room_o;
           }
@@ -274,6 +280,145 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
     warp_max = max(warp_max, (int)(nf + nb));
   }
   coincident = __any_sync(0xffffffffu, coincident);
+  if (lane == 0) {
+    if (overflow) flags->overflow = 1;
+    if (coincident) flags->nonfinite = 1;
+    if (warp_max > 0) atomicMax(&flags->max_row, warp_max);
+  }
+}
+
+// ------------------------------------ S3, cell_div = 1: one warp per cell ---
+// The 32 lanes hold up to 32 particles i of one cell and walk the candidates j of
+// the (2R+1)^2 cell runs in lock-step, so every candidate is ONE broadcast load
+// for the whole warp (no gathers) and the exact test costs 8 fp64 operations per
+// lane.  Hits are collected per lane in a shared-memory buffer of 8 entries and
+// written as whole 32-byte sectors (two 128-bit stores), front part upwards, back
+// part downwards (back_slot).  Entries come out in ascending slot order, as above.
+constexpr int CELL_TPB = 256;
+constexpr int CELL_WARPS = CELL_TPB / 32;
+constexpr int CELL_BATCH = 8;  // candidates tested per lane before the hits are appended
+
+__device__ __forceinline__ void flush_sector(uint32_t* dst, const uint32_t (*b)[32], int lane) {
+  uint4 lo = make_uint4(b[0][lane], b[1][lane], b[2][lane], b[3][lane]);
+  uint4 hi = make_uint4(b[4][lane], b[5][lane], b[6][lane], b[7][lane]);
+  reinterpret_cast<uint4*>(dst)[0] = lo;
+  reinterpret_cast<uint4*>(dst)[1] = hi;
+}
+
+__global__ void __launch_bounds__(CELL_TPB, 4)
+k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
+                  const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
+                  uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags) {
+  __shared__ uint32_t buf[2][CELL_WARPS][8][32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int gwarp = blockIdx.x * CELL_WARPS + wid;
+  const int nwarps = gridDim.x * CELL_WARPS;
+  uint32_t (*bn)[32] = buf[0][wid];
+  uint32_t (*bo)[32] = buf[1][wid];
+  // ghosts sit behind the last cell and have no neighbours
+  for (uint32_t i = cell_start[kc.ncells] + (uint32_t)(gwarp * 32 + lane); i < (uint32_t)kc.n;
+       i += (uint32_t)nwarps * 32u) {
+    cn[i] = 0;
+    co[i] = 0;
+  }
+  const int R = kc.R_lap, S = kc.stride;
+  const uint32_t cap = (uint32_t)kc.cap;
+  int lane_max = 0;
+  int coincident = 0, overflow = 0;
+  for (int c = gwarp; c < kc.ncells; c += nwarps) {
+    const uint32_t ps = cell_start[c], pe = cell_start[c + 1];
+    if (ps == pe) continue;
+    const int cx = c % kc.nx, cy = (c / kc.nx) % kc.ny, cz = c / (kc.nx * kc.ny);
+    const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
+    for (uint32_t base = ps; base < pe; base += 32) {
+      const uint32_t i = base + (uint32_t)lane;
+      const bool act = i < pe;
+      const uint32_t ii = act ? i : ps;
+      const double4 pi = pos4[ii];
+      uint32_t* row = nbr + (size_t)ii * (size_t)S;
+      uint32_t nf = 0, nb = 0;
+      for (int dz = -R; dz <= R; ++dz) {
+        const int z2 = cz + dz;
+        if (z2 < 0 || z2 >= kc.nz) continue;
+        for (int dy = -R; dy <= R; ++dy) {
+          const int y2 = cy + dy;
+          if (y2 < 0 || y2 >= kc.ny) continue;
+          const int cbase = kc.nx * (y2 + kc.ny * z2);
+          const uint32_t js = cell_start[cbase + x_lo];
+          const uint32_t je = cell_start[cbase + x_hi + 1];
+          for (uint32_t j0 = js; j0 < je; j0 += 32) {
+            // phase 1: up to 32 independent exact tests per lane; every load is a warp-uniform
+            // broadcast.  Slots past je (at most 31, inside the padded arrays) are masked off.
+            const uint32_t cnt = min(32u, je - j0);
+            uint32_t m_lap = 0, m_n = 0;
+            const double4* qp = pos4 + j0;
+            for (uint32_t g = 0; g < cnt; g += CELL_BATCH, qp += CELL_BATCH) {
+              uint32_t b_lap = 0, b_n = 0;
+#pragma unroll
+              for (int t = 0; t < CELL_BATCH; ++t) {
+                const double4 q = qp[t];
+                const double dx = __dsub_rn(q.x, pi.x), dy_ = __dsub_rn(q.y, pi.y), dz_ = __dsub_rn(q.z, pi.z);
+                const double r2 =
+                    __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
+                if (r2 < kc.re_lap2) b_lap |= 1u << t;
+                if (r2 < kc.re_n2) b_n |= 1u << t;
+              }
+              m_lap |= b_lap << g;
+              m_n |= b_n << g;
+            }
+            uint32_t keep = cnt == 32u ? 0xffffffffu : ((1u << cnt) - 1u);
+            if (i - j0 < 32u) keep &= ~(1u << (i - j0));  // j == i
+            m_lap = act ? (m_lap & keep) : 0u;
+            // capacity: keep the first hits that fit (ascending j), flag the rest
+            if (nf + nb + (uint32_t)__popc(m_lap) > cap) {
+              overflow = 1;
+              while (nf + nb + (uint32_t)__popc(m_lap) > cap) m_lap &= ~(0x80000000u >> __clz((int)m_lap));
+            }
+            m_n &= m_lap;
+            uint32_t m_o = m_lap & ~m_n;
+            // the chunk's row entries, one per lane
+            const uint32_t eb = ent[j0 + (uint32_t)lane];
+            // phase 2: every lane appends its hits in ascending j (warp-convergent loops)
+            while (__any_sync(0xffffffffu, m_n != 0u)) {
+              const int bit = __ffs((int)m_n) - 1;
+              const uint32_t e = __shfl_sync(0xffffffffu, eb, bit & 31);
+              if (m_n) {
+                m_n &= m_n - 1u;
+                bn[nf & 7u][lane] = e;
+                ++nf;
+                if ((nf & 7u) == 0u) flush_sector(row + (nf - 8u), bn, lane);
+              }
+            }
+            while (__any_sync(0xffffffffu, m_o != 0u)) {
+              const int bit = __ffs((int)m_o) - 1;
+              const uint32_t e = __shfl_sync(0xffffffffu, eb, bit & 31);
+              if (m_o) {
+                m_o &= m_o - 1u;
+                bo[nb & 7u][lane] = e;
+                ++nb;
+                if ((nb & 7u) == 0u) flush_sector(row + ((uint32_t)S - nb), bo, lane);
+              }
+            }
+          }
+        }
+      }
+      // coincident particles (r = 0 makes Eq. 3 infinite) can only be cell mates
+      for (uint32_t j = ps; j < pe; ++j) {
+        const double4 q = pos4[j];
+        if (act && j != i && q.x == pi.x && q.y == pi.y && q.z == pi.z) coincident = 1;
+      }
+      if (act) {
+        if (nf & 7u) flush_sector(row + (nf & ~7u), bn, lane);
+        if (nb & 7u) flush_sector(row + ((uint32_t)S - 8u * (nb / 8u + 1u)), bo, lane);
+        cn[i] = nf;
+        co[i] = nb;
+        lane_max = max(lane_max, (int)(nf + nb));
+      }
+    }
+  }
+  coincident = __any_sync(0xffffffffu, coincident != 0);
+  overflow = __any_sync(0xffffffffu, overflow != 0);
+  const int warp_max = __reduce_max_sync(0xffffffffu, lane_max);
   if (lane == 0) {
     if (overflow) flags->overflow = 1;
     if (coincident) flags->nonfinite = 1;
@@ -382,7 +527,7 @@ __global__ void k_nb_fill(int n, int cap_row, int radius_id, const uint32_t* __r
   if (base + m > cap) return;  // caller's buffer too small for this row: skip it
   // insertion sort by original index while writing
   for (uint32_t k = 0; k < m; ++k) {
-    uint32_t e = (k < nf) ? row[k] : row[cap_row - 1 - (k - nf)];
+    uint32_t e = (k < nf) ? row[k] : row[back_slot(cap_row, k - nf)];
     uint32_t v = oid[e & NB_INDEX];
     int64_t t = base + k;
     while (t > base && idx[t - 1] > v) { idx[t] = idx[t - 1]; --t; }
@@ -423,11 +568,17 @@ int mpsk_bin(mps_ctx* c) {
              c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key);
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_reorder, div_up(n, TPB), TPB, n, nc, c->key, c->cell_start,
              c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
-             c->vel4[nxt], c->tp[nxt], c->oid[nxt]);
+             c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent);
   c->cur = nxt;
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
-  MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc, c->pos4[nxt], c->tp[nxt],
-             c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags);
+  if (c->prm.cell_div == 1 && !c->rows_by_warp) {
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, c->kc, c->pos4[nxt],
+               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags);
+  } else {
+    // small cells hold only a few particles each: one warp per particle, lanes on candidates
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc,
+               c->pos4[nxt], c->tp[nxt], c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags);
+  }
   c->binned = true;
   c->ppe_ready = false;
   c->posw_is_p = false;

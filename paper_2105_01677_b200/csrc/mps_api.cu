@@ -58,7 +58,7 @@ static void free_all(mps_ctx* c) {
   for (int k = 0; k < 2; ++k) {
     cudaFree(c->pos4[k]); cudaFree(c->vel4[k]); cudaFree(c->tp[k]); cudaFree(c->oid[k]);
   }
-  cudaFree(c->key); cudaFree(c->key_tmp); cudaFree(c->rank); cudaFree(c->tmp_src);
+  cudaFree(c->ent); cudaFree(c->key); cudaFree(c->key_tmp); cudaFree(c->rank); cudaFree(c->tmp_src);
   cudaFree(c->tmp_oid); cudaFree(c->cell_count); cudaFree(c->cell_start); cudaFree(c->scan_tmp);
   cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co);
   cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
@@ -152,7 +152,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.nx = nc[0]; k.ny = nc[1]; k.nz = nc[2]; k.ncells = (int)ncells;
   k.R_lap = (int)ceil(prm->re_lap * k.inv_h);
   k.cap = prm->max_neighbours;
-  k.stride = (k.cap + 7) / 8 * 8;
+  k.stride = (k.cap + 14 + 7) / 8 * 8;
   k.grad_variant = prm->grad_variant; k.clamp_negative_p = prm->clamp_negative_p;
   k.rho_pair_mean = prm->rho_pair_mean; k.nu_pair_mean = prm->nu_pair_mean;
   k.n = (int)n;
@@ -162,9 +162,9 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
   const size_t N = (size_t)c->n_pad;
   for (int b = 0; b < 2; ++b) {
-    A(dalloc(&c->pos4[b], N)); A(dalloc(&c->vel4[b], N)); A(dalloc(&c->tp[b], N)); A(dalloc(&c->oid[b], N));
+    A(dalloc(&c->pos4[b], N + 32)); A(dalloc(&c->vel4[b], N)); A(dalloc(&c->tp[b], N)); A(dalloc(&c->oid[b], N));
   }
-  A(dalloc(&c->key, N)); A(dalloc(&c->key_tmp, N)); A(dalloc(&c->rank, N));
+  A(dalloc(&c->ent, N + 32)); A(dalloc(&c->key, N)); A(dalloc(&c->key_tmp, N)); A(dalloc(&c->rank, N));
   A(dalloc(&c->tmp_src, N + 1)); A(dalloc(&c->tmp_oid, N));
   A(dalloc(&c->cell_count, (size_t)ncells + 2)); A(dalloc(&c->cell_start, (size_t)ncells + 2));
   A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
@@ -187,6 +187,8 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   }
   {
     // lanes per row of the CG operator: 8 by default; MPS_B200_CG_LANES = 4 | 8 | 16 for tuning
+    const char* rw = getenv("MPS_B200_ROWS");
+    c->rows_by_warp = rw && !strcmp(rw, "warp");
     const char* ev = getenv("MPS_B200_CG_LANES");
     c->cg_lanes = ev ? atoi(ev) : 8;
     if (mpsk_ppe_plan(c) != MPS_OK) {
@@ -211,8 +213,9 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   cudaMemsetAsync(c->cn, 0, N * 4, s);
   cudaMemsetAsync(c->co, 0, N * 4, s);
   cudaMemsetAsync(c->key, 0, N * 4, s);
+  cudaMemsetAsync(c->ent, 0, (N + 32) * 4, s);
   for (int b = 0; b < 2; ++b) {
-    cudaMemsetAsync(c->pos4[b], 0, N * sizeof(double4), s);
+    cudaMemsetAsync(c->pos4[b], 0, (N + 32) * sizeof(double4), s);
     cudaMemsetAsync(c->vel4[b], 0, N * sizeof(double4), s);
     cudaMemsetAsync(c->tp[b], 0, N * 4, s);
     cudaMemsetAsync(c->oid[b], 0, N * 4, s);

@@ -16,17 +16,23 @@
 // tp[i]   = type | phase << 8.
 // oid[i]  = caller's original index of slot i (= perm).
 // nbr     = neighbour rows, row-major ELL: row of slot i starts at nbr + i * stride
-//           (stride = max_neighbours rounded up to a multiple of 8, so every row
-//           starts on a 32-byte sector).  Entries with r < re_n fill the row from
-//           the front (count cn[i], ascending slot order); entries with
-//           re_n <= r < re_lap fill it from the back (count co[i]).  The L lanes
-//           that share a row read L consecutive entries.  Entry = slot index of j
+//           (stride = max_neighbours + 14 rounded up to a multiple of 8, so every
+//           row starts on a 32-byte sector and the two parts never share one).
+//           Entries with r < re_n fill the row from the front (count cn[i],
+//           ascending slot order); entries with re_n <= r < re_lap fill it from the
+//           back in whole sectors (count co[i], see back_slot).  The L lanes that
+//           share a row read L consecutive entries.  Entry = slot index of j
 //           | NB_DUMMY if j is a dummy | NB_PHASE1 if j is of phase 1 | NB_WALL if
 //           j is a wall particle.
 #define NB_DUMMY 0x80000000u
 #define NB_PHASE1 0x40000000u
 #define NB_WALL 0x20000000u
 #define NB_INDEX 0x1fffffffu
+
+// position of back entry kk (0-based) in a row of `stride` entries
+__host__ __device__ __forceinline__ uint32_t back_slot(int stride, uint32_t kk) {
+  return (uint32_t)stride - 8u * (kk / 8u + 1u) + (kk & 7u);
+}
 
 struct CgScalars {
   double gamma, delta;          // r.r and r.Ar of the current iteration
@@ -63,7 +69,7 @@ struct KConst {  // by-value kernel parameter
   int nx, ny, nz, ncells;
   int R_lap;  // cells to each side for re_lap
   int cap;    // row capacity (max_neighbours)
-  int stride; // row stride in entries (cap rounded up to a multiple of 8)
+  int stride; // row stride in entries (cap + 14 rounded up to a multiple of 8)
   int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean;
   int n;      // particles
 };
@@ -80,6 +86,8 @@ struct mps_ctx {
   double4* vel4[2] = {nullptr, nullptr};
   uint32_t* tp[2] = {nullptr, nullptr};
   uint32_t* oid[2] = {nullptr, nullptr};
+  uint32_t* ent = nullptr;         // per slot: own index | NB_* flags (what a neighbour row stores)
+  bool rows_by_warp = false;       // MPS_B200_ROWS=warp forces the warp-per-particle row builder
   int cur = 0;
   // bin scratch
   uint32_t* key = nullptr;         // per slot (after bin: key of the slot)

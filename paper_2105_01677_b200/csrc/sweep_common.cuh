@@ -8,9 +8,10 @@ __device__ __forceinline__ const uint32_t* row_ptr(const uint32_t* nbr, int stri
   return nbr + (size_t)i * (size_t)stride;
 }
 // Entry k of a row with nf front entries: the re_n part grows from the front,
-// the re_n <= r < re_lap part from the back.
+// the re_n <= r < re_lap part from the back in whole 32-byte sectors (8 entries),
+// ascending inside each sector: back entry kk sits at stride - 8 (kk/8 + 1) + kk % 8.
 __device__ __forceinline__ uint32_t row_entry(const uint32_t* row, int stride, uint32_t nf, uint32_t k) {
-  return k < nf ? row[k] : row[stride - 1 - (k - nf)];
+  return k < nf ? row[k] : row[back_slot(stride, k - nf)];
 }
 
 // ---- 1/sqrt(x) in fp64: hardware seed (about 2^-22) plus one cubically convergent
