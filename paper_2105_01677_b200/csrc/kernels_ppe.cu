@@ -20,7 +20,22 @@
 
 namespace {
 
-constexpr int CG_TPB = 512;
+#ifdef MPS_CG_PROFILE
+#include <cstdio>
+#define TICK(slot) do { if (bid == 0 && tid == 0) { long long t_ = clock64(); prof[slot] += t_ - tlast; tlast = t_; } } while (0)
+#else
+#define TICK(slot) do { } while (0)
+#endif
+
+#ifndef MPS_CG_TPB
+#define MPS_CG_TPB 1024
+#endif
+#ifndef MPS_CG_MINB
+#define MPS_CG_MINB 1
+#endif
+constexpr int PPE_ILP = 4;  // independent neighbour gathers in flight per lane
+constexpr int CG_TPB = MPS_CG_TPB;
+constexpr int CG_MINB = MPS_CG_MINB;  // co-resident blocks per SM the register budget is set for
 
 struct PpeArgs {
   double4* pos4;  // .w: CG residual r during the solve, pressure at exit
@@ -46,48 +61,61 @@ struct PpeArgs {
 };
 
 // ---- block-wide sum of two values, result broadcast to every thread ---------------
+// warp shuffles, one partial per warp in shared memory, the first warp folds them in
+// a fixed order, the result is broadcast: two block barriers.
 template <int NT>
 __device__ __forceinline__ void block_sum2(double& a, double& b) {
   __shared__ double sh[2][NT / 32];
+  __shared__ double res[2];
   a = warp_sum(a);
   b = warp_sum(b);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  __syncthreads();  // sh may still be read from the previous call
   if (lane == 0) { sh[0][wid] = a; sh[1][wid] = b; }
   __syncthreads();
-  double sa = 0.0, sb = 0.0;
-#pragma unroll
-  for (int k = 0; k < NT / 32; ++k) { sa += sh[0][k]; sb += sh[1][k]; }
-  a = sa;
-  b = sb;
+  if (wid == 0) {
+    double sa = lane < NT / 32 ? sh[0][lane] : 0.0;
+    double sb = lane < NT / 32 ? sh[1][lane] : 0.0;
+    sa = warp_sum(sa);
+    sb = warp_sum(sb);
+    if (lane == 0) { res[0] = sa; res[1] = sb; }
+  }
+  __syncthreads();
+  a = res[0];
+  b = res[1];
+  // the next call's writes to sh/res come after its own first barrier at the earliest for
+  // sh (written before the barrier by lane 0 of each warp: all reads of sh above are done
+  // by warp 0 before the second barrier) and after both barriers for res
 }
 
 // ---- grid barrier (all blocks are co-resident: cooperative launch) ----------------
-// One thread per block arrives with a release fence and spins on the generation
-// word; the fence after the spin makes every later plain load of the block see the
-// other blocks' writes (it invalidates the SM's L1).  A spin that lasts longer than
-// about two seconds raises barrier_timeout and lets the kernel drain instead of hanging.
+// One monotonically increasing arrival counter: thread 0 of every block adds 1 with
+// release semantics and spins (acquire) until the count reaches nb x generation, so
+// a barrier costs one L2 round trip for the arrival plus the polls -- there is no
+// second "last block flips the flag" hop.  The fence after the spin makes every
+// later plain load of the block see the other blocks' writes (it invalidates the
+// SM's L1).  A spin that lasts longer than about two seconds raises barrier_timeout
+// and lets the kernel drain instead of hanging.
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
   unsigned int v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
+}
+__device__ __forceinline__ void red_release_add_u32(unsigned int* p, unsigned int v) {
+  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, CgScalars* cg) {
   __shared__ int dead;
   __syncthreads();
   if (threadIdx.x == 0) {
     dead = 0;
-    gen += 1u;
-    __threadfence();
-    const unsigned int prev = atomicAdd(&bar->count, 1u);
-    if (prev == gridDim.x - 1u) {
-      atomicExch(&bar->count, 0u);
-      __threadfence();
-      atomicExch(&bar->gen, gen);
-    } else {
-      const long long t0 = clock64();
-      while (ld_acquire_u32(&bar->gen) != gen) {
-        if (clock64() - t0 > 4000000000LL) {
+    gen += gridDim.x;  // arrivals expected once this barrier is complete
+    red_release_add_u32(&bar->count, 1u);
+    long long t0 = 0;
+    unsigned int polls = 0;
+    while ((int)(ld_acquire_u32(&bar->count) - gen) < 0) {
+      if ((++polls & 1023u) == 0u) {
+        if (t0 == 0) t0 = clock64();
+        else if (clock64() - t0 > 4000000000LL) {
           cg->barrier_timeout = 1;
           dead = 1;
           break;
@@ -118,21 +146,37 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
   const uint32_t m = live ? nf + co[i] : 0u;
   const double rho_i = TWO_PHASE ? kc.rho[(tp[i] >> 8) & 1] : kc.rho[0];
   double s = 0.0;
-#pragma unroll 2
-  for (uint32_t k = sub; k < m; k += L) {
-    const uint32_t e = row_entry(row, kc.stride, nf, k);
-    if (e & NB_DUMMY) continue;
-    const double4 q = pos4[e & NB_INDEX];
-    const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
-    double w = fma(kc.re_lap, rsqrt_f64(r2), -1.0);
-    if (TWO_PHASE) {
-      const double rho_j = kc.rho[(e & NB_PHASE1) ? 1 : 0];
-      const double rij =
-          kc.rho_pair_mean == 1 ? 2.0 * rho_i * rho_j / (rho_i + rho_j) : 0.5 * (rho_i + rho_j);
-      w = w / rij;
+  // batches of PPE_ILP entries per lane: entry loads, then gathers, then arithmetic, so the
+  // L2 round trips of one batch overlap (the L1 is invalidated by every grid barrier).
+  // An empty or dummy slot takes a point at distance re_lap on the x axis: its weight is
+  // re_lap / re_lap - 1 = 0 exactly.
+  for (uint32_t k = sub; k < m; k += PPE_ILP * L) {
+    uint32_t e[PPE_ILP];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const uint32_t kk = k + (uint32_t)(u * L);
+      e[u] = kk < m ? row_entry(row, kc.stride, nf, kk) : NB_DUMMY;
     }
-    s = fma(w, pi.w - q.w, s);
+    double4 q[PPE_ILP];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      if (e[u] & NB_DUMMY) q[u] = make_double4(pi.x + kc.re_lap, pi.y, pi.z, pi.w);
+      else q[u] = pos4[e[u] & NB_INDEX];
+    }
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const double dx = q[u].x - pi.x, dy = q[u].y - pi.y, dz = q[u].z - pi.z;
+      const double r2 = dx * dx + dy * dy + dz * dz;
+      double w = fma(kc.re_lap, rsqrt_f64(r2), -1.0);
+      if (TWO_PHASE) {
+        const double rho_j = kc.rho[(e[u] & NB_PHASE1) ? 1 : 0];
+        const double rij =
+            kc.rho_pair_mean == 1 ? 2.0 * rho_i * rho_j / (rho_i + rho_j) : 0.5 * (rho_i + rho_j);
+        w = w / rij;
+      }
+      if (e[u] & NB_DUMMY) w = 0.0;
+      s = fma(w, pi.w - q[u].w, s);
+    }
   }
   s = group_sum<L>(s);
   if (!TWO_PHASE) s *= 1.0 / kc.rho[0];
@@ -141,12 +185,15 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 
 // ---- the persistent solve -------------------------------------------------------------
 template <bool TWO_PHASE, int L>
-__global__ void __launch_bounds__(CG_TPB, 2)
+__global__ void __launch_bounds__(CG_TPB, CG_MINB)
 k_ppe_cg(KConst kc, PpeArgs a) {
   __shared__ uint32_t sh_cnt[2][CG_TPB / 32];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int nb = (int)gridDim.x, bid = (int)blockIdx.x;
   unsigned int gen = 0;
+#ifdef MPS_CG_PROFILE
+  long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
+#endif
 
   // -- S8b-1, S8b-2: flags and right-hand side over this block's contiguous chunk --------
   const int chunk = (kc.n + nb - 1) / nb;
@@ -233,6 +280,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
   }
   if (!grid_barrier(a.bar, gen, a.cg)) return;
 
+  TICK(0);
   // -- S8b-3, S8b-4: conjugate gradients ---------------------------------------------------
   const double tol2bb = a.tol2 * bb;
   int iters = 0, converged = (bb == 0.0) ? 1 : 0;
@@ -257,12 +305,15 @@ k_ppe_cg(KConst kc, PpeArgs a) {
           d_part = fma(ri, wi, d_part);
         }
       }
+      TICK(1);
       block_sum2<CG_TPB>(g_part, d_part);
       if (tid == 0) {
         a.part[2 * bid] = g_part;
         a.part[2 * bid + 1] = d_part;
       }
+      TICK(2);
       if (!grid_barrier(a.bar, gen, a.cg)) return;
+      TICK(3);
       double del = 0.0;
       gam = 0.0;
       for (int k = tid; k < nb; k += CG_TPB) {
@@ -270,6 +321,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         del += __ldcg(&a.part[2 * k + 1]);
       }
       block_sum2<CG_TPB>(gam, del);
+      TICK(4);
       if (gam <= tol2bb) { converged = 1; break; }
       if (iters >= a.maxit) break;
       double alpha, beta;
@@ -294,7 +346,9 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         a.x[i] = fma(alpha, pn, a.x[i]);
         a.pos4[i].w = fma(-alpha, sn, r);
       }
+      TICK(5);
       if (!grid_barrier(a.bar, gen, a.cg)) return;
+      TICK(6);
     }
   }
 
@@ -305,6 +359,11 @@ k_ppe_cg(KConst kc, PpeArgs a) {
     a.p[i] = v;
     a.pos4[i].w = v;
   }
+#ifdef MPS_CG_PROFILE
+  if (bid == 0 && tid == 0)
+    printf("cg profile (block 0, kcycles): setup %lld | phaseA %lld | blocksum %lld | barrier1 %lld | reduce %lld | phaseB %lld | barrier2 %lld | iters %d\n",
+           prof[0] / 1000, prof[1] / 1000, prof[2] / 1000, prof[3] / 1000, prof[4] / 1000, prof[5] / 1000, prof[6] / 1000, iters);
+#endif
   if (bid == 0 && tid == 0) {
     a.cg->gamma = gam;
     a.cg->bb = bb;
@@ -374,7 +433,7 @@ int mpsk_ppe_plan(mps_ctx* c) {
     default: c->cg_lanes = 8; per_sm = tp ? cg_blocks_per_sm<true, 8>() : cg_blocks_per_sm<false, 8>(); break;
   }
   if (per_sm < 1) return MPS_ERR_CUDA;
-  if (per_sm > 2) per_sm = 2;
+  if (per_sm > CG_MINB) per_sm = CG_MINB;
   c->cg_grid = per_sm * c->sm_count;
   return MPS_OK;
 }

@@ -188,7 +188,9 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   {
     // lanes per row of the CG operator: 8 by default; MPS_B200_CG_LANES = 4 | 8 | 16 for tuning
     const char* rw = getenv("MPS_B200_ROWS");
-    c->rows_by_warp = rw && !strcmp(rw, "warp");
+    // few occupied cells cannot fill the GPU with one warp per cell: small scenes use one
+    // warp per particle (measured crossover between scene 2, 89 k, and scene 3, 438 k)
+    c->rows_by_warp = rw ? !strcmp(rw, "warp") : (n < 200000);
     const char* ev = getenv("MPS_B200_CG_LANES");
     c->cg_lanes = ev ? atoi(ev) : 8;
     if (mpsk_ppe_plan(c) != MPS_OK) {

@@ -87,7 +87,7 @@ struct mps_ctx {
   uint32_t* tp[2] = {nullptr, nullptr};
   uint32_t* oid[2] = {nullptr, nullptr};
   uint32_t* ent = nullptr;         // per slot: own index | NB_* flags (what a neighbour row stores)
-  bool rows_by_warp = false;       // MPS_B200_ROWS=warp forces the warp-per-particle row builder
+  bool rows_by_warp = false;       // warp-per-particle row builder (small scenes; MPS_B200_ROWS=warp|cell overrides)
   int cur = 0;
   // bin scratch
   uint32_t* key = nullptr;         // per slot (after bin: key of the slot)

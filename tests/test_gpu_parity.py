@@ -92,9 +92,12 @@ def test_bin_after_motion_matches_oracle(B, O):
 
 
 # ----------------------------------------------------------- S3: neighbour sets ---
+@pytest.mark.parametrize("rows", ["warp", "cell"])
 @pytest.mark.parametrize("cell_div", [1, 2])
 @pytest.mark.parametrize("scene", ["tank_moved", "config1", "cloud"])
-def test_neighbour_sets_are_bit_exact(B, O, scene, cell_div):
+def test_neighbour_sets_are_bit_exact(B, O, scene, cell_div, rows, monkeypatch):
+    # both row builders (warp per particle / warp per cell; the library picks by size)
+    monkeypatch.setenv("MPS_B200_ROWS", rows)
     if scene == "cloud":
         s = scenes.random_cloud(3000, 10 * 0.031, seed=3)
         s.params.update(l0=0.01, re_n=0.021, re_lap=0.031)
@@ -298,7 +301,9 @@ def _trajectory(B, O, s, nsteps, route, **over):
     return d.max() / L, d.max() / s.params["l0"], moved / s.params["l0"], g, o
 
 
-def test_trajectory_config1_explicit_20_steps(B, O):
+@pytest.mark.parametrize("rows", ["warp", "cell"])
+def test_trajectory_config1_explicit_20_steps(B, O, rows, monkeypatch):
+    monkeypatch.setenv("MPS_B200_ROWS", rows)
     s = scenes.make_scene(1)
     eL, el0, moved, g, o = _trajectory(B, O, s, 20, 0)
     print(f"config 1, 20 explicit steps: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}; max displacement {moved:.2f} l0")
