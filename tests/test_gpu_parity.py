@@ -418,3 +418,46 @@ def test_full_size_sampled_config3(B, O):
     assert (np.diff(key[perm].astype(np.int64)) >= 0).all()
     same = np.diff(key[perm].astype(np.int64)) == 0
     assert (np.diff(perm.astype(np.int64))[same] > 0).all()
+
+
+@pytest.mark.parametrize("cfg,idx", [(3, 0), (5, 2)])
+def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx):
+    """Configs 3 (N = 438,208) and 5[2] (N = 1,011,096) in the launch configuration bench.py
+    times (warp-per-cell row builder, 148 x 1024 persistent CG): density, flags, right-hand
+    side and operator against the oracle on identical positions, and the GPU's CG solution
+    checked by its true residual under the ORACLE's operator."""
+    s = scenes.make_scene(cfg, sweep_index=idx)
+    g = B.Mps(s)
+    o = O.Oracle(s)
+    g.step(1, 1)                      # one whole PPE step moves the fluid off the lattice
+    for k in ("x", "y", "z", "u", "v", "w"):
+        o.set(k, g.get(k))
+    g.bin(); o.bin()
+    g.density(); o.density()
+    n0 = o.constants()["n0_n"]
+    assert relerr(g.get("n"), o.get("n"), n0) <= TOL
+    g.set("n", o.get("n"))
+    it, relres = g.pressure_ppe()
+    o.ppe_flags(); o.ppe_rhs()
+    bc = o.get("bc")
+    assert np.array_equal(g.get("bc"), bc)
+    b = o.get("b")
+    assert relerr(g.get("b"), b, 1.0) <= 1e-14
+    rows = bc == 0
+    v = np.where(rows, np.random.default_rng(1).standard_normal(s.n), 0.0)
+    assert relerr(g.ppe_apply(v), o.ppe_apply(v), 1e-30) <= TOL
+    x = g.get("xcg")
+    true_rel = np.linalg.norm(b - o.ppe_apply(x)) / np.linalg.norm(b)
+    print(f"config {cfg}[{idx}]: N {s.n}, rows {int(rows.sum())}, CG iters {it}, recurrence relres {relres:.2e}, "
+          f"true relres under the oracle's operator {true_rel:.2e}")
+    assert relres <= 1e-8 and true_rel <= 2e-8
+    # neighbour counts of the cell builder on sampled particles against the brute-force definition
+    cnt_l, _ = g.neighbours(B.RADIUS_LAP)
+    X, Y, Z = (g.get(k) for k in "xyz")
+    re = s.params["re_lap"]
+    for i in np.random.default_rng(2).choice(s.n, 100, replace=False):
+        dx, dy, dz = X - X[i], Y - Y[i], Z - Z[i]
+        r2 = (dx * dx + dy * dy) + dz * dz
+        m = r2 < re * re
+        m[i] = False
+        assert cnt_l[i] == m.sum()
