@@ -292,9 +292,14 @@ k_ppe_cg(KConst kc, PpeArgs a) {
     for (;;) {
       // phase A: w = A r, gamma = r.r, delta = r.w
       double g_part = 0.0, d_part = 0.0;
-      // warp-uniform trip count: g0 is the warp's first group
-      for (int g0 = (gtid & ~31) / L; g0 < n_rows; g0 += gthreads / L) {
-        const int g = g0 + (lane / L);
+      // Rows are dealt to the blocks in super-chunks of 8 warps (8 * 32 / L consecutive rows, so
+      // the warps that share an SM's L1 work on neighbouring rows) round-robin over the grid:
+      // every block gets an even sample of cheap (wall) and expensive (fluid) rows and at most
+      // one super-chunk more than any other.  The trip count is warp-uniform.
+      constexpr int GPW = 32 / L;        // row groups per warp
+      constexpr int SCW = 8;             // warps per super-chunk
+      for (int sc = (wid / SCW) * nb + bid; sc * (SCW * GPW) < n_rows; sc += (CG_TPB / 32 / SCW) * nb) {
+        const int g = sc * (SCW * GPW) + (wid % SCW) * GPW + (lane / L);
         const bool live = g < n_rows;
         const int i = live ? (int)a.rows[g] : 0;
         double ri;
