@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(ROWS_TPB)
 k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
              const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
              uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
-             DevFlags* __restrict__ flags) {
+             DevFlags* __restrict__ flags, int fluid_only) {
   const int lane = threadIdx.x & 31;
   const int warp = (blockIdx.x * ROWS_TPB + threadIdx.x) >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
@@ -213,7 +213,8 @@ k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
     const int i = warp * ROWS_PPW + t;
     if (i >= kc.n) break;
     const uint32_t k = key[i];
-    if (k >= (uint32_t)kc.ncells) {  // ghost
+    if (k >= (uint32_t)kc.ncells || (fluid_only && (tp[i] & 0xff) != MPS_FLUID)) {
+      // ghosts have no neighbours; the first bin of a step serves fluid rows only
       if (lane == 0) { cn[i] = 0; co[i] = 0; }
       continue;
     }
@@ -308,7 +309,8 @@ __device__ __forceinline__ void flush_sector(uint32_t* dst, const uint32_t (*b)[
 __global__ void __launch_bounds__(CELL_TPB, 4)
 k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
                   const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
-                  uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags) {
+                  uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags,
+                  int fluid_only) {
   __shared__ uint32_t buf[2][CELL_WARPS][8][32];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarp = blockIdx.x * CELL_WARPS + wid;
@@ -332,7 +334,15 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
     const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
     for (uint32_t base = ps; base < pe; base += 32) {
       const uint32_t i = base + (uint32_t)lane;
-      const bool act = i < pe;
+      bool act = i < pe;
+      if (fluid_only) {  // the first bin of a step serves viscosity: fluid rows only
+        if (act && (ent[i] & (NB_DUMMY | NB_WALL))) {
+          act = false;
+          cn[i] = 0;
+          co[i] = 0;
+        }
+        if (!__any_sync(0xffffffffu, act)) continue;
+      }
       const uint32_t ii = act ? i : ps;
       const double4 pi = pos4[ii];
       uint32_t* row = nbr + (size_t)ii * (size_t)S;
@@ -555,7 +565,8 @@ int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const doub
   return MPS_OK;
 }
 
-int mpsk_bin(mps_ctx* c) {
+int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
+  const int fo = fluid_rows_only ? 1 : 0;
   const int n = (int)c->n;
   const int nc = c->kc.ncells;
   const int cur = c->cur, nxt = cur ^ 1;
@@ -573,11 +584,11 @@ int mpsk_bin(mps_ctx* c) {
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
   if (c->prm.cell_div == 1 && !c->rows_by_warp) {
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, c->kc, c->pos4[nxt],
-               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags);
+               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
   } else {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc,
-               c->pos4[nxt], c->tp[nxt], c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags);
+               c->pos4[nxt], c->tp[nxt], c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
   }
   c->binned = true;
   c->ppe_ready = false;

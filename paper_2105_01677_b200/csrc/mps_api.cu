@@ -393,7 +393,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     return fail(c, MPS_ERR_ARG, "bad nsteps or pressure_route");
   int first_err = MPS_OK;
   for (int s = 0; s < nsteps; ++s) {
-    mpsk_bin(c);
+    mpsk_bin(c, /*fluid_rows_only=*/true);  // viscosity and nu_t are computed for fluid i only
     mpsk_viscosity(c);
     mpsk_predict(c);
     mpsk_bin(c);

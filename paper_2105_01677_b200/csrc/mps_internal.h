@@ -163,7 +163,9 @@ void mps_timer_drain(mps_ctx* c);
 static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // ---- stage launchers (defined in the .cu files) -----------------------------------
-int mpsk_bin(mps_ctx* c);                 // keys, counting sort, reorder, neighbour rows
+// keys, counting sort, reorder, neighbour rows (fluid_rows_only: rows of FLUID particles only,
+// all a viscosity sweep needs; used for the first bin of mps_step)
+int mpsk_bin(mps_ctx* c, bool fluid_rows_only = false);
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
                          uint32_t* tmp);
 int mpsk_density(mps_ctx* c);
