@@ -96,7 +96,7 @@ class ClockSampler(threading.Thread):
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", self.gpu_id, f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             for line in self.proc.stdout:
                 self.rows.append([c.strip() for c in line.split(",")])
         except Exception:
@@ -312,7 +312,8 @@ def run_b200(args):
         uses = {"bin_sort": 2 * K, "bin_list": 2 * K, "viscosity": K, "gradient": K, "ppe_setup": K,
                 **cg_uses}.get(top, ln)
         achieved = ab * uses / (ms * 1e-3) / 1e9
-        roof = {"kernel": top, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        roof = {"kernel": top, "bound": "hbm", "per": "use (cg_spmv: one operator application; one k_ppe_cg launch runs a whole solve)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, ROUTE_NAME[route], top)),
                 "peak_source": peak_src, "algorithmic_bytes_per_use": ab, "uses": uses,
                 "us_per_use": 1e3 * ms / max(uses, 1), "launches": ln,
