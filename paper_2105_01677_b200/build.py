@@ -42,5 +42,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_peaks() -> str:
+    """The stand-alone ceilings micro-benchmark (csrc/peaks.cu) -> ./mps_peaks."""
+    exe = os.path.join(HERE, "mps_peaks")
+    src = os.path.join(CSRC, "peaks.cu")
+    if _stale(exe, [src]):
+        subprocess.check_call([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo",
+                               "-std=c++17", "-o", exe, src])
+    return exe
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--peaks" in sys.argv:
+        print(build_peaks())
