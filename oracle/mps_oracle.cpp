@@ -41,6 +41,8 @@ struct Prm {
   int cg_maxit;
   double cs;
   int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean, cell_div;
+  int ppe_source;     // 0: Eq. 8; 1: higher-order source Eq. 15 (HS); 2: HS + error-compensating parts Eq. 17-18 (ECS)
+  int ppe_laplacian;  // 0: Eq. 10 form (Listing 2); 1: higher-order Laplacian Eq. 16 (HL)
   double dmin[3], dmax[3];
   int max_neighbours;
   double n0_n, n0_lap, lam;
@@ -74,7 +76,7 @@ void lattice_constants(int dim, double l0, double re, double* n0, double* lam, i
 struct Orc {
   Prm prm;
   int n = 0;
-  std::vector<double> f[18];  // x y z u v w n p ax ay az nut b phat gx gy gz xcg
+  std::vector<double> f[21];  // x y z u v w n p ax ay az nut b phat gx gy gz xcg dndt n_k dndt_k
   std::vector<int> type, phase, bc, key, perm, cell_start;
   double h = 0, inv_h = 0;
   int nc[3] = {0, 0, 0};
@@ -292,10 +294,57 @@ struct Orc {
       else bc[i] = 0;
     }
   }
-  // step 7b.2 (Eq.8 divided by -rho; Q5).
+  // NEXT-1, MPS-HS (Eq.15; Q22): the material derivative of the particle
+  // number density of Eq.5 with w = re/r - 1:  Dn/Dt = sum dw/dt = - sum re/r^3 (x_ij . u_ij),
+  // x_ij = x_j - x_i, u_ij = u_j - u_i (walls and dummies have u = 0), over N(i, r_n),
+  // every non-ghost i.  Written into field `dst` (18: current, 20: the copy kept from r^k).
+  void dndt(int dst) {
+    ensure_binned();
+    const double re = prm.re_n;
+    for (int i = 0; i < n; ++i) {
+      f[dst][i] = 0.0;
+      if (type[i] == GHOST) continue;
+      const bool si = (type[i] == WALL || type[i] == DUMMY);
+      const double ui[3] = {si ? 0.0 : f[3][i], si ? 0.0 : f[4][i], si ? 0.0 : f[5][i]};
+      double s = 0.0;
+      for_neighbours(i, re, [&](int j, double dx, double dy, double dz, double r2) {
+        const bool sj = (type[j] == WALL || type[j] == DUMMY);
+        const double uj[3] = {sj ? 0.0 : f[3][j], sj ? 0.0 : f[4][j], sj ? 0.0 : f[5][j]};
+        const double r = std::sqrt(r2);
+        s += re / (r2 * r) * (dx * (uj[0] - ui[0]) + dy * (uj[1] - ui[1]) + dz * (uj[2] - ui[2]));
+      });
+      f[dst][i] = -s;
+    }
+  }
+  // step 7b.2.  ppe_source 0: Eq.8 divided by -rho (Q5).
+  // ppe_source 1 (HS, Eq.15; Q22): b = relax / (n0 dt) (Dn/Dt)*.
+  // ppe_source 2 (ECS, Eq.17-18; Q22): b = relax / dt [ (Dn/Dt)* / n0 + ECS ],
+  //   ECS = |alpha| (Dn/Dt)^k / n0 + |beta| alpha / dt, alpha = (n^k - n0)/n0,
+  //   beta = dt (Dn/Dt)^k / n0, with n^k and (Dn/Dt)^k kept from the start of the step.
   void ppe_rhs() {
-    for (int i = 0; i < n; ++i)
-      f[12][i] = (bc[i] == 0) ? prm.ppe_relax / (prm.dt * prm.dt) * (f[6][i] - n0_n) / n0_n : 0.0;
+    const double dt = prm.dt;
+    for (int i = 0; i < n; ++i) {
+      double b = 0.0;
+      if (bc[i] == 0) {
+        if (prm.ppe_source == 0) {
+          b = prm.ppe_relax / (dt * dt) * (f[6][i] - n0_n) / n0_n;
+        } else if (prm.ppe_source == 1) {
+          b = prm.ppe_relax / (n0_n * dt) * f[18][i];
+        } else {
+          const double alpha = (f[19][i] - n0_n) / n0_n;
+          const double beta = dt / n0_n * f[20][i];
+          const double ecs = std::fabs(alpha) * (f[20][i] / n0_n) + std::fabs(beta) * (alpha / dt);
+          b = prm.ppe_relax / dt * (f[18][i] / n0_n + ecs);
+        }
+      }
+      f[12][i] = b;
+    }
+  }
+  // pair coefficient of the pressure Laplacian before the 1/rho_ij: Eq.10 form
+  // A_lap w(r) (Listing 2), or MPS-HL (Eq.16; Q23): 2 re / (n0 r^3).
+  double lap_coef(double re, double r2) const {
+    if (prm.ppe_laplacian == 1) return 2.0 * re / (n0_lap * r2 * std::sqrt(r2));
+    return A_lap * w_of(re, r2);
   }
   double rho_pair(int i, int j) const {
     const double ri = prm.rho[phase[i]], rj = prm.rho[phase[j]];
@@ -313,7 +362,7 @@ struct Orc {
       const double xi = xin[i];
       for_neighbours(i, re, [&](int j, double, double, double, double r2) {
         if (bc[j] == -1) return;
-        const double c = A_lap * w_of(re, r2) / rho_pair(i, j);
+        const double c = lap_coef(re, r2) / rho_pair(i, j);
         s += c * (xi - (bc[j] == 0 ? xin[j] : 0.0));
       });
       yout[i] = s + prm.compress / (prm.dt * prm.dt) * xi;
@@ -420,10 +469,16 @@ struct Orc {
   // STEP k -> k+1 (section 8(c).1 of SURVEY.md / DESIGN.md section 2).
   int step(int route) {
     bin();                // 1
+    if (route == 1 && prm.ppe_source == 2) {  // ECS keeps n^k and (Dn/Dt)^k (Eq.17)
+      density();
+      f[19] = f[6];
+      dndt(20);
+    }
     viscosity();          // 2, 3
     predict();            // 4
     bin();                // 5
     density();            // 6
+    if (route == 1 && prm.ppe_source >= 1) dndt(18);  // (Dn/Dt)* at r*, u* (Eq.15)
     int rc = 0;
     if (route == 0) pressure_explicit();  // 7a
     else rc = pressure_ppe();             // 7b
@@ -456,7 +511,7 @@ void* orc_create(const double* dp, const int* ip, int n, const double* x, const 
   p.n0_n = dp[24]; p.n0_lap = dp[25]; p.lam = dp[26];
   p.dim = ip[0]; p.n_phases = ip[1]; p.cg_maxit = ip[2]; p.grad_variant = ip[3];
   p.clamp_negative_p = ip[4]; p.rho_pair_mean = ip[5]; p.nu_pair_mean = ip[6];
-  p.cell_div = ip[7]; p.max_neighbours = ip[8];
+  p.cell_div = ip[7]; p.max_neighbours = ip[8]; p.ppe_source = ip[9]; p.ppe_laplacian = ip[10];
   o->n = n;
   for (auto& a : o->f) a.assign(n, 0.0);
   const double* src[6] = {x, y, z, u, v, w};
@@ -472,14 +527,14 @@ void orc_set_brute(void* h, int b) { ((Orc*)h)->brute = (b != 0); }
 
 int orc_set_f64(void* h, int field, const double* src) {
   Orc* o = (Orc*)h;
-  if (field < 0 || field >= 18) return -1;
+  if (field < 0 || field >= 21) return -1;
   std::copy(src, src + o->n, o->f[field].begin());
   if (field < 3) o->binned = false;
   return 0;
 }
 int orc_get_f64(void* h, int field, double* dst) {
   Orc* o = (Orc*)h;
-  if (field < 0 || field >= 18) return -1;
+  if (field < 0 || field >= 21) return -1;
   std::copy(o->f[field].begin(), o->f[field].end(), dst);
   return 0;
 }
@@ -554,6 +609,7 @@ int orc_ppe_rhs(void* h) { ((Orc*)h)->ppe_rhs(); return 0; }
 int orc_ppe_apply(void* h, const double* xin, double* yout) { ((Orc*)h)->ppe_apply(xin, yout); return 0; }
 int orc_ppe_solve(void* h, double rtol, int maxit) { return ((Orc*)h)->ppe_solve(rtol, maxit); }
 int orc_pressure_ppe(void* h) { return ((Orc*)h)->pressure_ppe(); }
+void orc_dndt(void* h, int dst) { ((Orc*)h)->dndt(dst == 20 ? 20 : 18); }
 int orc_phat(void* h) { ((Orc*)h)->phat(); return 0; }
 int orc_gradient(void* h) { ((Orc*)h)->gradient(); return 0; }
 int orc_correct(void* h) { ((Orc*)h)->correct(); return 0; }

@@ -15,7 +15,8 @@ from . import build as _build
 _lib = None
 
 F64 = {"x": 0, "y": 1, "z": 2, "u": 3, "v": 4, "w": 5, "n": 6, "p": 7, "ax": 8, "ay": 9,
-       "az": 10, "nut": 11, "b": 12, "phat": 13, "gx": 14, "gy": 15, "gz": 16, "xcg": 17}
+       "az": 10, "nut": 11, "b": 12, "phat": 13, "gx": 14, "gy": 15, "gz": 16, "xcg": 17,
+       "dndt": 18, "n_k": 19, "dndt_k": 20}
 I32 = {"type": 0, "phase": 1, "bc": 2, "key": 3, "perm": 4}
 
 _dp = C.POINTER(C.c_double)
@@ -44,6 +45,7 @@ def lib():
                    "orc_pressure_explicit", "orc_ppe_flags", "orc_ppe_rhs", "orc_pressure_ppe",
                    "orc_phat", "orc_gradient", "orc_correct"):
             getattr(L, nm).argtypes = [C.c_void_p]
+        L.orc_dndt.argtypes = [C.c_void_p, C.c_int]
         L.orc_ppe_apply.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_ppe_solve.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.orc_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
@@ -79,8 +81,9 @@ def pack_params(p: Dict[str, object]):
                    p["lam"]], dtype=np.float64)
     ip = np.array([p["dim"], p["n_phases"], p["cg_maxit"], p["grad_variant"],
                    p["clamp_negative_p"], p["rho_pair_mean"], p["nu_pair_mean"], p["cell_div"],
-                   p["max_neighbours"]], dtype=np.int32)
-    assert dp.size == 27 and ip.size == 9
+                   p["max_neighbours"], p.get("ppe_source", 0), p.get("ppe_laplacian", 0)],
+                  dtype=np.int32)
+    assert dp.size == 27 and ip.size == 11
     return dp, ip
 
 
@@ -166,6 +169,7 @@ class Oracle:
     def viscosity(self): self.L.orc_viscosity(self.h)
     def predict(self): self.L.orc_predict(self.h)
     def pressure_explicit(self): self.L.orc_pressure_explicit(self.h)
+    def dndt(self, keep: bool = False): self.L.orc_dndt(self.h, 20 if keep else 18)
     def ppe_flags(self): self.L.orc_ppe_flags(self.h)
     def ppe_rhs(self): self.L.orc_ppe_rhs(self.h)
     def pressure_ppe(self) -> int: return int(self.L.orc_pressure_ppe(self.h))

@@ -453,3 +453,124 @@ def test_T11_hydrostatic_explicit():
     rg = 1000.0 * 9.81
     assert slope == pytest.approx(rg, rel=0.20)
     assert bottom == pytest.approx(rg * H, rel=0.20)
+
+
+# ---- NEXT-1: higher-order source (HS, Eq. 15), higher-order Laplacian (HL, Eq. 16), ECS ----
+def _numpy_dndt(x, y, z, u, v, w, re):
+    """Brute force: Dn/Dt_i = d/dt sum_j (re/r_ij - 1) = -sum_j re/r^3 (x_ij . u_ij)."""
+    dx = x[None, :] - x[:, None]; dy = y[None, :] - y[:, None]; dz = z[None, :] - z[:, None]
+    du = u[None, :] - u[:, None]; dv = v[None, :] - v[:, None]; dw = w[None, :] - w[:, None]
+    r2 = (dx * dx + dy * dy) + dz * dz
+    m = r2 < re * re
+    np.fill_diagonal(m, False)
+    r2 = np.where(m, r2, 1.0)
+    return -(np.where(m, re / (r2 * np.sqrt(r2)) * (dx * du + dy * dv + dz * dw), 0.0)).sum(axis=1)
+
+
+def test_HS_dndt_uniform_dilation_closed_form():
+    # u = a x on the ideal lattice: x_ij . u_ij = a r^2, so Dn/Dt = -a sum re/r = -a (n0 + 32)
+    m = 9
+    s = scenes.fluid_blob(L0, (m, m, m))
+    a = 0.37
+    o = O.Oracle(s)
+    o.set("u", a * s.x); o.set("v", a * s.y); o.set("w", a * s.z)
+    o.bin(); o.dndt()
+    core = _interior_mask(s, m, 3)
+    expect = -a * (GOLD["n0_3d_2.1"] + GOLD["count_3d_2.1"])
+    assert core.sum() == 27
+    assert np.allclose(o.get("dndt")[core], expect, rtol=1e-12)
+
+
+def test_HS_dndt_equals_brute_force_and_finite_difference_of_density():
+    s = scenes.small_tank(shuffle=True)
+    rng = np.random.default_rng(4)
+    fl = s.type == scenes.FLUID
+    for k in "uvw":
+        getattr(s, k)[fl] = rng.standard_normal(fl.sum())
+    o = O.Oracle(s)
+    o.bin(); o.dndt()
+    d = o.get("dndt")
+    ref = _numpy_dndt(s.x, s.y, s.z, s.u, s.v, s.w, s.params["re_n"])
+    assert np.allclose(d, ref, rtol=1e-12, atol=1e-9 * np.abs(ref).max())
+    # it is the time derivative of Eq. 5 along the motion: central difference of the oracle's
+    # own density at r -/+ eps u (walls do not move), on particles with no pair near r_n
+    eps = 1e-9
+    dens = []
+    for sgn in (-1.0, 1.0):
+        o2 = O.Oracle(s)
+        for k, vel in zip("xyz", "uvw"):
+            o2.set(k, getattr(s, k) + sgn * eps * getattr(s, vel))
+        o2.bin(); o2.density()
+        dens.append(o2.get("n"))
+    fd = (dens[1] - dens[0]) / (2 * eps)
+    # exclude particles that have a pair within 1e-6 l0 of r_n (the weight has a kink there)
+    dx = s.x[None, :] - s.x[:, None]; dy = s.y[None, :] - s.y[:, None]; dz = s.z[None, :] - s.z[:, None]
+    r = np.sqrt(dx * dx + dy * dy + dz * dz)
+    near = (np.abs(r - s.params["re_n"]) < 1e-6 * s.params["l0"]).any(axis=1)
+    ok = ~near
+    assert ok.sum() > 0.9 * s.n
+    assert np.allclose(fd[ok], d[ok], rtol=2e-5, atol=2e-5 * np.abs(d).max())
+
+
+def test_HS_and_ECS_right_hand_side_worked_example():
+    # ideal lattice scaled by s (same 32 neighbours for 0.94 < s <= 1) with u = a X:
+    #   n^k = (n0 + 32)/s - 32,  (Dn/Dt)^k = -a (n0 + 32)/s   (every r scales by s)
+    m, sc, a = 9, 0.98, -0.8
+    n0, cnt = GOLD["n0_3d_2.1"], GOLD["count_3d_2.1"]
+    s = scenes.fluid_blob(L0, (m, m, m))
+    core = _interior_mask(s, m, 3)
+    for src in (1, 2):
+        o = O.Oracle(s, ppe_source=src, re_n=2.1 * L0, beta=0.0)
+        X, Y, Z = sc * s.x, sc * s.y, sc * s.z
+        o.set("x", X); o.set("y", Y); o.set("z", Z)
+        o.set("u", a * X); o.set("v", a * Y); o.set("w", a * Z)
+        o.bin(); o.density(); o.dndt(); o.dndt(keep=True)
+        nk = (n0 + cnt) / sc - cnt
+        dk = -a * (n0 + cnt) / sc
+        assert np.allclose(o.get("n")[core], nk, rtol=1e-12)
+        assert np.allclose(o.get("dndt_k")[core], dk, rtol=1e-12)
+        o.set("n_k", o.get("n"))
+        o.ppe_flags(); o.ppe_rhs()
+        dt = s.params["dt"]
+        if src == 1:      # Eq. 15 (sign: Q22): b = (Dn/Dt)* / (n0 dt)
+            expect = dk / (n0 * dt)
+        else:             # Eq. 17-18 by hand with alpha = (n^k - n0)/n0, beta = dt (Dn/Dt)^k / n0
+            alpha = (nk - n0) / n0
+            beta = dt * dk / n0
+            expect = (dk / n0 + abs(alpha) * dk / n0 + abs(beta) * alpha / dt) / dt
+        assert expect > 0  # compression (a < 0) must raise the pressure
+        assert np.allclose(o.get("b")[core], expect, rtol=1e-12)
+
+
+def test_HL_operator_closed_form_symmetry_and_dense_solve():
+    # Eq. 16 applied to phi = x^2 at an interior lattice particle: (1/n0) sum 2 x_ij^2 re / r^3
+    # = (2/3)(1/n0) sum re/r = (2/3)(n0 + 122)/n0 (cubic symmetry); the operator is -(1/rho) lap
+    m = 10
+    s = scenes.fluid_blob(L0, (m, m, m))
+    o = O.Oracle(s, ppe_laplacian=1, compress=0.0, beta=0.0)
+    o.bin(); o.density(); o.ppe_flags()
+    assert (o.get("bc") == 0).all()
+    y = o.ppe_apply(s.x ** 2)
+    core = _interior_mask(s, m, 4)
+    n0l, cnt = GOLD["n0_3d_3.1"], GOLD["count_3d_3.1"]
+    assert np.allclose(y[core], -(2.0 / 3.0) * (n0l + cnt) / n0l / 1000.0, rtol=1e-11)  # rho = 1000
+    # symmetric positive definite, and CG = dense solve
+    st = scenes.small_tank()
+    o = O.Oracle(st, ppe_laplacian=1)
+    o.bin(); o.density(); o.ppe_flags(); o.ppe_rhs()
+    rows = np.nonzero(o.get("bc") == 0)[0]
+    rng = np.random.default_rng(7)
+    xv = np.zeros(st.n); yv = np.zeros(st.n)
+    xv[rows] = rng.standard_normal(rows.size); yv[rows] = rng.standard_normal(rows.size)
+    Ax, Ay = o.ppe_apply(xv), o.ppe_apply(yv)
+    assert abs(xv @ Ay - Ax @ yv) <= 1e-12 * abs(xv @ Ay)
+    assert xv @ Ax > 0
+    A = np.zeros((rows.size, rows.size))
+    for k, i in enumerate(rows):
+        e = np.zeros(st.n); e[i] = 1.0
+        A[:, k] = o.ppe_apply(e)[rows]
+    b = o.get("b")[rows]
+    it = o.ppe_solve(1e-12, 5000)
+    assert it > 0
+    xd = np.linalg.solve(A, b)
+    assert np.linalg.norm(o.get("xcg")[rows] - xd) <= 1e-9 * np.linalg.norm(xd)
