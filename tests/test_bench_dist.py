@@ -25,7 +25,8 @@ n_all = bench.all_sum(world, scene.n, dev)
 import numpy as np
 out = dict(rank=rank, ms=ms, n_all=n_all, n=scene.n, route=route,
            x_sum=float(np.sum(scene.x)), name=bench.workload_name(argparse.Namespace(config=1, sweep_index=0), scene, route))
-print("RESULT " + json.dumps(out), flush=True)
+with open(os.path.join({out!r}, "rank%d.json" % rank), "w") as f:   # one file per rank: stdout lines can interleave
+    json.dump(out, f)
 torch.distributed.barrier()
 torch.distributed.destroy_process_group()
 """
@@ -40,10 +41,10 @@ def _torchrun(script_args, port):
 
 def test_world2_gloo_replicas(tmp_path):
     w = tmp_path / "worker.py"
-    w.write_text(WORKER.format(root=ROOT))
+    w.write_text(WORKER.format(root=ROOT, out=str(tmp_path)))
     r = _torchrun([str(w)], 29731)
     assert r.returncode == 0, r.stderr[-2000:]
-    res = [json.loads(l.split("RESULT ", 1)[1]) for l in r.stdout.splitlines() if "RESULT " in l]
+    res = [json.load(open(tmp_path / f"rank{k}.json")) for k in (0, 1)]
     assert sorted(x["rank"] for x in res) == [0, 1]
     a, b = sorted(res, key=lambda x: x["rank"])
     # max over ranks of the per-rank time, sum over ranks of the particle counts
