@@ -48,7 +48,7 @@ enum { MPS_ORDER_ORIGINAL = 0, MPS_ORDER_SORTED = 1 };
 enum { MPS_ROUTE_EXPLICIT = 0, MPS_ROUTE_PPE = 1 };
 enum { MPS_RADIUS_N = 0, MPS_RADIUS_LAP = 1 };
 
-/* field ids for mps_get_field / mps_set_field.  0..17 are fp64, 32..35 int32. */
+/* field ids for mps_get_field / mps_set_field.  0..20 are fp64, 32..35 int32. */
 enum {
   MPS_F_X = 0, MPS_F_Y = 1, MPS_F_Z = 2,       /* position r */
   MPS_F_U = 3, MPS_F_V = 4, MPS_F_W = 5,       /* velocity u */
@@ -60,6 +60,8 @@ enum {
   MPS_F_PHAT = 13,                             /* neighbourhood minimum pressure (Eq. 14, Q12) */
   MPS_F_GX = 14, MPS_F_GY = 15, MPS_F_GZ = 16, /* pressure gradient */
   MPS_F_XCG = 17,                              /* CG solution before the clamp (Q4) */
+  MPS_F_DNDT = 18,                             /* Dn/Dt of the last mps_dndt (Eq. 15, Q22) */
+  MPS_F_NK = 19, MPS_F_DNDTK = 20,             /* n and Dn/Dt kept from the start of the step (Eq. 17) */
   MPS_I_TYPE = 32, MPS_I_PHASE = 33,
   MPS_I_BC = 34,                               /* -1 dummy/ghost, 1 free surface, 0 PPE unknown (Eq. 6) */
   MPS_I_KEY = 35                               /* cell key of the last mps_bin (read only) */
@@ -78,7 +80,9 @@ typedef struct mps_params {
   int32_t key_mode;         /* 0: linear x-fastest cell key (the only mode supported) */
   int32_t cell_div;         /* (1) cell side h = max(re_n, re_lap) / cell_div; 1..3 */
   int32_t max_neighbours;   /* (300) P:286; capacity of one neighbour row */
-  int32_t reserved_i[2];
+  int32_t ppe_source;       /* (0) 0: Eq. 8; 1: higher-order source, Eq. 15 (MPS-HS); 2: HS plus the
+                               error-compensating parts, Eq. 17-18 (ECS); Q22 */
+  int32_t ppe_laplacian;    /* (0) 0: Eq. 10 form of Listing 2; 1: higher-order Laplacian, Eq. 16 (MPS-HL); Q23 */
   double l0;                /* initial particle spacing */
   double re_n;              /* radius for density, p-hat and gradient (2.1 l0) */
   double re_grad;           /* must equal re_n (one list serves both) */
@@ -169,6 +173,12 @@ int mps_pressure_explicit(mps_ctx* ctx);
  * Returns MPS_ERR_NOCONV if cg_maxit was reached (pressures still written). */
 int mps_pressure_ppe(mps_ctx* ctx, int32_t* iters_out, double* relres_out);
 
+/* mps_dndt: Dn/Dt_i = -sum_{j in N(i, re_n)} re_n / r^3 (x_ij . u_ij) at the current positions
+ * and velocities, every non-ghost i (Eq. 15, the material derivative of Eq. 5; sign:
+ * Q22).  keep = 0 writes MPS_F_DNDT; keep = 1 writes MPS_F_DNDTK and copies the ctx's n field to
+ * MPS_F_NK (the start-of-step values of Eq. 17).  Needs mps_bin at the current positions. */
+int mps_dndt(mps_ctx* ctx, int32_t keep);
+
 /* mps_gradient: p-hat (minimum over i and its non-dummy neighbours within re_n;
  * P:215, Q12) then the pressure gradient of fluid i, variant grad_variant
  * (Eq. 14; Q13). */
@@ -178,8 +188,8 @@ int mps_gradient(mps_ctx* ctx);
  * and dummies do not move (Q8, Q3, Q11).  Invalidates the bin. */
 int mps_correct(mps_ctx* ctx);
 
-/* mps_step: nsteps times { bin, viscosity, predict, bin, density, pressure
- * (route), gradient, correct }.  No host synchronisation inside except the CG
+/* mps_step: nsteps times { bin, [ppe_source 2: density, dndt(keep)], viscosity, predict, bin,
+ * density, [ppe_source >= 1: dndt], pressure (route), gradient, correct }.  No host synchronisation inside except the CG
  * convergence poll of the PPE route.  Returns the first error met. */
 int mps_step(mps_ctx* ctx, int32_t nsteps, int32_t pressure_route);
 

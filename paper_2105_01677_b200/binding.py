@@ -24,12 +24,13 @@ RADIUS_N, RADIUS_LAP = 0, 1
 
 FIELDS = {"x": 0, "y": 1, "z": 2, "u": 3, "v": 4, "w": 5, "n": 6, "p": 7, "ax": 8, "ay": 9,
           "az": 10, "nut": 11, "b": 12, "phat": 13, "gx": 14, "gy": 15, "gz": 16, "xcg": 17,
+          "dndt": 18, "nk": 19, "dndtk": 20,
           "type": 32, "phase": 33, "bc": 34, "key": 35}
 TIMERS = ["bin_sort", "bin_list", "viscosity", "predict", "density", "pressure_explicit",
           "ppe_setup", "cg_spmv", "cg_update", "gradient", "correct"]
 
 # Names the header declares (checked by tests/test_abi.py against include/mps_b200.h).
-SYMBOLS = ["mps_init", "mps_init_host", "mps_destroy", "mps_bin", "mps_density", "mps_viscosity",
+SYMBOLS = ["mps_init", "mps_init_host", "mps_destroy", "mps_bin", "mps_density", "mps_dndt", "mps_viscosity",
            "mps_predict", "mps_pressure_explicit", "mps_pressure_ppe", "mps_gradient",
            "mps_correct", "mps_step", "mps_step_host", "mps_upload_host", "mps_download_host",
            "mps_get_field", "mps_set_field",
@@ -44,7 +45,8 @@ class MpsParams(C.Structure):
         ("dim", C.c_int32), ("n_phases", C.c_int32), ("cg_maxit", C.c_int32),
         ("grad_variant", C.c_int32), ("clamp_negative_p", C.c_int32),
         ("rho_pair_mean", C.c_int32), ("nu_pair_mean", C.c_int32), ("key_mode", C.c_int32),
-        ("cell_div", C.c_int32), ("max_neighbours", C.c_int32), ("reserved_i", C.c_int32 * 2),
+        ("cell_div", C.c_int32), ("max_neighbours", C.c_int32), ("ppe_source", C.c_int32),
+        ("ppe_laplacian", C.c_int32),
         ("l0", C.c_double), ("re_n", C.c_double), ("re_grad", C.c_double),
         ("re_lap", C.c_double), ("dt", C.c_double), ("g", C.c_double * 3),
         ("rho", C.c_double * 2), ("nu", C.c_double * 2), ("c0", C.c_double),
@@ -80,6 +82,8 @@ def make_params(p: Dict[str, object]) -> MpsParams:
               "nu_pair_mean", "cell_div", "max_neighbours"):
         setattr(s, k, int(p[k]))
     s.key_mode = int(p.get("key_mode", 0))
+    s.ppe_source = int(p.get("ppe_source", 0))
+    s.ppe_laplacian = int(p.get("ppe_laplacian", 0))
     for k in ("l0", "re_n", "re_lap", "dt", "c0", "gamma", "beta", "compress", "ppe_relax",
               "cg_rtol", "cs", "n0_n", "n0_lap"):
         setattr(s, k, float(p[k]))
@@ -105,6 +109,7 @@ def _load():
     for nm in ("mps_bin", "mps_density", "mps_viscosity", "mps_predict", "mps_pressure_explicit",
                "mps_gradient", "mps_correct", "mps_sync"):
         getattr(L, nm).argtypes = [vp]
+    L.mps_dndt.argtypes = [vp, i32]
     L.mps_pressure_ppe.argtypes = [vp, C.POINTER(i32), C.POINTER(dbl)]
     L.mps_step.argtypes = [vp, i32, i32]
     L.mps_step_host.argtypes = [C.POINTER(MpsParams), i64] + [vp] * 6 + [vp, vp, vp, i32, i32,
@@ -197,6 +202,7 @@ class Mps:
     # ---- the path --------------------------------------------------------------
     def bin(self): self._ck(lib.mps_bin(self.h))
     def density(self): self._ck(lib.mps_density(self.h))
+    def dndt(self, keep: bool = False): self._ck(lib.mps_dndt(self.h, 1 if keep else 0))
     def viscosity(self): self._ck(lib.mps_viscosity(self.h))
     def predict(self): self._ck(lib.mps_predict(self.h))
     def pressure_explicit(self): self._ck(lib.mps_pressure_explicit(self.h))

@@ -163,7 +163,8 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
                           const double4* __restrict__ vel_in, const uint32_t* __restrict__ tp_in,
                           double4* __restrict__ pos_out, double4* __restrict__ vel_out,
                           uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out,
-                          uint32_t* __restrict__ ent_out) {
+                          uint32_t* __restrict__ ent_out, const double2* __restrict__ keep_in,
+                          double2* __restrict__ keep_out) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   uint32_t c = key[s];
@@ -181,6 +182,7 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
   const uint32_t ty = tj & 0xff;
   tp_out[f] = tj;
   oid_out[f] = me;
+  if (keep_in) keep_out[f] = keep_in[src];  // (n^k, (Dn/Dt)^k) of Eq. 17 follow their particle
   // the neighbour-row entry that names this particle (flags of mps_internal.h)
   ent_out[f] = f | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
                ((tj & 0x100) ? NB_PHASE1 : 0u);
@@ -445,7 +447,8 @@ __global__ void k_count_ghosts(int n, int ncells, const uint32_t* __restrict__ c
 __global__ void k_get_f64(int n, int field, int order, const double4* __restrict__ pos4,
                           const double4* __restrict__ vel4, const double4* __restrict__ acc4,
                           const double4* __restrict__ grad4, const double* __restrict__ scalar,
-                          const uint32_t* __restrict__ oid, double* __restrict__ dst) {
+                          const double2* __restrict__ keep2, const uint32_t* __restrict__ oid,
+                          double* __restrict__ dst) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double v;
@@ -462,6 +465,8 @@ __global__ void k_get_f64(int n, int field, int order, const double4* __restrict
     case MPS_F_GX: v = grad4[i].x; break;
     case MPS_F_GY: v = grad4[i].y; break;
     case MPS_F_GZ: v = grad4[i].z; break;
+    case MPS_F_NK: v = keep2[i].x; break;
+    case MPS_F_DNDTK: v = keep2[i].y; break;
     default: v = scalar[i]; break;
   }
   dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = v;
@@ -469,7 +474,8 @@ __global__ void k_get_f64(int n, int field, int order, const double4* __restrict
 __global__ void k_set_f64(int n, int field, int order, double4* __restrict__ pos4,
                           double4* __restrict__ vel4, double4* __restrict__ acc4,
                           double4* __restrict__ grad4, double* __restrict__ scalar,
-                          const uint32_t* __restrict__ oid, const double* __restrict__ src) {
+                          double2* __restrict__ keep2, const uint32_t* __restrict__ oid,
+                          const double* __restrict__ src) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double v = src[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i];
@@ -486,6 +492,8 @@ __global__ void k_set_f64(int n, int field, int order, double4* __restrict__ pos
     case MPS_F_GX: grad4[i].x = v; break;
     case MPS_F_GY: grad4[i].y = v; break;
     case MPS_F_GZ: grad4[i].z = v; break;
+    case MPS_F_NK: keep2[i].x = v; break;
+    case MPS_F_DNDTK: keep2[i].y = v; break;
     default: scalar[i] = v; break;
   }
 }
@@ -579,7 +587,8 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
              c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key);
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_reorder, div_up(n, TPB), TPB, n, nc, c->key, c->cell_start,
              c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
-             c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent);
+             c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent,
+             c->prm.ppe_source == 2 ? c->keep2[cur] : nullptr, c->keep2[nxt]);
   c->cur = nxt;
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
   if (c->prm.cell_div == 1 && !c->rows_by_warp) {
@@ -604,6 +613,7 @@ static const double* scalar_field(mps_ctx* c, int field) {
     case MPS_F_B: return c->b;
     case MPS_F_PHAT: return c->phat;
     case MPS_F_XCG: return c->cg_x;
+    case MPS_F_DNDT: return c->dndt;
   }
   return nullptr;
 }
@@ -611,9 +621,10 @@ static const double* scalar_field(mps_ctx* c, int field) {
 int mpsk_get_field(mps_ctx* c, int field, void* dst, int order) {
   int n = (int)c->n;
   int cur = c->cur;
-  if (field >= 0 && field <= MPS_F_XCG) {
+  if (field >= 0 && field <= MPS_F_DNDTK) {
     MPS_LAUNCH(c, MPS_T_BIN_SORT, k_get_f64, div_up(n, TPB), TPB, n, field, order, c->pos4[cur],
-               c->vel4[cur], c->acc4, c->grad4, scalar_field(c, field), c->oid[cur], (double*)dst);
+               c->vel4[cur], c->acc4, c->grad4, scalar_field(c, field), c->keep2[cur], c->oid[cur],
+               (double*)dst);
     return MPS_OK;
   }
   if (field >= MPS_I_TYPE && field <= MPS_I_KEY) {
@@ -627,10 +638,10 @@ int mpsk_get_field(mps_ctx* c, int field, void* dst, int order) {
 int mpsk_set_field(mps_ctx* c, int field, const void* src, int order) {
   int n = (int)c->n;
   int cur = c->cur;
-  if (field >= 0 && field <= MPS_F_XCG) {
+  if (field >= 0 && field <= MPS_F_DNDTK) {
     MPS_LAUNCH(c, MPS_T_BIN_SORT, k_set_f64, div_up(n, TPB), TPB, n, field, order, c->pos4[cur],
-               c->vel4[cur], c->acc4, c->grad4, (double*)scalar_field(c, field), c->oid[cur],
-               (const double*)src);
+               c->vel4[cur], c->acc4, c->grad4, (double*)scalar_field(c, field), c->keep2[cur],
+               c->oid[cur], (const double*)src);
     if (field <= MPS_F_Z) { c->binned = false; c->ppe_ready = false; }
     if (field == MPS_F_P) c->posw_is_p = false;
     return MPS_OK;

@@ -41,6 +41,8 @@ struct PpeArgs {
   double4* pos4;  // .w: CG residual r during the solve, pressure at exit
   const uint32_t* tp;
   const double* dens;
+  const double* dndt;      // (Dn/Dt)* (ppe_source >= 1)
+  const double2* keep2;    // (n^k, (Dn/Dt)^k) (ppe_source == 2)
   int8_t* bc;
   double* b;
   double* x;
@@ -145,6 +147,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
   const uint32_t nf = live ? cn[i] : 0u;
   const uint32_t m = live ? nf + co[i] : 0u;
   const double rho_i = TWO_PHASE ? kc.rho[(tp[i] >> 8) & 1] : kc.rho[0];
+  const bool hl = kc.ppe_laplacian == 1;
   double s = 0.0;
   // batches of PPE_ILP entries per lane: entry loads, then gathers, then arithmetic, so the
   // L2 round trips of one batch overlap (the L1 is invalidated by every grid barrier).
@@ -167,7 +170,9 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
     for (int u = 0; u < PPE_ILP; ++u) {
       const double dx = q[u].x - pi.x, dy = q[u].y - pi.y, dz = q[u].z - pi.z;
       const double r2 = dx * dx + dy * dy + dz * dz;
-      double w = fma(kc.re_lap, rsqrt_f64(r2), -1.0);
+      const double ir = rsqrt_f64(r2);
+      // Eq. 10 form: A_lap (re/r - 1); MPS-HL (Eq. 16, Q23): (2 re / n0) / r^3
+      double w = hl ? ir * ir * ir : fma(kc.re_lap, ir, -1.0);
       if (TWO_PHASE) {
         const double rho_j = kc.rho[(e[u] & NB_PHASE1) ? 1 : 0];
         const double rij =
@@ -180,7 +185,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
   }
   s = group_sum<L>(s);
   if (!TWO_PHASE) s *= 1.0 / kc.rho[0];
-  return fma(kc.A_lap, s, kc.compress_dt2 * pi.w);
+  return fma(hl ? kc.hl_c : kc.A_lap, s, kc.compress_dt2 * pi.w);
 }
 
 // ---- the persistent solve -------------------------------------------------------------
@@ -211,7 +216,17 @@ k_ppe_cg(KConst kc, PpeArgs a) {
       else {
         f = 0;
         ++n_rows;
-        bi = kc.relax_dt2 * (ni - kc.n0_n) / kc.n0_n;
+        if (kc.ppe_source == 0) {         // Eq. 8 divided by -rho (Q5)
+          bi = kc.relax_dt2 * (ni - kc.n0_n) / kc.n0_n;
+        } else if (kc.ppe_source == 1) {  // MPS-HS, Eq. 15 (Q22)
+          bi = kc.relax / (kc.n0_n * kc.dt) * a.dndt[i];
+        } else {                          // HS + error-compensating parts, Eq. 17-18 (Q22)
+          const double2 kk = a.keep2[i];
+          const double alpha = (kk.x - kc.n0_n) / kc.n0_n;
+          const double beta = kc.dt / kc.n0_n * kk.y;
+          const double ecs = fabs(alpha) * (kk.y / kc.n0_n) + fabs(beta) * (alpha / kc.dt);
+          bi = kc.relax / kc.dt * (a.dndt[i] / kc.n0_n + ecs);
+        }
       }
       a.bc[i] = f;
       a.b[i] = bi;
@@ -446,7 +461,7 @@ int mpsk_ppe_plan(mps_ctx* c) {
 int mpsk_pressure_ppe(mps_ctx* c) {
   const int cur = c->cur;
   PpeArgs a;
-  a.pos4 = c->pos4[cur]; a.tp = c->tp[cur]; a.dens = c->dens; a.bc = c->bc; a.b = c->b;
+  a.pos4 = c->pos4[cur]; a.tp = c->tp[cur]; a.dens = c->dens; a.dndt = c->dndt; a.keep2 = c->keep2[cur]; a.bc = c->bc; a.b = c->b;
   a.x = c->cg_x; a.pv = c->cg_p; a.sv = c->cg_s; a.wv = c->cg_w; a.p = c->p;
   a.nbr = c->nbr; a.cn = c->cn; a.co = c->co; a.rows = c->cg_rows; a.bcount = c->cg_bcount;
   a.part = c->cg_part; a.cg = c->cg; a.bar = c->cg_bar;

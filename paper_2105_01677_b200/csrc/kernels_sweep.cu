@@ -37,6 +37,37 @@ k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restric
   if (row_live && sub == 0) dens[i] = s;
 }
 
+// ---------------------------------------------------- NEXT-1: Dn/Dt (MPS-HS) ---
+// Dn/Dt_i = d/dt sum_j (re_n / r_ij - 1) = -sum_{j in N(i, re_n)} re_n / r^3 (x_ij . u_ij),
+// x_ij = x_j - x_i, u_ij = u_j - u_i; walls and dummies hold u = 0 in vel4 (P:224-228
+// Eq. 15; sign: Q22).  keep: also store (n_i, Dn/Dt_i) as the start-of-step pair of Eq. 17.
+__global__ void __launch_bounds__(TPB)
+k_dndt(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ vel4,
+       const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn,
+       const double* __restrict__ dens, double* __restrict__ dndt, double2* __restrict__ keep2) {
+  ROW_GROUP(i, sub);
+  const double4 pi = pos4[ii];
+  const double4 vi = vel4[ii];
+  const uint32_t* row = row_ptr(nbr, kc.stride, ii);
+  const uint32_t m = row_live ? cn[ii] : 0u;
+  double s = 0.0;
+  for (uint32_t k = sub; k < m; k += L) {
+    const uint32_t j = row[k] & NB_INDEX;
+    const double4 q = pos4[j];
+    const double4 vj = vel4[j];
+    const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double ir = rsqrt_f64(r2);
+    const double xu = dx * (vj.x - vi.x) + dy * (vj.y - vi.y) + dz * (vj.z - vi.z);
+    s = fma(ir * ir * ir, xu, s);
+  }
+  s = -kc.re_n * group_sum<L>(s);
+  if (row_live && sub == 0) {
+    if (keep2) keep2[i] = make_double2(dens[i], s);
+    else dndt[i] = s;
+  }
+}
+
 // --------------------------------------------------- S5 Smagorinsky + nu_eff ---
 // G_ab = (d/n0) sum (u_b,j - u_b,i)(x_a,j - x_a,i) / r^2 w(r) over N(i, re_n);
 // S = (G + G^T)/2; nu_t = (Cs l0)^2 sqrt(2 S:S) (Eq. 13; Q10).
@@ -297,6 +328,14 @@ int mpsk_density(mps_ctx* c) {
   int n = (int)c->n;
   MPS_LAUNCH(c, MPS_T_DENSITY, k_density, group_grid(n), TPB, c->kc, c->pos4[c->cur], c->nbr, c->cn,
              c->dens);
+  return MPS_OK;
+}
+
+int mpsk_dndt(mps_ctx* c, int keep) {
+  int n = (int)c->n;
+  int cur = c->cur;
+  MPS_LAUNCH(c, MPS_T_DENSITY, k_dndt, group_grid(n), TPB, c->kc, c->pos4[cur], c->vel4[cur], c->nbr,
+             c->cn, c->dens, c->dndt, keep ? c->keep2[cur] : nullptr);
   return MPS_OK;
 }
 

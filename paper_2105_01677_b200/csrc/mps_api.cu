@@ -62,7 +62,7 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->tmp_oid); cudaFree(c->cell_count); cudaFree(c->cell_start); cudaFree(c->scan_tmp);
   cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co);
   cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
-  cudaFree(c->phat); cudaFree(c->grad4); cudaFree(c->bc);
+  cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
   cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
   cudaFree(c->cg_rows); cudaFree(c->cg_bcount); cudaFree(c->cg_bar);
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
@@ -85,6 +85,8 @@ static int check_params(const mps_params* p, int64_t n) {
   if (p->n_phases < 1 || p->n_phases > 2) return fail(nullptr, MPS_ERR_ARG, "n_phases must be 1 or 2");
   if (p->max_neighbours < 1 || p->max_neighbours > 4096)
     return fail(nullptr, MPS_ERR_ARG, "max_neighbours must be in [1, 4096]");
+  if (p->ppe_source < 0 || p->ppe_source > 2) return fail(nullptr, MPS_ERR_ARG, "ppe_source must be 0..2");
+  if (p->ppe_laplacian < 0 || p->ppe_laplacian > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_laplacian must be 0 or 1");
   if (p->grad_variant < 0 || p->grad_variant > 2) return fail(nullptr, MPS_ERR_ARG, "grad_variant must be 0..2");
   if (!(p->rho[0] > 0) || (p->n_phases == 2 && !(p->rho[1] > 0)))
     return fail(nullptr, MPS_ERR_ARG, "densities must be positive");
@@ -136,6 +138,9 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.relax_dt2 = prm->ppe_relax / (prm->dt * prm->dt);
   k.cs_l0_sq = (prm->cs * prm->l0) * (prm->cs * prm->l0);
   k.d_over_n0 = (double)prm->dim / k.n0_n;
+  k.relax = prm->ppe_relax;
+  k.hl_c = 2.0 * prm->re_lap / k.n0_lap;
+  k.ppe_source = prm->ppe_source; k.ppe_laplacian = prm->ppe_laplacian;
   c->h = std::max(prm->re_n, prm->re_lap) / prm->cell_div;
   k.inv_h = 1.0 / c->h;
   int64_t ncells = 1;
@@ -170,7 +175,8 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
   A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
   A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
-  A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->grad4, N)); A(dalloc(&c->bc, N));
+  A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->dndt, N));
+  A(dalloc(&c->keep2[0], N)); A(dalloc(&c->keep2[1], N)); A(dalloc(&c->grad4, N)); A(dalloc(&c->bc, N));
   A(dalloc(&c->cg_x, N)); A(dalloc(&c->cg_p, N)); A(dalloc(&c->cg_s, N)); A(dalloc(&c->cg_w, N));
   A(dalloc(&c->cg_part, (size_t)2 * (c->sm_count * 8 + 8)));
   A(dalloc(&c->cg_rows, N)); A(dalloc(&c->cg_bcount, (size_t)2 * (c->sm_count * 8 + 8)));
@@ -207,7 +213,8 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   cudaMemsetAsync(c->cg_bar, 0, sizeof(GridBar), s);
   cudaMemsetAsync(c->cg_rows, 0, N * 4, s);
   cudaMemsetAsync(c->flags, 0, sizeof(DevFlags), s);
-  double* zero_d[] = {c->dens, c->p, c->nut, c->b, c->phat, c->cg_x, c->cg_p, c->cg_s, c->cg_w};
+  double* zero_d[] = {c->dens, c->p, c->nut, c->b, c->phat, c->dndt, c->cg_x, c->cg_p, c->cg_s, c->cg_w};
+  for (int b = 0; b < 2; ++b) cudaMemsetAsync(c->keep2[b], 0, N * sizeof(double2), s);
   for (double* z : zero_d) cudaMemsetAsync(z, 0, N * sizeof(double), s);
   cudaMemsetAsync(c->acc4, 0, N * sizeof(double4), s);
   cudaMemsetAsync(c->grad4, 0, N * sizeof(double4), s);
@@ -346,6 +353,12 @@ int mps_density(mps_ctx* c) {
   CK(cudaGetLastError());
   return MPS_OK;
 }
+int mps_dndt(mps_ctx* c, int32_t keep) {
+  NEED_BIN(c);
+  mpsk_dndt(c, keep ? 1 : 0);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
 int mps_viscosity(mps_ctx* c) {
   NEED_BIN(c);
   mpsk_viscosity(c);
@@ -392,12 +405,20 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
   if (nsteps < 0 || (route != MPS_ROUTE_EXPLICIT && route != MPS_ROUTE_PPE))
     return fail(c, MPS_ERR_ARG, "bad nsteps or pressure_route");
   int first_err = MPS_OK;
+  const bool ecs = route == MPS_ROUTE_PPE && c->prm.ppe_source == 2;
+  const bool hs = route == MPS_ROUTE_PPE && c->prm.ppe_source >= 1;
   for (int s = 0; s < nsteps; ++s) {
-    mpsk_bin(c, /*fluid_rows_only=*/true);  // viscosity and nu_t are computed for fluid i only
+    // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
+    mpsk_bin(c, /*fluid_rows_only=*/!ecs);
+    if (ecs) {
+      mpsk_density(c);
+      mpsk_dndt(c, 1);
+    }
     mpsk_viscosity(c);
     mpsk_predict(c);
     mpsk_bin(c);
     mpsk_density(c);
+    if (hs) mpsk_dndt(c, 0);
     if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
     else {
       int rc = mpsk_pressure_ppe(c);

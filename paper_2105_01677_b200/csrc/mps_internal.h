@@ -65,6 +65,8 @@ struct KConst {  // by-value kernel parameter
   double rho[2], nu[2];
   double c0, gamma, beta, compress_dt2, relax_dt2;
   double cs_l0_sq, d_over_n0;
+  double relax, hl_c;  // ppe_relax; 2 re_lap / n0_lap (Eq. 16)
+  int ppe_source, ppe_laplacian;
   double dmin[3], inv_h;
   int nx, ny, nz, ncells;
   int R_lap;  // cells to each side for re_lap
@@ -109,6 +111,8 @@ struct mps_ctx {
   double* nut = nullptr;
   double* b = nullptr;
   double* phat = nullptr;
+  double* dndt = nullptr;
+  double2* keep2[2] = {nullptr, nullptr};  // (n^k, (Dn/Dt)^k) of Eq. 17, carried through the re-sort
   double4* grad4 = nullptr;
   int8_t* bc = nullptr;
   // CG vectors
@@ -169,6 +173,7 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only = false);
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
                          uint32_t* tmp);
 int mpsk_density(mps_ctx* c);
+int mpsk_dndt(mps_ctx* c, int keep);
 int mpsk_viscosity(mps_ctx* c);
 int mpsk_predict(mps_ctx* c);
 int mpsk_pressure_explicit(mps_ctx* c);

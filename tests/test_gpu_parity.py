@@ -461,3 +461,56 @@ def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx):
         m = r2 < re * re
         m[i] = False
         assert cnt_l[i] == m.sum()
+
+
+# ------------------------------- NEXT-1: higher-order source, Laplacian, ECS (Eq. 15-18) ---
+def test_dndt(B, O):
+    s = scenes.small_tank(shuffle=True)
+    g, o = _pair(B, O, s)
+    g.dndt(); o.dndt()
+    ref = o.get("dndt")
+    assert np.abs(ref).max() > 0
+    assert relerr(g.get("dndt"), ref, 1e-30) <= TOL
+
+
+@pytest.mark.parametrize("src,lap", [(1, 0), (2, 0), (0, 1), (2, 1)])
+def test_ppe_higher_order_source_and_laplacian(B, O, src, lap):
+    s = scenes.small_tank(shuffle=True)
+    over = dict(ppe_source=src, ppe_laplacian=lap)
+    g, o = _pair(B, O, s, **over)
+    # start-of-step pair of Eq. 17 at r^k, u^k
+    g.density(); g.dndt(keep=True)
+    o.density(); o.set("n_k", o.get("n")); o.dndt(keep=True)
+    assert relerr(g.get("nk"), o.get("n_k"), 1.0) <= TOL
+    assert relerr(g.get("dndtk"), o.get("dndt_k"), 1e-30) <= TOL
+    o.viscosity(); o.predict()
+    inject(g, o, ("x", "y", "z", "u", "v", "w"))
+    g.set("nk", o.get("n_k")); g.set("dndtk", o.get("dndt_k"))
+    g.bin()                      # with ECS the kept pair follows its particle through the re-sort
+    if src == 2:
+        assert np.array_equal(g.get("nk"), o.get("n_k"))
+        assert np.array_equal(g.get("dndtk"), o.get("dndt_k"))
+    g.density(); g.dndt(); o.density(); o.dndt()
+    g.set("n", o.get("n")); g.set("dndt", o.get("dndt"))
+    it_g, relres_g = g.pressure_ppe()
+    o.ppe_flags(); o.ppe_rhs()
+    bc = o.get("bc")
+    assert np.array_equal(g.get("bc"), bc)
+    b = o.get("b")
+    assert relerr(g.get("b"), b, 1e-30) <= 1e-13
+    rows = bc == 0
+    v = np.where(rows, np.random.default_rng(0).standard_normal(s.n), 0.0)
+    assert relerr(g.ppe_apply(v), o.ppe_apply(v), 1e-30) <= TOL
+    x = g.get("xcg")
+    true_rel = np.linalg.norm(b - o.ppe_apply(x)) / np.linalg.norm(b)
+    assert relres_g <= 1e-8 and true_rel <= 2e-8
+    it_o = o.ppe_solve(o.params["cg_rtol"], 5000)
+    assert abs(it_g - it_o) <= 3
+
+
+@pytest.mark.parametrize("src,lap", [(1, 1), (2, 1)])
+def test_trajectory_small_tank_hs_hl_ecs(B, O, src, lap):
+    s = scenes.small_tank(shuffle=True)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 12, 1, ppe_source=src, ppe_laplacian=lap)
+    print(f"small tank, 12 PPE steps, source {src} laplacian {lap}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
+    assert eL <= 1e-7 and moved > 0.01
