@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="scene 1..5 (SURVEY.md 8(d)); default 2 = BASELINE configs[1]")
+    ap.add_argument("--config", type=int, default=2, help="scene 1..5 (SURVEY.md 8(d)); default 2 = BASELINE configs[1]; 6 = paper-shaped 2D dam break")
     ap.add_argument("--sweep-index", type=int, default=0, help="size index 0..4 of scene 5")
     ap.add_argument("--route", default=None, choices=[None, "explicit", "ppe"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -66,14 +66,14 @@ def peaks():
 
 def workload_name(args, scene, route):
     tag = f"scene{args.config}"
-    if args.config == 5:
+    if args.config >= 5:
         tag += f"[{args.sweep_index}]"
     return f"{tag}:{scene.name}:N={scene.n}:fluid={scene.n_fluid}:route={ROUTE_NAME[route]}"
 
 
 def make_scene(args, rank=0):
     from paper_2105_01677_b200 import scenes
-    seed = scenes.BASE_SEED + args.config + (args.sweep_index if args.config == 5 else 0) + 1000 * rank
+    seed = scenes.BASE_SEED + args.config + (args.sweep_index if args.config >= 5 else 0) + 1000 * rank
     s = scenes.make_scene(args.config, seed=seed, sweep_index=args.sweep_index)
     route = s.route if args.route is None else {"explicit": 0, "ppe": 1}[args.route]
     return s, route
@@ -370,7 +370,8 @@ def run_b200(args):
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args, scene, route),
-                       "baseline_config": f"BASELINE.json configs[{args.config - 1}]",
+                       "baseline_config": (f"BASELINE.json configs[{args.config - 1}]" if args.config <= 5 else
+                                           "none: the paper's own 2D dam-break shape (PAPER.md:397), context only"),
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
                        "l2": "flushed before every timed step (256 MiB write, untimed)",
                        "timing": "CUDA events on the ctx stream around each mps_step(1), summed; max over ranks"},

@@ -70,7 +70,8 @@ enum {
 /* Parameters: a POD struct copied at mps_init.  Every reading of DESIGN.md
  * section 3 is a field here.  Defaults in parentheses are what the tests use. */
 typedef struct mps_params {
-  int32_t dim;              /* 3 (only 3 is supported; P:292 item 1 also offers 2) */
+  int32_t dim;              /* 3, or 2 (P:292 item 1): d of Eq. 10/14 and the lattice sums of n0, lambda;
+                               in 2D the caller keeps z constant, w = 0 and g[2] = 0 */
   int32_t n_phases;         /* 1 or 2 */
   int32_t cg_maxit;         /* (2000) then MPS_ERR_NOCONV; Q15 */
   int32_t grad_variant;     /* 0: (p_j - phat_i) standard [8]; 1: Eq. 14 as printed; 2: (p_i + p_j); Q13 */

@@ -75,7 +75,9 @@ static void free_all(mps_ctx* c) {
 static int check_params(const mps_params* p, int64_t n) {
   if (!p) return fail(nullptr, MPS_ERR_ARG, "params is NULL");
   if (n <= 0 || n > (int64_t)NB_INDEX) return fail(nullptr, MPS_ERR_ARG, "n must be in [1, 2^29)");
-  if (p->dim != 3) return fail(nullptr, MPS_ERR_ARG, "only dim = 3 is supported");
+  if (p->dim != 2 && p->dim != 3) return fail(nullptr, MPS_ERR_ARG, "dim must be 2 or 3");
+  if (p->dim == 2 && p->ppe_laplacian == 1)
+    return fail(nullptr, MPS_ERR_ARG, "the higher-order Laplacian (Eq. 16) is given for 3D only");
   if (!(p->l0 > 0) || !(p->re_n > 0) || !(p->re_lap > 0) || !(p->dt > 0))
     return fail(nullptr, MPS_ERR_ARG, "l0, re_n, re_lap and dt must be positive");
   if (p->re_grad != p->re_n) return fail(nullptr, MPS_ERR_ARG, "re_grad must equal re_n");

@@ -196,6 +196,49 @@ def fluid_blob(l0: float, m: Tuple[int, int, int], seed: int = 0, jitter: float 
     return s
 
 
+def dam_break_2d(l0: float, tank: Tuple[int, int], fluid: Tuple[int, int], seed: int,
+                 name: str = "dam_break_2d", jitter: float = 1.0e-3, shuffle: bool = False) -> Scene:
+    """Two-dimensional dam break in the x-y plane (gravity along -y, z = 0 for every particle):
+    the shape of the paper's own timed scenes (section 5.2 and PAPER.md:397:
+    column height = 2 x column length, floor = 4 x column length).  Walls as in 3D: 3 layers on
+    the floor and both sides, innermost WALL, outer two DUMMY; open top."""
+    nx, ny = tank
+    L = 3
+    ix = np.arange(-L, nx + L, dtype=np.int64)
+    iy = np.arange(-L, ny, dtype=np.int64)
+    Y, X = np.meshgrid(iy, ix, indexing="ij")  # y slowest, x fastest
+    X = X.ravel()
+    Y = Y.ravel()
+    inside = (X >= 0) & (X < nx) & (Y >= 0)
+    in_wall_box = (X >= -1) & (X < nx + 1) & (Y >= -1)
+    typ = np.full(X.shape, -1, dtype=np.int32)
+    typ[(X >= 0) & (X < fluid[0]) & (Y >= 0) & (Y < fluid[1])] = FLUID
+    typ[~inside & in_wall_box] = WALL
+    typ[~inside & ~in_wall_box] = DUMMY
+    keep = typ >= 0
+    X, Y, typ = X[keep], Y[keep], typ[keep]
+    x = (X.astype(np.float64) + 0.5) * l0
+    y = (Y.astype(np.float64) + 0.5) * l0
+    fl = np.nonzero(typ == FLUID)[0]
+    if jitter > 0.0 and fl.size:
+        rng = np.random.Generator(np.random.PCG64(seed))
+        d = rng.uniform(-jitter * l0, jitter * l0, size=(fl.size, 2))
+        x[fl] += d[:, 0]
+        y[fl] += d[:, 1]
+    n = x.shape[0]
+    if shuffle:
+        prm = np.random.Generator(np.random.PCG64(seed ^ 0x5EED)).permutation(n)
+        x, y, typ = x[prm], y[prm], typ[prm]
+    p = default_params(l0)
+    p.update(dim=2, g=(0.0, -9.81, 0.0))
+    p["domain_min"] = (-L * l0, -L * l0, -0.5 * l0)
+    p["domain_max"] = ((nx + L) * l0, ny * l0, 0.5 * l0)
+    zeros = np.zeros(n, dtype=np.float64)
+    return Scene(name=name, x=np.ascontiguousarray(x), y=np.ascontiguousarray(y), z=zeros.copy(),
+                 u=zeros.copy(), v=zeros.copy(), w=zeros.copy(), type=np.ascontiguousarray(typ),
+                 phase=np.zeros(n, dtype=np.int32), params=p)
+
+
 SWEEP_M = (23, 40, 69, 89, 147)  # config 5: N = 66k / 250k / 1.0M / 2.0M / 7.9M
 
 
@@ -234,6 +277,13 @@ def make_scene(config: int, seed: Optional[int] = None, shuffle: bool = False,
         s = dam_break(0.005, (4 * m, m, 2 * m), (2 * m, m, m), seed,
                       f"config5_sweep_m{m}", shuffle=shuffle)
         s.route, s.steps = 0, 50
+    elif config == 6:
+        # not a BASELINE.json config: the paper's own timed workload shape (2D dam break,
+        # PAPER.md:397, "about 1 fps at about 200,000 particles"), context only
+        c = (100, 316, 700)[sweep_index] if sweep_index < 3 else 316
+        s = dam_break_2d(0.005, (4 * c, 3 * c), (c, 2 * c), seed, f"paper_shape_2d_dam_c{c}",
+                         shuffle=shuffle)
+        s.route, s.steps = 1, 50
     else:
         raise ValueError(f"unknown config {config}")
     return s

@@ -514,3 +514,37 @@ def test_trajectory_small_tank_hs_hl_ecs(B, O, src, lap):
     eL, el0, moved, g, o = _trajectory(B, O, s, 12, 1, ppe_source=src, ppe_laplacian=lap)
     print(f"small tank, 12 PPE steps, source {src} laplacian {lap}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
     assert eL <= 1e-7 and moved > 0.01
+
+
+# ----------------------------------------------------- NEXT-3 (part): 2D mode ---
+@pytest.mark.parametrize("rows", ["warp", "cell"])
+def test_2d_bin_neighbours_and_fields(B, O, rows, monkeypatch):
+    monkeypatch.setenv("MPS_B200_ROWS", rows)
+    s = scenes.dam_break_2d(0.01, (60, 40), (20, 30), seed=9, shuffle=True)
+    o = moved_state(O, s, 3)
+    g = B.Mps(s)
+    inject(g, o, ("x", "y", "z", "u", "v", "w"))
+    key, perm, cs = o.bin()
+    g.bin()
+    assert g.grid() == o.grid() and g.grid()[2] == 1
+    assert np.array_equal(g.perm(), perm) and np.array_equal(g.cell_start(), cs)
+    for rid, re in ((B.RADIUS_N, s.params["re_n"]), (B.RADIUS_LAP, s.params["re_lap"])):
+        co, io = o.neighbours(re)
+        cg, ig = g.neighbours(rid)
+        assert np.array_equal(cg, co) and np.array_equal(ig, io)
+    c = g.constants(); oc = o.constants()
+    for k in ("n0_n", "n0_lap", "lam"):
+        assert abs(c[k] - oc[k]) <= 1e-14 * oc[k]
+    g.density(); o.density()
+    assert relerr(g.get("n"), o.get("n"), oc["n0_n"]) <= TOL
+    g.viscosity(); o.viscosity()
+    assert vec_relerr([g.get(k) for k in ("ax", "ay", "az")], [o.get(k) for k in ("ax", "ay", "az")], 9.81) <= TOL
+
+
+@pytest.mark.parametrize("route", [0, 1])
+def test_2d_trajectory_20_steps(B, O, route):
+    s = scenes.dam_break_2d(0.01, (60, 40), (20, 30), seed=9, shuffle=True)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, route)
+    print(f"2D dam break, 20 steps, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
+    assert eL <= 1e-7 and moved > 0.02
+    assert (g.get("z") == 0).all() and (g.get("w") == 0).all()

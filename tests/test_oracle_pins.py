@@ -574,3 +574,74 @@ def test_HL_operator_closed_form_symmetry_and_dense_solve():
     assert it > 0
     xd = np.linalg.solve(A, b)
     assert np.linalg.norm(o.get("xcg")[rows] - xd) <= 1e-9 * np.linalg.norm(xd)
+
+
+# ---- NEXT-3 (part): two-dimensional mode (P:292 item 1; the paper's timed scenes are 2D) ----
+def _lattice_2d(m, l0=L0):
+    i = np.arange(m)
+    Y, X = np.meshgrid(i, i, indexing="ij")
+    x = (X.ravel() + 0.5) * l0; y = (Y.ravel() + 0.5) * l0
+    s = scenes.dam_break_2d(l0, (m, m), (m, m), seed=1, jitter=0.0)
+    keep = s.type == scenes.FLUID
+    for k in ("x", "y", "z", "u", "v", "w", "type", "phase"):
+        setattr(s, k, np.ascontiguousarray(getattr(s, k)[keep]))
+    pad = 8.0 * l0
+    s.params["domain_min"] = (-pad, -pad, -0.5 * l0)
+    s.params["domain_max"] = (m * l0 + pad, m * l0 + pad, 0.5 * l0)
+    assert np.allclose(np.sort(s.x), np.sort(x)) and np.allclose(np.sort(s.y), np.sort(y))
+    return s
+
+
+def test_2d_density_laplacian_and_gradient_closed_forms():
+    m = 12
+    s = _lattice_2d(m)
+    ix = np.rint(s.x / L0 - 0.5).astype(int); iy = np.rint(s.y / L0 - 0.5).astype(int)
+    core = (ix >= 4) & (ix < m - 4) & (iy >= 4) & (iy < m - 4)
+    o = O.Oracle(s, nu=(1.0, 1.0), g=(0.0, 0.0, 0.0))
+    c = o.constants()
+    assert abs(c["n0_n"] - GOLD["n0_2d_2.1"]) <= 1e-12 * GOLD["n0_2d_2.1"]
+    assert abs(c["n0_lap"] - GOLD["n0_2d_3.1"]) <= 1e-12 * GOLD["n0_2d_3.1"]
+    assert abs(c["lam"] / L0 ** 2 - GOLD["lambda_2d_3.1"]) <= 1e-12 * GOLD["lambda_2d_3.1"]
+    o.bin(); o.density()
+    assert np.allclose(o.get("n")[core], GOLD["n0_2d_2.1"], rtol=1e-12)
+    cnt, _ = o.neighbours(s.params["re_lap"])
+    assert (cnt[core] == GOLD["count_2d_3.1"]).all()
+    # Eq. 10 with d = 2 on a quadratic: 2 (a_x + a_y)
+    a = np.array([1.7, -0.6])
+    o.set("u", a[0] * s.x ** 2 + a[1] * s.y ** 2 + 0.3 * s.x - 2.0 * s.y + 1.0)
+    o.viscosity()
+    assert np.allclose(o.get("ax")[core], 2 * a.sum(), rtol=1e-11)
+    # gradient of a linear pressure with d = 2: variants 0 and 2 return the slope
+    gvec = np.array([3.0, -2.0])
+    p = gvec[0] * s.x + gvec[1] * s.y + 50.0
+    for variant in (0, 2):
+        o2 = O.Oracle(s, grad_variant=variant)
+        o2.bin(); o2.set("p", p); o2.phat(); o2.gradient()
+        gx, gy = o2.get("gx")[core], o2.get("gy")[core]
+        if variant == 0:   # (p_j - phat_i): the constant phat_i drops out on the symmetric lattice
+            assert np.allclose(gx, gvec[0], rtol=1e-10) and np.allclose(gy, gvec[1], rtol=1e-10)
+        else:              # (p_i + p_j): same, the 2 p_i part cancels by symmetry
+            assert np.allclose(gx, gvec[0], rtol=1e-10) and np.allclose(gy, gvec[1], rtol=1e-10)
+        assert np.abs(o2.get("gz")).max() == 0.0
+
+
+def test_2d_neighbour_sets_equal_numpy_brute_force_and_cg_equals_dense():
+    s = scenes.dam_break_2d(L0, (24, 20), (8, 14), seed=5)
+    o = O.Oracle(s)
+    o.bin()
+    valid = np.ones(s.n, bool)
+    for re in (s.params["re_n"], s.params["re_lap"]):
+        cnt, idx = o.neighbours(re)
+        assert np.array_equal(csr_to_mask(cnt, idx, s.n), brute_sets_numpy(s.x, s.y, s.z, valid, re))
+    o.density(); o.ppe_flags(); o.ppe_rhs()
+    rows = np.nonzero(o.get("bc") == 0)[0]
+    assert 50 < rows.size < 600
+    A = np.zeros((rows.size, rows.size))
+    for k, i in enumerate(rows):
+        e = np.zeros(s.n); e[i] = 1.0
+        A[:, k] = o.ppe_apply(e)[rows]
+    assert np.allclose(A, A.T, rtol=0, atol=1e-12 * np.abs(A).max())
+    b = o.get("b")[rows]
+    assert o.ppe_solve(1e-12, 5000) > 0
+    xd = np.linalg.solve(A, b)
+    assert np.linalg.norm(o.get("xcg")[rows] - xd) <= 1e-9 * np.linalg.norm(xd)
