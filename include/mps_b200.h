@@ -84,6 +84,9 @@ typedef struct mps_params {
   int32_t ppe_source;       /* (0) 0: Eq. 8; 1: higher-order source, Eq. 15 (MPS-HS); 2: HS plus the
                                error-compensating parts, Eq. 17-18 (ECS); Q22 */
   int32_t ppe_laplacian;    /* (0) 0: Eq. 10 form of Listing 2; 1: higher-order Laplacian, Eq. 16 (MPS-HL); Q23 */
+  int32_t kernel;           /* (0) 0: w = re/r - 1 (Eq. 3); 1: w = (1 - r/re)^3 (Eq. 4, the paper's
+                               recommendation for the explicit route); n0 and lambda follow the kernel */
+  int32_t reserved_i;
   double l0;                /* initial particle spacing */
   double re_n;              /* radius for density, p-hat and gradient (2.1 l0) */
   double re_grad;           /* must equal re_n (one list serves both) */

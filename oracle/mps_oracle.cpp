@@ -43,6 +43,7 @@ struct Prm {
   int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean, cell_div;
   int ppe_source;     // 0: Eq. 8; 1: higher-order source Eq. 15 (HS); 2: HS + error-compensating parts Eq. 17-18 (ECS)
   int ppe_laplacian;  // 0: Eq. 10 form (Listing 2); 1: higher-order Laplacian Eq. 16 (HL)
+  int kernel;         // 0: w = re/r - 1 (Eq. 3); 1: w = (1 - r/re)^3 (Eq. 4)
   double dmin[3], dmax[3];
   int max_neighbours;
   double n0_n, n0_lap, lam;
@@ -50,7 +51,13 @@ struct Prm {
 
 // I2 (Eq.5 on the initial lattice; "weighted average of
 // r_ij^2"): sums over the ideal cubic lattice, o in Z^dim \ {0}, |o| l0 < re.
-void lattice_constants(int dim, double l0, double re, double* n0, double* lam, int* count) {
+// P:123 Eq.3 (kernel 0) and P:128 Eq.4 (kernel 1), for 0 <= r < re.
+double kernel_w(int kernel, double re, double r) {
+  if (kernel == 1) { const double t = 1.0 - r / re; return t * t * t; }
+  return re / r - 1.0;
+}
+
+void lattice_constants(int dim, double l0, double re, double* n0, double* lam, int* count, int kernel = 0) {
   int R = (int)std::ceil(re / l0) + 1;
   double sw = 0.0, sr2w = 0.0;
   int cnt = 0;
@@ -62,7 +69,7 @@ void lattice_constants(int dim, double l0, double re, double* n0, double* lam, i
         double r2 = (dx * dx + dy * dy) + dz * dz;
         if (r2 < re * re) {
           double r = std::sqrt(r2);
-          double w = re / r - 1.0;  // P:123 Eq.3
+          double w = kernel_w(kernel, re, r);  // P:123 Eq.3 / P:128 Eq.4
           sw += w;
           sr2w += r2 * w;
           ++cnt;
@@ -96,9 +103,9 @@ struct Orc {
     int c;
     double lam_n;
     // I1-I3
-    if (prm.n0_n > 0) n0_n = prm.n0_n; else lattice_constants(prm.dim, prm.l0, prm.re_n, &n0_n, &lam_n, &c);
+    if (prm.n0_n > 0) n0_n = prm.n0_n; else lattice_constants(prm.dim, prm.l0, prm.re_n, &n0_n, &lam_n, &c, prm.kernel);
     double n0l, lm;
-    lattice_constants(prm.dim, prm.l0, prm.re_lap, &n0l, &lm, &c);
+    lattice_constants(prm.dim, prm.l0, prm.re_lap, &n0l, &lm, &c, prm.kernel);
     n0_lap = prm.n0_lap > 0 ? prm.n0_lap : n0l;
     lam = prm.lam > 0 ? prm.lam : lm;
     A_lap = 2.0 * prm.dim / (n0_lap * lam);  // P:170 Eq.10
@@ -181,7 +188,7 @@ struct Orc {
     }
   }
 
-  double w_of(double re, double r2) const { return re / std::sqrt(r2) - 1.0; }  // P:123 Eq.3
+  double w_of(double re, double r2) const { return kernel_w(prm.kernel, re, std::sqrt(r2)); }  // Eq.3 / Eq.4
 
   // step 6 (Eq.5): all non-ghost i; all non-ghost j count.
   void density() {
@@ -511,7 +518,7 @@ void* orc_create(const double* dp, const int* ip, int n, const double* x, const 
   p.n0_n = dp[24]; p.n0_lap = dp[25]; p.lam = dp[26];
   p.dim = ip[0]; p.n_phases = ip[1]; p.cg_maxit = ip[2]; p.grad_variant = ip[3];
   p.clamp_negative_p = ip[4]; p.rho_pair_mean = ip[5]; p.nu_pair_mean = ip[6];
-  p.cell_div = ip[7]; p.max_neighbours = ip[8]; p.ppe_source = ip[9]; p.ppe_laplacian = ip[10];
+  p.cell_div = ip[7]; p.max_neighbours = ip[8]; p.ppe_source = ip[9]; p.ppe_laplacian = ip[10]; p.kernel = ip[11];
   o->n = n;
   for (auto& a : o->f) a.assign(n, 0.0);
   const double* src[6] = {x, y, z, u, v, w};
@@ -617,6 +624,12 @@ int orc_step(void* h, int nsteps, int route) {
   int rc = 0;
   for (int s = 0; s < nsteps; ++s) rc = ((Orc*)h)->step(route);
   return rc;
+}
+void orc_lattice_constants_k(int dim, double l0, double re, int kernel, double* out) {
+  double n0, lam;
+  int c;
+  lattice_constants(dim, l0, re, &n0, &lam, &c, kernel);
+  out[0] = n0; out[1] = lam; out[2] = c;
 }
 void orc_lattice_constants(int dim, double l0, double re, double* out) {
   double n0, lam; int c;

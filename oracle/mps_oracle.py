@@ -50,6 +50,7 @@ def lib():
         L.orc_ppe_solve.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.orc_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_lattice_constants.argtypes = [C.c_int, C.c_double, C.c_double, _dp]
+        L.orc_lattice_constants_k.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int, _dp]
         L.orc_eos.restype = C.c_double
         L.orc_eos.argtypes = [C.c_double] * 5
         _lib = L
@@ -64,9 +65,9 @@ def _i(a):
     return a.ctypes.data_as(_ip)
 
 
-def lattice_constants(dim: int, l0: float, re: float) -> Tuple[float, float, int]:
+def lattice_constants(dim: int, l0: float, re: float, kernel: int = 0) -> Tuple[float, float, int]:
     out = np.zeros(3)
-    lib().orc_lattice_constants(dim, l0, re, _d(out))
+    lib().orc_lattice_constants_k(dim, l0, re, kernel, _d(out))
     return float(out[0]), float(out[1]), int(out[2])
 
 
@@ -81,9 +82,9 @@ def pack_params(p: Dict[str, object]):
                    p["lam"]], dtype=np.float64)
     ip = np.array([p["dim"], p["n_phases"], p["cg_maxit"], p["grad_variant"],
                    p["clamp_negative_p"], p["rho_pair_mean"], p["nu_pair_mean"], p["cell_div"],
-                   p["max_neighbours"], p.get("ppe_source", 0), p.get("ppe_laplacian", 0)],
-                  dtype=np.int32)
-    assert dp.size == 27 and ip.size == 11
+                   p["max_neighbours"], p.get("ppe_source", 0), p.get("ppe_laplacian", 0),
+                   p.get("kernel", 0)], dtype=np.int32)
+    assert dp.size == 27 and ip.size == 12
     return dp, ip
 
 

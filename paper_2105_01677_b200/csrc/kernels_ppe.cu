@@ -172,7 +172,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
       const double r2 = dx * dx + dy * dy + dz * dz;
       const double ir = rsqrt_f64(r2);
       // Eq. 10 form: A_lap (re/r - 1); MPS-HL (Eq. 16, Q23): (2 re / n0) / r^3
-      double w = hl ? ir * ir * ir : fma(kc.re_lap, ir, -1.0);
+      double w = hl ? ir * ir * ir : kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, ir);
       if (TWO_PHASE) {
         const double rho_j = kc.rho[(e[u] & NB_PHASE1) ? 1 : 0];
         const double rij =

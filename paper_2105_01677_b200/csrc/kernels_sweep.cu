@@ -31,7 +31,7 @@ k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restric
     const double4 q = pos4[row[k] & NB_INDEX];
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = dx * dx + dy * dy + dz * dz;
-    s += fma(kc.re_n, rsqrt_f64(r2), -1.0);
+    s += kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, rsqrt_f64(r2));
   }
   s = group_sum<L>(s);
   if (row_live && sub == 0) dens[i] = s;
@@ -94,7 +94,7 @@ k_nu_eff(KConst kc, int with_sps, const double4* __restrict__ pos4, double4* __r
       const double du[3] = {vj.x - vi.x, vj.y - vi.y, vj.z - vi.z};
       const double r2 = dr[0] * dr[0] + dr[1] * dr[1] + dr[2] * dr[2];
       const double ir = rsqrt_f64(r2);
-      const double c = fma(kc.re_n, ir, -1.0) * ir * ir;
+      const double c = kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, ir) * ir * ir;
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -147,7 +147,7 @@ k_viscosity(KConst kc, const double4* __restrict__ pos4, const double4* __restri
     const double4 vj = vel4[j];
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = dx * dx + dy * dy + dz * dz;
-    const double w = fma(kc.re_lap, rsqrt_f64(r2), -1.0);
+    const double w = kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, rsqrt_f64(r2));
     double nuij;
     if (e & (NB_DUMMY | NB_WALL)) {
       nuij = nui;
@@ -286,7 +286,7 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     if (VARIANT == 0) coef = q.w - phi;
     else if (VARIANT == 1) coef = (pi.w + q.w) - (phi + phat[j]);
     else coef = pi.w + q.w;
-    const double c = coef * fma(kc.re_n, ir, -1.0) * ir * ir;
+    const double c = coef * kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, ir) * ir * ir;
     sx += c * dx;
     sy += c * dy;
     sz += c * dz;

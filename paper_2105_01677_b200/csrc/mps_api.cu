@@ -29,7 +29,7 @@ static int fail(mps_ctx* c, int code, const char* msg) {
 // ---- lattice closed forms (I2; Eq. 5) -------------------------
 // n0 = sum over lattice offsets o != 0 with |o| l0 < re of (re / (|o| l0) - 1),
 // lambda = sum |o|^2 l0^2 w / sum w.
-static void lattice_sums(int dim, double l0, double re, double* n0, double* lam) {
+static void lattice_sums(int dim, int kernel, double l0, double re, double* n0, double* lam) {
   const int R = (int)ceil(re / l0) + 1;
   double sw = 0.0, sr2w = 0.0;
   const int Rz = dim == 3 ? R : 0;
@@ -40,7 +40,8 @@ static void lattice_sums(int dim, double l0, double re, double* n0, double* lam)
         const double ex = k * l0, ey = b * l0, ez = a * l0;
         const double r2 = (ex * ex + ey * ey) + ez * ez;
         if (r2 < re * re) {
-          const double w = re / sqrt(r2) - 1.0;
+          const double r = sqrt(r2);
+          const double w = kernel == 1 ? (1.0 - r / re) * (1.0 - r / re) * (1.0 - r / re) : re / r - 1.0;
           sw += w;
           sr2w += r2 * w;
         }
@@ -89,6 +90,9 @@ static int check_params(const mps_params* p, int64_t n) {
     return fail(nullptr, MPS_ERR_ARG, "max_neighbours must be in [1, 4096]");
   if (p->ppe_source < 0 || p->ppe_source > 2) return fail(nullptr, MPS_ERR_ARG, "ppe_source must be 0..2");
   if (p->ppe_laplacian < 0 || p->ppe_laplacian > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_laplacian must be 0 or 1");
+  if (p->kernel < 0 || p->kernel > 1) return fail(nullptr, MPS_ERR_ARG, "kernel must be 0 (Eq. 3) or 1 (Eq. 4)");
+  if (p->kernel == 1 && (p->ppe_source != 0 || p->ppe_laplacian != 0))
+    return fail(nullptr, MPS_ERR_ARG, "Eq. 15-18 are derived for the Eq. 3 kernel: kernel 1 needs ppe_source = ppe_laplacian = 0");
   if (p->grad_variant < 0 || p->grad_variant > 2) return fail(nullptr, MPS_ERR_ARG, "grad_variant must be 0..2");
   if (!(p->rho[0] > 0) || (p->n_phases == 2 && !(p->rho[1] > 0)))
     return fail(nullptr, MPS_ERR_ARG, "densities must be positive");
@@ -123,8 +127,8 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   KConst& k = c->kc;
   memset(&k, 0, sizeof(k));
   double n0n, lam_n, n0l, lam_l;
-  lattice_sums(prm->dim, prm->l0, prm->re_n, &n0n, &lam_n);
-  lattice_sums(prm->dim, prm->l0, prm->re_lap, &n0l, &lam_l);
+  lattice_sums(prm->dim, prm->kernel, prm->l0, prm->re_n, &n0n, &lam_n);
+  lattice_sums(prm->dim, prm->kernel, prm->l0, prm->re_lap, &n0l, &lam_l);
   k.n0_n = prm->n0_n > 0 ? prm->n0_n : n0n;
   k.n0_lap = prm->n0_lap > 0 ? prm->n0_lap : n0l;
   k.lam = prm->lambda > 0 ? prm->lambda : lam_l;
@@ -143,6 +147,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.relax = prm->ppe_relax;
   k.hl_c = 2.0 * prm->re_lap / k.n0_lap;
   k.ppe_source = prm->ppe_source; k.ppe_laplacian = prm->ppe_laplacian;
+  k.kernel = prm->kernel; k.inv_re_n = 1.0 / prm->re_n; k.inv_re_lap = 1.0 / prm->re_lap;
   c->h = std::max(prm->re_n, prm->re_lap) / prm->cell_div;
   k.inv_h = 1.0 / c->h;
   int64_t ncells = 1;

@@ -67,6 +67,8 @@ struct KConst {  // by-value kernel parameter
   double cs_l0_sq, d_over_n0;
   double relax, hl_c;  // ppe_relax; 2 re_lap / n0_lap (Eq. 16)
   int ppe_source, ppe_laplacian;
+  int kernel;          // 0: Eq. 3, 1: Eq. 4
+  double inv_re_n, inv_re_lap;
   double dmin[3], inv_h;
   int nx, ny, nz, ncells;
   int R_lap;  // cells to each side for re_lap

@@ -28,6 +28,16 @@ __device__ __forceinline__ double rsqrt_f64(double x) {
   return fma(y, c, y);
 }
 
+// ---- kernel function w(r), 0 <= r < re, from r^2 and ir = 1/r: Eq. 3 re/r - 1, or
+// Eq. 4 (1 - r/re)^3 when kernel == 1 (a warp-uniform switch).
+__device__ __forceinline__ double kernel_w(int kernel, double re, double inv_re, double r2, double ir) {
+  if (kernel == 1) {
+    const double t = fma(-(r2 * ir), inv_re, 1.0);
+    return t * t * t;
+  }
+  return fma(re, ir, -1.0);
+}
+
 // ---- 32-byte particle record loads -------------------------------------------------
 // Coherent (ld.global, L1-cached, invalidated by a gpu-scope fence): used inside the
 // persistent CG kernel where pos4.w changes between phases.

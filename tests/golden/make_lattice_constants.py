@@ -12,9 +12,11 @@ R3 = {1: 6, 2: 12, 3: 8, 4: 6, 5: 24, 6: 24, 7: 0, 8: 12, 9: 30}
 R2 = {1: 4, 2: 4, 3: 0, 4: 4, 5: 8, 6: 0, 7: 0, 8: 4, 9: 4}
 
 
-def consts(mult, re):
-    sw = sum(m * (re / math.sqrt(k) - 1.0) for k, m in mult.items() if k < re * re)
-    sr = sum(m * k * (re / math.sqrt(k) - 1.0) for k, m in mult.items() if k < re * re)
+def consts(mult, re, w=None):
+    if w is None:
+        w = lambda r: re / r - 1.0                      # PAPER.md:123 Eq.3
+    sw = sum(m * w(math.sqrt(k)) for k, m in mult.items() if k < re * re)
+    sr = sum(m * k * w(math.sqrt(k)) for k, m in mult.items() if k < re * re)
     cnt = sum(m for k, m in mult.items() if k < re * re)
     return sw, sr / sw, cnt
 
@@ -27,6 +29,11 @@ def main():
             rows.append((f"n0_{tag}_{re}", n0, "P:134 Eq.5 + P:123 Eq.3 on the cubic lattice"))
             rows.append((f"lambda_{tag}_{re}", lam, "P:174, in units of l0^2"))
             rows.append((f"count_{tag}_{re}", cnt, "number of lattice neighbours"))
+    for tag, mult in (("3d", R3), ("2d", R2)):
+        for re in (2.1, 3.1):
+            n0, lam, cnt = consts(mult, re, lambda r: (1.0 - r / re) ** 3)   # PAPER.md:128 Eq.4
+            rows.append((f"n0_eq4_{tag}_{re}", n0, "P:134 Eq.5 + P:128 Eq.4 on the cubic lattice"))
+            rows.append((f"lambda_eq4_{tag}_{re}", lam, "P:174 with the Eq.4 kernel, in units of l0^2"))
     n0 = consts(R3, 2.1)[0]
     w = lambda k: 2.1 / math.sqrt(k) - 1.0
     rows.append(("n_depth1_3d_2.1", n0 - w(4), "misses one (2,0,0) neighbour (T3)"))

@@ -34,9 +34,9 @@ def test_library_exports_every_declared_symbol(B):
 
 
 def test_struct_layout_matches_header(B):
-    # 12 int32 then 28 doubles, no padding
-    assert C.sizeof(B.MpsParams) == 12 * 4 + 28 * 8
-    assert B.MpsParams.l0.offset == 48
+    # 14 int32 then 28 doubles, no padding
+    assert C.sizeof(B.MpsParams) == 14 * 4 + 28 * 8
+    assert B.MpsParams.l0.offset == 56
     assert C.sizeof(B.MpsStats) == 56
     # field ids in the binding equal the header's enum
     src = open(os.path.join(ROOT, "include", "mps_b200.h")).read()
@@ -66,7 +66,7 @@ def _init_rc(B, **over):
 
 
 @pytest.mark.parametrize("over", [
-    dict(dim=4), dict(dim=2, ppe_laplacian=1), dict(ppe_source=3), dict(l0=0.0), dict(dt=-1.0), dict(re_grad=0.5), dict(re_lap=0.001),
+    dict(dim=4), dict(dim=2, ppe_laplacian=1), dict(ppe_source=3), dict(kernel=2), dict(kernel=1, ppe_source=1), dict(l0=0.0), dict(dt=-1.0), dict(re_grad=0.5), dict(re_lap=0.001),
     dict(cell_div=0), dict(cell_div=4), dict(key_mode=1), dict(n_phases=3), dict(max_neighbours=0),
     dict(grad_variant=3), dict(rho=(0.0, 1.0)), dict(cg_rtol=0.0), dict(domain_max=(0.0, 1.0, 1.0)),
 ])

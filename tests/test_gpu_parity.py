@@ -548,3 +548,25 @@ def test_2d_trajectory_20_steps(B, O, route):
     print(f"2D dam break, 20 steps, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
     assert eL <= 1e-7 and moved > 0.02
     assert (g.get("z") == 0).all() and (g.get("w") == 0).all()
+
+
+# ----------------------------------------- NEXT-3 (part): the Eq. 4 kernel (1 - r/re)^3 ---
+def test_eq4_kernel_fields_and_trajectory(B, O):
+    s = scenes.small_tank(shuffle=True)
+    g, o = _pair(B, O, s, kernel=1, cs=0.12)
+    c, oc = g.constants(), o.constants()
+    for k in ("n0_n", "n0_lap", "lam"):
+        assert abs(c[k] - oc[k]) <= 1e-14 * oc[k]
+    g.density(); o.density()
+    assert relerr(g.get("n"), o.get("n"), oc["n0_n"]) <= TOL
+    g.viscosity(); o.viscosity()
+    assert relerr(g.get("nut"), o.get("nut"), 1e-30) <= TOL
+    assert vec_relerr([g.get(k) for k in ("ax", "ay", "az")], [o.get(k) for k in ("ax", "ay", "az")], 9.81) <= TOL
+    g.pressure_explicit(); o.pressure_explicit()
+    g.gradient(); o.phat(); o.gradient()
+    assert vec_relerr([g.get(k) for k in ("gx", "gy", "gz")], [o.get(k) for k in ("gx", "gy", "gz")], 1.0) <= TOL
+    # the paper recommends Eq. 4 for the explicit route; the PPE route must agree too
+    for route in (0, 1):
+        eL, el0, moved, g2, o2 = _trajectory(B, O, scenes.small_tank(shuffle=True), 12, route, kernel=1)
+        print(f"Eq. 4 kernel, 12 steps, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.3f} l0")
+        assert eL <= 1e-7

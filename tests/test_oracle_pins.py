@@ -645,3 +645,42 @@ def test_2d_neighbour_sets_equal_numpy_brute_force_and_cg_equals_dense():
     assert o.ppe_solve(1e-12, 5000) > 0
     xd = np.linalg.solve(A, b)
     assert np.linalg.norm(o.get("xcg")[rows] - xd) <= 1e-9 * np.linalg.norm(xd)
+
+
+# ---- NEXT-3 (part): the (1 - r/re)^3 kernel of Eq. 4 ---------------------------------
+@pytest.mark.parametrize("dim,tag", [(3, "3d"), (2, "2d")])
+@pytest.mark.parametrize("re", [2.1, 3.1])
+def test_eq4_kernel_lattice_constants(dim, tag, re):
+    n0, lam, cnt = O.lattice_constants(dim, L0, re * L0, kernel=1)
+    assert abs(n0 - GOLD[f"n0_eq4_{tag}_{re}"]) <= 1e-13 * n0
+    assert abs(lam / L0 ** 2 - GOLD[f"lambda_eq4_{tag}_{re}"]) <= 1e-13 * lam / L0 ** 2
+    assert cnt == GOLD[f"count_{tag}_{re}"]
+
+
+def test_eq4_kernel_density_laplacian_gradient():
+    # density = NumPy brute force of Eq. 5 with Eq. 4 on a jittered tank
+    s = scenes.small_tank(shuffle=True)
+    o = O.Oracle(s, kernel=1)
+    o.bin(); o.density()
+    re = s.params["re_n"]
+    dx = s.x[None, :] - s.x[:, None]; dy = s.y[None, :] - s.y[:, None]; dz = s.z[None, :] - s.z[:, None]
+    r = np.sqrt((dx * dx + dy * dy) + dz * dz)
+    m = r < re
+    np.fill_diagonal(m, False)
+    ref = np.where(m, (1.0 - r / re) ** 3, 0.0).sum(axis=1)
+    assert np.allclose(o.get("n"), ref, rtol=1e-12, atol=1e-13)
+    # lambda makes Eq. 10 exact on a quadratic for any kernel; the gradient model is exact on a
+    # linear field on the symmetric lattice for any kernel
+    mm = 10
+    b = scenes.fluid_blob(L0, (mm, mm, mm))
+    core = _interior_mask(b, mm, 4)
+    a = np.array([0.9, 1.4, -2.2])
+    o = O.Oracle(b, kernel=1, nu=(1.0, 1.0), g=(0.0, 0.0, 0.0))
+    o.set("u", a[0] * b.x ** 2 + a[1] * b.y ** 2 + a[2] * b.z ** 2 - 3.0 * b.x + 7.0)
+    o.viscosity()
+    assert np.allclose(o.get("ax")[core], 2 * a.sum(), rtol=1e-11)
+    gvec = np.array([2.0, -1.0, 0.5])
+    o2 = O.Oracle(b, kernel=1, grad_variant=2)
+    o2.bin(); o2.set("p", gvec[0] * b.x + gvec[1] * b.y + gvec[2] * b.z + 10.0); o2.phat(); o2.gradient()
+    for k, comp in enumerate(("gx", "gy", "gz")):
+        assert np.allclose(o2.get(comp)[core], gvec[k], rtol=1e-10)
