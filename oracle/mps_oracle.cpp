@@ -44,6 +44,7 @@ struct Prm {
   int ppe_source;     // 0: Eq. 8; 1: higher-order source Eq. 15 (HS); 2: HS + error-compensating parts Eq. 17-18 (ECS)
   int ppe_laplacian;  // 0: Eq. 10 form (Listing 2); 1: higher-order Laplacian Eq. 16 (HL)
   int kernel;         // 0: w = re/r - 1 (Eq. 3); 1: w = (1 - r/re)^3 (Eq. 4)
+  int rebin_every;    // 1: exact sets at every sweep (Q7); K > 1: the paper's list reuse (Q24)
   double dmin[3], dmax[3];
   int max_neighbours;
   double n0_n, n0_lap, lam;
@@ -151,7 +152,26 @@ struct Orc {
     }
     binned = true;
   }
-  void ensure_binned() { if (!binned) bin(); }
+  // NEXT-3 list reuse ("constant for that entire step", "every four steps"; Q24):
+  // the neighbour lists of both radii as built by the last scheduled BIN, each row ascending.
+  std::vector<int> lst_off[2], lst_idx[2];
+  bool use_lists = false;
+  long step_count = 0;
+  void build_lists() {
+    const double radius[2] = {prm.re_n, prm.re_lap};
+    for (int w = 0; w < 2; ++w) {
+      lst_off[w].assign(n + 1, 0);
+      lst_idx[w].clear();
+      for (int i = 0; i < n; ++i) {
+        std::vector<int> row;
+        for_neighbours(i, radius[w], [&](int j, double, double, double, double) { row.push_back(j); });
+        std::sort(row.begin(), row.end());
+        lst_idx[w].insert(lst_idx[w].end(), row.begin(), row.end());
+        lst_off[w][i + 1] = (int)lst_idx[w].size();
+      }
+    }
+  }
+  void ensure_binned() { if (!use_lists && !binned) bin(); }
 
   // NEIGHBOURS(i, re) (Eq.3, strict r < re; Q2 rounding of the test).
   template <class F>
@@ -165,6 +185,11 @@ struct Orc {
       if (r2 < re2) fn(j, dx, dy, dz, r2);
     };
     if (type[i] == GHOST) return;
+    if (use_lists) {  // stored list of that radius, re-tested at the current distance (Q24)
+      const int w = (re == prm.re_n) ? 0 : 1;
+      for (int k = lst_off[w][i]; k < lst_off[w][i + 1]; ++k) test(lst_idx[w][k]);
+      return;
+    }
     if (brute) {
       for (int j = 0; j < n; ++j) test(j);
       return;
@@ -473,8 +498,37 @@ struct Orc {
     }
     binned = false;
   }
+  // STEP with list reuse (Q24): BIN and the lists of both radii only when step_count is a
+  // multiple of rebin_every, at r^k; every sweep of this and the next rebin_every - 1 steps walks
+  // those lists and keeps the pairs whose CURRENT distance is below the radius.
+  int step_reuse(int route) {
+    if (step_count % prm.rebin_every == 0) {
+      use_lists = false;
+      bin();
+      build_lists();
+    }
+    use_lists = true;
+    if (route == 1 && prm.ppe_source == 2) {
+      density();
+      f[19] = f[6];
+      dndt(20);
+    }
+    viscosity();
+    predict();
+    density();
+    if (route == 1 && prm.ppe_source >= 1) dndt(18);
+    int rc = 0;
+    if (route == 0) pressure_explicit();
+    else rc = pressure_ppe();
+    phat();
+    gradient();
+    correct();
+    ++step_count;
+    return rc;
+  }
   // STEP k -> k+1 (section 8(c).1 of SURVEY.md / DESIGN.md section 2).
   int step(int route) {
+    if (prm.rebin_every > 1) return step_reuse(route);
     bin();                // 1
     if (route == 1 && prm.ppe_source == 2) {  // ECS keeps n^k and (Dn/Dt)^k (Eq.17)
       density();
@@ -518,7 +572,7 @@ void* orc_create(const double* dp, const int* ip, int n, const double* x, const 
   p.n0_n = dp[24]; p.n0_lap = dp[25]; p.lam = dp[26];
   p.dim = ip[0]; p.n_phases = ip[1]; p.cg_maxit = ip[2]; p.grad_variant = ip[3];
   p.clamp_negative_p = ip[4]; p.rho_pair_mean = ip[5]; p.nu_pair_mean = ip[6];
-  p.cell_div = ip[7]; p.max_neighbours = ip[8]; p.ppe_source = ip[9]; p.ppe_laplacian = ip[10]; p.kernel = ip[11];
+  p.cell_div = ip[7]; p.max_neighbours = ip[8]; p.ppe_source = ip[9]; p.ppe_laplacian = ip[10]; p.kernel = ip[11]; p.rebin_every = ip[12] < 1 ? 1 : ip[12];
   o->n = n;
   for (auto& a : o->f) a.assign(n, 0.0);
   const double* src[6] = {x, y, z, u, v, w};
@@ -620,6 +674,12 @@ void orc_dndt(void* h, int dst) { ((Orc*)h)->dndt(dst == 20 ? 20 : 18); }
 int orc_phat(void* h) { ((Orc*)h)->phat(); return 0; }
 int orc_gradient(void* h) { ((Orc*)h)->gradient(); return 0; }
 int orc_correct(void* h) { ((Orc*)h)->correct(); return 0; }
+// list reuse for the tests: BIN + lists at the current positions, then walk them (1) or drop them (0)
+void orc_freeze_lists(void* h, int on) {
+  Orc* o = (Orc*)h;
+  o->use_lists = false;
+  if (on) { o->bin(); o->build_lists(); o->use_lists = true; }
+}
 int orc_step(void* h, int nsteps, int route) {
   int rc = 0;
   for (int s = 0; s < nsteps; ++s) rc = ((Orc*)h)->step(route);

@@ -46,6 +46,7 @@ def lib():
                    "orc_phat", "orc_gradient", "orc_correct"):
             getattr(L, nm).argtypes = [C.c_void_p]
         L.orc_dndt.argtypes = [C.c_void_p, C.c_int]
+        L.orc_freeze_lists.argtypes = [C.c_void_p, C.c_int]
         L.orc_ppe_apply.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_ppe_solve.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.orc_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
@@ -83,8 +84,8 @@ def pack_params(p: Dict[str, object]):
     ip = np.array([p["dim"], p["n_phases"], p["cg_maxit"], p["grad_variant"],
                    p["clamp_negative_p"], p["rho_pair_mean"], p["nu_pair_mean"], p["cell_div"],
                    p["max_neighbours"], p.get("ppe_source", 0), p.get("ppe_laplacian", 0),
-                   p.get("kernel", 0)], dtype=np.int32)
-    assert dp.size == 27 and ip.size == 12
+                   p.get("kernel", 0), p.get("rebin_every", 1)], dtype=np.int32)
+    assert dp.size == 27 and ip.size == 13
     return dp, ip
 
 
@@ -170,6 +171,7 @@ class Oracle:
     def viscosity(self): self.L.orc_viscosity(self.h)
     def predict(self): self.L.orc_predict(self.h)
     def pressure_explicit(self): self.L.orc_pressure_explicit(self.h)
+    def freeze_lists(self, on: bool = True): self.L.orc_freeze_lists(self.h, 1 if on else 0)
     def dndt(self, keep: bool = False): self.L.orc_dndt(self.h, 20 if keep else 18)
     def ppe_flags(self): self.L.orc_ppe_flags(self.h)
     def ppe_rhs(self): self.L.orc_ppe_rhs(self.h)

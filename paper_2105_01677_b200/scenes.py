@@ -88,6 +88,7 @@ def default_params(l0: float) -> Dict[str, object]:
         ppe_source=0,        # 0 Eq. 8; 1 higher-order source (Eq. 15); 2 + error-compensating parts (Eq. 17-18)
         ppe_laplacian=0,     # 0 Eq. 10 form; 1 higher-order Laplacian (Eq. 16)
         kernel=0,            # 0 w = re/r - 1 (Eq. 3); 1 w = (1 - r/re)^3 (Eq. 4)
+        rebin_every=1,       # 1 exact sets at every sweep; K > 1 the paper's list reuse
         clamp_negative_p=1,
         rho_pair_mean=0,
         nu_pair_mean=1,

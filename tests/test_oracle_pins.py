@@ -684,3 +684,42 @@ def test_eq4_kernel_density_laplacian_gradient():
     o2.bin(); o2.set("p", gvec[0] * b.x + gvec[1] * b.y + gvec[2] * b.z + 10.0); o2.phat(); o2.gradient()
     for k, comp in enumerate(("gx", "gy", "gz")):
         assert np.allclose(o2.get(comp)[core], gvec[k], rtol=1e-10)
+
+
+# ---- NEXT-3 (part): neighbour-list reuse (Q24) -------------------------------------
+def test_list_reuse_is_the_stored_set_retested_at_the_current_distance():
+    s = scenes.small_tank(shuffle=True)
+    o = O.Oracle(s, rebin_every=4)
+    o.freeze_lists()                                   # lists of both radii at positions A
+    rng = np.random.default_rng(11)
+    fl = s.type == scenes.FLUID
+    xb, yb, zb = s.x.copy(), s.y.copy(), s.z.copy()
+    for arr in (xb, yb, zb):
+        arr[fl] += rng.uniform(-0.3, 0.3, fl.sum()) * s.params["l0"]   # positions B: sets change
+    o.set("x", xb); o.set("y", yb); o.set("z", zb)
+    o.density()
+    re = s.params["re_n"]
+    valid = np.ones(s.n, bool)
+    at_a = brute_sets_numpy(s.x, s.y, s.z, valid, re)
+    at_b = brute_sets_numpy(xb, yb, zb, valid, re)
+    assert (at_a != at_b).sum() > 100                  # the move does change the exact sets
+    dx = xb[None, :] - xb[:, None]; dy = yb[None, :] - yb[:, None]; dz = zb[None, :] - zb[:, None]
+    r = np.sqrt((dx * dx + dy * dy) + dz * dz)
+    r = np.where(at_a & at_b, r, 1.0)
+    ref = np.where(at_a & at_b, re / r - 1.0, 0.0).sum(axis=1)
+    assert np.allclose(o.get("n"), ref, rtol=1e-12, atol=1e-12)
+    # dropping the lists gives the exact sets at B again
+    o.freeze_lists(False)
+    o.density()
+    r = np.where(at_b, np.sqrt((dx * dx + dy * dy) + dz * dz), 1.0)
+    assert np.allclose(o.get("n"), np.where(at_b, re / r - 1.0, 0.0).sum(axis=1), rtol=1e-12, atol=1e-12)
+
+
+def test_list_reuse_equals_exact_mode_while_no_pair_crosses_a_radius():
+    # a fluid at rest in a full tank barely moves in 4 steps: same sets, so the same trajectory
+    # up to the order of the sums
+    s = scenes.hydrostatic_tank(foot=(8, 8), depth=6, height=9)
+    a = O.Oracle(s); b = O.Oracle(s, rebin_every=4)
+    a.step(4, 0); b.step(4, 0)
+    for k in "xyz":
+        assert np.abs(a.get(k) - b.get(k)).max() <= 1e-12 * s.params["l0"]
