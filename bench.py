@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="scene 1..5 (SURVEY.md 8(d)); default 2 = BASELINE configs[1]; 6 = paper-shaped 2D dam break")
     ap.add_argument("--sweep-index", type=int, default=0, help="size index 0..4 of scene 5")
     ap.add_argument("--route", default=None, choices=[None, "explicit", "ppe"])
+    ap.add_argument("--rebin-every", type=int, default=1,
+                    help="K > 1: the paper's neighbour-list reuse (PAPER.md:433), NOT the BASELINE workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-replay", action="store_true", help="skip the instrumented per-kernel replay")
@@ -76,6 +78,9 @@ def make_scene(args, rank=0):
     seed = scenes.BASE_SEED + args.config + (args.sweep_index if args.config >= 5 else 0) + 1000 * rank
     s = scenes.make_scene(args.config, seed=seed, sweep_index=args.sweep_index)
     route = s.route if args.route is None else {"explicit": 0, "ppe": 1}[args.route]
+    if getattr(args, "rebin_every", 1) > 1:
+        s.params["rebin_every"] = int(args.rebin_every)
+        s.name += f"_reuse{args.rebin_every}"
     return s, route
 
 

@@ -86,7 +86,9 @@ typedef struct mps_params {
   int32_t ppe_laplacian;    /* (0) 0: Eq. 10 form of Listing 2; 1: higher-order Laplacian, Eq. 16 (MPS-HL); Q23 */
   int32_t kernel;           /* (0) 0: w = re/r - 1 (Eq. 3); 1: w = (1 - r/re)^3 (Eq. 4, the paper's
                                recommendation for the explicit route); n0 and lambda follow the kernel */
-  int32_t reserved_i;
+  int32_t rebin_every;      /* (1) 1: exact neighbour sets at both bins of every step (Q7).  K > 1: the paper's
+                               list reuse: mps_step bins once every K steps, at r^k, and every
+                               sweep keeps the stored pairs whose current distance is below the radius; Q24 */
   double l0;                /* initial particle spacing */
   double re_n;              /* radius for density, p-hat and gradient (2.1 l0) */
   double re_grad;           /* must equal re_n (one list serves both) */

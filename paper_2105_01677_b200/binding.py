@@ -46,7 +46,7 @@ class MpsParams(C.Structure):
         ("grad_variant", C.c_int32), ("clamp_negative_p", C.c_int32),
         ("rho_pair_mean", C.c_int32), ("nu_pair_mean", C.c_int32), ("key_mode", C.c_int32),
         ("cell_div", C.c_int32), ("max_neighbours", C.c_int32), ("ppe_source", C.c_int32),
-        ("ppe_laplacian", C.c_int32), ("kernel", C.c_int32), ("reserved_i", C.c_int32),
+        ("ppe_laplacian", C.c_int32), ("kernel", C.c_int32), ("rebin_every", C.c_int32),
         ("l0", C.c_double), ("re_n", C.c_double), ("re_grad", C.c_double),
         ("re_lap", C.c_double), ("dt", C.c_double), ("g", C.c_double * 3),
         ("rho", C.c_double * 2), ("nu", C.c_double * 2), ("c0", C.c_double),
@@ -85,6 +85,7 @@ def make_params(p: Dict[str, object]) -> MpsParams:
     s.ppe_source = int(p.get("ppe_source", 0))
     s.ppe_laplacian = int(p.get("ppe_laplacian", 0))
     s.kernel = int(p.get("kernel", 0))
+    s.rebin_every = int(p.get("rebin_every", 1))
     for k in ("l0", "re_n", "re_lap", "dt", "c0", "gamma", "beta", "compress", "ppe_relax",
               "cg_rtol", "cs", "n0_n", "n0_lap"):
         setattr(s, k, float(p[k]))

@@ -169,7 +169,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 #pragma unroll
     for (int u = 0; u < PPE_ILP; ++u) {
       const double dx = q[u].x - pi.x, dy = q[u].y - pi.y, dz = q[u].z - pi.z;
-      const double r2 = dx * dx + dy * dy + dz * dz;
+      const double r2 = pair_r2(dx, dy, dz, kc.stale);
       const double ir = rsqrt_f64(r2);
       // Eq. 10 form: A_lap (re/r - 1); MPS-HL (Eq. 16, Q23): (2 re / n0) / r^3
       double w = hl ? ir * ir * ir : kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, ir);
@@ -179,7 +179,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
             kc.rho_pair_mean == 1 ? 2.0 * rho_i * rho_j / (rho_i + rho_j) : 0.5 * (rho_i + rho_j);
         w = w / rij;
       }
-      if (e[u] & NB_DUMMY) w = 0.0;
+      if ((e[u] & NB_DUMMY) || (kc.stale && !(r2 < kc.re_lap2))) w = 0.0;  // dummy, empty slot, or left the radius
       s = fma(w, pi.w - q[u].w, s);
     }
   }

@@ -30,7 +30,8 @@ k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restric
   for (uint32_t k = sub; k < m; k += L) {
     const double4 q = pos4[row[k] & NB_INDEX];
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r2 = pair_r2(dx, dy, dz, kc.stale);
+    if (kc.stale && !(r2 < kc.re_n2)) continue;  // reused row: the pair has left the radius
     s += kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, rsqrt_f64(r2));
   }
   s = group_sum<L>(s);
@@ -56,7 +57,8 @@ k_dndt(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ 
     const double4 q = pos4[j];
     const double4 vj = vel4[j];
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r2 = pair_r2(dx, dy, dz, kc.stale);
+    if (kc.stale && !(r2 < kc.re_n2)) continue;
     const double ir = rsqrt_f64(r2);
     const double xu = dx * (vj.x - vi.x) + dy * (vj.y - vi.y) + dz * (vj.z - vi.z);
     s = fma(ir * ir * ir, xu, s);
@@ -92,7 +94,8 @@ k_nu_eff(KConst kc, int with_sps, const double4* __restrict__ pos4, double4* __r
       const double4 vj = vel4[j];  // walls and dummies hold u = 0
       const double dr[3] = {q.x - pi.x, q.y - pi.y, q.z - pi.z};
       const double du[3] = {vj.x - vi.x, vj.y - vi.y, vj.z - vi.z};
-      const double r2 = dr[0] * dr[0] + dr[1] * dr[1] + dr[2] * dr[2];
+      const double r2 = pair_r2(dr[0], dr[1], dr[2], kc.stale);
+      if (kc.stale && !(r2 < kc.re_n2)) continue;
       const double ir = rsqrt_f64(r2);
       const double c = kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, ir) * ir * ir;
 #pragma unroll
@@ -146,7 +149,8 @@ k_viscosity(KConst kc, const double4* __restrict__ pos4, const double4* __restri
     const double4 q = pos4[j];
     const double4 vj = vel4[j];
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r2 = pair_r2(dx, dy, dz, kc.stale);
+    if (kc.stale && !(r2 < kc.re_lap2)) continue;
     const double w = kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, rsqrt_f64(r2));
     double nuij;
     if (e & (NB_DUMMY | NB_WALL)) {
@@ -232,11 +236,14 @@ k_phat(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__
   const bool on = row_live && (ty == MPS_FLUID || ty == MPS_WALL);
   const uint32_t* row = row_ptr(nbr, kc.stride, ii);
   const uint32_t m = on ? cn[ii] : 0u;
-  double mn = pos4[ii].w;
+  const double4 pi = pos4[ii];
+  double mn = pi.w;
   for (uint32_t k = sub; k < m; k += L) {
     const uint32_t e = row[k];
     if (e & NB_DUMMY) continue;
-    mn = fmin(mn, pos4[e & NB_INDEX].w);
+    const double4 q = pos4[e & NB_INDEX];
+    if (kc.stale && !(pair_r2(q.x - pi.x, q.y - pi.y, q.z - pi.z, 1) < kc.re_n2)) continue;
+    mn = fmin(mn, q.w);
   }
   mn = group_min<L>(mn);
   if (row_live && sub == 0) phat[i] = on ? mn : 0.0;
@@ -267,7 +274,9 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     for (uint32_t k = sub; k < m; k += L) {
       const uint32_t e = row[k];
       if (e & NB_DUMMY) continue;
-      mn = fmin(mn, pos4[e & NB_INDEX].w);
+      const double4 q = pos4[e & NB_INDEX];
+      if (kc.stale && !(pair_r2(q.x - pi.x, q.y - pi.y, q.z - pi.z, 1) < kc.re_n2)) continue;
+      mn = fmin(mn, q.w);
     }
     phi = group_min<L>(mn);
     if (row_live && sub == 0) phat[i] = (fluid || wall) ? phi : 0.0;
@@ -280,7 +289,8 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     const uint32_t j = e & NB_INDEX;
     const double4 q = pos4[j];
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r2 = pair_r2(dx, dy, dz, kc.stale);
+    if (kc.stale && !(r2 < kc.re_n2)) continue;
     const double ir = rsqrt_f64(r2);
     double coef;
     if (VARIANT == 0) coef = q.w - phi;

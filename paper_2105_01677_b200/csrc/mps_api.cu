@@ -90,6 +90,7 @@ static int check_params(const mps_params* p, int64_t n) {
     return fail(nullptr, MPS_ERR_ARG, "max_neighbours must be in [1, 4096]");
   if (p->ppe_source < 0 || p->ppe_source > 2) return fail(nullptr, MPS_ERR_ARG, "ppe_source must be 0..2");
   if (p->ppe_laplacian < 0 || p->ppe_laplacian > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_laplacian must be 0 or 1");
+  if (p->rebin_every < 1 || p->rebin_every > 1000) return fail(nullptr, MPS_ERR_ARG, "rebin_every must be in [1, 1000]");
   if (p->kernel < 0 || p->kernel > 1) return fail(nullptr, MPS_ERR_ARG, "kernel must be 0 (Eq. 3) or 1 (Eq. 4)");
   if (p->kernel == 1 && (p->ppe_source != 0 || p->ppe_laplacian != 0))
     return fail(nullptr, MPS_ERR_ARG, "Eq. 15-18 are derived for the Eq. 3 kernel: kernel 1 needs ppe_source = ppe_laplacian = 0");
@@ -414,16 +415,28 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
   int first_err = MPS_OK;
   const bool ecs = route == MPS_ROUTE_PPE && c->prm.ppe_source == 2;
   const bool hs = route == MPS_ROUTE_PPE && c->prm.ppe_source >= 1;
+  const int K = c->prm.rebin_every;
   for (int s = 0; s < nsteps; ++s) {
-    // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
-    mpsk_bin(c, /*fluid_rows_only=*/!ecs);
+    if (K > 1) {
+      // list reuse (Q24): bin (all rows, both radii) once every K steps at r^k; every sweep of
+      // these steps walks the stored rows and re-tests the current distance
+      if (c->reuse_count % K == 0) {
+        c->kc.stale = 0;
+        mpsk_bin(c);
+      }
+      c->kc.stale = 1;
+      ++c->reuse_count;
+    } else {
+      // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
+      mpsk_bin(c, /*fluid_rows_only=*/!ecs);
+    }
     if (ecs) {
       mpsk_density(c);
       mpsk_dndt(c, 1);
     }
     mpsk_viscosity(c);
     mpsk_predict(c);
-    mpsk_bin(c);
+    if (K == 1) mpsk_bin(c);
     mpsk_density(c);
     if (hs) mpsk_dndt(c, 0);
     if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
@@ -436,6 +449,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     mpsk_correct(c);
     c->stats.steps_total++;
   }
+  c->kc.stale = 0;  // API-level sweeps always run on exact rows (they need mps_bin first)
   CK(cudaGetLastError());
   int fl = read_flags(c);
   if (fl) return fl;
@@ -492,6 +506,7 @@ int mps_upload_host(mps_ctx* c, const double* x, const double* y, const double* 
   CK(cudaGetLastError());
   c->binned = false;
   c->ppe_ready = false;
+  c->reuse_count = 0;  // new particle order: the stored rows are void
   return MPS_OK;
 }
 

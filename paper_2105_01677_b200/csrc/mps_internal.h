@@ -68,6 +68,7 @@ struct KConst {  // by-value kernel parameter
   double relax, hl_c;  // ppe_relax; 2 re_lap / n0_lap (Eq. 16)
   int ppe_source, ppe_laplacian;
   int kernel;          // 0: Eq. 3, 1: Eq. 4
+  int stale;           // 1 while mps_step walks reused rows: every pair is re-tested (Q24)
   double inv_re_n, inv_re_lap;
   double dmin[3], inv_h;
   int nx, ny, nz, ncells;
@@ -137,6 +138,7 @@ struct mps_ctx {
   cudaEvent_t poll_event = nullptr;
   // state
   bool binned = false;
+  int64_t reuse_count = 0;  // steps since the ctx started reusing rows (rebin_every > 1)
   bool ppe_ready = false;
   int sticky_error = 0;
   mps_stats stats{};

@@ -38,6 +38,13 @@ __device__ __forceinline__ double kernel_w(int kernel, double re, double inv_re,
   return fma(re, ir, -1.0);
 }
 
+// ---- squared distance of a pair: fused arithmetic, or -- while rows are reused (Q24) -- the
+// rounding of reading Q2, so that the re-test r2 < re^2 decides exactly as the oracle's does.
+__device__ __forceinline__ double pair_r2(double dx, double dy, double dz, int stale) {
+  if (stale) return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  return dx * dx + dy * dy + dz * dz;
+}
+
 // ---- 32-byte particle record loads -------------------------------------------------
 // Coherent (ld.global, L1-cached, invalidated by a gpu-scope fence): used inside the
 // persistent CG kernel where pos4.w changes between phases.

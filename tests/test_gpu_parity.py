@@ -570,3 +570,24 @@ def test_eq4_kernel_fields_and_trajectory(B, O):
         eL, el0, moved, g2, o2 = _trajectory(B, O, scenes.small_tank(shuffle=True), 12, route, kernel=1)
         print(f"Eq. 4 kernel, 12 steps, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.3f} l0")
         assert eL <= 1e-7
+
+
+# -------------------------------------- NEXT-3 (part): neighbour-list reuse ---
+@pytest.mark.parametrize("route", [0, 1])
+@pytest.mark.parametrize("rows", ["warp", "cell"])
+def test_list_reuse_every_four_steps(B, O, route, rows, monkeypatch):
+    monkeypatch.setenv("MPS_B200_ROWS", rows)
+    s = scenes.small_tank(shuffle=True)
+    rng = np.random.default_rng(3)
+    fl = s.type == scenes.FLUID
+    for k in "uvw":                      # enough motion that pairs do cross the radii within 4 steps
+        getattr(s, k)[fl] = 0.4 * rng.standard_normal(fl.sum())
+    eL, el0, moved, g, o = _trajectory(B, O, s, 10, route, rebin_every=4)
+    print(f"list reuse every 4 steps, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
+    assert moved > 0.3 and eL <= 1e-7
+    assert relerr(g.get("n"), o.get("n"), 14.4) <= 1e-9
+    assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-6
+    # and it is a different trajectory from the exact mode (the stored sets do go stale)
+    o1 = O.Oracle(s)
+    o1.step(10, route)
+    assert np.abs(o1.get("x") - o.get("x")).max() > 1e-9 * s.params["l0"]
