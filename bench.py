@@ -301,12 +301,13 @@ def run_b200(args):
         cg_iters_timed = st_r["cg_iters_total"] - (stats["cg_iters_total"] - cg_timed_main)
         cg_uses = {"cg_spmv": cg_iters_timed + K, "cg_update": cg_iters_timed}
         peak, peak_src = peaks()
+        n_bins = tm["bin_list"][1]          # one row-builder launch per bin (2 per step; fewer with list reuse)
         for cat, (ms, ln) in tm.items():
             if ln == 0:
                 continue
             ab = algorithmic_bytes(cat, scene.n, rows, kn, kl, klr)
             # categories with several kernels per use: bytes are per use, not per launch
-            uses = {"bin_sort": 2 * K, "bin_list": 2 * K, "viscosity": K, "gradient": K,
+            uses = {"bin_sort": n_bins, "bin_list": n_bins, "viscosity": K, "gradient": K,
                     "ppe_setup": K, **cg_uses}.get(cat, ln)
             kernels[cat] = {"ms_per_step": ms / K, "launches_per_step": ln / K,
                             "us_per_launch": 1e3 * ms / ln,
@@ -314,7 +315,7 @@ def run_b200(args):
         top = max(kernels, key=lambda c: kernels[c]["ms_per_step"])
         ab = algorithmic_bytes(top, scene.n, rows, kn, kl, klr)
         ms, ln = tm[top]
-        uses = {"bin_sort": 2 * K, "bin_list": 2 * K, "viscosity": K, "gradient": K, "ppe_setup": K,
+        uses = {"bin_sort": n_bins, "bin_list": n_bins, "viscosity": K, "gradient": K, "ppe_setup": K,
                 **cg_uses}.get(top, ln)
         achieved = ab * uses / (ms * 1e-3) / 1e9
         roof = {"kernel": top, "bound": "hbm", "per": "use (cg_spmv: one operator application; one k_ppe_cg launch runs a whole solve)",
