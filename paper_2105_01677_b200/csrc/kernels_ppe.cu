@@ -36,6 +36,7 @@ namespace {
 constexpr int PPE_ILP = 4;  // independent neighbour gathers in flight per lane
 constexpr int CG_TPB = MPS_CG_TPB;
 constexpr int CG_MINB = MPS_CG_MINB;  // co-resident blocks per SM the register budget is set for
+static_assert(CG_TPB % 256 == 0, "phase A deals rows in super-chunks of 8 warps");
 
 struct PpeArgs {
   double4* pos4;  // .w: CG residual r during the solve, pressure at exit

@@ -69,7 +69,6 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
   if (c->cg_host) cudaFreeHost(c->cg_host);
   if (c->flags_host) cudaFreeHost(c->flags_host);
-  if (c->poll_event) cudaEventDestroy(c->poll_event);
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
 }
 
@@ -192,7 +191,6 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->cg, 1)); A(dalloc(&c->flags, 1)); A(dalloc(&c->io_tmp, N));
   A(cudaMallocHost((void**)&c->cg_host, sizeof(CgScalars)));
   A(cudaMallocHost((void**)&c->flags_host, sizeof(DevFlags)));
-  A(cudaEventCreateWithFlags(&c->poll_event, cudaEventDisableTiming));
   if (e != cudaSuccess) {
     g_init_error = std::string("allocation failed: ") + cudaGetErrorString(e);
     free_all(c);

@@ -34,21 +34,18 @@ __host__ __device__ __forceinline__ uint32_t back_slot(int stride, uint32_t kk) 
   return (uint32_t)stride - 8u * (kk / 8u + 1u) + (kk & 7u);
 }
 
-struct CgScalars {
-  double gamma, delta;          // r.r and r.Ar of the current iteration
-  double gamma_old, alpha_old;
-  double alpha, beta;
-  double bb, tol2bb;
+struct CgScalars {  // what k_ppe_cg reports at exit (block 0)
+  double gamma;                 // r.r of the last iteration
+  double bb, tol2bb;            // b.b and cg_rtol^2 b.b
   int iters, done, converged, maxit;
-  unsigned int blocks_done, pad;
   int n_surface, n_rows;
-  int barrier_timeout, pad2;
+  int barrier_timeout, pad;
 };
 
 // Grid-wide barrier state of the persistent CG kernel (zeroed at init).
 struct GridBar {
-  unsigned int count;
-  unsigned int gen;
+  unsigned int count;  // arrivals since the launch (monotonic; a barrier waits for nb x generation)
+  unsigned int pad;
 };
 
 struct DevFlags {
@@ -135,7 +132,6 @@ struct mps_ctx {
   DevFlags* flags = nullptr;
   DevFlags* flags_host = nullptr;  // pinned
   double* io_tmp = nullptr;   // n doubles, staging for get/set
-  cudaEvent_t poll_event = nullptr;
   // state
   bool binned = false;
   int64_t reuse_count = 0;  // steps since the ctx started reusing rows (rebin_every > 1)

@@ -45,19 +45,6 @@ __device__ __forceinline__ double pair_r2(double dx, double dy, double dz, int s
   return dx * dx + dy * dy + dz * dz;
 }
 
-// ---- 32-byte particle record loads -------------------------------------------------
-// Coherent (ld.global, L1-cached, invalidated by a gpu-scope fence): used inside the
-// persistent CG kernel where pos4.w changes between phases.
-__device__ __forceinline__ double4 ld_pos4(const double4* p) {
-  double4 v;
-  asm volatile("ld.global.v2.f64 {%0, %1}, [%4];\n\t"
-               "ld.global.v2.f64 {%2, %3}, [%4+16];"
-               : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w)
-               : "l"(p)
-               : "memory");
-  return v;
-}
-
 // ---- reductions over the L lanes that share a row (L a power of two <= 32) -----------
 template <int L>
 __device__ __forceinline__ double group_sum(double v) {
