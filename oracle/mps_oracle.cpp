@@ -84,7 +84,7 @@ void lattice_constants(int dim, double l0, double re, double* n0, double* lam, i
 struct Orc {
   Prm prm;
   int n = 0;
-  std::vector<double> f[21];  // x y z u v w n p ax ay az nut b phat gx gy gz xcg dndt n_k dndt_k
+  std::vector<double> f[22];  // x y z u v w n p ax ay az nut b phat gx gy gz xcg dndt n_k dndt_k rho_s
   std::vector<int> type, phase, bc, key, perm, cell_start;
   double h = 0, inv_h = 0;
   int nc[3] = {0, 0, 0};
@@ -461,9 +461,49 @@ struct Orc {
       f[13][i] = m;
     }
   }
+  // NEXT-2 (Q25): the smoothed density <rho>_i "set for each particle before starting
+  // the simulation": kernel-weighted mean of the neighbours' densities over N(i, r_n).
+  bool rho_s_ready = false;
+  void smooth_density() {
+    ensure_binned();
+    const double re = prm.re_n;
+    for (int i = 0; i < n; ++i) {
+      double sw = 0.0, srw = 0.0;
+      for_neighbours(i, re, [&](int j, double, double, double, double r2) {
+        const double w = w_of(re, r2);
+        sw += w;
+        srw += prm.rho[phase[j]] * w;
+      });
+      f[21][i] = sw > 0.0 ? srw / sw : prm.rho[phase[i]];
+    }
+    rho_s_ready = true;
+  }
+  // step 9, variant 3 (Eq.11-12; Q25): the multi-density pressure term of the
+  // weakly-compressible model, alpha_i = p_i / rho_i (Eq.12 times nothing: p_i = rho_i alpha_i),
+  //   (1/rho_i) <grad p>_i = (d/n0) sum ((<rho>_j / <rho>_i) alpha_j - alpha_i) / r^2 r_ij w,
+  // stored as G_i = rho_i x that, so that the corrector's (dt / rho_i) G_i applies it as is.
+  void gradient_multiphase() {
+    ensure_binned();
+    const double re = prm.re_n, d = prm.dim;
+    for (int i = 0; i < n; ++i) {
+      f[14][i] = f[15][i] = f[16][i] = 0.0;
+      if (type[i] != FLUID) continue;
+      const double rho_i = prm.rho[phase[i]];
+      const double ai = f[7][i] / rho_i, rsi = f[21][i];
+      double s[3] = {0, 0, 0};
+      for_neighbours(i, re, [&](int j, double dx, double dy, double dz, double r2) {
+        if (type[j] == DUMMY) return;
+        const double aj = f[7][j] / prm.rho[phase[j]];
+        const double c = (f[21][j] / rsi * aj - ai) / r2 * w_of(re, r2);
+        s[0] += c * dx; s[1] += c * dy; s[2] += c * dz;
+      });
+      for (int a = 0; a < 3; ++a) f[14 + a][i] = rho_i * (d / n0_n * s[a]);
+    }
+  }
   // step 9 (variant 0: cited method [8], BASELINE cfg 2; variant 1: Eq.14
   // as printed; variant 2: BASELINE cfg 3 wording "(P_i+P_j)/r^2"; Q13).
   void gradient() {
+    if (prm.grad_variant == 3) { gradient_multiphase(); return; }
     ensure_binned();
     const double re = prm.re_n, d = prm.dim;
     for (int i = 0; i < n; ++i) {
@@ -505,6 +545,7 @@ struct Orc {
     if (step_count % prm.rebin_every == 0) {
       use_lists = false;
       bin();
+      if (prm.grad_variant == 3 && !rho_s_ready) smooth_density();
       build_lists();
     }
     use_lists = true;
@@ -530,6 +571,7 @@ struct Orc {
   int step(int route) {
     if (prm.rebin_every > 1) return step_reuse(route);
     bin();                // 1
+    if (prm.grad_variant == 3 && !rho_s_ready) smooth_density();  // once, at the initial positions
     if (route == 1 && prm.ppe_source == 2) {  // ECS keeps n^k and (Dn/Dt)^k (Eq.17)
       density();
       f[19] = f[6];
@@ -588,14 +630,15 @@ void orc_set_brute(void* h, int b) { ((Orc*)h)->brute = (b != 0); }
 
 int orc_set_f64(void* h, int field, const double* src) {
   Orc* o = (Orc*)h;
-  if (field < 0 || field >= 21) return -1;
+  if (field < 0 || field >= 22) return -1;
   std::copy(src, src + o->n, o->f[field].begin());
   if (field < 3) o->binned = false;
+  if (field == 21) o->rho_s_ready = true;
   return 0;
 }
 int orc_get_f64(void* h, int field, double* dst) {
   Orc* o = (Orc*)h;
-  if (field < 0 || field >= 21) return -1;
+  if (field < 0 || field >= 22) return -1;
   std::copy(o->f[field].begin(), o->f[field].end(), dst);
   return 0;
 }
@@ -670,6 +713,7 @@ int orc_ppe_rhs(void* h) { ((Orc*)h)->ppe_rhs(); return 0; }
 int orc_ppe_apply(void* h, const double* xin, double* yout) { ((Orc*)h)->ppe_apply(xin, yout); return 0; }
 int orc_ppe_solve(void* h, double rtol, int maxit) { return ((Orc*)h)->ppe_solve(rtol, maxit); }
 int orc_pressure_ppe(void* h) { return ((Orc*)h)->pressure_ppe(); }
+void orc_smooth_density(void* h) { ((Orc*)h)->smooth_density(); }
 void orc_dndt(void* h, int dst) { ((Orc*)h)->dndt(dst == 20 ? 20 : 18); }
 int orc_phat(void* h) { ((Orc*)h)->phat(); return 0; }
 int orc_gradient(void* h) { ((Orc*)h)->gradient(); return 0; }

@@ -16,7 +16,7 @@ _lib = None
 
 F64 = {"x": 0, "y": 1, "z": 2, "u": 3, "v": 4, "w": 5, "n": 6, "p": 7, "ax": 8, "ay": 9,
        "az": 10, "nut": 11, "b": 12, "phat": 13, "gx": 14, "gy": 15, "gz": 16, "xcg": 17,
-       "dndt": 18, "n_k": 19, "dndt_k": 20}
+       "dndt": 18, "n_k": 19, "dndt_k": 20, "rho_s": 21}
 I32 = {"type": 0, "phase": 1, "bc": 2, "key": 3, "perm": 4}
 
 _dp = C.POINTER(C.c_double)
@@ -41,7 +41,7 @@ def lib():
         L.orc_get_cell_start.argtypes = [C.c_void_p, _ip]
         L.orc_neighbours.restype = C.c_longlong
         L.orc_neighbours.argtypes = [C.c_void_p, C.c_double, _ip, _ip, C.c_longlong]
-        for nm in ("orc_bin", "orc_density", "orc_viscosity", "orc_predict",
+        for nm in ("orc_smooth_density", "orc_bin", "orc_density", "orc_viscosity", "orc_predict",
                    "orc_pressure_explicit", "orc_ppe_flags", "orc_ppe_rhs", "orc_pressure_ppe",
                    "orc_phat", "orc_gradient", "orc_correct"):
             getattr(L, nm).argtypes = [C.c_void_p]
@@ -171,6 +171,7 @@ class Oracle:
     def viscosity(self): self.L.orc_viscosity(self.h)
     def predict(self): self.L.orc_predict(self.h)
     def pressure_explicit(self): self.L.orc_pressure_explicit(self.h)
+    def smooth_density(self): self.L.orc_smooth_density(self.h)
     def freeze_lists(self, on: bool = True): self.L.orc_freeze_lists(self.h, 1 if on else 0)
     def dndt(self, keep: bool = False): self.L.orc_dndt(self.h, 20 if keep else 18)
     def ppe_flags(self): self.L.orc_ppe_flags(self.h)

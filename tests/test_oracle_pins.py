@@ -723,3 +723,78 @@ def test_list_reuse_equals_exact_mode_while_no_pair_crosses_a_radius():
     a.step(4, 0); b.step(4, 0)
     for k in "xyz":
         assert np.abs(a.get(k) - b.get(k)).max() <= 1e-12 * s.params["l0"]
+
+
+# ---- NEXT-2: multi-density pressure term of the weakly-compressible model (Eq. 11-12) ----
+def test_smoothed_density_closed_form_at_a_flat_interface():
+    # lattice block, lower half rho_a, upper half rho_b.  A particle in the layer just below the
+    # interface sees, above it, the offsets (0,0,1), 4 x (1,0,1), 4 x (1,1,1), (0,0,2) within 2.1 l0:
+    # S1 = 1.1 + 4 (2.1/sqrt2 - 1) + 4 (2.1/sqrt3 - 1) + 0.05; <rho> = (rho_a (n0 - S1) + rho_b S1)/n0
+    m = 10
+    s = scenes.fluid_blob(L0, (m, m, m))
+    iz = np.rint(s.z / L0 - 0.5).astype(int)
+    s.phase[iz >= m // 2] = 1
+    ra, rb = 1000.0, 800.0
+    o = O.Oracle(s, n_phases=2, rho=(ra, rb), grad_variant=3)
+    o.bin(); o.smooth_density()
+    rs = o.get("rho_s")
+    n0 = GOLD["n0_3d_2.1"]
+    S1 = 1.1 + 4 * (2.1 / math.sqrt(2) - 1) + 4 * (2.1 / math.sqrt(3) - 1) + 0.05
+    S2 = 0.05                                             # two layers below: only (0,0,2) reaches across
+    core_xy = _interior_mask(s, m, 3)
+    below1 = core_xy & (iz == m // 2 - 1); below2 = core_xy & (iz == m // 2 - 2)
+    above1 = core_xy & (iz == m // 2)
+    assert below1.sum() > 0 and below2.sum() > 0
+    assert np.allclose(rs[below1], (ra * (n0 - S1) + rb * S1) / n0, rtol=1e-13)
+    assert np.allclose(rs[below2], (ra * (n0 - S2) + rb * S2) / n0, rtol=1e-13)
+    assert np.allclose(rs[above1], (rb * (n0 - S1) + ra * S1) / n0, rtol=1e-13)
+    # single phase: <rho> = rho exactly
+    o1 = O.Oracle(scenes.small_tank(), grad_variant=3)
+    o1.bin(); o1.smooth_density()
+    assert np.allclose(o1.get("rho_s"), 1000.0, rtol=1e-14, atol=0)
+
+
+def test_multiphase_pressure_term_brute_force_and_single_phase_limit():
+    s = scenes.small_tank(shuffle=True)
+    s.phase[s.z > 0.03] = 1
+    rho = np.array([1000.0, 800.0])
+    o = O.Oracle(s, n_phases=2, rho=tuple(rho), grad_variant=3)
+    o.bin(); o.smooth_density()
+    rng = np.random.default_rng(9)
+    p = rng.uniform(0.0, 500.0, s.n)
+    p[s.type == scenes.DUMMY] = 0.0
+    o.set("p", p); o.gradient()
+    re = s.params["re_n"]
+    dx = s.x[None, :] - s.x[:, None]; dy = s.y[None, :] - s.y[:, None]; dz = s.z[None, :] - s.z[:, None]
+    r2 = (dx * dx + dy * dy) + dz * dz
+    m = (r2 < re * re) & (s.type != scenes.DUMMY)[None, :]
+    np.fill_diagonal(m, False)
+    r2s = np.where(m, r2, 1.0)
+    w = np.where(m, re / np.sqrt(r2s) - 1.0, 0.0)
+    # smoothed density (all neighbours, dummies included)
+    mall = r2 < re * re
+    np.fill_diagonal(mall, False)
+    wall_ = np.where(mall, re / np.sqrt(np.where(mall, r2, 1.0)) - 1.0, 0.0)
+    rj = rho[s.phase]
+    rs = (wall_ * rj[None, :]).sum(axis=1) / wall_.sum(axis=1)
+    assert np.allclose(o.get("rho_s"), rs, rtol=1e-12)
+    al = p / rj
+    coef = (rs[None, :] / rs[:, None]) * al[None, :] - al[:, None]
+    c = coef / r2s * w
+    n0 = GOLD["n0_3d_2.1"]
+    fluid = s.type == scenes.FLUID
+    for comp, d in (("gx", dx), ("gy", dy), ("gz", dz)):
+        ref = rj * (3.0 / n0) * (c * d).sum(axis=1)
+        got = o.get(comp)
+        assert np.allclose(got[fluid], ref[fluid], rtol=1e-11, atol=1e-9 * np.abs(ref[fluid]).max())
+        assert (got[~fluid] == 0).all()
+    # single phase, linear pressure on the lattice: G = grad p exactly ((p_j - p_i) form)
+    mm = 10
+    b = scenes.fluid_blob(L0, (mm, mm, mm))
+    core = _interior_mask(b, mm, 3)
+    gvec = np.array([4.0, -3.0, 2.0])
+    o2 = O.Oracle(b, grad_variant=3)
+    o2.bin(); o2.smooth_density()
+    o2.set("p", gvec[0] * b.x + gvec[1] * b.y + gvec[2] * b.z + 30.0); o2.gradient()
+    for k, comp in enumerate(("gx", "gy", "gz")):
+        assert np.allclose(o2.get(comp)[core], gvec[k], rtol=1e-10)
