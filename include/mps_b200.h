@@ -48,7 +48,7 @@ enum { MPS_ORDER_ORIGINAL = 0, MPS_ORDER_SORTED = 1 };
 enum { MPS_ROUTE_EXPLICIT = 0, MPS_ROUTE_PPE = 1 };
 enum { MPS_RADIUS_N = 0, MPS_RADIUS_LAP = 1 };
 
-/* field ids for mps_get_field / mps_set_field.  0..20 are fp64, 32..35 int32. */
+/* field ids for mps_get_field / mps_set_field.  0..21 are fp64, 32..35 int32. */
 enum {
   MPS_F_X = 0, MPS_F_Y = 1, MPS_F_Z = 2,       /* position r */
   MPS_F_U = 3, MPS_F_V = 4, MPS_F_W = 5,       /* velocity u */
@@ -62,6 +62,7 @@ enum {
   MPS_F_XCG = 17,                              /* CG solution before the clamp (Q4) */
   MPS_F_DNDT = 18,                             /* Dn/Dt of the last mps_dndt (Eq. 15, Q22) */
   MPS_F_NK = 19, MPS_F_DNDTK = 20,             /* n and Dn/Dt kept from the start of the step (Eq. 17) */
+  MPS_F_RHOS = 21,                             /* smoothed density <rho> of the multi-density model (Q25) */
   MPS_I_TYPE = 32, MPS_I_PHASE = 33,
   MPS_I_BC = 34,                               /* -1 dummy/ghost, 1 free surface, 0 PPE unknown (Eq. 6) */
   MPS_I_KEY = 35                               /* cell key of the last mps_bin (read only) */
@@ -74,7 +75,8 @@ typedef struct mps_params {
                                in 2D the caller keeps z constant, w = 0 and g[2] = 0 */
   int32_t n_phases;         /* 1 or 2 */
   int32_t cg_maxit;         /* (2000) then MPS_ERR_NOCONV; Q15 */
-  int32_t grad_variant;     /* 0: (p_j - phat_i) standard [8]; 1: Eq. 14 as printed; 2: (p_i + p_j); Q13 */
+  int32_t grad_variant;     /* 0: (p_j - phat_i) standard [8]; 1: Eq. 14 as printed; 2: (p_i + p_j); Q13;
+                               3: multi-density term of the weakly-compressible model, Eq. 11-12; Q25 */
   int32_t clamp_negative_p; /* (1) p < 0 -> 0 after either pressure route; Q4 */
   int32_t rho_pair_mean;    /* 0 arithmetic (default), 1 harmonic; Q6 */
   int32_t nu_pair_mean;     /* 1 harmonic (default), 0 arithmetic; Q9 */
@@ -179,6 +181,12 @@ int mps_pressure_explicit(mps_ctx* ctx);
  * Returns MPS_ERR_NOCONV if cg_maxit was reached (pressures still written). */
 int mps_pressure_ppe(mps_ctx* ctx, int32_t* iters_out, double* relres_out);
 
+/* mps_smooth_density: <rho>_i = sum_j rho_j w / sum_j w over N(i, re_n) at the current positions
+ * ("set for each particle before starting the simulation"; Q25); the value follows its
+ * particle through later sorts.  mps_step calls it once, before the first step, when
+ * grad_variant = 3.  Needs mps_bin. */
+int mps_smooth_density(mps_ctx* ctx);
+
 /* mps_dndt: Dn/Dt_i = -sum_{j in N(i, re_n)} re_n / r^3 (x_ij . u_ij) at the current positions
  * and velocities, every non-ghost i (Eq. 15, the material derivative of Eq. 5; sign:
  * Q22).  keep = 0 writes MPS_F_DNDT; keep = 1 writes MPS_F_DNDTK and copies the ctx's n field to
@@ -187,7 +195,8 @@ int mps_dndt(mps_ctx* ctx, int32_t keep);
 
 /* mps_gradient: p-hat (minimum over i and its non-dummy neighbours within re_n;
  * P:215, Q12) then the pressure gradient of fluid i, variant grad_variant
- * (Eq. 14; Q13). */
+ * (Eq. 14; Q13).  Variant 3: G_i = rho_i (d/n0) sum ((<rho>_j/<rho>_i) alpha_j - alpha_i)/r^2
+ * (r_j - r_i) w, alpha = p/rho (Eq. 11-12; Q25), no p-hat. */
 int mps_gradient(mps_ctx* ctx);
 
 /* mps_correct: u = u* - (dt / rho_i) G; r = r* + dt (u - u*) for fluid; walls

@@ -24,13 +24,13 @@ RADIUS_N, RADIUS_LAP = 0, 1
 
 FIELDS = {"x": 0, "y": 1, "z": 2, "u": 3, "v": 4, "w": 5, "n": 6, "p": 7, "ax": 8, "ay": 9,
           "az": 10, "nut": 11, "b": 12, "phat": 13, "gx": 14, "gy": 15, "gz": 16, "xcg": 17,
-          "dndt": 18, "nk": 19, "dndtk": 20,
+          "dndt": 18, "nk": 19, "dndtk": 20, "rhos": 21,
           "type": 32, "phase": 33, "bc": 34, "key": 35}
 TIMERS = ["bin_sort", "bin_list", "viscosity", "predict", "density", "pressure_explicit",
           "ppe_setup", "cg_spmv", "cg_update", "gradient", "correct"]
 
 # Names the header declares (checked by tests/test_abi.py against include/mps_b200.h).
-SYMBOLS = ["mps_init", "mps_init_host", "mps_destroy", "mps_bin", "mps_density", "mps_dndt", "mps_viscosity",
+SYMBOLS = ["mps_init", "mps_init_host", "mps_destroy", "mps_bin", "mps_density", "mps_dndt", "mps_smooth_density", "mps_viscosity",
            "mps_predict", "mps_pressure_explicit", "mps_pressure_ppe", "mps_gradient",
            "mps_correct", "mps_step", "mps_step_host", "mps_upload_host", "mps_download_host",
            "mps_get_field", "mps_set_field",
@@ -108,7 +108,7 @@ def _load():
     L.mps_init.argtypes = [C.POINTER(vp), C.POINTER(MpsParams), i64] + [vp] * 8 + [vp]
     L.mps_init_host.argtypes = L.mps_init.argtypes
     L.mps_destroy.argtypes = [vp]
-    for nm in ("mps_bin", "mps_density", "mps_viscosity", "mps_predict", "mps_pressure_explicit",
+    for nm in ("mps_smooth_density", "mps_bin", "mps_density", "mps_viscosity", "mps_predict", "mps_pressure_explicit",
                "mps_gradient", "mps_correct", "mps_sync"):
         getattr(L, nm).argtypes = [vp]
     L.mps_dndt.argtypes = [vp, i32]
@@ -204,6 +204,7 @@ class Mps:
     # ---- the path --------------------------------------------------------------
     def bin(self): self._ck(lib.mps_bin(self.h))
     def density(self): self._ck(lib.mps_density(self.h))
+    def smooth_density(self): self._ck(lib.mps_smooth_density(self.h))
     def dndt(self, keep: bool = False): self._ck(lib.mps_dndt(self.h, 1 if keep else 0))
     def viscosity(self): self._ck(lib.mps_viscosity(self.h))
     def predict(self): self._ck(lib.mps_predict(self.h))

@@ -164,7 +164,8 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
                           double4* __restrict__ pos_out, double4* __restrict__ vel_out,
                           uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out,
                           uint32_t* __restrict__ ent_out, const double2* __restrict__ keep_in,
-                          double2* __restrict__ keep_out) {
+                          double2* __restrict__ keep_out, const double* __restrict__ rs_in,
+                          double* __restrict__ rs_out) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   uint32_t c = key[s];
@@ -183,6 +184,7 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
   tp_out[f] = tj;
   oid_out[f] = me;
   if (keep_in) keep_out[f] = keep_in[src];  // (n^k, (Dn/Dt)^k) of Eq. 17 follow their particle
+  if (rs_in) rs_out[f] = rs_in[src];        // so does the smoothed density of Eq. 11
   // the neighbour-row entry that names this particle (flags of mps_internal.h)
   ent_out[f] = f | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
                ((tj & 0x100) ? NB_PHASE1 : 0u);
@@ -588,7 +590,8 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_reorder, div_up(n, TPB), TPB, n, nc, c->key, c->cell_start,
              c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
              c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent,
-             c->prm.ppe_source == 2 ? c->keep2[cur] : nullptr, c->keep2[nxt]);
+             c->prm.ppe_source == 2 ? c->keep2[cur] : nullptr, c->keep2[nxt],
+             c->prm.grad_variant == 3 ? c->rho_s[cur] : nullptr, c->rho_s[nxt]);
   c->cur = nxt;
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
   if (c->prm.cell_div == 1 && !c->rows_by_warp) {
@@ -614,6 +617,7 @@ static const double* scalar_field(mps_ctx* c, int field) {
     case MPS_F_PHAT: return c->phat;
     case MPS_F_XCG: return c->cg_x;
     case MPS_F_DNDT: return c->dndt;
+    case MPS_F_RHOS: return c->rho_s[c->cur];
   }
   return nullptr;
 }
@@ -621,7 +625,7 @@ static const double* scalar_field(mps_ctx* c, int field) {
 int mpsk_get_field(mps_ctx* c, int field, void* dst, int order) {
   int n = (int)c->n;
   int cur = c->cur;
-  if (field >= 0 && field <= MPS_F_DNDTK) {
+  if (field >= 0 && field <= MPS_F_RHOS) {
     MPS_LAUNCH(c, MPS_T_BIN_SORT, k_get_f64, div_up(n, TPB), TPB, n, field, order, c->pos4[cur],
                c->vel4[cur], c->acc4, c->grad4, scalar_field(c, field), c->keep2[cur], c->oid[cur],
                (double*)dst);
@@ -638,7 +642,8 @@ int mpsk_get_field(mps_ctx* c, int field, void* dst, int order) {
 int mpsk_set_field(mps_ctx* c, int field, const void* src, int order) {
   int n = (int)c->n;
   int cur = c->cur;
-  if (field >= 0 && field <= MPS_F_DNDTK) {
+  if (field >= 0 && field <= MPS_F_RHOS) {
+    if (field == MPS_F_RHOS) c->rho_s_ready = true;
     MPS_LAUNCH(c, MPS_T_BIN_SORT, k_set_f64, div_up(n, TPB), TPB, n, field, order, c->pos4[cur],
                c->vel4[cur], c->acc4, c->grad4, (double*)scalar_field(c, field), c->keep2[cur],
                c->oid[cur], (const double*)src);

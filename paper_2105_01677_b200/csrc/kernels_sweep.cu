@@ -38,6 +38,39 @@ k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restric
   if (row_live && sub == 0) dens[i] = s;
 }
 
+// ------------------------------------ NEXT-2: smoothed density of the multi-density model ---
+// <rho>_i = sum_j rho_j w(r_ij) / sum_j w(r_ij) over N(i, re_n), every non-ghost i; rho_j comes
+// from the phase bit of the row entry (Q25).  No neighbour: the particle's own density.
+__global__ void __launch_bounds__(TPB)
+k_smooth_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
+                 const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn,
+                 double* __restrict__ rho_s) {
+  ROW_GROUP(i, sub);
+  const double4 pi = pos4[ii];
+  const uint32_t* row = row_ptr(nbr, kc.stride, ii);
+  const uint32_t m = row_live ? cn[ii] : 0u;
+  double sw = 0.0, srw = 0.0;
+  for (uint32_t k = sub; k < m; k += L) {
+    const uint32_t e = row[k];
+    const double4 q = pos4[e & NB_INDEX];
+    const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double w = kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, rsqrt_f64(r2));
+    sw += w;
+    srw = fma(kc.rho[(e & NB_PHASE1) ? 1 : 0], w, srw);
+  }
+  sw = group_sum<L>(sw);
+  srw = group_sum<L>(srw);
+  if (row_live && sub == 0) rho_s[i] = sw > 0.0 ? srw / sw : kc.rho[(tp[i] >> 8) & 1];
+}
+
+// stage beta_i = <rho>_i alpha_i = <rho>_i p_i / rho_i into pos4.w for the variant-3 gradient
+__global__ void k_stage_beta(KConst kc, const double* __restrict__ p, const double* __restrict__ rho_s,
+                             const uint32_t* __restrict__ tp, double4* __restrict__ pos4) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < kc.n) pos4[i].w = rho_s[i] * (p[i] / kc.rho[(tp[i] >> 8) & 1]);
+}
+
 // ---------------------------------------------------- NEXT-1: Dn/Dt (MPS-HS) ---
 // Dn/Dt_i = d/dt sum_j (re_n / r_ij - 1) = -sum_{j in N(i, re_n)} re_n / r^3 (x_ij . u_ij),
 // x_ij = x_j - x_i, u_ij = u_j - u_i; walls and dummies hold u = 0 in vel4 (P:224-228
@@ -266,8 +299,10 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
   const double4 pi = pos4[ii];  // .w = p_i
   const uint32_t* row = row_ptr(nbr, kc.stride, ii);
   const uint32_t m = (fluid || wall) ? cn[ii] : 0u;
-  double phi;
-  if (VARIANT == 1) {
+  double phi = 0.0;
+  if (VARIANT == 3) {
+    // pi.w = beta_i; phat carries <rho> (see mpsk_gradient): nothing to pre-compute
+  } else if (VARIANT == 1) {
     phi = phat[ii];
   } else {
     double mn = pi.w;
@@ -280,6 +315,12 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     }
     phi = group_min<L>(mn);
     if (row_live && sub == 0) phat[i] = (fluid || wall) ? phi : 0.0;
+  }
+  double inv_rsi = 0.0, ai = 0.0, scale = kc.d_over_n0;
+  if (VARIANT == 3) {
+    inv_rsi = 1.0 / phat[ii];     // phat points at <rho> for this variant
+    ai = pi.w * inv_rsi;          // alpha_i = beta_i / <rho>_i
+    scale *= kc.rho[(tp[ii] >> 8) & 1];  // stored as rho_i x Eq. 11: the corrector divides by rho_i
   }
   double sx = 0.0, sy = 0.0, sz = 0.0;
   const uint32_t mg = fluid ? m : 0u;
@@ -295,7 +336,8 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     double coef;
     if (VARIANT == 0) coef = q.w - phi;
     else if (VARIANT == 1) coef = (pi.w + q.w) - (phi + phat[j]);
-    else coef = pi.w + q.w;
+    else if (VARIANT == 2) coef = pi.w + q.w;
+    else coef = fma(q.w, inv_rsi, -ai);  // (<rho>_j / <rho>_i) alpha_j - alpha_i, Eq. 11
     const double c = coef * kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, ir) * ir * ir;
     sx += c * dx;
     sy += c * dy;
@@ -305,7 +347,7 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
   sy = group_sum<L>(sy);
   sz = group_sum<L>(sz);
   if (row_live && sub == 0)
-    grad4[i] = make_double4(kc.d_over_n0 * sx, kc.d_over_n0 * sy, kc.d_over_n0 * sz, 0.0);
+    grad4[i] = make_double4(scale * sx, scale * sy, scale * sz, 0.0);
 }
 
 // --------------------------------------------------------------- S11 corrector ---
@@ -338,6 +380,15 @@ int mpsk_density(mps_ctx* c) {
   int n = (int)c->n;
   MPS_LAUNCH(c, MPS_T_DENSITY, k_density, group_grid(n), TPB, c->kc, c->pos4[c->cur], c->nbr, c->cn,
              c->dens);
+  return MPS_OK;
+}
+
+int mpsk_smooth_density(mps_ctx* c) {
+  int n = (int)c->n;
+  int cur = c->cur;
+  MPS_LAUNCH(c, MPS_T_DENSITY, k_smooth_density, group_grid(n), TPB, c->kc, c->pos4[cur], c->tp[cur],
+             c->nbr, c->cn, c->rho_s[cur]);
+  c->rho_s_ready = true;
   return MPS_OK;
 }
 
@@ -385,6 +436,14 @@ int mpsk_pressure_explicit(mps_ctx* c) {
 int mpsk_gradient(mps_ctx* c) {
   int n = (int)c->n;
   int cur = c->cur;
+  if (c->prm.grad_variant == 3) {
+    MPS_LAUNCH(c, MPS_T_GRADIENT, k_stage_beta, div_up(n, 256), 256, c->kc, c->p, c->rho_s[cur], c->tp[cur],
+               c->pos4[cur]);
+    c->posw_is_p = false;
+    MPS_LAUNCH(c, MPS_T_GRADIENT, k_gradient<3>, group_grid(n), TPB, c->kc, c->pos4[cur], c->rho_s[cur],
+               c->tp[cur], c->nbr, c->cn, c->grad4);
+    return MPS_OK;
+  }
   if (!c->posw_is_p) {
     MPS_LAUNCH(c, MPS_T_GRADIENT, k_stage_p, div_up(n, 256), 256, n, c->p, c->pos4[cur]);
     c->posw_is_p = true;

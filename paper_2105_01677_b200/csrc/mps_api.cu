@@ -63,7 +63,7 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->tmp_oid); cudaFree(c->cell_count); cudaFree(c->cell_start); cudaFree(c->scan_tmp);
   cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co);
   cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
-  cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
+  cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->rho_s[0]); cudaFree(c->rho_s[1]); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
   cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
   cudaFree(c->cg_rows); cudaFree(c->cg_bcount); cudaFree(c->cg_bar);
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
@@ -93,7 +93,7 @@ static int check_params(const mps_params* p, int64_t n) {
   if (p->kernel < 0 || p->kernel > 1) return fail(nullptr, MPS_ERR_ARG, "kernel must be 0 (Eq. 3) or 1 (Eq. 4)");
   if (p->kernel == 1 && (p->ppe_source != 0 || p->ppe_laplacian != 0))
     return fail(nullptr, MPS_ERR_ARG, "Eq. 15-18 are derived for the Eq. 3 kernel: kernel 1 needs ppe_source = ppe_laplacian = 0");
-  if (p->grad_variant < 0 || p->grad_variant > 2) return fail(nullptr, MPS_ERR_ARG, "grad_variant must be 0..2");
+  if (p->grad_variant < 0 || p->grad_variant > 3) return fail(nullptr, MPS_ERR_ARG, "grad_variant must be 0..3");
   if (!(p->rho[0] > 0) || (p->n_phases == 2 && !(p->rho[1] > 0)))
     return fail(nullptr, MPS_ERR_ARG, "densities must be positive");
   if (!(p->gamma > 0) || !(p->cg_rtol > 0) || p->cg_maxit < 1)
@@ -183,7 +183,8 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
   A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
   A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->dndt, N));
-  A(dalloc(&c->keep2[0], N)); A(dalloc(&c->keep2[1], N)); A(dalloc(&c->grad4, N)); A(dalloc(&c->bc, N));
+  A(dalloc(&c->keep2[0], N)); A(dalloc(&c->keep2[1], N));
+  A(dalloc(&c->rho_s[0], N)); A(dalloc(&c->rho_s[1], N)); A(dalloc(&c->grad4, N)); A(dalloc(&c->bc, N));
   A(dalloc(&c->cg_x, N)); A(dalloc(&c->cg_p, N)); A(dalloc(&c->cg_s, N)); A(dalloc(&c->cg_w, N));
   A(dalloc(&c->cg_part, (size_t)2 * (c->sm_count * 8 + 8)));
   A(dalloc(&c->cg_rows, N)); A(dalloc(&c->cg_bcount, (size_t)2 * (c->sm_count * 8 + 8)));
@@ -220,7 +221,10 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   cudaMemsetAsync(c->cg_rows, 0, N * 4, s);
   cudaMemsetAsync(c->flags, 0, sizeof(DevFlags), s);
   double* zero_d[] = {c->dens, c->p, c->nut, c->b, c->phat, c->dndt, c->cg_x, c->cg_p, c->cg_s, c->cg_w};
-  for (int b = 0; b < 2; ++b) cudaMemsetAsync(c->keep2[b], 0, N * sizeof(double2), s);
+  for (int b = 0; b < 2; ++b) {
+    cudaMemsetAsync(c->keep2[b], 0, N * sizeof(double2), s);
+    cudaMemsetAsync(c->rho_s[b], 0, N * sizeof(double), s);
+  }
   for (double* z : zero_d) cudaMemsetAsync(z, 0, N * sizeof(double), s);
   cudaMemsetAsync(c->acc4, 0, N * sizeof(double4), s);
   cudaMemsetAsync(c->grad4, 0, N * sizeof(double4), s);
@@ -359,6 +363,12 @@ int mps_density(mps_ctx* c) {
   CK(cudaGetLastError());
   return MPS_OK;
 }
+int mps_smooth_density(mps_ctx* c) {
+  NEED_BIN(c);
+  mpsk_smooth_density(c);
+  CK(cudaGetLastError());
+  return MPS_OK;
+}
 int mps_dndt(mps_ctx* c, int32_t keep) {
   NEED_BIN(c);
   mpsk_dndt(c, keep ? 1 : 0);
@@ -414,6 +424,11 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
   const bool ecs = route == MPS_ROUTE_PPE && c->prm.ppe_source == 2;
   const bool hs = route == MPS_ROUTE_PPE && c->prm.ppe_source >= 1;
   const int K = c->prm.rebin_every;
+  if (nsteps > 0 && c->prm.grad_variant == 3 && !c->rho_s_ready) {
+    // the smoothed density is set once, at the initial positions, from rows of every particle
+    mpsk_bin(c);
+    mpsk_smooth_density(c);
+  }
   for (int s = 0; s < nsteps; ++s) {
     if (K > 1) {
       // list reuse (Q24): bin (all rows, both radii) once every K steps at r^k; every sweep of
@@ -505,6 +520,7 @@ int mps_upload_host(mps_ctx* c, const double* x, const double* y, const double* 
   c->binned = false;
   c->ppe_ready = false;
   c->reuse_count = 0;  // new particle order: the stored rows are void
+  c->rho_s_ready = false;
   return MPS_OK;
 }
 

@@ -112,6 +112,8 @@ struct mps_ctx {
   double* b = nullptr;
   double* phat = nullptr;
   double* dndt = nullptr;
+  double* rho_s[2] = {nullptr, nullptr};   // smoothed density (grad_variant 3), carried through the re-sort
+  bool rho_s_ready = false;
   double2* keep2[2] = {nullptr, nullptr};  // (n^k, (Dn/Dt)^k) of Eq. 17, carried through the re-sort
   double4* grad4 = nullptr;
   int8_t* bc = nullptr;
@@ -174,6 +176,7 @@ void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out,
                          uint32_t* tmp);
 int mpsk_density(mps_ctx* c);
 int mpsk_dndt(mps_ctx* c, int keep);
+int mpsk_smooth_density(mps_ctx* c);
 int mpsk_viscosity(mps_ctx* c);
 int mpsk_predict(mps_ctx* c);
 int mpsk_pressure_explicit(mps_ctx* c);

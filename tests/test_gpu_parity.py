@@ -591,3 +591,31 @@ def test_list_reuse_every_four_steps(B, O, route, rows, monkeypatch):
     o1 = O.Oracle(s)
     o1.step(10, route)
     assert np.abs(o1.get("x") - o.get("x")).max() > 1e-9 * s.params["l0"]
+
+
+# ------------------- NEXT-2: multi-density pressure term of the WC model (Eq. 11-12) ---
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_multiphase_wc_pressure_term(B, O, kernel):
+    s = scenes.small_tank(shuffle=True)
+    s.phase[s.z > 0.03] = 1
+    over = dict(n_phases=2, rho=(1000.0, 800.0), nu=(1e-6, 5e-6), grad_variant=3, kernel=kernel)
+    g = B.Mps(s, **over); o = O.Oracle(s, **over)
+    g.bin(); g.smooth_density(); o.bin(); o.smooth_density()
+    rs = o.get("rho_s")
+    assert rs.min() >= 800.0 - 1e-9 and rs.max() <= 1000.0 + 1e-9 and np.unique(np.round(rs, 6)).size > 10
+    assert relerr(g.get("rhos"), rs, 1.0) <= TOL
+    # the value follows its particle through a re-sort after motion
+    o.step(2, 0)
+    inject(g, o, ("x", "y", "z", "u", "v", "w"))
+    g.set("rhos", o.get("rho_s"))
+    g.bin()
+    assert np.array_equal(g.get("rhos"), o.get("rho_s"))
+    g.density(); o.bin(); o.density()
+    g.pressure_explicit(); o.pressure_explicit()
+    g.gradient(); o.gradient()
+    assert vec_relerr([g.get(k) for k in ("gx", "gy", "gz")], [o.get(k) for k in ("gx", "gy", "gz")], 1.0) <= TOL
+    # whole steps: smoothing is done once by the first mps_step
+    eL, el0, moved, g2, o2 = _trajectory(B, O, s, 12, 0, **over)
+    print(f"multi-density WC term, kernel {kernel}, 12 explicit steps: max |dr|/L = {eL:.2e}, moved {moved:.3f} l0")
+    assert eL <= 1e-7
+    assert relerr(g2.get("rhos"), o2.get("rho_s"), 1.0) <= TOL
