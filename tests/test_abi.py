@@ -66,7 +66,7 @@ def _init_rc(B, **over):
 
 
 @pytest.mark.parametrize("over", [
-    dict(dim=4), dict(dim=2, ppe_laplacian=1), dict(ppe_source=3), dict(kernel=2), dict(kernel=1, ppe_source=1), dict(rebin_every=0), dict(l0=0.0), dict(dt=-1.0), dict(re_grad=0.5), dict(re_lap=0.001),
+    dict(dim=4), dict(dim=2, ppe_laplacian=1), dict(ppe_source=3), dict(kernel=2), dict(kernel=1, ppe_source=1), dict(rebin_every=0), dict(_n=0), dict(_n=-5), dict(l0=0.0), dict(dt=-1.0), dict(re_grad=0.5), dict(re_lap=0.001),
     dict(cell_div=0), dict(cell_div=4), dict(key_mode=1), dict(n_phases=3), dict(max_neighbours=0),
     dict(grad_variant=4), dict(rho=(0.0, 1.0)), dict(cg_rtol=0.0), dict(domain_max=(0.0, 1.0, 1.0)),
 ])

@@ -619,3 +619,36 @@ def test_multiphase_wc_pressure_term(B, O, kernel):
     print(f"multi-density WC term, kernel {kernel}, 12 explicit steps: max |dr|/L = {eL:.2e}, moved {moved:.3f} l0")
     assert eL <= 1e-7
     assert relerr(g2.get("rhos"), o2.get("rho_s"), 1.0) <= TOL
+
+
+def test_max_size_8m_sampled(B, O):
+    """The largest configured size (config 5[4], N = 7,932,816; 32-bit slot indices, 921k cells,
+    10 GB of neighbour rows): sort invariants, and neighbour counts and densities of sampled
+    particles against the brute-force definition."""
+    s = scenes.make_scene(5, sweep_index=4)
+    assert s.n == 7932816
+    g = B.Mps(s)
+    g.bin(); g.density()
+    st = g.stats()
+    assert st["device_error"] == 0 and st["n_ghost"] == 0 and 100 < st["max_neighbours"] <= 300
+    key = g.get("key"); perm = g.perm()
+    ks = key[perm].astype(np.int64)
+    assert (np.diff(ks) >= 0).all()
+    assert (np.diff(perm.astype(np.int64))[np.diff(ks) == 0] > 0).all()       # stable
+    assert np.array_equal(np.sort(perm), np.arange(s.n, dtype=perm.dtype))    # a permutation
+    cs = g.cell_start()
+    assert cs[0] == 0 and cs[-1] == s.n and (np.diff(cs.astype(np.int64)) >= 0).all()
+    n = g.get("n")
+    cnt_l = g.neighbour_counts(B.RADIUS_LAP)
+    rn, rl = s.params["re_n"], s.params["re_lap"]
+    for i in np.random.default_rng(8).choice(s.n, 40, replace=False):
+        dx, dy, dz = s.x - s.x[i], s.y - s.y[i], s.z - s.z[i]
+        r2 = (dx * dx + dy * dy) + dz * dz
+        ml = r2 < rl * rl
+        ml[i] = False
+        assert cnt_l[i] == ml.sum()
+        mn = r2 < rn * rn
+        mn[i] = False
+        assert abs(n[i] - (rn / np.sqrt(r2[mn]) - 1.0).sum()) <= 1e-10 * 14.4
+    g.step(1, 0)                     # one whole explicit step at this size
+    assert g.stats()["device_error"] == 0 and np.isfinite(g.get("p")).all()
