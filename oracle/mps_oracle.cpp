@@ -21,7 +21,10 @@
 // hand-computed n0 / lambda shells, lattice densities, free-surface counts,
 // Laplacian of a quadratic, gradient of a linear field, Eq. 7 value, operator
 // symmetry / row sums, CG vs dense Cholesky, momentum conservation, hydrostatic
-// rho*g*h.  Whole-step trajectories in a moving fluid: the paper prints no
+// rho*g*h; NEXT rows: Dn/Dt (dilation closed form, brute force, finite difference of the density),
+// HS/ECS worked example, HL shell sum and dense solve, 2D constants and closed forms, Eq. 4 shell
+// sums, list reuse against brute force on the stored sets, smoothed density at a flat interface and
+// the multi-density term by brute force.  Whole-step trajectories in a moving fluid: the paper prints no
 // values => "parity unpinned" against the paper for those (pinned on the parts).
 #include <algorithm>
 #include <cmath>
