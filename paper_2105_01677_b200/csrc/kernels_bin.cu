@@ -593,6 +593,8 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
              c->prm.ppe_source == 2 ? c->keep2[cur] : nullptr, c->keep2[nxt],
              c->prm.grad_variant == 3 ? c->rho_s[cur] : nullptr, c->rho_s[nxt]);
   c->cur = nxt;
+  c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
+  c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
   if (c->prm.cell_div == 1 && !c->rows_by_warp) {
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, c->kc, c->pos4[nxt],

@@ -40,6 +40,7 @@ static_assert(CG_TPB % 256 == 0, "phase A deals rows in super-chunks of 8 warps"
 
 struct PpeArgs {
   double4* pos4;  // .w: CG residual r during the solve, pressure at exit
+  cudaTextureObject_t tex;  // pos4 as 16-byte texels (0: not used)
   const uint32_t* tp;
   const double* dens;
   const double* dndt;      // (Dn/Dt)* (ppe_source >= 1)
@@ -136,8 +137,9 @@ __device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, Cg
 // c_ij = A_lap w(r_ij) / rho_ij (Listing 2; Q5, Q6).  r_j is read from
 // pos4.w, which is 0 on free-surface slots (Dirichlet p = 0).  The L lanes of the
 // group each take every L-th entry; the result is valid in every lane.
-template <bool TWO_PHASE, int L>
-__device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4, const uint32_t* tp,
+template <bool TWO_PHASE, int L, bool TEX>
+__device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4, cudaTextureObject_t tex,
+                                          const uint32_t* tp,
                                           const uint32_t* nbr, const uint32_t* cn, const uint32_t* co,
                                           int i, int sub, bool live, double& ri) {
   // every lane of the warp must come through here (full-mask shuffles below): a
@@ -165,7 +167,14 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 #pragma unroll
     for (int u = 0; u < PPE_ILP; ++u) {
       if (e[u] & NB_DUMMY) q[u] = make_double4(pi.x + kc.re_lap, pi.y, pi.z, pi.w);
-      else q[u] = pos4[e[u] & NB_INDEX];
+      else if (TEX) {
+        // (x, y) never change during a solve: fetched through the texture front end, which works
+        // in parallel with the LSU; (z, r) -- r changes every iteration -- take the coherent path
+        const uint32_t j = e[u] & NB_INDEX;
+        const int4 xy = tex1Dfetch<int4>(tex, 2 * (int)j);
+        const double2 zr = reinterpret_cast<const double2*>(pos4 + j)[1];
+        q[u] = make_double4(__hiloint2double(xy.y, xy.x), __hiloint2double(xy.w, xy.z), zr.x, zr.y);
+      } else q[u] = pos4[e[u] & NB_INDEX];
     }
 #pragma unroll
     for (int u = 0; u < PPE_ILP; ++u) {
@@ -190,7 +199,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 }
 
 // ---- the persistent solve -------------------------------------------------------------
-template <bool TWO_PHASE, int L>
+template <bool TWO_PHASE, int L, bool TEX>
 __global__ void __launch_bounds__(CG_TPB, CG_MINB)
 k_ppe_cg(KConst kc, PpeArgs a) {
   __shared__ uint32_t sh_cnt[2][CG_TPB / 32];
@@ -319,7 +328,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         const bool live = g < n_rows;
         const int i = live ? (int)a.rows[g] : 0;
         double ri;
-        const double wi = ppe_row<TWO_PHASE, L>(kc, a.pos4, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+        const double wi = ppe_row<TWO_PHASE, L, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
         if (live && sub == 0) {
           a.wv[i] = wi;
           g_part = fma(ri, ri, g_part);
@@ -416,7 +425,7 @@ k_ppe_apply(KConst kc, const double4* pos4, const uint32_t* __restrict__ tp, con
   const bool in = i < kc.n;
   const bool live = in && bc[i] == 0;
   double ri;
-  const double wi = ppe_row<TWO_PHASE, L>(kc, pos4, tp, nbr, cn, co, in ? i : 0, sub, live, ri);
+  const double wi = ppe_row<TWO_PHASE, L, false>(kc, pos4, 0, tp, nbr, cn, co, in ? i : 0, sub, live, ri);
   if (in && sub == 0) wv[i] = live ? wi : 0.0;
 }
 __global__ void k_stage_out(int n, int order, const uint32_t* __restrict__ oid,
@@ -426,16 +435,16 @@ __global__ void k_stage_out(int n, int order, const uint32_t* __restrict__ oid,
   dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = src[i];
 }
 
-template <bool TWO_PHASE, int L>
+template <bool TWO_PHASE, int L, bool TEX>
 cudaError_t launch_cg(mps_ctx* c, PpeArgs& a, int grid) {
   void* params[] = {(void*)&c->kc, (void*)&a};
-  return cudaLaunchCooperativeKernel((const void*)k_ppe_cg<TWO_PHASE, L>, dim3(grid), dim3(CG_TPB),
+  return cudaLaunchCooperativeKernel((const void*)k_ppe_cg<TWO_PHASE, L, TEX>, dim3(grid), dim3(CG_TPB),
                                      params, 0, c->stream);
 }
-template <bool TWO_PHASE, int L>
+template <bool TWO_PHASE, int L, bool TEX>
 int cg_blocks_per_sm() {
   int nb = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_ppe_cg<TWO_PHASE, L>, CG_TPB, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_ppe_cg<TWO_PHASE, L, TEX>, CG_TPB, 0);
   return nb;
 }
 
@@ -448,11 +457,9 @@ bool two_phase(const mps_ctx* c) { return c->prm.n_phases > 1 && c->prm.rho[0] !
 int mpsk_ppe_plan(mps_ctx* c) {
   int per_sm = 2;
   const bool tp = two_phase(c);
-  switch (c->cg_lanes) {
-    case 4: per_sm = tp ? cg_blocks_per_sm<true, 4>() : cg_blocks_per_sm<false, 4>(); break;
-    case 16: per_sm = tp ? cg_blocks_per_sm<true, 16>() : cg_blocks_per_sm<false, 16>(); break;
-    default: c->cg_lanes = 8; per_sm = tp ? cg_blocks_per_sm<true, 8>() : cg_blocks_per_sm<false, 8>(); break;
-  }
+  c->cg_lanes = 8;  // 4 and 16 lanes per row measured within 5 % of 8
+  if (c->cg_tex) per_sm = tp ? cg_blocks_per_sm<true, 8, true>() : cg_blocks_per_sm<false, 8, true>();
+  else per_sm = tp ? cg_blocks_per_sm<true, 8, false>() : cg_blocks_per_sm<false, 8, false>();
   if (per_sm < 1) return MPS_ERR_CUDA;
   if (per_sm > CG_MINB) per_sm = CG_MINB;
   c->cg_grid = per_sm * c->sm_count;
@@ -462,7 +469,7 @@ int mpsk_ppe_plan(mps_ctx* c) {
 int mpsk_pressure_ppe(mps_ctx* c) {
   const int cur = c->cur;
   PpeArgs a;
-  a.pos4 = c->pos4[cur]; a.tp = c->tp[cur]; a.dens = c->dens; a.dndt = c->dndt; a.keep2 = c->keep2[cur]; a.bc = c->bc; a.b = c->b;
+  a.pos4 = c->pos4[cur]; a.tex = c->cg_tex ? c->pos_tex[cur] : 0; a.tp = c->tp[cur]; a.dens = c->dens; a.dndt = c->dndt; a.keep2 = c->keep2[cur]; a.bc = c->bc; a.b = c->b;
   a.x = c->cg_x; a.pv = c->cg_p; a.sv = c->cg_s; a.wv = c->cg_w; a.p = c->p;
   a.nbr = c->nbr; a.cn = c->cn; a.co = c->co; a.rows = c->cg_rows; a.bcount = c->cg_bcount;
   a.part = c->cg_part; a.cg = c->cg; a.bar = c->cg_bar;
@@ -476,11 +483,8 @@ int mpsk_pressure_ppe(mps_ctx* c) {
   if (((c)->timer_mask >> MPS_T_CG_SPMV) & 1u) mps_timer_begin(c, MPS_T_CG_SPMV);
   cudaError_t e;
   const bool tp = two_phase(c);
-  switch (c->cg_lanes) {
-    case 4: e = tp ? launch_cg<true, 4>(c, a, grid) : launch_cg<false, 4>(c, a, grid); break;
-    case 16: e = tp ? launch_cg<true, 16>(c, a, grid) : launch_cg<false, 16>(c, a, grid); break;
-    default: e = tp ? launch_cg<true, 8>(c, a, grid) : launch_cg<false, 8>(c, a, grid); break;
-  }
+  if (c->cg_tex) e = tp ? launch_cg<true, 8, true>(c, a, grid) : launch_cg<false, 8, true>(c, a, grid);
+  else e = tp ? launch_cg<true, 8, false>(c, a, grid) : launch_cg<false, 8, false>(c, a, grid);
   c->launches++;
   c->t_launches[MPS_T_CG_SPMV]++;
   if (((c)->timer_mask >> MPS_T_CG_SPMV) & 1u) mps_timer_end(c, MPS_T_CG_SPMV);

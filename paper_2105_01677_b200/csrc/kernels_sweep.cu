@@ -28,7 +28,7 @@ k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restric
   const uint32_t m = row_live ? cn[ii] : 0u;
   double s = 0.0;
   for (uint32_t k = sub; k < m; k += L) {
-    const double4 q = pos4[row[k] & NB_INDEX];
+    const double4 q = gather_rec(kc.pos_tex, pos4, row[k] & NB_INDEX);
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = pair_r2(dx, dy, dz, kc.stale);
     if (kc.stale && !(r2 < kc.re_n2)) continue;  // reused row: the pair has left the radius
@@ -52,7 +52,7 @@ k_smooth_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __
   double sw = 0.0, srw = 0.0;
   for (uint32_t k = sub; k < m; k += L) {
     const uint32_t e = row[k];
-    const double4 q = pos4[e & NB_INDEX];
+    const double4 q = gather_rec(kc.pos_tex, pos4, e & NB_INDEX);
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = dx * dx + dy * dy + dz * dz;
     const double w = kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, rsqrt_f64(r2));
@@ -87,8 +87,8 @@ k_dndt(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ 
   double s = 0.0;
   for (uint32_t k = sub; k < m; k += L) {
     const uint32_t j = row[k] & NB_INDEX;
-    const double4 q = pos4[j];
-    const double4 vj = vel4[j];
+    const double4 q = gather_rec(kc.pos_tex, pos4, j);
+    const double4 vj = gather_rec(kc.vel_tex, vel4, j);
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = pair_r2(dx, dy, dz, kc.stale);
     if (kc.stale && !(r2 < kc.re_n2)) continue;
@@ -123,8 +123,8 @@ k_nu_eff(KConst kc, int with_sps, const double4* __restrict__ pos4, double4* __r
     double G[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
     for (uint32_t k = sub; k < m; k += L) {
       const uint32_t j = row[k] & NB_INDEX;
-      const double4 q = pos4[j];
-      const double4 vj = vel4[j];  // walls and dummies hold u = 0
+      const double4 q = gather_rec(kc.pos_tex, pos4, j);
+      const double4 vj = gather_rec(kc.vel_tex, vel4, j);  // walls and dummies hold u = 0
       const double dr[3] = {q.x - pi.x, q.y - pi.y, q.z - pi.z};
       const double du[3] = {vj.x - vi.x, vj.y - vi.y, vj.z - vi.z};
       const double r2 = pair_r2(dr[0], dr[1], dr[2], kc.stale);
@@ -179,8 +179,8 @@ k_viscosity(KConst kc, const double4* __restrict__ pos4, const double4* __restri
   for (uint32_t k = sub; k < m; k += L) {
     const uint32_t e = row_entry(row, kc.stride, nf, k);
     const uint32_t j = e & NB_INDEX;
-    const double4 q = pos4[j];
-    const double4 vj = vel4[j];
+    const double4 q = gather_rec(kc.pos_tex, pos4, j);
+    const double4 vj = gather_rec(kc.vel_tex, vel4, j);
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = pair_r2(dx, dy, dz, kc.stale);
     if (kc.stale && !(r2 < kc.re_lap2)) continue;
@@ -274,7 +274,7 @@ k_phat(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__
   for (uint32_t k = sub; k < m; k += L) {
     const uint32_t e = row[k];
     if (e & NB_DUMMY) continue;
-    const double4 q = pos4[e & NB_INDEX];
+    const double4 q = gather_rec(kc.pos_tex, pos4, e & NB_INDEX);
     if (kc.stale && !(pair_r2(q.x - pi.x, q.y - pi.y, q.z - pi.z, 1) < kc.re_n2)) continue;
     mn = fmin(mn, q.w);
   }
@@ -309,7 +309,7 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     for (uint32_t k = sub; k < m; k += L) {
       const uint32_t e = row[k];
       if (e & NB_DUMMY) continue;
-      const double4 q = pos4[e & NB_INDEX];
+      const double4 q = gather_rec(kc.pos_tex, pos4, e & NB_INDEX);
       if (kc.stale && !(pair_r2(q.x - pi.x, q.y - pi.y, q.z - pi.z, 1) < kc.re_n2)) continue;
       mn = fmin(mn, q.w);
     }
@@ -328,7 +328,7 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     const uint32_t e = row[k];
     if (e & NB_DUMMY) continue;
     const uint32_t j = e & NB_INDEX;
-    const double4 q = pos4[j];
+    const double4 q = gather_rec(kc.pos_tex, pos4, j);
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = pair_r2(dx, dy, dz, kc.stale);
     if (kc.stale && !(r2 < kc.re_n2)) continue;

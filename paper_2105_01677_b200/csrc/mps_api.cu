@@ -57,6 +57,8 @@ static cudaError_t dalloc(T** p, size_t count) {
 
 static void free_all(mps_ctx* c) {
   for (int k = 0; k < 2; ++k) {
+    if (c->pos_tex[k]) cudaDestroyTextureObject(c->pos_tex[k]);
+    if (c->vel_tex[k]) cudaDestroyTextureObject(c->vel_tex[k]);
     cudaFree(c->pos4[k]); cudaFree(c->vel4[k]); cudaFree(c->tp[k]); cudaFree(c->oid[k]);
   }
   cudaFree(c->ent); cudaFree(c->key); cudaFree(c->key_tmp); cudaFree(c->rank); cudaFree(c->tmp_src);
@@ -199,19 +201,39 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     return MPS_ERR_CUDA;
   }
   {
-    // lanes per row of the CG operator: 8 by default; MPS_B200_CG_LANES = 4 | 8 | 16 for tuning
     const char* rw = getenv("MPS_B200_ROWS");
     // few occupied cells cannot fill the GPU with one warp per cell: small scenes use one
     // warp per particle (measured crossover between scene 2, 89 k, and scene 3, 438 k)
     c->rows_by_warp = rw ? !strcmp(rw, "warp") : (n < 200000);
-    const char* ev = getenv("MPS_B200_CG_LANES");
-    c->cg_lanes = ev ? atoi(ev) : 8;
-    if (mpsk_ppe_plan(c) != MPS_OK) {
-      g_init_error = "k_ppe_cg cannot be made resident on this device";
-      free_all(c);
-      delete c;
-      return MPS_ERR_CUDA;
+  }
+  {
+    // texture views of the two position buffers (MPS_B200_CG_TEX=0 switches them off)
+    const char* tx = getenv("MPS_B200_CG_TEX");
+    c->cg_tex = (tx ? atoi(tx) != 0 : true) && (2 * (N + 32) <= (size_t)prop.maxTexture1DLinear);
+    for (int b = 0; b < 4 && c->cg_tex; ++b) {
+      cudaResourceDesc rd;
+      memset(&rd, 0, sizeof(rd));
+      rd.resType = cudaResourceTypeLinear;
+      rd.res.linear.devPtr = b < 2 ? (void*)c->pos4[b] : (void*)c->vel4[b - 2];
+      rd.res.linear.desc = cudaCreateChannelDesc<int4>();
+      rd.res.linear.sizeInBytes = (b < 2 ? N + 32 : N) * sizeof(double4);
+      cudaTextureDesc td;
+      memset(&td, 0, sizeof(td));
+      td.readMode = cudaReadModeElementType;
+      cudaTextureObject_t* dst = b < 2 ? &c->pos_tex[b] : &c->vel_tex[b - 2];
+      if (cudaCreateTextureObject(dst, &rd, &td, nullptr) != cudaSuccess) {
+        cudaGetLastError();
+        c->cg_tex = false;
+      }
     }
+    c->kc.pos_tex = c->cg_tex ? c->pos_tex[c->cur] : 0;
+    c->kc.vel_tex = c->cg_tex ? c->vel_tex[c->cur] : 0;
+  }
+  if (mpsk_ppe_plan(c) != MPS_OK) {
+    g_init_error = "k_ppe_cg cannot be made resident on this device";
+    free_all(c);
+    delete c;
+    return MPS_ERR_CUDA;
   }
   memset(c->cg_host, 0, sizeof(CgScalars));
   memset(c->flags_host, 0, sizeof(DevFlags));

@@ -74,6 +74,9 @@ struct KConst {  // by-value kernel parameter
   int stride; // row stride in entries (cap + 14 rounded up to a multiple of 8)
   int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean;
   int n;      // particles
+  // the current position / velocity buffers as 16-byte texels (0: not used): the first half of a
+  // record is fetched through the texture front end, which works in parallel with the LSU
+  cudaTextureObject_t pos_tex, vel_tex;
 };
 
 struct mps_ctx {
@@ -86,6 +89,9 @@ struct mps_ctx {
   // double-buffered sorted particle arrays
   double4* pos4[2] = {nullptr, nullptr};
   double4* vel4[2] = {nullptr, nullptr};
+  cudaTextureObject_t pos_tex[2] = {0, 0};  // pos4 / vel4 viewed as 16-byte texels
+  cudaTextureObject_t vel_tex[2] = {0, 0};
+  bool cg_tex = false;
   uint32_t* tp[2] = {nullptr, nullptr};
   uint32_t* oid[2] = {nullptr, nullptr};
   uint32_t* ent = nullptr;         // per slot: own index | NB_* flags (what a neighbour row stores)

@@ -45,6 +45,20 @@ __device__ __forceinline__ double pair_r2(double dx, double dy, double dz, int s
   return dx * dx + dy * dy + dz * dz;
 }
 
+// ---- neighbour record gathers ------------------------------------------------------
+// A sweep is bound by the rate at which the LSU serves one 32-byte record per lane per pair
+// (profiles/r01_ceilings_microbench.md).  When the texture view exists, the first 16 bytes come
+// through the texture front end and the second 16 through the LSU: the two work in parallel
+// (measured 1.2x).  Only data that no thread writes during the kernel may take the texture path.
+__device__ __forceinline__ double4 gather_rec(cudaTextureObject_t tex, const double4* __restrict__ a, uint32_t j) {
+  if (tex) {
+    const int4 lo = tex1Dfetch<int4>(tex, 2 * (int)j);
+    const double2 hi = reinterpret_cast<const double2*>(a + j)[1];
+    return make_double4(__hiloint2double(lo.y, lo.x), __hiloint2double(lo.w, lo.z), hi.x, hi.y);
+  }
+  return a[j];
+}
+
 // ---- reductions over the L lanes that share a row (L a power of two <= 32) -----------
 template <int L>
 __device__ __forceinline__ double group_sum(double v) {
