@@ -47,10 +47,11 @@ __device__ __forceinline__ double rsqrt_f64(double x) {
   double t = x * y, e = fma(-t, y, 1.0), q = fma(e, 0.375, 0.5);
   return fma(y, q * e, y);
 }
-template <int L, bool MATH>
+// SPLIT: first 16 bytes of the record through the texture unit, second 16 through the LSU
+template <int L, bool MATH, bool SPLIT>
 __global__ void __launch_bounds__(1024)
-k_gather(const double4* __restrict__ pos, const uint32_t* __restrict__ list, int NE, int nrows,
-         double* __restrict__ y) {
+k_gather(const double4* __restrict__ pos, cudaTextureObject_t tex, const uint32_t* __restrict__ list,
+         int NE, int nrows, double* __restrict__ y) {
   const int sub = threadIdx.x & (L - 1);
   const int gstride = gridDim.x * blockDim.x / L;
   for (int r = (blockIdx.x * blockDim.x + threadIdx.x) / L; r < nrows; r += gstride) {
@@ -59,7 +60,15 @@ k_gather(const double4* __restrict__ pos, const uint32_t* __restrict__ list, int
     double s = 0.0;
 #pragma unroll 4
     for (int k = sub; k < NE; k += L) {
-      const double4 q = pos[row[k]];
+      double4 q;
+      if (SPLIT) {
+        const uint32_t j = row[k];
+        const int4 lo = tex1Dfetch<int4>(tex, 2 * (int)j);
+        const double2 hi = reinterpret_cast<const double2*>(pos + j)[1];
+        q = make_double4(__hiloint2double(lo.y, lo.x), __hiloint2double(lo.w, lo.z), hi.x, hi.y);
+      } else {
+        q = pos[row[k]];
+      }
       if (MATH) {
         const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
         const double r2 = dx * dx + dy * dy + dz * dz;
@@ -132,11 +141,20 @@ int main() {
     CK(cudaMalloc(&dy, (size_t)N * 8));
     CK(cudaMemcpy(dp, hp.data(), (size_t)N * 32, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(dl, hl.data(), hl.size() * 4, cudaMemcpyHostToDevice));
+    cudaResourceDesc rd = {};
+    rd.resType = cudaResourceTypeLinear;
+    rd.res.linear.devPtr = dp;
+    rd.res.linear.desc = cudaCreateChannelDesc<int4>();
+    rd.res.linear.sizeInBytes = (size_t)N * 32;
+    cudaTextureDesc td = {};
+    td.readMode = cudaReadModeElementType;
+    cudaTextureObject_t tex;
+    CK(cudaCreateTextureObject(&tex, &rd, &td, nullptr));
     auto run = [&](auto kern, const char* name) {
-      kern<<<sms, 1024>>>(dp, dl, NE, N, dy);
+      kern<<<sms, 1024>>>(dp, tex, dl, NE, N, dy);
       cudaDeviceSynchronize();
       cudaEventRecord(e0);
-      for (int r = 0; r < 5; ++r) kern<<<sms, 1024>>>(dp, dl, NE, N, dy);
+      for (int r = 0; r < 5; ++r) kern<<<sms, 1024>>>(dp, tex, dl, NE, N, dy);
       cudaEventRecord(e1);
       cudaDeviceSynchronize();
       cudaEventElapsedTime(&ms, e0, e1);
@@ -145,10 +163,12 @@ int main() {
              name, ms * 1e9 / N, NE, ms * 1e-3 * ghz * 1e9 * sms / ((double)N * NE) * 32,
              (double)N * (NE * 4 + 41) / (ms * 1e-3) / 1e9);
     };
-    run(k_gather<8, true>, "L=8, pair arithmetic");
-    run(k_gather<8, false>, "L=8, loads only");
-    run(k_gather<16, true>, "L=16, pair arithmetic");
-    run(k_gather<32, true>, "L=32, pair arithmetic");
+    run(k_gather<8, true, false>, "L=8, pair arithmetic");
+    run(k_gather<8, false, false>, "L=8, loads only");
+    run(k_gather<16, true, false>, "L=16, pair arithmetic");
+    run(k_gather<32, true, false>, "L=32, pair arithmetic");
+    run(k_gather<8, true, true>, "L=8, TEX+LSU split, arith.");
+    run(k_gather<8, false, true>, "L=8, TEX+LSU split, loads");
   }
   return 0;
 }
