@@ -149,7 +149,9 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
   const uint32_t* row = row_ptr(nbr, kc.stride, i);
   const uint32_t nf = live ? cn[i] : 0u;
   const uint32_t m = live ? nf + co[i] : 0u;
-  const double rho_i = TWO_PHASE ? kc.rho[(tp[i] >> 8) & 1] : kc.rho[0];
+  // 1 / rho_ij for a neighbour of phase 0 and of phase 1 (Q6): two values per row, no division per pair
+  const int ph_i = TWO_PHASE ? (int)((tp[i] >> 8) & 1) : 0;
+  const double inv_rij0 = kc.inv_rho_pair[ph_i][0], inv_rij1 = kc.inv_rho_pair[ph_i][1];
   const bool hl = kc.ppe_laplacian == 1;
   double s = 0.0;
   // batches of PPE_ILP entries per lane: entry loads, then gathers, then arithmetic, so the
@@ -184,10 +186,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
       // Eq. 10 form: A_lap (re/r - 1); MPS-HL (Eq. 16, Q23): (2 re / n0) / r^3
       double w = hl ? ir * ir * ir : kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, ir);
       if (TWO_PHASE) {
-        const double rho_j = kc.rho[(e[u] & NB_PHASE1) ? 1 : 0];
-        const double rij =
-            kc.rho_pair_mean == 1 ? 2.0 * rho_i * rho_j / (rho_i + rho_j) : 0.5 * (rho_i + rho_j);
-        w = w / rij;
+        w *= (e[u] & NB_PHASE1) ? inv_rij1 : inv_rij0;
       }
       if ((e[u] & NB_DUMMY) || (kc.stale && !(r2 < kc.re_lap2))) w = 0.0;  // dummy, empty slot, or left the radius
       s = fma(w, pi.w - q[u].w, s);

@@ -146,6 +146,11 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.relax_dt2 = prm->ppe_relax / (prm->dt * prm->dt);
   k.cs_l0_sq = (prm->cs * prm->l0) * (prm->cs * prm->l0);
   k.d_over_n0 = (double)prm->dim / k.n0_n;
+  for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b) {
+      const double ra = k.rho[a], rb = k.rho[b];
+      k.inv_rho_pair[a][b] = 1.0 / (prm->rho_pair_mean == 1 ? 2.0 * ra * rb / (ra + rb) : 0.5 * (ra + rb));
+    }
   k.relax = prm->ppe_relax;
   k.hl_c = 2.0 * prm->re_lap / k.n0_lap;
   k.ppe_source = prm->ppe_source; k.ppe_laplacian = prm->ppe_laplacian;

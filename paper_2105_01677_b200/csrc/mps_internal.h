@@ -62,6 +62,7 @@ struct KConst {  // by-value kernel parameter
   double rho[2], nu[2];
   double c0, gamma, beta, compress_dt2, relax_dt2;
   double cs_l0_sq, d_over_n0;
+  double inv_rho_pair[2][2];  // 1 / rho_ij by the phases of i and j (arithmetic or harmonic mean, Q6)
   double relax, hl_c;  // ppe_relax; 2 re_lap / n0_lap (Eq. 16)
   int ppe_source, ppe_laplacian;
   int kernel;          // 0: Eq. 3, 1: Eq. 4
