@@ -396,9 +396,9 @@ def run_b200(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by
 # hand from the ncu --set full capture summarised under profiles/ (key: scene, route, category).
 NCU_TRAFFIC = {
-    # profiles/r01b_scene2_scene3_ppe.md: per operator application (whole-solve DRAM bytes / applications)
-    (2, "ppe", "cg_spmv"): (20.14e6 + 0.25e6) / 53,
-    (3, "ppe", "cg_spmv"): (9.214e9 + 0.958e9) / 62,
+    # profiles/r01d_scene2_scene3_ppe.md: per operator application (whole-solve DRAM bytes / applications)
+    (2, "ppe", "cg_spmv"): (20.16e6 + 0.38e6) / 53,
+    (3, "ppe", "cg_spmv"): (9.293e9 + 1.011e9) / 62,
 }
 
 
