@@ -420,12 +420,12 @@ def test_full_size_sampled_config3(B, O):
     assert (np.diff(perm.astype(np.int64))[same] > 0).all()
 
 
-@pytest.mark.parametrize("cfg,idx", [(3, 0), (5, 2)])
+@pytest.mark.parametrize("cfg,idx", [(3, 0), (4, 0), (5, 2)])
 def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx):
-    """Configs 3 (N = 438,208) and 5[2] (N = 1,011,096) in the launch configuration bench.py
-    times (warp-per-cell row builder, 148 x 1024 persistent CG): density, flags, right-hand
-    side and operator against the oracle on identical positions, and the GPU's CG solution
-    checked by its true residual under the ORACLE's operator."""
+    """Configs 3 (N = 438,208), 4 (two-phase, Smagorinsky, N = 634,808) and 5[2] (N = 1,011,096)
+    in the launch configuration bench.py times (warp-per-cell row builder, 148 x 1024 persistent
+    CG): density, flags, right-hand side and operator against the oracle on identical positions,
+    and the GPU's CG solution checked by its true residual under the ORACLE's operator."""
     s = scenes.make_scene(cfg, sweep_index=idx)
     g = B.Mps(s)
     o = O.Oracle(s)
@@ -433,6 +433,11 @@ def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx):
     for k in ("x", "y", "z", "u", "v", "w"):
         o.set(k, g.get(k))
     g.bin(); o.bin()
+    if s.params["cs"] > 0:            # config 4: eddy viscosity and the two-viscosity Laplacian
+        g.viscosity(); o.viscosity()
+        assert o.get("nut").max() > 0
+        assert relerr(g.get("nut"), o.get("nut"), 1e-30) <= TOL
+        assert vec_relerr([g.get(k) for k in ("ax", "ay", "az")], [o.get(k) for k in ("ax", "ay", "az")], 9.81) <= TOL
     g.density(); o.density()
     n0 = o.constants()["n0_n"]
     assert relerr(g.get("n"), o.get("n"), n0) <= TOL
