@@ -332,6 +332,17 @@ def run_b200(args):
                 "units": {"N": scene.n, "ppe_rows": rows, "mean_k_re_n": kn, "mean_k_re_lap": kl,
                           "mean_k_re_lap_rows": klr},
                 "ms_per_step_instrumented": ms_replay / K}
+        if top == "cg_spmv" and rows:
+            # the two on-chip ceilings of a list-driven sweep (profiles/r01_ceilings_microbench.md):
+            # 15 fp64 instructions per pair at 1.86e13/s, and the record gather at 30.8 SM-cycles
+            # per 32 pairs (texture + LSU split) on 148 SMs at 1.965 GHz
+            pairs = rows * klr
+            t_use = 1e-3 * ms / max(uses, 1)
+            roof["on_chip_ceilings"] = {
+                "fp64_pipe_frac": pairs * 15.0 / 1.86e13 / t_use,
+                "l1_gather_frac": pairs / 32.0 * 30.8 / (148 * 1.965e9) / t_use,
+                "note": "fractions of the time of one operator application that the fp64 pipe and the "
+                        "L1 record gather would need at their measured peaks; the gather binds"}
 
     # ---- end to end: pinned host buffers in, one step, host buffers out, every step ----
     e2e = None
