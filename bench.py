@@ -295,6 +295,7 @@ def run_b200(args):
     if not args.no_replay:
         g = B.Mps(scene, device=str(dev))
         g.step(W, route)
+        cg_before_replay = g.stats()["cg_iters_total"]
         g.timers_enable((1 << len(B.TIMERS)) - 1)
         ms_replay = timed_steps(torch, 1, g, route, K, flush, stream)
         tm = g.timers_read()
@@ -303,7 +304,7 @@ def run_b200(args):
         g.close()
         # full operator applications / vector updates actually performed (launches issued after
         # convergence return at once; their time stays in the category's total)
-        cg_iters_timed = st_r["cg_iters_total"] - (stats["cg_iters_total"] - cg_timed_main)
+        cg_iters_timed = st_r["cg_iters_total"] - cg_before_replay
         cg_uses = {"cg_spmv": cg_iters_timed + K, "cg_update": cg_iters_timed}
         peak, peak_src = peaks()
         n_bins = tm["bin_list"][1]          # one row-builder launch per bin (2 per step; fewer with list reuse)
