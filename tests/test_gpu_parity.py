@@ -1,5 +1,5 @@
 """GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element
-by element on the same seeded inputs.  Bars (north_star / DESIGN.md section 5):
+by element on the same seeded inputs.  Bars (north_star / DESIGN.md section 4):
 bit-exact keys, sort, cell table and neighbour sets; single-step fp64 fields
 within 1e-10 (max-norm, relative to the field's scale); PPE pressure: true
 relative residual under the ORACLE's operator <= 2e-8; 20-step trajectories
