@@ -199,36 +199,79 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
 // front of the row, the others to the back; entries come out in ascending slot
 // order, so every later sum has a fixed order.
 constexpr int ROWS_TPB = 256;
-constexpr int ROWS_PPW = 4;  // particles per warp (consecutive slots: same candidate cells)
+constexpr int ROWS_PPW = 4;  // particles per warp (consecutive slots: almost always one cell)
+
+// Append the hits of one 32-candidate trip to the row of one particle: ballot compaction,
+// front part upwards, back part downwards (back_slot).  On overflow keep what fits, in order.
+__device__ __forceinline__ void row_append(uint32_t* row, int stride, uint32_t cap, uint32_t lt_mask,
+                                           bool in_n, bool in_o, uint32_t e, uint32_t& nf,
+                                           uint32_t& nb, bool& overflow) {
+  const uint32_t m_n = __ballot_sync(0xffffffffu, in_n);
+  const uint32_t m_o = __ballot_sync(0xffffffffu, in_o);
+  if ((m_n | m_o) == 0u) return;
+  const uint32_t add_n = (uint32_t)__popc(m_n), add_o = (uint32_t)__popc(m_o);
+  const uint32_t pn = (uint32_t)__popc(m_n & lt_mask), po = (uint32_t)__popc(m_o & lt_mask);
+  if (nf + nb + add_n + add_o <= cap) {
+    if (in_n) row[nf + pn] = e;
+    else if (in_o) row[back_slot(stride, nb + po)] = e;
+    nf += add_n;
+    nb += add_o;
+  } else {
+    overflow = true;
+    const uint32_t room = cap - (nf + nb);
+    if (in_n && pn < room) row[nf + pn] = e;
+    const uint32_t took_n = add_n < room ? add_n : room;
+    const uint32_t room_o = room - took_n;
+    if (in_o && po < room_o) row[back_slot(stride, nb + po)] = e;
+    nf += took_n;
+    nb += add_o < room_o ? add_o : room_o;
+  }
+}
+
+// exact squared distance of reading Q2
+__device__ __forceinline__ double r2_exact(const double4& q, const double4& p) {
+  const double dx = __dsub_rn(q.x, p.x), dy = __dsub_rn(q.y, p.y), dz = __dsub_rn(q.z, p.z);
+  return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
 
 __global__ void __launch_bounds__(ROWS_TPB)
 k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
-             const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
-             uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
-             DevFlags* __restrict__ flags, int fluid_only) {
+             const uint32_t* __restrict__ ent, const uint32_t* __restrict__ key,
+             const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
+             uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags,
+             int fluid_only) {
   const int lane = threadIdx.x & 31;
   const int warp = (blockIdx.x * ROWS_TPB + threadIdx.x) >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
-  const int R = kc.R_lap;
+  const int R = kc.R_lap, S = kc.stride;
   const uint32_t cap = (uint32_t)kc.cap;
+  const int i0 = warp * ROWS_PPW;
+  if (i0 >= kc.n) return;
   int warp_max = 0;
   bool coincident = false, overflow = false;
+  // which of the warp's particles want a row, and do they share one cell?
+  bool want[ROWS_PPW];
+  uint32_t kk[ROWS_PPW];
+  bool same = true;
+#pragma unroll
   for (int t = 0; t < ROWS_PPW; ++t) {
-    const int i = warp * ROWS_PPW + t;
-    if (i >= kc.n) break;
-    const uint32_t k = key[i];
-    if (k >= (uint32_t)kc.ncells || (fluid_only && (tp[i] & 0xff) != MPS_FLUID)) {
-      // ghosts have no neighbours; the first bin of a step serves fluid rows only
-      if (lane == 0) { cn[i] = 0; co[i] = 0; }
-      continue;
-    }
-    const double4 pi = pos4[i];
+    const int i = i0 + t;
+    kk[t] = i < kc.n ? key[i] : 0xffffffffu;
+    want[t] = i < kc.n && kk[t] < (uint32_t)kc.ncells && !(fluid_only && (tp[i] & 0xff) != MPS_FLUID);
+    if (i < kc.n && !want[t] && lane == 0) { cn[i] = 0; co[i] = 0; }  // ghost, or not needed by this bin
+    same = same && (kk[t] == kk[0]);
+  }
+  if (same && kk[0] < (uint32_t)kc.ncells) {
+    // ---- one candidate load per trip serves all ROWS_PPW particles -----------------------
+    const uint32_t k = kk[0];
     const int cx = (int)(k % (uint32_t)kc.nx);
     const int cy = (int)((k / (uint32_t)kc.nx) % (uint32_t)kc.ny);
     const int cz = (int)(k / ((uint32_t)kc.nx * (uint32_t)kc.ny));
     const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
-    uint32_t* row = nbr + (size_t)i * (size_t)kc.stride;
-    uint32_t nf = 0, nb = 0;  // warp-uniform
+    double4 pi[ROWS_PPW];
+    uint32_t nf[ROWS_PPW], nb[ROWS_PPW];
+#pragma unroll
+    for (int t = 0; t < ROWS_PPW; ++t) { pi[t] = pos4[i0 + t]; nf[t] = 0; nb[t] = 0; }
     for (int dz = -R; dz <= R; ++dz) {
       const int z2 = cz + dz;
       if (z2 < 0 || z2 >= kc.nz) continue;
@@ -240,49 +283,69 @@ k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
         const uint32_t je = cell_start[cbase + x_hi + 1];
         for (uint32_t j0 = js; j0 < je; j0 += 32) {
           const uint32_t j = j0 + (uint32_t)lane;
-          bool in_lap = false, in_n = false;
+          const bool valid = j < je;
+          double4 q = make_double4(0.0, 0.0, 0.0, 0.0);
           uint32_t e = 0;
-          if (j < je) {
-            const double4 q = pos4[j];
-            const double dx = __dsub_rn(q.x, pi.x), dy_ = __dsub_rn(q.y, pi.y), dz_ = __dsub_rn(q.z, pi.z);
-            const double r2 =
-                __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
-            in_lap = (r2 < kc.re_lap2) && (j != (uint32_t)i);
-            if (in_lap) {
-              in_n = r2 < kc.re_n2;
-              if (r2 == 0.0) coincident = true;
-              const uint32_t tj = tp[j];
-              const uint32_t ty = tj & 0xff;
-              e = j | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
-                  ((tj & 0x100) ? NB_PHASE1 : 0u);
-            }
-          }
-          const uint32_t m_n = __ballot_sync(0xffffffffu, in_n);
-          const uint32_t m_o = __ballot_sync(0xffffffffu, in_lap && !in_n);
-          const uint32_t add_n = (uint32_t)__popc(m_n), add_o = (uint32_t)__popc(m_o);
-          if (nf + nb + add_n + add_o <= cap) {
-            if (in_n) row[nf + (uint32_t)__popc(m_n & lt_mask)] = e;
-            else if (in_lap) row[back_slot(kc.stride, nb + (uint32_t)__popc(m_o & lt_mask))] = e;
-            nf += add_n;
-            nb += add_o;
-          } else {
-            // keep what fits (front entries first, in order), then stop storing
-            overflow = true;
-            const uint32_t room = cap - (nf + nb);
-            const uint32_t pn = (uint32_t)__popc(m_n & lt_mask);
-            if (in_n && pn < room) row[nf + pn] = e;
-            const uint32_t took_n = add_n < room ? add_n : room;
-            const uint32_t room_o = room - took_n;
-            const uint32_t po = (uint32_t)__popc(m_o & lt_mask);
-            if (in_lap && !in_n && po < room_o) row[back_slot(kc.stride, nb + po)] = e;
-            nf += took_n;
-            nb += add_o < room_o ? add_o : room_o;
+          if (valid) { q = pos4[j]; e = ent[j]; }
+#pragma unroll
+          for (int t = 0; t < ROWS_PPW; ++t) {
+            if (!want[t]) continue;  // warp-uniform
+            const double r2 = r2_exact(q, pi[t]);
+            const bool in_lap = valid && (r2 < kc.re_lap2) && (j != (uint32_t)(i0 + t));
+            const bool in_n = in_lap && (r2 < kc.re_n2);
+            if (in_lap && r2 == 0.0) coincident = true;
+            row_append(nbr + (size_t)(i0 + t) * (size_t)S, S, cap, lt_mask, in_n, in_lap && !in_n, e, nf[t],
+                       nb[t], overflow);
           }
         }
       }
     }
-    if (lane == 0) { cn[i] = nf; co[i] = nb; }
-    warp_max = max(warp_max, (int)(nf + nb));
+#pragma unroll
+    for (int t = 0; t < ROWS_PPW; ++t) {
+      if (!want[t]) continue;
+      if (lane == 0) { cn[i0 + t] = nf[t]; co[i0 + t] = nb[t]; }
+      warp_max = max(warp_max, (int)(nf[t] + nb[t]));
+    }
+  } else {
+    // ---- the warp straddles cells (or holds ghosts): one particle after the other ----------
+    for (int t = 0; t < ROWS_PPW; ++t) {
+      if (!want[t]) continue;
+      const int i = i0 + t;
+      const uint32_t k = kk[t];
+      const double4 pi = pos4[i];
+      const int cx = (int)(k % (uint32_t)kc.nx);
+      const int cy = (int)((k / (uint32_t)kc.nx) % (uint32_t)kc.ny);
+      const int cz = (int)(k / ((uint32_t)kc.nx * (uint32_t)kc.ny));
+      const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
+      uint32_t* row = nbr + (size_t)i * (size_t)S;
+      uint32_t nf = 0, nb = 0;  // warp-uniform
+      for (int dz = -R; dz <= R; ++dz) {
+        const int z2 = cz + dz;
+        if (z2 < 0 || z2 >= kc.nz) continue;
+        for (int dy = -R; dy <= R; ++dy) {
+          const int y2 = cy + dy;
+          if (y2 < 0 || y2 >= kc.ny) continue;
+          const int cbase = kc.nx * (y2 + kc.ny * z2);
+          const uint32_t js = cell_start[cbase + x_lo];
+          const uint32_t je = cell_start[cbase + x_hi + 1];
+          for (uint32_t j0 = js; j0 < je; j0 += 32) {
+            const uint32_t j = j0 + (uint32_t)lane;
+            bool in_lap = false, in_n = false;
+            uint32_t e = 0;
+            if (j < je) {
+              const double r2 = r2_exact(pos4[j], pi);
+              in_lap = (r2 < kc.re_lap2) && (j != (uint32_t)i);
+              in_n = in_lap && (r2 < kc.re_n2);
+              if (in_lap && r2 == 0.0) coincident = true;
+              e = ent[j];
+            }
+            row_append(row, S, cap, lt_mask, in_n, in_lap && !in_n, e, nf, nb, overflow);
+          }
+        }
+      }
+      if (lane == 0) { cn[i] = nf; co[i] = nb; }
+      warp_max = max(warp_max, (int)(nf + nb));
+    }
   }
   coincident = __any_sync(0xffffffffu, coincident);
   if (lane == 0) {
@@ -602,7 +665,7 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
   } else {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc,
-               c->pos4[nxt], c->tp[nxt], c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
+               c->pos4[nxt], c->tp[nxt], c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
   }
   c->binned = true;
   c->ppe_ready = false;
