@@ -140,12 +140,38 @@ __global__ void k_scan_apply(const uint32_t* __restrict__ in, uint32_t* __restri
   }
 }
 
+// Small inputs (a few tiles): the whole scan in ONE block, tile after tile with a running carry
+// -- one launch instead of three.
+__global__ void __launch_bounds__(TPB) k_scan_small(const uint32_t* __restrict__ in,
+                                                    uint32_t* __restrict__ out, int64_t n) {
+  uint32_t carry = 0;
+  for (int64_t tile = 0; tile < n; tile += SCAN_TILE) {
+    const int64_t base = tile + (int64_t)threadIdx.x * SCAN_ITEMS;
+    uint32_t v[SCAN_ITEMS];
+    uint32_t s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+      v[k] = (base + k < n) ? in[base + k] : 0;
+      s += v[k];
+    }
+    uint32_t tot;
+    uint32_t ex = block_exclusive_scan(s, &tot) + carry;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+      if (base + k < n) out[base + k] = ex;
+      ex += v[k];
+    }
+    carry += tot;
+  }
+}
+
 // ------------------------------------------------------- S2: scatter + reorder ---
 __global__ void k_scatter(int n, const uint32_t* __restrict__ key_tmp, const uint32_t* __restrict__ rank,
                           const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ oid,
                           uint32_t* __restrict__ tmp_src, uint32_t* __restrict__ tmp_oid,
-                          uint32_t* __restrict__ key) {
+                          uint32_t* __restrict__ key, int ncells, DevFlags* __restrict__ flags) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) flags->n_ghost = n - (int)cell_start[ncells];  // ghosts sit behind the last cell
   if (i >= n) return;
   uint32_t k = key_tmp[i];
   uint32_t dst = cell_start[k] + rank[i];
@@ -503,11 +529,6 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
   }
 }
 
-__global__ void k_count_ghosts(int n, int ncells, const uint32_t* __restrict__ cell_start,
-                               DevFlags* __restrict__ flags) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) flags->n_ghost = n - (int)cell_start[ncells];
-}
-
 // ---------------------------------------------------------- field get / set ---
 __global__ void k_get_f64(int n, int field, int order, const double4* __restrict__ pos4,
                           const double4* __restrict__ vel4, const double4* __restrict__ acc4,
@@ -624,6 +645,10 @@ __global__ void k_nb_fill(int n, int cap_row, int radius_id, const uint32_t* __r
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
                          uint32_t* tmp) {
   int ntiles = div_up(n, SCAN_TILE);
+  if (ntiles <= 16) {  // up to 32k entries: one block is faster than three launches
+    MPS_LAUNCH(c, cat, k_scan_small, 1, TPB, in, out, n);
+    return;
+  }
   MPS_LAUNCH(c, cat, k_scan_reduce, ntiles, TPB, in, n, tmp);
   MPS_LAUNCH(c, cat, k_scan_spine, 1, TPB, tmp, ntiles);
   MPS_LAUNCH(c, cat, k_scan_apply, ntiles, TPB, in, out, n, tmp);
@@ -649,7 +674,7 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
              c->key_tmp, c->rank, c->cell_count, c->flags);
   mpsk_exclusive_scan(c, MPS_T_BIN_SORT, c->cell_count, c->cell_start, nc + 2, c->scan_tmp);
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_scatter, div_up(n, TPB), TPB, n, c->key_tmp, c->rank,
-             c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key);
+             c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key, nc, c->flags);
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_reorder, div_up(n, TPB), TPB, n, nc, c->key, c->cell_start,
              c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
              c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent,
@@ -658,7 +683,6 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
   c->cur = nxt;
   c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
   c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;
-  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_count_ghosts, 1, 32, n, nc, c->cell_start, c->flags);
   if (c->prm.cell_div == 1 && !c->rows_by_warp) {
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, c->kc, c->pos4[nxt],
                c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
