@@ -50,6 +50,10 @@ def parse_args():
     ap.add_argument("--route", default=None, choices=[None, "explicit", "ppe"])
     ap.add_argument("--rebin-every", type=int, default=1,
                     help="K > 1: the paper's neighbour-list reuse (PAPER.md:433), NOT the BASELINE workload")
+    ap.add_argument("--ppe-operator", type=int, default=None, choices=[0, 1],
+                    help="0 matrix-free, 1 assembled once per solve (library default)")
+    ap.add_argument("--warm-start", action="store_true", help="cg_warm_start = 1")
+    ap.add_argument("--key-mode", type=int, default=None, choices=[0, 1], help="0 linear cell key, 1 Morton")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-replay", action="store_true", help="skip the instrumented per-kernel replay")
@@ -78,6 +82,12 @@ def make_scene(args, rank=0):
     seed = scenes.BASE_SEED + args.config + (args.sweep_index if args.config >= 5 else 0) + 1000 * rank
     s = scenes.make_scene(args.config, seed=seed, sweep_index=args.sweep_index)
     route = s.route if args.route is None else {"explicit": 0, "ppe": 1}[args.route]
+    if getattr(args, "ppe_operator", None) is not None:
+        s.params["ppe_operator"] = int(args.ppe_operator)
+    if getattr(args, "warm_start", False):
+        s.params["cg_warm_start"] = 1
+    if getattr(args, "key_mode", None) is not None:
+        s.params["key_mode"] = int(args.key_mode)
     if getattr(args, "rebin_every", 1) > 1:
         s.params["rebin_every"] = int(args.rebin_every)
         s.name += f"_reuse{args.rebin_every}"
@@ -270,13 +280,15 @@ def run_b200(args):
     while time.perf_counter() < t_end and len(sampler.rows) < 3:
         g.step(1, route)               # untimed: keep the GPU under load until the sampler reports
     l0 = g.launch_count()
-    cg_before = g.stats()["cg_iters_total"]
+    st0 = g.stats()
+    cg_before, loop_before = st0["cg_iters_total"], st0["cg_loop_ms_total"]
     ms_rank = timed_steps(torch, world, g, route, K, flush, stream)
     launches = g.launch_count() - l0
     clocks = sampler.stop()
     ms_total = barrier_and_max(world, ms_rank, dev)
     stats = g.stats()
     cg_timed_main = stats["cg_iters_total"] - cg_before
+    cg_loop_ms = stats["cg_loop_ms_total"] - loop_before   # device-timed (%globaltimer) CG loops of the timed steps
     n_all = all_sum(world, scene.n, dev)
     value = n_all * K / (ms_total * 1e-3)
 
@@ -432,6 +444,12 @@ def run_b200(args):
         }
         if route == 1:
             out["cg_iters_per_sec"] = cg_timed_main / (ms_total * 1e-3)
+            out["cg"] = {"operator": {0: "matrix-free", 1: "assembled once per solve"}[int(scene.params.get("ppe_operator", 1))],
+                         "rows": int(stats["n_rows"]), "loop_ms_per_step": cg_loop_ms / K,
+                         "setup_ms_last_solve": stats["cg_setup_ms"],
+                         "us_per_iteration": 1e3 * cg_loop_ms / max(cg_timed_main, 1),
+                         "ps_per_row_per_iteration": 1e9 * cg_loop_ms / max(cg_timed_main, 1) / max(int(stats["n_rows"]), 1),
+                         "timing": "%globaltimer of block 0 inside k_ppe_cg around the iteration loop"}
         print(json.dumps(out))
     if world > 1:
         torch.distributed.destroy_process_group()

@@ -91,6 +91,14 @@ typedef struct mps_params {
   int32_t rebin_every;      /* (1) 1: exact neighbour sets at both bins of every step (Q7).  K > 1: the paper's
                                list reuse: mps_step bins once every K steps, at r^k, and every
                                sweep keeps the stored pairs whose current distance is below the radius; Q24 */
+  int32_t ppe_operator;     /* (1) how the CG applies A of Listing 2.  0: matrix-free -- rows hold
+                               neighbour indices only and every application recomputes c_ij from the positions;
+                               1: assembled -- the coefficients of the rows bc = 0 are computed once per solve
+                               (positions are fixed during a solve) into a compact ELL matrix (fp64 value +
+                               uint32 column, the paper's poiss[] of P:272-282 without its N x 300 stride over all
+                               particles) and every application streams it.  Same operator, same parity bars. */
+  int32_t cg_warm_start;    /* (0) 1: CG starts from the previous step's pressure of the particle (x0 = p^k on
+                               the rows bc = 0) instead of x0 = 0 (Q15); one extra operator application per solve */
   double l0;                /* initial particle spacing */
   double re_n;              /* radius for density, p-hat and gradient (2.1 l0) */
   double re_grad;           /* must equal re_n (one list serves both) */
@@ -124,7 +132,11 @@ typedef struct mps_stats {
   int64_t cg_iters_total;   /* summed over the life of the ctx */
   int64_t steps_total;
   int32_t device_error;     /* sticky MPS_ERR_* raised on the device, 0 if none */
-  int32_t reserved;
+  int32_t cg_noconv_total;  /* solves that hit cg_maxit, summed over the life of the ctx */
+  double cg_setup_ms;       /* last solve, timed on the device (%globaltimer, block 0): flags, rhs,
+                               compaction and (ppe_operator 1) assembly ... */
+  double cg_loop_ms;        /* ... and the CG iterations alone */
+  double cg_loop_ms_total;  /* cg_loop_ms summed over the life of the ctx */
 } mps_stats;
 
 /* mps_init: create a ctx and copy n particles in (device pointers, caller's

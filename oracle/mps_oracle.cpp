@@ -48,6 +48,8 @@ struct Prm {
   int ppe_laplacian;  // 0: Eq. 10 form (Listing 2); 1: higher-order Laplacian Eq. 16 (HL)
   int kernel;         // 0: w = re/r - 1 (Eq. 3); 1: w = (1 - r/re)^3 (Eq. 4)
   int rebin_every;    // 1: exact sets at every sweep (Q7); K > 1: the paper's list reuse (Q24)
+  int key_mode;       // 0: linear x-fastest cell key; 1: Morton key, 3 x 10-bit interleave (north_star "Morton- or cell-sorted")
+  int cg_warm_start;  // 0: x0 = 0 (Q15); 1: x0 = the particle's previous pressure
   double dmin[3], dmax[3];
   int max_neighbours;
   double n0_n, n0_lap, lam;
@@ -91,7 +93,8 @@ struct Orc {
   std::vector<int> type, phase, bc, key, perm, cell_start;
   double h = 0, inv_h = 0;
   int nc[3] = {0, 0, 0};
-  int ncells = 0;
+  int ncells = 0;       // size of the key space: n_x n_y n_z (linear) or 8^bits (Morton)
+  std::vector<int> ccx, ccy, ccz;  // cell coordinates of every particle (last BIN)
   bool brute = false;
   bool binned = false;
   double n0_n = 0, n0_lap = 0, lam = 0, A_lap = 0;
@@ -122,11 +125,30 @@ struct Orc {
       if (nc[a] < 1) nc[a] = 1;
       ncells *= nc[a];
     }
+    if (prm.key_mode == 1) {  // Morton keys live in [0, 8^bits), bits = smallest with 2^bits >= every n_a
+      int bits = 0;
+      while ((1 << bits) < std::max(nc[0], std::max(nc[1], nc[2]))) ++bits;
+      ncells = 1 << (3 * bits);
+    }
+  }
+  // Morton key: bit k of c_x goes to bit 3k, of c_y to bit 3k+1, of c_z to bit 3k+2 (k = 0..9).
+  static int morton3(int cx, int cy, int cz) {
+    int key = 0;
+    for (int k = 0; k < 10; ++k) {
+      key |= ((cx >> k) & 1) << (3 * k);
+      key |= ((cy >> k) & 1) << (3 * k + 1);
+      key |= ((cz >> k) & 1) << (3 * k + 2);
+    }
+    return key;
+  }
+  int cell_key(int cx, int cy, int cz) const {
+    return prm.key_mode == 1 ? morton3(cx, cy, cz) : cx + nc[0] * (cy + nc[1] * cz);
   }
 
   // BIN: B1-B4.
   void bin() {
     key.assign(n, 0);
+    ccx.assign(n, 0); ccy.assign(n, 0); ccz.assign(n, 0);
     n_ghost = 0;
     for (int i = 0; i < n; ++i) {
       const double pos[3] = {f[0][i], f[1][i], f[2][i]};
@@ -138,7 +160,7 @@ struct Orc {
         else c[a] = (int)fl;
       }
       if (out) { type[i] = GHOST; key[i] = ncells; ++n_ghost; }  // B1, B2
-      else key[i] = c[0] + nc[0] * (c[1] + nc[1] * c[2]);
+      else { key[i] = cell_key(c[0], c[1], c[2]); ccx[i] = c[0]; ccy[i] = c[1]; ccz[i] = c[2]; }
     }
     // B3: stable sort by key, ties by ascending original index.
     perm.resize(n);
@@ -198,8 +220,7 @@ struct Orc {
       return;
     }
     int R = (int)std::ceil(re * inv_h);
-    int k = key[i];
-    int cx = k % nc[0], cy = (k / nc[0]) % nc[1], cz = k / (nc[0] * nc[1]);
+    int cx = ccx[i], cy = ccy[i], cz = ccz[i];
     for (int dz = -R; dz <= R; ++dz) {
       int z2 = cz + dz;
       if (z2 < 0 || z2 >= nc[2]) continue;
@@ -209,7 +230,7 @@ struct Orc {
         for (int dx = -R; dx <= R; ++dx) {
           int x2 = cx + dx;
           if (x2 < 0 || x2 >= nc[0]) continue;
-          int c = x2 + nc[0] * (y2 + nc[1] * z2);
+          int c = cell_key(x2, y2, z2);
           for (int s = cell_start[c]; s < cell_start[c + 1]; ++s) test(perm[s]);
         }
       }
@@ -387,6 +408,32 @@ struct Orc {
   }
   // step 7b.3 (Listing 2: off-diagonal -val, diagonal += val, diagonal
   // += 1.00e-7/dt^2, dummy neighbours give 0, rows only where bcon == 0).
+  // Positions are fixed during a solve, so ppe_solve() records, for every row, the neighbours and
+  // r2 in the order for_neighbours() visits them and the later applications walk that record:
+  // the same pairs, the same numbers, the same order of additions -- only the search is skipped
+  // (this is Listing 2's neigh[] list).
+  std::vector<long long> nbc_off;
+  std::vector<int> nbc_j;
+  std::vector<double> nbc_r2;
+  bool nbc_on = false;
+  void nbc_build() {
+    const double re = prm.re_lap;
+    nbc_off.assign(n + 1, 0);
+    nbc_j.clear();
+    nbc_r2.clear();
+    for (int i = 0; i < n; ++i) {
+      if (bc[i] == 0)
+        for_neighbours(i, re, [&](int j, double, double, double, double r2) { nbc_j.push_back(j); nbc_r2.push_back(r2); });
+      nbc_off[i + 1] = (long long)nbc_j.size();
+    }
+    nbc_on = true;
+  }
+  void nbc_drop() { nbc_on = false; nbc_off.clear(); nbc_j.clear(); nbc_r2.clear(); nbc_j.shrink_to_fit(); nbc_r2.shrink_to_fit(); }
+  template <class F>
+  void for_lap_neighbours(int i, F&& fn) {
+    if (nbc_on) { for (long long k = nbc_off[i]; k < nbc_off[i + 1]; ++k) fn(nbc_j[k], nbc_r2[k]); }
+    else for_neighbours(i, prm.re_lap, [&](int j, double, double, double, double r2) { fn(j, r2); });
+  }
   void ppe_apply(const double* xin, double* yout) {
     ensure_binned();
     const double re = prm.re_lap;
@@ -395,7 +442,7 @@ struct Orc {
       if (bc[i] != 0) continue;
       double s = 0.0;
       const double xi = xin[i];
-      for_neighbours(i, re, [&](int j, double, double, double, double r2) {
+      for_lap_neighbours(i, [&](int j, double r2) {
         if (bc[j] == -1) return;
         const double c = lap_coef(re, r2) / rho_pair(i, j);
         s += c * (xi - (bc[j] == 0 ? xin[j] : 0.0));
@@ -403,17 +450,28 @@ struct Orc {
       yout[i] = s + prm.compress / (prm.dt * prm.dt) * xi;
     }
   }
-  // step 7b.4 (Eq.9, P:176 CG part; Q15): textbook CG, x0 = 0.
+  // step 7b.4 (Eq.9, P:176 CG part; Q15): textbook CG, x0 = 0 (or, cg_warm_start = 1, the
+  // particle's previous pressure on the rows: r0 = b - A x0).
+  bool nbc_keep = false;  // set by the preconditioned solvers, which build the record themselves
   int ppe_solve(double rtol, int maxit) {
     std::vector<double>& x = f[17];
     std::vector<double> r(n), p(n), Ap(n);
     const std::vector<double>& b = f[12];
     double rr = 0.0, bb = 0.0;
-    for (int i = 0; i < n; ++i) { x[i] = 0.0; r[i] = b[i]; p[i] = r[i]; }
+    ensure_binned();
+    nbc_build();
+    for (int i = 0; i < n; ++i) { x[i] = 0.0; r[i] = b[i]; }
+    if (prm.cg_warm_start) {
+      for (int i = 0; i < n; ++i) x[i] = (bc[i] == 0) ? f[7][i] : 0.0;
+      ppe_apply(x.data(), Ap.data());
+      for (int i = 0; i < n; ++i) r[i] = (bc[i] == 0) ? b[i] - Ap[i] : 0.0;
+    }
+    for (int i = 0; i < n; ++i) p[i] = r[i];
     for (int i = 0; i < n; ++i) if (bc[i] == 0) { rr += r[i] * r[i]; bb += b[i] * b[i]; }
     cg_iters = 0;
     cg_relres = 0.0;
-    if (bb == 0.0) return 0;
+    if (bb == 0.0) { for (int i = 0; i < n; ++i) x[i] = 0.0; nbc_drop(); return 0; }
+    if (rr <= rtol * rtol * bb) { cg_relres = std::sqrt(rr / bb); nbc_drop(); return 0; }
     int it;
     bool conv = false;
     for (it = 1; it <= maxit; ++it) {
@@ -434,6 +492,7 @@ struct Orc {
     }
     cg_iters = conv ? it : maxit;
     cg_relres = std::sqrt(rr / bb);
+    nbc_drop();
     return conv ? cg_iters : -cg_iters;
   }
   // step 7b (whole) incl. 7b.5 (Q4 clamp).
@@ -618,6 +677,7 @@ void* orc_create(const double* dp, const int* ip, int n, const double* x, const 
   p.dim = ip[0]; p.n_phases = ip[1]; p.cg_maxit = ip[2]; p.grad_variant = ip[3];
   p.clamp_negative_p = ip[4]; p.rho_pair_mean = ip[5]; p.nu_pair_mean = ip[6];
   p.cell_div = ip[7]; p.max_neighbours = ip[8]; p.ppe_source = ip[9]; p.ppe_laplacian = ip[10]; p.kernel = ip[11]; p.rebin_every = ip[12] < 1 ? 1 : ip[12];
+  p.key_mode = ip[13]; p.cg_warm_start = ip[14];
   o->n = n;
   for (auto& a : o->f) a.assign(n, 0.0);
   const double* src[6] = {x, y, z, u, v, w};
@@ -715,6 +775,7 @@ int orc_ppe_flags(void* h) { ((Orc*)h)->ppe_flags(); return 0; }
 int orc_ppe_rhs(void* h) { ((Orc*)h)->ppe_rhs(); return 0; }
 int orc_ppe_apply(void* h, const double* xin, double* yout) { ((Orc*)h)->ppe_apply(xin, yout); return 0; }
 int orc_ppe_solve(void* h, double rtol, int maxit) { return ((Orc*)h)->ppe_solve(rtol, maxit); }
+int orc_morton3(int cx, int cy, int cz) { return Orc::morton3(cx, cy, cz); }
 int orc_pressure_ppe(void* h) { return ((Orc*)h)->pressure_ppe(); }
 void orc_smooth_density(void* h) { ((Orc*)h)->smooth_density(); }
 void orc_dndt(void* h, int dst) { ((Orc*)h)->dndt(dst == 20 ? 20 : 18); }

@@ -50,6 +50,7 @@ def lib():
         L.orc_ppe_apply.argtypes = [C.c_void_p, _dp, _dp]
         L.orc_ppe_solve.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.orc_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.orc_morton3.argtypes = [C.c_int, C.c_int, C.c_int]
         L.orc_lattice_constants.argtypes = [C.c_int, C.c_double, C.c_double, _dp]
         L.orc_lattice_constants_k.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int, _dp]
         L.orc_eos.restype = C.c_double
@@ -72,6 +73,10 @@ def lattice_constants(dim: int, l0: float, re: float, kernel: int = 0) -> Tuple[
     return float(out[0]), float(out[1]), int(out[2])
 
 
+def morton3(cx: int, cy: int, cz: int) -> int:
+    return int(lib().orc_morton3(cx, cy, cz))
+
+
 def eos(rho, c0, gamma, n, n0) -> float:
     return float(lib().orc_eos(rho, c0, gamma, n, n0))
 
@@ -84,8 +89,9 @@ def pack_params(p: Dict[str, object]):
     ip = np.array([p["dim"], p["n_phases"], p["cg_maxit"], p["grad_variant"],
                    p["clamp_negative_p"], p["rho_pair_mean"], p["nu_pair_mean"], p["cell_div"],
                    p["max_neighbours"], p.get("ppe_source", 0), p.get("ppe_laplacian", 0),
-                   p.get("kernel", 0), p.get("rebin_every", 1)], dtype=np.int32)
-    assert dp.size == 27 and ip.size == 13
+                   p.get("kernel", 0), p.get("rebin_every", 1), p.get("key_mode", 0),
+                   p.get("cg_warm_start", 0)], dtype=np.int32)
+    assert dp.size == 27 and ip.size == 15
     return dp, ip
 
 

@@ -47,6 +47,7 @@ class MpsParams(C.Structure):
         ("rho_pair_mean", C.c_int32), ("nu_pair_mean", C.c_int32), ("key_mode", C.c_int32),
         ("cell_div", C.c_int32), ("max_neighbours", C.c_int32), ("ppe_source", C.c_int32),
         ("ppe_laplacian", C.c_int32), ("kernel", C.c_int32), ("rebin_every", C.c_int32),
+        ("ppe_operator", C.c_int32), ("cg_warm_start", C.c_int32),
         ("l0", C.c_double), ("re_n", C.c_double), ("re_grad", C.c_double),
         ("re_lap", C.c_double), ("dt", C.c_double), ("g", C.c_double * 3),
         ("rho", C.c_double * 2), ("nu", C.c_double * 2), ("c0", C.c_double),
@@ -62,7 +63,8 @@ class MpsStats(C.Structure):
         ("cg_iters", C.c_int32), ("cg_converged", C.c_int32), ("cg_relres", C.c_double),
         ("max_neighbours", C.c_int32), ("n_surface", C.c_int32), ("n_ghost", C.c_int32),
         ("n_rows", C.c_int32), ("cg_iters_total", C.c_int64), ("steps_total", C.c_int64),
-        ("device_error", C.c_int32), ("reserved", C.c_int32),
+        ("device_error", C.c_int32), ("cg_noconv_total", C.c_int32),
+        ("cg_setup_ms", C.c_double), ("cg_loop_ms", C.c_double), ("cg_loop_ms_total", C.c_double),
     ]
 
     def as_dict(self) -> Dict[str, float]:
@@ -86,6 +88,8 @@ def make_params(p: Dict[str, object]) -> MpsParams:
     s.ppe_laplacian = int(p.get("ppe_laplacian", 0))
     s.kernel = int(p.get("kernel", 0))
     s.rebin_every = int(p.get("rebin_every", 1))
+    s.ppe_operator = int(p.get("ppe_operator", 1))
+    s.cg_warm_start = int(p.get("cg_warm_start", 0))
     for k in ("l0", "re_n", "re_lap", "dt", "c0", "gamma", "beta", "compress", "ppe_relax",
               "cg_rtol", "cs", "n0_n", "n0_lap"):
         setattr(s, k, float(p[k]))

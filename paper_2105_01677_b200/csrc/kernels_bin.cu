@@ -191,7 +191,7 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
                           uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out,
                           uint32_t* __restrict__ ent_out, const double2* __restrict__ keep_in,
                           double2* __restrict__ keep_out, const double* __restrict__ rs_in,
-                          double* __restrict__ rs_out) {
+                          double* __restrict__ rs_out, int carry_w) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   uint32_t c = key[s];
@@ -202,7 +202,7 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
   for (uint32_t t = lo; t < hi; ++t) f += (tmp_oid[t] < me) ? 1u : 0u;
   uint32_t src = tmp_src[s];
   double4 q = pos_in[src];
-  q.w = 0.0;
+  if (!carry_w) q.w = 0.0;  // cg_warm_start: the previous pressure follows its particle
   pos_out[f] = q;
   vel_out[f] = vel_in[src];
   const uint32_t tj = tp_in[src];
@@ -679,7 +679,7 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
              c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
              c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent,
              c->prm.ppe_source == 2 ? c->keep2[cur] : nullptr, c->keep2[nxt],
-             c->prm.grad_variant == 3 ? c->rho_s[cur] : nullptr, c->rho_s[nxt]);
+             c->prm.grad_variant == 3 ? c->rho_s[cur] : nullptr, c->rho_s[nxt], c->prm.cg_warm_start);
   c->cur = nxt;
   c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
   c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;

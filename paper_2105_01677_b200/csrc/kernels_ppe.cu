@@ -1,45 +1,45 @@
 // kernels_ppe.cu -- the semi-implicit pressure route (S8b of DESIGN.md):
 // free-surface flags (Eq. 6), right-hand side (Eq. 8; Q5), the
-// matrix-free operator with the structure of Listing 2, and the
+// operator with the structure of Listing 2, and the
 // conjugate-gradient solve (Eq. 9; Q15).
 //
 // The whole solve is ONE persistent cooperative kernel (k_ppe_cg): flags and
-// right-hand side, ordered compaction of the unknown rows, then the CG loop in its
-// single-reduction (Chronopoulos-Gear) form with two grid barriers per iteration:
-//   phase A  w = A r fused with the dot products r.r and r.w (L lanes per row,
+// right-hand side, ordered compaction of the unknown rows, (ppe_operator 1) assembly of
+// the coefficients, then the CG loop in its single-reduction (Chronopoulos-Gear) form
+// with two grid barriers per iteration:
+//   phase A  w = A r fused with the dot products r.r and r.w (8 lanes per row,
 //            shuffles inside the row group, one partial per block)
 //   barrier  every block adds the partials in index order -> identical alpha, beta
 //   phase B  p = r + beta p; s = w + beta s; x += alpha p; r -= alpha s
-//   barrier  r (kept in pos4.w, so a neighbour gather is one 32-byte sector) is visible
+//   barrier  r is visible to every block
 // All scalars stay on the device and the convergence test is taken by every block
 // from the same numbers, so there is no host poll.  In exact arithmetic the
-// iterates are those of textbook CG; the matrix is never stored.
+// iterates are those of textbook CG.
+//
+// Two forms of the operator (mps_params.ppe_operator), same numbers up to rounding:
+//   0  matrix-free: r lives in pos4.w (a neighbour gather is one 32-byte record) and
+//      c_ij = A_lap w(r_ij) / rho_ij is recomputed at every application;
+//   1  assembled: positions are fixed during a solve, so the c_ij of the rows bc = 0 are
+//      computed once into a compact ELL matrix (fp64 value + uint32 column in the numbering
+//      of the compacted rows; neighbours on the free surface fold into a per-row diagonal
+//      term, dummies drop out).  An application streams 12 bytes per pair, coalesced, and
+//      gathers 8 bytes from a dense vector in which neighbouring rows share cache lines.
 #include <algorithm>
+#include <stdlib.h>
 
 #include "sweep_common.cuh"
 
 namespace {
 
-#ifdef MPS_CG_PROFILE
-#include <cstdio>
-#define TICK(slot) do { if (bid == 0 && tid == 0) { long long t_ = clock64(); prof[slot] += t_ - tlast; tlast = t_; } } while (0)
-#else
-#define TICK(slot) do { } while (0)
-#endif
-
-#ifndef MPS_CG_TPB
-#define MPS_CG_TPB 1024
-#endif
-#ifndef MPS_CG_MINB
-#define MPS_CG_MINB 1
-#endif
-constexpr int PPE_ILP = 4;  // independent neighbour gathers in flight per lane
-constexpr int CG_TPB = MPS_CG_TPB;
-constexpr int CG_MINB = MPS_CG_MINB;  // co-resident blocks per SM the register budget is set for
-static_assert(CG_TPB % 256 == 0, "phase A deals rows in super-chunks of 8 warps");
+constexpr int PPE_ILP = 4;   // independent neighbour gathers in flight per lane
+constexpr int CG_TPB = 1024;
+constexpr int L = 8;         // lanes per row
+constexpr int GPW = 32 / L;  // row groups per warp
+constexpr int SCW = 8;       // warps per super-chunk of consecutive rows
+static_assert(CG_TPB % (32 * SCW) == 0, "phase A deals rows in super-chunks of 8 warps");
 
 struct PpeArgs {
-  double4* pos4;  // .w: CG residual r during the solve, pressure at exit
+  double4* pos4;  // matrix-free: .w is the CG residual r during the solve; pressure at exit
   cudaTextureObject_t tex;  // pos4 as 16-byte texels (0: not used)
   const uint32_t* tp;
   const double* dens;
@@ -47,8 +47,8 @@ struct PpeArgs {
   const double2* keep2;    // (n^k, (Dn/Dt)^k) (ppe_source == 2)
   int8_t* bc;
   double* b;
-  double* x;
-  double* pv;
+  double* x;               // per slot: the solution (matrix-free: the CG iterate itself)
+  double* pv;              // p, s, w: per slot (matrix-free) or compact (assembled)
   double* sv;
   double* wv;
   double* p;
@@ -60,9 +60,25 @@ struct PpeArgs {
   double* part;      // 2 per block
   CgScalars* cg;
   GridBar* bar;
+  // assembled operator
+  uint32_t* rowmap;
+  double* mval;
+  uint32_t* mcol;
+  uint32_t* mcnt;
+  double* mdex;
+  double* rc;
+  double* xc;
   double tol2;
+  long long timeout_cycles;
   int maxit;
+  int warm;
 };
+
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 
 // ---- block-wide sum of two values, result broadcast to every thread ---------------
 // warp shuffles, one partial per warp in shared memory, the first warp folds them in
@@ -86,19 +102,18 @@ __device__ __forceinline__ void block_sum2(double& a, double& b) {
   __syncthreads();
   a = res[0];
   b = res[1];
-  // the next call's writes to sh/res come after its own first barrier at the earliest for
-  // sh (written before the barrier by lane 0 of each warp: all reads of sh above are done
-  // by warp 0 before the second barrier) and after both barriers for res
+  // the next call's writes to sh come before its first barrier (lane 0 of each warp) and every
+  // read of sh above is done by warp 0 before the second barrier; res is rewritten only
+  // between the next call's two barriers
 }
 
 // ---- grid barrier (all blocks are co-resident: cooperative launch) ----------------
 // One monotonically increasing arrival counter: thread 0 of every block adds 1 with
 // release semantics and spins (acquire) until the count reaches nb x generation, so
-// a barrier costs one L2 round trip for the arrival plus the polls -- there is no
-// second "last block flips the flag" hop.  The fence after the spin makes every
-// later plain load of the block see the other blocks' writes (it invalidates the
-// SM's L1).  A spin that lasts longer than about two seconds raises barrier_timeout
-// and lets the kernel drain instead of hanging.
+// a barrier costs one L2 round trip for the arrival plus the polls.  The fence after
+// the spin makes every later plain load of the block see the other blocks' writes.
+// A spin longer than timeout_cycles (0: no limit) raises bar->timeout and lets the
+// kernel drain instead of hanging.
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
   unsigned int v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -107,7 +122,7 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
 __device__ __forceinline__ void red_release_add_u32(unsigned int* p, unsigned int v) {
   asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-__device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, CgScalars* cg) {
+__device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, long long timeout_cycles) {
   __shared__ int dead;
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -118,11 +133,14 @@ __device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, Cg
     unsigned int polls = 0;
     while ((int)(ld_acquire_u32(&bar->count) - gen) < 0) {
       if ((++polls & 1023u) == 0u) {
-        if (t0 == 0) t0 = clock64();
-        else if (clock64() - t0 > 4000000000LL) {
-          cg->barrier_timeout = 1;
-          dead = 1;
-          break;
+        if (ld_acquire_u32(&bar->timeout)) { dead = 1; break; }  // some block gave up: follow it
+        if (timeout_cycles > 0) {
+          if (t0 == 0) t0 = clock64();
+          else if (clock64() - t0 > timeout_cycles) {
+            bar->timeout = 1u;
+            dead = 1;
+            break;
+          }
         }
       }
     }
@@ -132,12 +150,24 @@ __device__ __forceinline__ bool grid_barrier(GridBar* bar, unsigned int& gen, Cg
   return dead == 0;
 }
 
-// ---- one row of y = A r ------------------------------------------------------------
+// ---- pair coefficient before the row's common factor ---------------------------------
+// Eq. 10 form (Listing 2): w(r) (then times A_lap); MPS-HL (Eq. 16; Q23): 1 / r^3 (then
+// times 2 re / n0); both times 1 / rho_ij (Q6).
+template <bool TWO_PHASE>
+__device__ __forceinline__ double pair_coef(const KConst& kc, bool hl, double r2, uint32_t e,
+                                            double inv_rij0, double inv_rij1) {
+  const double ir = rsqrt_f64(r2);
+  double w = hl ? ir * ir * ir : kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, ir);
+  if (TWO_PHASE) w *= (e & NB_PHASE1) ? inv_rij1 : inv_rij0;
+  return w;
+}
+
+// ---- one row of y = A r, matrix-free ---------------------------------------------------
 // (A r)_i = sum_{j in N(i, re_lap), j not dummy} c_ij (r_i - r_j) + compress/dt^2 r_i,
 // c_ij = A_lap w(r_ij) / rho_ij (Listing 2; Q5, Q6).  r_j is read from
 // pos4.w, which is 0 on free-surface slots (Dirichlet p = 0).  The L lanes of the
 // group each take every L-th entry; the result is valid in every lane.
-template <bool TWO_PHASE, int L, bool TEX>
+template <bool TWO_PHASE, bool TEX>
 __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4, cudaTextureObject_t tex,
                                           const uint32_t* tp,
                                           const uint32_t* nbr, const uint32_t* cn, const uint32_t* co,
@@ -182,12 +212,7 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
     for (int u = 0; u < PPE_ILP; ++u) {
       const double dx = q[u].x - pi.x, dy = q[u].y - pi.y, dz = q[u].z - pi.z;
       const double r2 = pair_r2(dx, dy, dz, kc.stale);
-      const double ir = rsqrt_f64(r2);
-      // Eq. 10 form: A_lap (re/r - 1); MPS-HL (Eq. 16, Q23): (2 re / n0) / r^3
-      double w = hl ? ir * ir * ir : kernel_w(kc.kernel, kc.re_lap, kc.inv_re_lap, r2, ir);
-      if (TWO_PHASE) {
-        w *= (e[u] & NB_PHASE1) ? inv_rij1 : inv_rij0;
-      }
+      double w = pair_coef<TWO_PHASE>(kc, hl, r2, e[u], inv_rij0, inv_rij1);
       if ((e[u] & NB_DUMMY) || (kc.stale && !(r2 < kc.re_lap2))) w = 0.0;  // dummy, empty slot, or left the radius
       s = fma(w, pi.w - q[u].w, s);
     }
@@ -197,17 +222,109 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
   return fma(hl ? kc.hl_c : kc.A_lap, s, kc.compress_dt2 * pi.w);
 }
 
+// ---- assembly of one row (ppe_operator 1) ----------------------------------------------
+// Walks the neighbour row of slot i once, computes c_ij as ppe_row does and writes the pairs
+// whose j is an unknown too as (value, compact column), in the row's order, at the start of
+// ELL row g; neighbours on the free surface (p = 0) only add to the diagonal term.
+// Every lane of the warp must come through here with a warp-uniform trip count m_max.
+template <bool TWO_PHASE>
+__device__ __forceinline__ void assemble_row(const KConst& kc, const PpeArgs& a, int g, int i, int sub,
+                                             int grp, bool live, uint32_t m_max) {
+  const double4 pi = a.pos4[i];
+  const uint32_t* row = row_ptr(a.nbr, kc.stride, i);
+  const uint32_t nf = live ? a.cn[i] : 0u;
+  const uint32_t m = live ? nf + a.co[i] : 0u;
+  const int ph_i = TWO_PHASE ? (int)((a.tp[i] >> 8) & 1) : 0;
+  const double inv_rij0 = kc.inv_rho_pair[ph_i][0], inv_rij1 = kc.inv_rho_pair[ph_i][1];
+  const bool hl = kc.ppe_laplacian == 1;
+  const double scale = (hl ? kc.hl_c : kc.A_lap) * (TWO_PHASE ? 1.0 : 1.0 / kc.rho[0]);
+  double* vrow = a.mval + (size_t)g * (size_t)kc.stride;
+  uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
+  const uint32_t lt = (1u << sub) - 1u;
+  uint32_t cnt = 0;
+  double dex = 0.0;
+  for (uint32_t k0 = 0; k0 < m_max; k0 += PPE_ILP * L) {
+    uint32_t e[PPE_ILP], rm[PPE_ILP];
+    double4 q[PPE_ILP];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const uint32_t kk = k0 + (uint32_t)(u * L + sub);
+      e[u] = kk < m ? row_entry(row, kc.stride, nf, kk) : NB_DUMMY;
+    }
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const bool use = !(e[u] & NB_DUMMY);
+      const uint32_t j = e[u] & NB_INDEX;
+      q[u] = use ? a.pos4[j] : make_double4(pi.x + kc.re_lap, pi.y, pi.z, 0.0);
+      rm[u] = use ? a.rowmap[j] : ROW_NONE;
+    }
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const double dx = q[u].x - pi.x, dy = q[u].y - pi.y, dz = q[u].z - pi.z;
+      const double r2 = pair_r2(dx, dy, dz, kc.stale);
+      double c = scale * pair_coef<TWO_PHASE>(kc, hl, r2, e[u], inv_rij0, inv_rij1);
+      if (kc.stale && !(r2 < kc.re_lap2)) rm[u] = ROW_NONE;  // reused row: the pair has left the radius
+      const bool off = rm[u] < ROW_SURFACE;
+      if (rm[u] == ROW_SURFACE) dex += c;
+      const uint32_t m8 = (__ballot_sync(0xffffffffu, off) >> (grp * L)) & ((1u << L) - 1u);
+      if (off) {
+        const uint32_t at = cnt + (uint32_t)__popc(m8 & lt);
+        vrow[at] = c;
+        crow[at] = rm[u];
+      }
+      cnt += (uint32_t)__popc(m8);
+    }
+  }
+  dex = group_sum<L>(dex);
+  if (live && sub == 0) {
+    a.mcnt[g] = cnt;
+    a.mdex[g] = dex + kc.compress_dt2;
+  }
+}
+
+// ---- one row of y = A v with the assembled operator -------------------------------------
+// y_g = sum_k val_k (v_g - v_col_k) + dex_g v_g: the same sum as ppe_row, pair by pair.
+// Matrix entries are read once per application: streaming loads; v is gathered through L1.
+__device__ __forceinline__ double asm_row(const KConst& kc, const PpeArgs& a, const double* __restrict__ v,
+                                          int g, int sub, bool live, double& vg) {
+  vg = v[g];
+  const uint32_t n = live ? a.mcnt[g] : 0u;
+  const double* vrow = a.mval + (size_t)g * (size_t)kc.stride;
+  const uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
+  double s0 = 0.0, s1 = 0.0;
+  for (uint32_t k = sub; k < n; k += PPE_ILP * L) {
+    double c[PPE_ILP];
+    uint32_t j[PPE_ILP];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const uint32_t kk = k + (uint32_t)(u * L);
+      const bool in = kk < n;
+      c[u] = in ? __ldcs(vrow + kk) : 0.0;
+      j[u] = in ? __ldcs(crow + kk) : (uint32_t)g;
+    }
+    double vj[PPE_ILP];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) vj[u] = v[j[u]];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; u += 2) {
+      s0 = fma(c[u], vg - vj[u], s0);
+      s1 = fma(c[u + 1], vg - vj[u + 1], s1);
+    }
+  }
+  const double s = group_sum<L>(s0 + s1);
+  return fma(live ? a.mdex[g] : 0.0, vg, s);
+}
+
 // ---- the persistent solve -------------------------------------------------------------
-template <bool TWO_PHASE, int L, bool TEX>
-__global__ void __launch_bounds__(CG_TPB, CG_MINB)
+template <bool TWO_PHASE, bool ASM, bool TEX>
+__global__ void __launch_bounds__(CG_TPB, 1)
 k_ppe_cg(KConst kc, PpeArgs a) {
   __shared__ uint32_t sh_cnt[2][CG_TPB / 32];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int nb = (int)gridDim.x, bid = (int)blockIdx.x;
   unsigned int gen = 0;
-#ifdef MPS_CG_PROFILE
-  long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
-#endif
+  unsigned long long t_start = 0, t_loop = 0;
+  if (bid == 0 && tid == 0) t_start = global_ns();
 
   // -- S8b-1, S8b-2: flags and right-hand side over this block's contiguous chunk --------
   const int chunk = (kc.n + nb - 1) / nb;
@@ -237,12 +354,18 @@ k_ppe_cg(KConst kc, PpeArgs a) {
           bi = kc.relax / kc.dt * (a.dndt[i] / kc.n0_n + ecs);
         }
       }
+      // warm start (Q15 option): the particle's previous pressure, carried in pos4.w by the sort
+      const double x0 = (a.warm && f == 0) ? a.pos4[i].w : 0.0;
       a.bc[i] = f;
       a.b[i] = bi;
-      a.x[i] = 0.0;
-      a.pv[i] = 0.0;
-      a.sv[i] = 0.0;
-      a.pos4[i].w = bi;  // r0 = b
+      a.x[i] = x0;
+      if (ASM) {
+        a.rowmap[i] = f == 1 ? ROW_SURFACE : ROW_NONE;  // rows get their index in the compaction below
+      } else {
+        a.pv[i] = 0.0;
+        a.sv[i] = 0.0;
+        a.pos4[i].w = a.warm ? x0 : bi;  // r0 = b (the warm start applies A to x0 first)
+      }
       bb += bi * bi;
     }
     block_sum2<CG_TPB>(bb, dummy);
@@ -259,7 +382,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
       a.part[2 * bid + 1] = 0.0;
     }
   }
-  if (!grid_barrier(a.bar, gen, a.cg)) return;
+  if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
 
   // -- totals and this block's offset into the compacted row list ------------------------
   double bb = 0.0;
@@ -299,50 +422,102 @@ k_ppe_cg(KConst kc, PpeArgs a) {
       if (k < wid) off += ck;
       tot += ck;
     }
-    if (is_row) a.rows[row_off + off + (uint32_t)__popc(m & ((1u << lane) - 1u))] = (uint32_t)i;
+    if (is_row) {
+      const uint32_t g = (uint32_t)row_off + off + (uint32_t)__popc(m & ((1u << lane) - 1u));
+      a.rows[g] = (uint32_t)i;
+      if (ASM) a.rowmap[i] = g;
+    }
     row_off += (int)tot;
   }
-  if (!grid_barrier(a.bar, gen, a.cg)) return;
+  if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
 
-  TICK(0);
+  const int gthreads = nb * CG_TPB;
+  const int gtid = bid * CG_TPB + tid;
+  const int sub = tid & (L - 1);
+  const int grp = lane / L;
+  // Rows are dealt to the blocks in super-chunks of 8 warps (8 * 32 / L consecutive rows, so
+  // the warps that share an SM's L1 work on neighbouring rows) round-robin over the grid:
+  // every block gets an even sample of cheap (wall) and expensive (fluid) rows and at most
+  // one super-chunk more than any other.  The trip count is warp-uniform.
+  const int sc_first = (wid / SCW) * nb + bid;
+  const int sc_step = (CG_TPB / 32 / SCW) * nb;
+  const int g_in_sc = (wid % SCW) * GPW + grp;
+
+  // -- ppe_operator 1: assemble the rows, set up the compact vectors ------------------------
+  if (ASM) {
+    for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
+      const int g = sc * (SCW * GPW) + g_in_sc;
+      const bool live = g < n_rows;
+      const int i = live ? (int)a.rows[g] : 0;
+      uint32_t m = live ? a.cn[i] + a.co[i] : 0u;
+      m = __reduce_max_sync(0xffffffffu, m);
+      assemble_row<TWO_PHASE>(kc, a, live ? g : 0, i, sub, grp, live, m);
+      if (live && sub == 0) {
+        a.xc[g] = a.x[i];
+        a.rc[g] = a.b[i];
+        a.pv[g] = 0.0;
+        a.sv[g] = 0.0;
+      }
+    }
+    if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
+  }
+  // -- warm start: r0 = b - A x0 ---------------------------------------------------------------
+  if (a.warm) {
+    for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
+      const int g = sc * (SCW * GPW) + g_in_sc;
+      const bool live = g < n_rows;
+      double xi;
+      if (ASM) {
+        const double t = asm_row(kc, a, a.xc, live ? g : 0, sub, live, xi);
+        if (live && sub == 0) a.rc[g] = a.rc[g] - t;
+      } else {
+        const int i = live ? (int)a.rows[g] : 0;
+        const double t = ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, xi);
+        if (live && sub == 0) a.wv[i] = t;
+      }
+    }
+    if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
+    if (!ASM) {  // every gather of x0 is done: pos4.w <- r0
+      for (int g = gtid; g < n_rows; g += gthreads) {
+        const int i = (int)a.rows[g];
+        a.pos4[i].w = a.b[i] - a.wv[i];
+      }
+      if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
+    }
+  }
+  if (bid == 0 && tid == 0) t_loop = global_ns();
+
   // -- S8b-3, S8b-4: conjugate gradients ---------------------------------------------------
   const double tol2bb = a.tol2 * bb;
   int iters = 0, converged = (bb == 0.0) ? 1 : 0;
   double gam = bb, gamma_old = 1.0, alpha_old = 1.0;
-  const int gthreads = nb * CG_TPB;
-  const int gtid = bid * CG_TPB + tid;
-  const int sub = tid & (L - 1);
   if (!converged) {
     for (;;) {
       // phase A: w = A r, gamma = r.r, delta = r.w
       double g_part = 0.0, d_part = 0.0;
-      // Rows are dealt to the blocks in super-chunks of 8 warps (8 * 32 / L consecutive rows, so
-      // the warps that share an SM's L1 work on neighbouring rows) round-robin over the grid:
-      // every block gets an even sample of cheap (wall) and expensive (fluid) rows and at most
-      // one super-chunk more than any other.  The trip count is warp-uniform.
-      constexpr int GPW = 32 / L;        // row groups per warp
-      constexpr int SCW = 8;             // warps per super-chunk
-      for (int sc = (wid / SCW) * nb + bid; sc * (SCW * GPW) < n_rows; sc += (CG_TPB / 32 / SCW) * nb) {
-        const int g = sc * (SCW * GPW) + (wid % SCW) * GPW + (lane / L);
+      for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
+        const int g = sc * (SCW * GPW) + g_in_sc;
         const bool live = g < n_rows;
-        const int i = live ? (int)a.rows[g] : 0;
-        double ri;
-        const double wi = ppe_row<TWO_PHASE, L, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+        double ri, wi;
+        if (ASM) {
+          wi = asm_row(kc, a, a.rc, live ? g : 0, sub, live, ri);
+          if (live && sub == 0) a.wv[g] = wi;
+        } else {
+          const int i = live ? (int)a.rows[g] : 0;
+          wi = ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+          if (live && sub == 0) a.wv[i] = wi;
+        }
         if (live && sub == 0) {
-          a.wv[i] = wi;
           g_part = fma(ri, ri, g_part);
           d_part = fma(ri, wi, d_part);
         }
       }
-      TICK(1);
       block_sum2<CG_TPB>(g_part, d_part);
       if (tid == 0) {
         a.part[2 * bid] = g_part;
         a.part[2 * bid + 1] = d_part;
       }
-      TICK(2);
-      if (!grid_barrier(a.bar, gen, a.cg)) return;
-      TICK(3);
+      if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
       double del = 0.0;
       gam = 0.0;
       for (int k = tid; k < nb; k += CG_TPB) {
@@ -350,7 +525,6 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         del += __ldcg(&a.part[2 * k + 1]);
       }
       block_sum2<CG_TPB>(gam, del);
-      TICK(4);
       if (gam <= tol2bb) { converged = 1; break; }
       if (iters >= a.maxit) break;
       double alpha, beta;
@@ -365,34 +539,48 @@ k_ppe_cg(KConst kc, PpeArgs a) {
       alpha_old = alpha;
       ++iters;
       // phase B: p = r + beta p; s = w + beta s; x += alpha p; r -= alpha s
-      for (int g = gtid; g < n_rows; g += gthreads) {
-        const int i = (int)a.rows[g];
-        const double r = a.pos4[i].w;
-        const double pn = fma(beta, a.pv[i], r);
-        const double sn = fma(beta, a.sv[i], a.wv[i]);
-        a.pv[i] = pn;
-        a.sv[i] = sn;
-        a.x[i] = fma(alpha, pn, a.x[i]);
-        a.pos4[i].w = fma(-alpha, sn, r);
+      if (ASM) {
+        for (int g = gtid; g < n_rows; g += gthreads) {
+          const double r = a.rc[g];
+          const double pn = fma(beta, a.pv[g], r);
+          const double sn = fma(beta, a.sv[g], a.wv[g]);
+          a.pv[g] = pn;
+          a.sv[g] = sn;
+          a.xc[g] = fma(alpha, pn, a.xc[g]);
+          a.rc[g] = fma(-alpha, sn, r);
+        }
+      } else {
+        for (int g = gtid; g < n_rows; g += gthreads) {
+          const int i = (int)a.rows[g];
+          const double r = a.pos4[i].w;
+          const double pn = fma(beta, a.pv[i], r);
+          const double sn = fma(beta, a.sv[i], a.wv[i]);
+          a.pv[i] = pn;
+          a.sv[i] = sn;
+          a.x[i] = fma(alpha, pn, a.x[i]);
+          a.pos4[i].w = fma(-alpha, sn, r);
+        }
       }
-      TICK(5);
-      if (!grid_barrier(a.bar, gen, a.cg)) return;
-      TICK(6);
+      if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
     }
   }
+  const unsigned long long t_end = (bid == 0 && tid == 0) ? global_ns() : 0ull;
 
   // -- S8b-5: pressures from x (Q4), staged into pos4.w for the gradient ------------------
   for (int i = gtid; i < kc.n; i += gthreads) {
-    double v = (a.bc[i] == 0) ? a.x[i] : 0.0;
+    double v;
+    if (ASM) {
+      const uint32_t g = a.rowmap[i];
+      v = g < ROW_SURFACE ? a.xc[g] : 0.0;
+      a.x[i] = v;
+    } else {
+      v = (a.bc[i] == 0) ? a.x[i] : 0.0;
+    }
+    if (bb == 0.0) v = 0.0;  // b = 0: the solution is 0 whatever the start
     if (kc.clamp_negative_p && v < 0.0) v = 0.0;
     a.p[i] = v;
     a.pos4[i].w = v;
   }
-#ifdef MPS_CG_PROFILE
-  if (bid == 0 && tid == 0)
-    printf("cg profile (block 0, kcycles): setup %lld | phaseA %lld | blocksum %lld | barrier1 %lld | reduce %lld | phaseB %lld | barrier2 %lld | iters %d\n",
-           prof[0] / 1000, prof[1] / 1000, prof[2] / 1000, prof[3] / 1000, prof[4] / 1000, prof[5] / 1000, prof[6] / 1000, iters);
-#endif
   if (bid == 0 && tid == 0) {
     a.cg->gamma = gam;
     a.cg->bb = bb;
@@ -403,6 +591,11 @@ k_ppe_cg(KConst kc, PpeArgs a) {
     a.cg->converged = converged;
     a.cg->n_rows = n_rows;
     a.cg->n_surface = n_surf;
+    a.cg->iters_total += iters;
+    a.cg->noconv_total += converged ? 0 : 1;
+    a.cg->t_setup_ns = t_loop - t_start;
+    a.cg->t_loop_ns = t_end - t_loop;
+    a.cg->t_loop_ns_total += t_end - t_loop;
   }
 }
 
@@ -414,7 +607,7 @@ __global__ void k_stage_in(int n, int order, const int8_t* __restrict__ bc, cons
   double v = src[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i];
   pos4[i].w = (bc[i] == 0) ? v : 0.0;
 }
-template <bool TWO_PHASE, int L>
+template <bool TWO_PHASE>
 __global__ void __launch_bounds__(256)
 k_ppe_apply(KConst kc, const double4* pos4, const uint32_t* __restrict__ tp, const int8_t* __restrict__ bc,
             const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn,
@@ -424,7 +617,7 @@ k_ppe_apply(KConst kc, const double4* pos4, const uint32_t* __restrict__ tp, con
   const bool in = i < kc.n;
   const bool live = in && bc[i] == 0;
   double ri;
-  const double wi = ppe_row<TWO_PHASE, L, false>(kc, pos4, 0, tp, nbr, cn, co, in ? i : 0, sub, live, ri);
+  const double wi = ppe_row<TWO_PHASE, false>(kc, pos4, 0, tp, nbr, cn, co, in ? i : 0, sub, live, ri);
   if (in && sub == 0) wv[i] = live ? wi : 0.0;
 }
 __global__ void k_stage_out(int n, int order, const uint32_t* __restrict__ oid,
@@ -433,57 +626,130 @@ __global__ void k_stage_out(int n, int order, const uint32_t* __restrict__ oid,
   if (i >= n) return;
   dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = src[i];
 }
+// the same through the matrix assembled by the last solve (compact numbering)
+__global__ void k_stage_in_c(int n_rows, int order, const uint32_t* __restrict__ rows,
+                             const uint32_t* __restrict__ oid, const double* __restrict__ src,
+                             double* __restrict__ vc) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n_rows) return;
+  const uint32_t i = rows[g];
+  vc[g] = src[order == MPS_ORDER_ORIGINAL ? oid[i] : i];
+}
+__global__ void __launch_bounds__(256)
+k_ppe_apply_c(KConst kc, PpeArgs a, int n_rows, const double* __restrict__ vc, double* __restrict__ yc) {
+  const int g = (int)((blockIdx.x * 256u + threadIdx.x) / L);
+  const int sub = threadIdx.x & (L - 1);
+  const bool live = g < n_rows;
+  double vg;
+  const double y = asm_row(kc, a, vc, live ? g : 0, sub, live, vg);
+  if (live && sub == 0) yc[g] = y;
+}
+__global__ void k_stage_out_c(int n, int order, const uint32_t* __restrict__ rowmap,
+                              const uint32_t* __restrict__ oid, const double* __restrict__ yc,
+                              double* __restrict__ dst) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t g = rowmap[i];
+  dst[order == MPS_ORDER_ORIGINAL ? oid[i] : (uint32_t)i] = g < ROW_SURFACE ? yc[g] : 0.0;
+}
 
-template <bool TWO_PHASE, int L, bool TEX>
+template <bool TWO_PHASE, bool ASM, bool TEX>
 cudaError_t launch_cg(mps_ctx* c, PpeArgs& a, int grid) {
   void* params[] = {(void*)&c->kc, (void*)&a};
-  return cudaLaunchCooperativeKernel((const void*)k_ppe_cg<TWO_PHASE, L, TEX>, dim3(grid), dim3(CG_TPB),
+  return cudaLaunchCooperativeKernel((const void*)k_ppe_cg<TWO_PHASE, ASM, TEX>, dim3(grid), dim3(CG_TPB),
                                      params, 0, c->stream);
 }
-template <bool TWO_PHASE, int L, bool TEX>
+template <bool TWO_PHASE, bool ASM, bool TEX>
 int cg_blocks_per_sm() {
   int nb = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_ppe_cg<TWO_PHASE, L, TEX>, CG_TPB, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_ppe_cg<TWO_PHASE, ASM, TEX>, CG_TPB, 0);
   return nb;
 }
 
 bool two_phase(const mps_ctx* c) { return c->prm.n_phases > 1 && c->prm.rho[0] != c->prm.rho[1]; }
+
+PpeArgs make_args(mps_ctx* c) {
+  const int cur = c->cur;
+  PpeArgs a;
+  a.pos4 = c->pos4[cur]; a.tex = c->cg_tex ? c->pos_tex[cur] : 0; a.tp = c->tp[cur]; a.dens = c->dens;
+  a.dndt = c->dndt; a.keep2 = c->keep2[cur]; a.bc = c->bc; a.b = c->b;
+  a.x = c->cg_x; a.pv = c->cg_p; a.sv = c->cg_s; a.wv = c->cg_w; a.p = c->p;
+  a.nbr = c->nbr; a.cn = c->cn; a.co = c->co; a.rows = c->cg_rows; a.bcount = c->cg_bcount;
+  a.part = c->cg_part; a.cg = c->cg; a.bar = c->cg_bar;
+  a.rowmap = c->rowmap; a.mval = c->mat_val; a.mcol = c->mat_col; a.mcnt = c->mat_cnt; a.mdex = c->mat_dex;
+  a.rc = c->cg_rc; a.xc = c->cg_xc;
+  a.tol2 = c->prm.cg_rtol * c->prm.cg_rtol;
+  a.timeout_cycles = c->cg_timeout_cycles;
+  a.maxit = c->prm.cg_maxit;
+  a.warm = c->prm.cg_warm_start ? 1 : 0;
+  return a;
+}
 
 }  // namespace
 
 // ============================================================ host launchers ===
 // Number of co-resident blocks of the persistent kernel (called once at init).
 int mpsk_ppe_plan(mps_ctx* c) {
-  int per_sm = 2;
+  int per_sm;
   const bool tp = two_phase(c);
-  c->cg_lanes = 8;  // 4 and 16 lanes per row measured within 5 % of 8
-  if (c->cg_tex) per_sm = tp ? cg_blocks_per_sm<true, 8, true>() : cg_blocks_per_sm<false, 8, true>();
-  else per_sm = tp ? cg_blocks_per_sm<true, 8, false>() : cg_blocks_per_sm<false, 8, false>();
+  const bool as = c->prm.ppe_operator == 1;
+  if (as) per_sm = tp ? cg_blocks_per_sm<true, true, false>() : cg_blocks_per_sm<false, true, false>();
+  else if (c->cg_tex) per_sm = tp ? cg_blocks_per_sm<true, false, true>() : cg_blocks_per_sm<false, false, true>();
+  else per_sm = tp ? cg_blocks_per_sm<true, false, false>() : cg_blocks_per_sm<false, false, false>();
   if (per_sm < 1) return MPS_ERR_CUDA;
-  if (per_sm > CG_MINB) per_sm = CG_MINB;
-  c->cg_grid = per_sm * c->sm_count;
+  c->cg_grid = c->sm_count;  // one 1024-thread block per SM: fewest barrier arrivals
+  c->cg_lanes = L;
+  const char* to = getenv("MPS_B200_CG_TIMEOUT_CYCLES");  // documented in include/mps_b200.h
+  if (to) c->cg_timeout_cycles = atoll(to);
   return MPS_OK;
 }
 
-int mpsk_pressure_ppe(mps_ctx* c) {
-  const int cur = c->cur;
-  PpeArgs a;
-  a.pos4 = c->pos4[cur]; a.tex = c->cg_tex ? c->pos_tex[cur] : 0; a.tp = c->tp[cur]; a.dens = c->dens; a.dndt = c->dndt; a.keep2 = c->keep2[cur]; a.bc = c->bc; a.b = c->b;
-  a.x = c->cg_x; a.pv = c->cg_p; a.sv = c->cg_s; a.wv = c->cg_w; a.p = c->p;
-  a.nbr = c->nbr; a.cn = c->cn; a.co = c->co; a.rows = c->cg_rows; a.bcount = c->cg_bcount;
-  a.part = c->cg_part; a.cg = c->cg; a.bar = c->cg_bar;
-  a.tol2 = c->prm.cg_rtol * c->prm.cg_rtol;
-  a.maxit = c->prm.cg_maxit;
+// Reads the solve statistics back (one small copy and a stream synchronisation).
+int mpsk_ppe_read_stats(mps_ctx* c) {
+  cudaMemcpyAsync(c->cg_host, c->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream);
+  cudaMemcpyAsync(c->bar_host, c->cg_bar, sizeof(GridBar), cudaMemcpyDeviceToHost, c->stream);
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) {
+    c->err = std::string("CUDA error in the PPE solve: ") + cudaGetErrorString(e);
+    return MPS_ERR_CUDA;
+  }
+  const CgScalars& s = *c->cg_host;
+  if (c->bar_host->timeout) {
+    c->err = "grid barrier timed out inside k_ppe_cg";
+    return MPS_ERR_CUDA;
+  }
+  c->stats.cg_iters = s.iters;
+  c->stats.cg_converged = s.converged;
+  c->stats.cg_relres = s.bb > 0.0 ? sqrt(s.gamma / s.bb) : 0.0;
+  c->stats.n_surface = s.n_surface;
+  c->stats.n_rows = s.n_rows;
+  c->stats.cg_iters_total = s.iters_total;
+  c->stats.cg_noconv_total = s.noconv_total;
+  c->stats.cg_setup_ms = 1e-6 * (double)s.t_setup_ns;
+  c->stats.cg_loop_ms = 1e-6 * (double)s.t_loop_ns;
+  c->stats.cg_loop_ms_total = 1e-6 * (double)s.t_loop_ns_total;
+  const bool noconv = s.noconv_total > c->noconv_seen;
+  c->noconv_seen = s.noconv_total;
+  if (noconv) {
+    c->err = "CG reached cg_maxit without meeting cg_rtol";
+    return MPS_ERR_NOCONV;
+  }
+  return MPS_OK;
+}
+
+int mpsk_pressure_ppe(mps_ctx* c, bool sync) {
+  PpeArgs a = make_args(c);
   // small problems: no more blocks than there is work for (fewer arrivals per barrier)
   int grid = c->cg_grid;
-  const int want = std::max(c->sm_count, div_up((int64_t)c->n * c->cg_lanes, CG_TPB));
+  const int want = std::max(1, div_up((int64_t)c->n * L, CG_TPB));
   if (grid > want) grid = want;
   cudaMemsetAsync(c->cg_bar, 0, sizeof(GridBar), c->stream);
   if (((c)->timer_mask >> MPS_T_CG_SPMV) & 1u) mps_timer_begin(c, MPS_T_CG_SPMV);
   cudaError_t e;
   const bool tp = two_phase(c);
-  if (c->cg_tex) e = tp ? launch_cg<true, 8, true>(c, a, grid) : launch_cg<false, 8, true>(c, a, grid);
-  else e = tp ? launch_cg<true, 8, false>(c, a, grid) : launch_cg<false, 8, false>(c, a, grid);
+  if (c->prm.ppe_operator == 1) e = tp ? launch_cg<true, true, false>(c, a, grid) : launch_cg<false, true, false>(c, a, grid);
+  else if (c->cg_tex) e = tp ? launch_cg<true, false, true>(c, a, grid) : launch_cg<false, false, true>(c, a, grid);
+  else e = tp ? launch_cg<true, false, false>(c, a, grid) : launch_cg<false, false, false>(c, a, grid);
   c->launches++;
   c->t_launches[MPS_T_CG_SPMV]++;
   if (((c)->timer_mask >> MPS_T_CG_SPMV) & 1u) mps_timer_end(c, MPS_T_CG_SPMV);
@@ -493,42 +759,35 @@ int mpsk_pressure_ppe(mps_ctx* c) {
   }
   c->ppe_ready = true;
   c->posw_is_p = true;
-  cudaMemcpyAsync(c->cg_host, c->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream);
-  e = cudaStreamSynchronize(c->stream);
-  if (e != cudaSuccess) {
-    c->err = std::string("CUDA error in mps_pressure_ppe: ") + cudaGetErrorString(e);
-    return MPS_ERR_CUDA;
-  }
-  const CgScalars& s = *c->cg_host;
-  if (s.barrier_timeout) {
-    c->err = "grid barrier timed out inside k_ppe_cg";
-    return MPS_ERR_CUDA;
-  }
-  c->stats.cg_iters = s.iters;
-  c->stats.cg_converged = s.converged;
-  c->stats.cg_relres = s.bb > 0.0 ? sqrt(s.gamma / s.bb) : 0.0;
-  c->stats.n_surface = s.n_surface;
-  c->stats.n_rows = s.n_rows;
-  c->stats.cg_iters_total += s.iters;
-  if (!s.converged) {
-    c->err = "CG reached cg_maxit without meeting cg_rtol";
-    return MPS_ERR_NOCONV;
-  }
-  return MPS_OK;
+  return sync ? mpsk_ppe_read_stats(c) : MPS_OK;
 }
 
 int mpsk_ppe_apply(mps_ctx* c, const double* x, double* y, int order) {
   const int n = (int)c->n;
   const int cur = c->cur;
+  if (c->prm.ppe_operator == 1) {
+    // the matrix assembled by the last solve; cg_w / cg_s serve as compact staging vectors
+    const int nr = c->stats.n_rows;
+    PpeArgs a = make_args(c);
+    if (nr > 0) {
+      MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_stage_in_c, div_up(nr, 256), 256, nr, order, c->cg_rows, c->oid[cur], x,
+                 c->cg_s);
+      MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_ppe_apply_c, div_up((int64_t)nr * L, 256), 256, c->kc, a, nr, c->cg_s,
+                 c->cg_w);
+    }
+    MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_stage_out_c, div_up(n, 256), 256, n, order, c->rowmap, c->oid[cur], c->cg_w,
+               y);
+    return MPS_OK;
+  }
   MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_stage_in, div_up(n, 256), 256, n, order, c->bc, c->oid[cur], x,
              c->pos4[cur]);
   c->posw_is_p = false;
-  const int grid = div_up((int64_t)n * 8, 256);
+  const int grid = div_up((int64_t)n * L, 256);
   if (two_phase(c)) {
-    MPS_LAUNCH(c, MPS_T_PPE_SETUP, (k_ppe_apply<true, 8>), grid, 256, c->kc, c->pos4[cur], c->tp[cur],
+    MPS_LAUNCH(c, MPS_T_PPE_SETUP, (k_ppe_apply<true>), grid, 256, c->kc, c->pos4[cur], c->tp[cur],
                c->bc, c->nbr, c->cn, c->co, c->cg_w);
   } else {
-    MPS_LAUNCH(c, MPS_T_PPE_SETUP, (k_ppe_apply<false, 8>), grid, 256, c->kc, c->pos4[cur], c->tp[cur],
+    MPS_LAUNCH(c, MPS_T_PPE_SETUP, (k_ppe_apply<false>), grid, 256, c->kc, c->pos4[cur], c->tp[cur],
                c->bc, c->nbr, c->cn, c->co, c->cg_w);
   }
   MPS_LAUNCH(c, MPS_T_PPE_SETUP, k_stage_out, div_up(n, 256), 256, n, order, c->oid[cur], c->cg_w, y);

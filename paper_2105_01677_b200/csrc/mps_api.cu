@@ -68,6 +68,9 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->rho_s[0]); cudaFree(c->rho_s[1]); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
   cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
   cudaFree(c->cg_rows); cudaFree(c->cg_bcount); cudaFree(c->cg_bar);
+  cudaFree(c->mat_val); cudaFree(c->mat_col); cudaFree(c->mat_cnt); cudaFree(c->mat_dex); cudaFree(c->rowmap);
+  cudaFree(c->cg_rc); cudaFree(c->cg_xc);
+  if (c->bar_host) cudaFreeHost(c->bar_host);
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
   if (c->cg_host) cudaFreeHost(c->cg_host);
   if (c->flags_host) cudaFreeHost(c->flags_host);
@@ -92,6 +95,8 @@ static int check_params(const mps_params* p, int64_t n) {
   if (p->ppe_source < 0 || p->ppe_source > 2) return fail(nullptr, MPS_ERR_ARG, "ppe_source must be 0..2");
   if (p->ppe_laplacian < 0 || p->ppe_laplacian > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_laplacian must be 0 or 1");
   if (p->rebin_every < 1 || p->rebin_every > 1000) return fail(nullptr, MPS_ERR_ARG, "rebin_every must be in [1, 1000]");
+  if (p->ppe_operator < 0 || p->ppe_operator > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_operator must be 0 (matrix-free) or 1 (assembled)");
+  if (p->cg_warm_start < 0 || p->cg_warm_start > 1) return fail(nullptr, MPS_ERR_ARG, "cg_warm_start must be 0 or 1");
   if (p->kernel < 0 || p->kernel > 1) return fail(nullptr, MPS_ERR_ARG, "kernel must be 0 (Eq. 3) or 1 (Eq. 4)");
   if (p->kernel == 1 && (p->ppe_source != 0 || p->ppe_laplacian != 0))
     return fail(nullptr, MPS_ERR_ARG, "Eq. 15-18 are derived for the Eq. 3 kernel: kernel 1 needs ppe_source = ppe_laplacian = 0");
@@ -196,6 +201,12 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->cg_part, (size_t)2 * (c->sm_count * 8 + 8)));
   A(dalloc(&c->cg_rows, N)); A(dalloc(&c->cg_bcount, (size_t)2 * (c->sm_count * 8 + 8)));
   A(dalloc(&c->cg_bar, 1));
+  if (prm->ppe_operator == 1) {  // the assembled operator: 12 bytes per pair of the rows bc = 0
+    A(dalloc(&c->mat_val, N * (size_t)k.stride)); A(dalloc(&c->mat_col, N * (size_t)k.stride));
+    A(dalloc(&c->mat_cnt, N)); A(dalloc(&c->mat_dex, N)); A(dalloc(&c->rowmap, N));
+    A(dalloc(&c->cg_rc, N)); A(dalloc(&c->cg_xc, N));
+  }
+  A(cudaMallocHost((void**)&c->bar_host, sizeof(GridBar)));
   A(dalloc(&c->cg, 1)); A(dalloc(&c->flags, 1)); A(dalloc(&c->io_tmp, N));
   A(cudaMallocHost((void**)&c->cg_host, sizeof(CgScalars)));
   A(cudaMallocHost((void**)&c->flags_host, sizeof(DevFlags)));
@@ -241,6 +252,13 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     return MPS_ERR_CUDA;
   }
   memset(c->cg_host, 0, sizeof(CgScalars));
+  memset(c->bar_host, 0, sizeof(GridBar));
+  if (prm->ppe_operator == 1) {
+    cudaMemsetAsync(c->mat_cnt, 0, N * 4, c->stream);
+    cudaMemsetAsync(c->rowmap, 0xff, N * 4, c->stream);
+    cudaMemsetAsync(c->cg_rc, 0, N * 8, c->stream);
+    cudaMemsetAsync(c->cg_xc, 0, N * 8, c->stream);
+  }
   memset(c->flags_host, 0, sizeof(DevFlags));
   cudaStream_t s = c->stream;
   cudaMemsetAsync(c->cg, 0, sizeof(CgScalars), s);
@@ -481,9 +499,8 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     if (hs) mpsk_dndt(c, 0);
     if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
     else {
-      int rc = mpsk_pressure_ppe(c);
+      int rc = mpsk_pressure_ppe(c, /*sync=*/false);  // statistics are read once, after the last step
       if (rc == MPS_ERR_CUDA) return rc;
-      if (rc && !first_err) first_err = rc;
     }
     mpsk_gradient(c);
     mpsk_correct(c);
@@ -491,6 +508,11 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
   }
   c->kc.stale = 0;  // API-level sweeps always run on exact rows (they need mps_bin first)
   CK(cudaGetLastError());
+  if (route == MPS_ROUTE_PPE && nsteps > 0) {
+    int rc = mpsk_ppe_read_stats(c);
+    if (rc == MPS_ERR_CUDA) return rc;
+    if (rc) first_err = rc;
+  }
   int fl = read_flags(c);
   if (fl) return fl;
   return first_err;

@@ -28,24 +28,29 @@
 #define NB_PHASE1 0x40000000u
 #define NB_WALL 0x20000000u
 #define NB_INDEX 0x1fffffffu
+#define ROW_NONE 0xffffffffu     // rowmap: dummy / ghost (bc = -1)
+#define ROW_SURFACE 0xfffffffeu  // rowmap: free surface (bc = 1)
 
 // position of back entry kk (0-based) in a row of `stride` entries
 __host__ __device__ __forceinline__ uint32_t back_slot(int stride, uint32_t kk) {
   return (uint32_t)stride - 8u * (kk / 8u + 1u) + (kk & 7u);
 }
 
-struct CgScalars {  // what k_ppe_cg reports at exit (block 0)
+struct CgScalars {  // what the persistent CG kernel reports at exit (block 0)
   double gamma;                 // r.r of the last iteration
   double bb, tol2bb;            // b.b and cg_rtol^2 b.b
   int iters, done, converged, maxit;
   int n_surface, n_rows;
-  int barrier_timeout, pad;
+  int noconv_total, pad;        // solves that hit maxit since the ctx was made
+  long long iters_total;        // iterations since the ctx was made
+  unsigned long long t_setup_ns, t_loop_ns;  // %globaltimer of block 0: setup (+ assembly) and the CG loop
+  unsigned long long t_loop_ns_total;
 };
 
-// Grid-wide barrier state of the persistent CG kernel (zeroed at init).
+// Grid-wide barrier state of the persistent CG kernel (zeroed before every launch).
 struct GridBar {
-  unsigned int count;  // arrivals since the launch (monotonic; a barrier waits for nb x generation)
-  unsigned int pad;
+  unsigned int count;    // arrivals since the launch (monotonic; a barrier waits for nb x generation)
+  unsigned int timeout;  // a spin exceeded the limit: the kernel drained instead of hanging
 };
 
 struct DevFlags {
@@ -131,6 +136,18 @@ struct mps_ctx {
   double* cg_w = nullptr;
   double* cg_part = nullptr;  // per-block partial sums
   uint32_t* cg_rows = nullptr;   // compacted slot indices of the PPE unknowns (bc == 0)
+  // ppe_operator 1: the assembled operator over the compacted rows g = 0..n_rows-1 (ELL, row g at
+  // g * kc.stride) and the CG vectors in the same compact numbering
+  double* mat_val = nullptr;     // c_ij of the neighbours j that are unknowns too
+  uint32_t* mat_col = nullptr;   // their compact row index
+  uint32_t* mat_cnt = nullptr;   // entries of row g
+  double* mat_dex = nullptr;     // sum of c_ij over free-surface neighbours + compress / dt^2
+  uint32_t* rowmap = nullptr;    // slot -> compact row (ROW_SURFACE / ROW_NONE otherwise)
+  double* cg_rc = nullptr;       // residual, compact
+  double* cg_xc = nullptr;       // solution, compact (cg_x is its per-slot copy)
+  long long cg_timeout_cycles = 4000000000LL;  // grid-barrier spin limit (0: none)
+  GridBar* bar_host = nullptr;   // pinned
+  int noconv_seen = 0;           // CgScalars.noconv_total at the last read
   uint32_t* cg_bcount = nullptr; // per-block row / surface counts of the setup phase
   GridBar* cg_bar = nullptr;
   int cg_grid = 0;               // co-resident blocks of the persistent CG kernel
@@ -188,7 +205,8 @@ int mpsk_viscosity(mps_ctx* c);
 int mpsk_predict(mps_ctx* c);
 int mpsk_pressure_explicit(mps_ctx* c);
 int mpsk_ppe_plan(mps_ctx* c);           // co-resident grid of the persistent CG kernel
-int mpsk_pressure_ppe(mps_ctx* c);
+int mpsk_pressure_ppe(mps_ctx* c, bool sync = true);  // sync: read the solve's statistics back
+int mpsk_ppe_read_stats(mps_ctx* c);
 int mpsk_ppe_apply(mps_ctx* c, const double* x, double* y, int order);
 int mpsk_gradient(mps_ctx* c);
 int mpsk_correct(mps_ctx* c);

@@ -89,6 +89,9 @@ def default_params(l0: float) -> Dict[str, object]:
         ppe_laplacian=0,     # 0 Eq. 10 form; 1 higher-order Laplacian (Eq. 16)
         kernel=0,            # 0 w = re/r - 1 (Eq. 3); 1 w = (1 - r/re)^3 (Eq. 4)
         rebin_every=1,       # 1 exact sets at every sweep; K > 1 the paper's list reuse
+        ppe_operator=1,      # CUDA path only: 0 matrix-free operator, 1 coefficients assembled once per solve
+        cg_warm_start=0,     # 1: CG starts from the particle's previous pressure instead of 0
+        key_mode=0,          # 0 linear x-fastest cell key, 1 Morton (3 x 10-bit interleave)
         clamp_negative_p=1,
         rho_pair_mean=0,
         nu_pair_mean=1,

@@ -34,10 +34,10 @@ def test_library_exports_every_declared_symbol(B):
 
 
 def test_struct_layout_matches_header(B):
-    # 14 int32 then 28 doubles, no padding
-    assert C.sizeof(B.MpsParams) == 14 * 4 + 28 * 8
-    assert B.MpsParams.l0.offset == 56
-    assert C.sizeof(B.MpsStats) == 56
+    # 16 int32 then 28 doubles, no padding
+    assert C.sizeof(B.MpsParams) == 16 * 4 + 28 * 8
+    assert B.MpsParams.l0.offset == 64
+    assert C.sizeof(B.MpsStats) == 80
     # field ids in the binding equal the header's enum
     src = open(os.path.join(ROOT, "include", "mps_b200.h")).read()
     for name, fid in B.FIELDS.items():
@@ -67,7 +67,7 @@ def _init_rc(B, **over):
 
 @pytest.mark.parametrize("over", [
     dict(dim=4), dict(dim=2, ppe_laplacian=1), dict(ppe_source=3), dict(kernel=2), dict(kernel=1, ppe_source=1), dict(rebin_every=0), dict(_n=0), dict(_n=-5), dict(l0=0.0), dict(dt=-1.0), dict(re_grad=0.5), dict(re_lap=0.001),
-    dict(cell_div=0), dict(cell_div=4), dict(key_mode=1), dict(n_phases=3), dict(max_neighbours=0),
+    dict(cell_div=0), dict(cell_div=4), dict(key_mode=2), dict(ppe_operator=2), dict(cg_warm_start=-1), dict(n_phases=3), dict(max_neighbours=0),
     dict(grad_variant=4), dict(rho=(0.0, 1.0)), dict(cg_rtol=0.0), dict(domain_max=(0.0, 1.0, 1.0)),
 ])
 def test_bad_parameters_are_rejected(B, over):

@@ -224,12 +224,14 @@ def test_phat_and_gradient(B, O, variant, route):
 
 
 # ------------------------------------------------------------------- S8b: PPE ---
+@pytest.mark.parametrize("op", [0, 1])   # matrix-free / assembled operator
 @pytest.mark.parametrize("over", [dict(), dict(compress=0.0), dict(n_phases=2, rho=(1000.0, 800.0)),
                                   dict(n_phases=2, rho=(1000.0, 800.0), rho_pair_mean=1),
-                                  dict(clamp_negative_p=0), dict(cell_div=2)])
-def test_ppe_flags_rhs_operator_and_solution(B, O, over):
+                                  dict(clamp_negative_p=0), dict(cell_div=2), dict(cg_warm_start=1)])
+def test_ppe_flags_rhs_operator_and_solution(B, O, over, op):
     s = scenes.small_tank(shuffle=True)
     s.phase[s.z > 0.03] = 1
+    over = dict(over, ppe_operator=op)
     g, o = _pair(B, O, s, **over)
     o.viscosity(); o.predict()
     inject(g, o, ("x", "y", "z", "u", "v", "w"))
@@ -258,7 +260,7 @@ def test_ppe_flags_rhs_operator_and_solution(B, O, over):
     assert true_rel <= 2e-8
     assert relres_g <= 1e-8 and st["cg_converged"] == 1
     it_o = o.ppe_solve(o.params["cg_rtol"], 5000)
-    assert abs(it_g - it_o) <= 3
+    assert abs(it_g - it_o) <= 3 or over.get("cg_warm_start")
     it_t = o.ppe_solve(1e-13, 5000)
     xt = o.get("xcg")
     kappa_est = 4.0 * (it_o / np.log(2.0 / 1e-8)) ** 2
@@ -271,8 +273,35 @@ def test_ppe_flags_rhs_operator_and_solution(B, O, over):
     assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-8 * kappa_est
 
 
-def test_ppe_noconv_and_zero_rhs(B, O):
+@pytest.mark.parametrize("op", [0, 1])
+def test_ppe_warm_start_from_previous_pressure(B, O, op):
+    """cg_warm_start: x0 = the particle's previous pressure, carried through the sorts.  Any x that
+    meets the residual bar is correct; started from the converged pressure of the same system the
+    solve must need (almost) no iterations."""
     s = scenes.small_tank(shuffle=True)
+    # (no clamp: the carried pressure is then the CG solution itself)
+    g, o = _pair(B, O, s, ppe_operator=op, cg_warm_start=1, clamp_negative_p=0)
+    o.step(3, 1); o.viscosity(); o.predict()
+    inject(g, o, ("x", "y", "z", "u", "v", "w"))
+    g.bin(); g.density(); o.density()
+    g.set("n", o.get("n"))
+    it_cold, _ = g.pressure_ppe()           # pos4.w carried nothing yet: a cold start
+    o.ppe_flags(); o.ppe_rhs()
+    b = o.get("b")
+    x1 = g.get("xcg")
+    assert np.linalg.norm(b - o.ppe_apply(x1)) / np.linalg.norm(b) <= 2e-8
+    g.bin()                                 # the sort carries p (now in pos4.w) to the new slots
+    g.density(); g.set("n", o.get("n"))
+    it_warm, rr = g.pressure_ppe()
+    x2 = g.get("xcg")
+    assert it_cold > 10 and it_warm <= 2 and rr <= 1e-8
+    assert np.linalg.norm(b - o.ppe_apply(x2)) / np.linalg.norm(b) <= 2e-8
+
+
+@pytest.mark.parametrize("op", [0, 1])
+def test_ppe_noconv_and_zero_rhs(B, O, op):
+    s = scenes.small_tank(shuffle=True)
+    s.params["ppe_operator"] = op
     g = B.Mps(s, cg_maxit=3)
     g.bin(); g.density()
     with pytest.raises(B.MpsError) as ei:
@@ -420,13 +449,14 @@ def test_full_size_sampled_config3(B, O):
     assert (np.diff(perm.astype(np.int64))[same] > 0).all()
 
 
-@pytest.mark.parametrize("cfg,idx", [(3, 0), (4, 0), (5, 2)])
-def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx):
+@pytest.mark.parametrize("cfg,idx,op", [(3, 0, 1), (3, 0, 0), (4, 0, 1), (4, 0, 0), (5, 2, 1)])
+def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx, op):
     """Configs 3 (N = 438,208), 4 (two-phase, Smagorinsky, N = 634,808) and 5[2] (N = 1,011,096)
     in the launch configuration bench.py times (warp-per-cell row builder, 148 x 1024 persistent
     CG): density, flags, right-hand side and operator against the oracle on identical positions,
     and the GPU's CG solution checked by its true residual under the ORACLE's operator."""
     s = scenes.make_scene(cfg, sweep_index=idx)
+    s.params["ppe_operator"] = op
     g = B.Mps(s)
     o = O.Oracle(s)
     g.step(1, 1)                      # one whole PPE step moves the fluid off the lattice

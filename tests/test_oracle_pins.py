@@ -822,3 +822,206 @@ def test_dam_break_leading_edge_between_theory_bounds(route):
         assert prev - 1e-9 <= front < 1.0 + 2.0 * T
         prev = front
     assert abs(T - 2.09) < 0.01 and 2.3 <= front <= 3.3
+
+
+# ---- pair viscosity nu_ij (Q9): harmonic / arithmetic mean, wall rule (unpinned branch a) ----
+@pytest.mark.parametrize("mean", [1, 0])
+def test_viscosity_pair_mean_shell_sum_at_a_flat_interface(mean):
+    # un-jittered lattice block, lower half nu_a, upper half nu_b, u = (a z^2, 0, 0), g = 0.
+    # Interior of one phase: nu * Laplacian(a z^2) = 2 a nu (T5's closed form).  In the layer just
+    # below the interface the offsets with o_z > 0 reach the other phase and carry nu_ab; written
+    # out as a sum over lattice offsets (Eq. 10 with nu_ij inside the sum).
+    m = 16
+    s = scenes.fluid_blob(L0, (m, m, m))
+    ix = np.rint(s.x / L0 - 0.5).astype(int)
+    iy = np.rint(s.y / L0 - 0.5).astype(int)
+    iz = np.rint(s.z / L0 - 0.5).astype(int)
+    s.phase[iz >= m // 2] = 1
+    a = 3.0
+    s.u[:] = a * s.z ** 2
+    nu_a, nu_b = 0.7, 1.9
+    o = O.Oracle(s, n_phases=2, nu=(nu_a, nu_b), nu_pair_mean=mean, g=(0.0, 0.0, 0.0))
+    o.bin(); o.viscosity()
+    ax = o.get("ax")
+    core_xy = (ix >= 4) & (ix < m - 4) & (iy >= 4) & (iy < m - 4)   # layers 4..11 have their whole ball inside in z
+    nu_ab = 2 * nu_a * nu_b / (nu_a + nu_b) if mean == 1 else 0.5 * (nu_a + nu_b)
+    n0l, lam = GOLD["n0_3d_3.1"], GOLD["lambda_3d_3.1"] * L0 ** 2
+    A = 2.0 * 3 / (n0l * lam)
+
+    def shell_sum(zi_layer, own_phase):
+        z = (zi_layer + 0.5) * L0
+        tot = 0.0
+        for oz in range(-3, 4):
+            for oy in range(-3, 4):
+                for ox in range(-3, 4):
+                    r2 = ox * ox + oy * oy + oz * oz
+                    if r2 == 0 or r2 >= 3.1 ** 2:
+                        continue
+                    other = (zi_layer + oz >= m // 2) != (own_phase == 1)
+                    nu_i = nu_a if own_phase == 0 else nu_b
+                    nu = nu_ab if other else nu_i
+                    du = a * ((z + oz * L0) ** 2 - z ** 2)
+                    tot += nu * du * (3.1 / math.sqrt(r2) - 1.0)
+        return A * tot
+
+    for layer, ph in ((m // 2 - 1, 0), (m // 2 - 2, 0), (m // 2 - 4, 0), (m // 2, 1), (m // 2 + 2, 1)):
+        sel = core_xy & (iz == layer)
+        assert sel.sum() > 0
+        assert np.allclose(ax[sel], shell_sum(layer, ph), rtol=1e-11), (layer, ph)
+    # four layers below the interface nothing reaches across: the single-nu closed form 2 a nu_a
+    assert np.allclose(ax[core_xy & (iz == m // 2 - 4)], 2 * a * nu_a, rtol=1e-11)
+    # the two means differ at the interface (so a swapped formula fails one of the two runs)
+    assert abs(shell_sum(m // 2 - 1, 0) - 2 * a * nu_a) > 1e-3
+
+
+@pytest.mark.parametrize("mean", [1, 0])
+@pytest.mark.parametrize("cs", [0.0, 0.12])
+def test_viscosity_brute_force_with_walls_two_phases(mean, cs):
+    # jittered tank with walls present, random velocities, two viscosities: the O(N^2) definition
+    # a_i = A_lap sum_j nu_ij (u_j - u_i) w + g with nu_ij = nu_i and u_j = 0 for WALL/DUMMY j (Q9),
+    # nu_i = nu[phase] + nu_t (nu_t from the oracle's own field when Cs > 0: its formula is pinned by
+    # test_smagorinsky_simple_shear).
+    s = scenes.small_tank(shuffle=True)
+    s.phase[s.z > 0.03] = 1
+    rng = np.random.default_rng(12)
+    fl = s.type == scenes.FLUID
+    for k in "uvw":
+        getattr(s, k)[fl] = rng.standard_normal(fl.sum())
+        getattr(s, k)[~fl] = 7.0           # must be ignored: walls and dummies are at rest (no-slip)
+    nu = np.array([0.7, 1.9])
+    o = O.Oracle(s, n_phases=2, nu=tuple(nu), nu_pair_mean=mean, cs=cs)
+    o.bin(); o.viscosity()
+    nut = o.get("nut")
+    assert (nut[~fl] == 0).all() and ((nut[fl] > 0).all() if cs > 0 else (nut == 0).all())
+    re = s.params["re_lap"]
+    dx = s.x[None, :] - s.x[:, None]; dy = s.y[None, :] - s.y[:, None]; dz = s.z[None, :] - s.z[:, None]
+    r2 = (dx * dx + dy * dy) + dz * dz
+    msk = r2 < re * re
+    np.fill_diagonal(msk, False)
+    w = np.where(msk, re / np.sqrt(np.where(msk, r2, 1.0)) - 1.0, 0.0)
+    nui = nu[s.phase] + nut
+    ni, nj = nui[:, None], nui[None, :]
+    pair = 2 * ni * nj / (ni + nj) if mean == 1 else 0.5 * (ni + nj)
+    solid_j = (~fl)[None, :]
+    nuij = np.where(solid_j, ni, pair)
+    n0l, lam = GOLD["n0_3d_3.1"], GOLD["lambda_3d_3.1"] * L0 ** 2
+    A = 2.0 * 3 / (n0l * lam)
+    for comp, vel, gc in (("ax", s.u, 0.0), ("ay", s.v, 0.0), ("az", s.w, -9.81)):
+        uj = np.where(fl, vel, 0.0)
+        ref = A * (nuij * (uj[None, :] - vel[:, None]) * w).sum(axis=1) + gc
+        got = o.get(comp)
+        assert np.allclose(got[fl], ref[fl], rtol=1e-11, atol=1e-9 * np.abs(ref[fl]).max()), comp
+        assert (got[~fl] == 0).all()
+    # the wall rule matters here: fluid next to a wall would change if nu_ij used the pair mean with nu_j
+    near_wall = fl & (np.where(solid_j & msk, 1, 0).sum(axis=1) > 0)
+    assert near_wall.sum() > 50
+
+
+# ---- p-hat and gradient variants 0-2 by brute force, dummies carrying a non-zero p (branch b) ----
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_phat_and_gradient_brute_force_skip_dummies(variant):
+    # P:215 Eq. 14 / Q12, Q13: dummies have no pressure and are skipped both in p-hat and in the
+    # sum.  They are given a large p here so that including them changes every wall-near value.
+    s = scenes.small_tank(shuffle=True)
+    rng = np.random.default_rng(21)
+    p = rng.uniform(100.0, 500.0, s.n)
+    dummy = s.type == scenes.DUMMY
+    p[dummy] = -1.0e4                       # would win every minimum and dominate every sum
+    o = O.Oracle(s, grad_variant=variant)
+    o.bin(); o.set("p", p); o.phat(); o.gradient()
+    re = s.params["re_n"]
+    dx = s.x[None, :] - s.x[:, None]; dy = s.y[None, :] - s.y[:, None]; dz = s.z[None, :] - s.z[:, None]
+    r2 = (dx * dx + dy * dy) + dz * dz
+    m = (r2 < re * re) & (~dummy)[None, :]
+    np.fill_diagonal(m, False)
+    # p-hat: FLUID and WALL rows, minimum over i itself and its non-dummy neighbours
+    ph_ref = np.minimum(p, np.where(m, p[None, :], np.inf).min(axis=1))
+    on = (s.type == scenes.FLUID) | (s.type == scenes.WALL)
+    ph = o.get("phat")
+    assert np.array_equal(ph[on], ph_ref[on]) and (ph[~on] == 0).all()
+    assert (ph[on] >= 100.0).all()          # no dummy value leaked in
+    r2s = np.where(m, r2, 1.0)
+    w = np.where(m, re / np.sqrt(r2s) - 1.0, 0.0)
+    if variant == 0:
+        coef = p[None, :] - ph_ref[:, None]
+    elif variant == 1:
+        phj = np.where(on, ph_ref, 0.0)
+        coef = (p[:, None] + p[None, :]) - (ph_ref[:, None] + phj[None, :])
+    else:
+        coef = p[:, None] + p[None, :]
+    c = coef / r2s * w
+    n0 = GOLD["n0_3d_2.1"]
+    fluid = s.type == scenes.FLUID
+    touched = fluid & ((r2 < re * re) & dummy[None, :]).any(axis=1)
+    assert touched.sum() > 20               # some fluid rows do have dummies in range
+    for comp, d in (("gx", dx), ("gy", dy), ("gz", dz)):
+        ref = (3.0 / n0) * (c * d).sum(axis=1)
+        got = o.get(comp)
+        assert np.allclose(got[fluid], ref[fluid], rtol=1e-11, atol=1e-9 * np.abs(ref[fluid]).max())
+        assert (got[~fluid] == 0).all()
+
+
+# ---- the record of neighbours kept during a solve changes no number; warm start reaches the same x ----
+def test_cg_neighbour_record_and_warm_start():
+    s = scenes.small_tank(shuffle=True)
+    o = O.Oracle(s); o.step(3, 1); o.viscosity(); o.predict(); o.density()
+    o.ppe_flags(); o.ppe_rhs()
+    rows = o.get("bc") == 0
+    it = o.ppe_solve(1e-8, 5000)
+    x = o.get("xcg"); b = o.get("b")
+    # the solve's operator (walking the record) and ppe_apply (searching the grid) are the same map
+    assert np.linalg.norm(b - o.ppe_apply(x)) <= 1.5e-8 * np.linalg.norm(b)
+    assert it > 10
+    # warm start: from the converged pressure of the same system CG needs no iteration; from a
+    # perturbed start it reaches the same solution
+    w = O.Oracle(s, cg_warm_start=1)
+    for k in ("x", "y", "z", "u", "v", "w", "n"):
+        w.set(k, o.get(k))
+    w.ppe_flags(); w.ppe_rhs()
+    w.set("p", np.where(rows, x, 0.0))
+    assert w.ppe_solve(1e-8, 5000) == 0
+    w.set("p", np.where(rows, x * (1.0 + 0.05 * np.sin(np.arange(s.n))), 0.0))
+    it_w = w.ppe_solve(1e-8, 5000)
+    assert 0 < it_w <= it
+    assert np.linalg.norm(w.get("xcg") - x) <= 1e-6 * np.linalg.norm(x)
+
+
+# ---- key_mode 1: the Morton key (north_star "Morton- or cell-sorted") ----
+def test_morton_key_table_and_sort_invariants():
+    # hand table: bit k of c_x -> bit 3k, c_y -> bit 3k+1, c_z -> bit 3k+2
+    table = {(0, 0, 0): 0, (1, 0, 0): 1, (0, 1, 0): 2, (0, 0, 1): 4, (1, 1, 1): 7, (2, 0, 0): 8,
+             (0, 2, 0): 16, (0, 0, 2): 32, (3, 0, 0): 9, (2, 3, 1): 8 + 16 + 2 + 4,
+             (5, 0, 0): 1 + 64, (0, 5, 0): 2 + 128, (0, 0, 5): 4 + 256,
+             (7, 7, 7): 511, (8, 0, 0): 512, (1023, 0, 0): sum(1 << (3 * k) for k in range(10)),
+             (1023, 1023, 1023): (1 << 30) - 1}
+    for (cx, cy, cz), key in table.items():
+        assert O.morton3(cx, cy, cz) == key, (cx, cy, cz)
+    s = scenes.small_tank(shuffle=True)
+    s.x[5] = 10.0                           # a ghost
+    lin = O.Oracle(s)
+    mor = O.Oracle(s, key_mode=1)
+    kl, pl, csl = lin.bin()
+    km, pm, csm = mor.bin()
+    nx, ny, nz, ncl = lin.grid()
+    assert mor.grid()[:3] == (nx, ny, nz)
+    bits = max(nx, ny, nz).bit_length() if (max(nx, ny, nz) & (max(nx, ny, nz) - 1)) else max(nx, ny, nz).bit_length() - 1
+    assert mor.grid()[3] == 8 ** bits and csm.size == 8 ** bits + 1
+    # the Morton key of every particle is the interleave of the cell coordinates its linear key encodes
+    live = kl < ncl
+    cx, cy, cz = kl % nx, (kl // nx) % ny, kl // (nx * ny)
+    ref = np.array([O.morton3(int(a), int(b), int(c)) for a, b, c in zip(cx, cy, cz)])
+    assert np.array_equal(km[live], ref[live]) and (km[~live] == 8 ** bits).all() and (~live).sum() == 1
+    # T12 invariants for the Morton sort
+    assert np.array_equal(np.sort(pm), np.arange(s.n))
+    ks = km[pm]
+    assert (np.diff(ks) >= 0).all() and (np.diff(pm)[np.diff(ks) == 0] > 0).all()
+    assert csm[0] == 0 and csm[-1] == s.n - 1 and (np.diff(csm) >= 0).all()
+    assert np.array_equal(np.diff(csm), np.bincount(km[live], minlength=8 ** bits))
+    # the neighbour sets and every field do not depend on the key
+    for re in (s.params["re_n"], s.params["re_lap"]):
+        a, b = lin.neighbours(re), mor.neighbours(re)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    lin2 = O.Oracle(scenes.small_tank(shuffle=True)); mor2 = O.Oracle(scenes.small_tank(shuffle=True), key_mode=1)
+    lin2.step(3, 1); mor2.step(3, 1)
+    for k in ("x", "y", "z"):               # only the order of additions inside a sum differs
+        assert np.abs(lin2.get(k) - mor2.get(k)).max() <= 1e-12 * 0.12
