@@ -495,6 +495,186 @@ struct Orc {
     nbc_drop();
     return conv ? cg_iters : -cg_iters;
   }
+
+  // ---- NEXT-4 ("incomplete Cholesky conjugate gradient"): preconditioned CG ------------
+  // The rows bc = 0 of Listing 2's matrix written out as CSR in the order of the
+  // cell-sorted slots (perm): diagonal = sum of c_ij over non-dummy neighbours + compress/dt^2,
+  // off-diagonal -c_ij where j is an unknown too.  precond: 0 none, 1 Jacobi (diagonal),
+  // 2 block Jacobi with the grid cells as blocks (dense Cholesky of each block), 3 incomplete Cholesky
+  // with zero fill-in IC(0) (the paper's ICCG), 4 Chebyshev polynomial of degree `degree` on
+  // [lmax / ratio, lmax].  Textbook PCG (Saad, Alg. 9.1) from x0 = 0; the stopping rule is the
+  // oracle's: ||r|| <= rtol ||b|| on the unpreconditioned residual.
+  struct Csr { int m = 0; std::vector<int> off, col; std::vector<double> val, diag; std::vector<int> row_of, slot; };
+  Csr pcg_assemble() {
+    Csr A;
+    ensure_binned();
+    const double re = prm.re_lap;
+    A.row_of.assign(n, -1);
+    for (int s = 0; s < n; ++s) { int i = perm[s]; if (bc[i] == 0) { A.row_of[i] = A.m++; A.slot.push_back(i); } }
+    A.off.assign(A.m + 1, 0); A.diag.assign(A.m, 0.0);
+    for (int r = 0; r < A.m; ++r) {
+      const int i = A.slot[r];
+      std::vector<std::pair<int, double>> ent;
+      double d = prm.compress / (prm.dt * prm.dt);
+      for_neighbours(i, re, [&](int j, double, double, double, double r2) {
+        if (bc[j] == -1) return;
+        const double c = lap_coef(re, r2) / rho_pair(i, j);
+        d += c;
+        if (bc[j] == 0) ent.push_back({A.row_of[j], -c});
+      });
+      std::sort(ent.begin(), ent.end());
+      for (auto& e : ent) { A.col.push_back(e.first); A.val.push_back(e.second); }
+      A.diag[r] = d;
+      A.off[r + 1] = (int)A.col.size();
+    }
+    return A;
+  }
+  static void csr_apply(const Csr& A, const std::vector<double>& x, std::vector<double>& y) {
+    for (int r = 0; r < A.m; ++r) {
+      double s = A.diag[r] * x[r];
+      for (int k = A.off[r]; k < A.off[r + 1]; ++k) s += A.val[k] * x[A.col[k]];
+      y[r] = s;
+    }
+  }
+  int pcg_iters = 0;
+  double pcg_relres = 0.0;
+  int ppe_solve_pcg(double rtol, int maxit, int precond, int degree, double ratio) {
+    Csr A = pcg_assemble();
+    const int m = A.m;
+    std::vector<double> b(m), x(m, 0.0), r(m), z(m), p(m), Ap(m);
+    for (int q = 0; q < m; ++q) b[q] = f[12][A.slot[q]];
+    // --- set-up of M
+    std::vector<double> Ld;                 // IC(0): diagonal of L; lower part shares A's pattern
+    std::vector<double> Lv;
+    std::vector<int> blk_of, blk_off, blk_rows;  // block Jacobi
+    std::vector<std::vector<double>> blkL;
+    double lmax = 0.0;
+    if (precond == 3) {
+      Lv = A.val; Ld = A.diag;
+      // row-oriented IC(0): for row r, for each lower entry (r, k): L_rk = (a_rk - sum_{j<k} L_rj L_kj) / L_kk
+      for (int r2 = 0; r2 < m; ++r2) {
+        for (int a = A.off[r2]; a < A.off[r2 + 1] && A.col[a] < r2; ++a) {
+          const int k = A.col[a];
+          double sum = Lv[a];
+          int pa = A.off[r2], pb = A.off[k];
+          while (pa < a && pb < A.off[k + 1] && A.col[pb] < k) {
+            if (A.col[pa] == A.col[pb]) { sum -= Lv[pa] * Lv[pb]; ++pa; ++pb; }
+            else if (A.col[pa] < A.col[pb]) ++pa; else ++pb;
+          }
+          Lv[a] = sum / Ld[k];
+        }
+        double d = A.diag[r2];
+        for (int a = A.off[r2]; a < A.off[r2 + 1] && A.col[a] < r2; ++a) d -= Lv[a] * Lv[a];
+        if (!(d > 0.0)) return -1000000;  // breakdown (cannot happen for this M-matrix)
+        Ld[r2] = std::sqrt(d);
+      }
+    } else if (precond == 2) {
+      // blocks = grid cells (rows are in cell-sorted order, so a block is a run of consecutive rows)
+      blk_of.assign(m, 0);
+      int nb = 0, last = -1;
+      for (int q = 0; q < m; ++q) { int kq = key[A.slot[q]]; if (kq != last) { blk_off.push_back(q); last = kq; ++nb; } blk_of[q] = nb - 1; }
+      blk_off.push_back(m);
+      blkL.resize(nb);
+      for (int bq = 0; bq < nb; ++bq) {
+        const int lo = blk_off[bq], sz = blk_off[bq + 1] - lo;
+        std::vector<double>& M = blkL[bq];
+        M.assign((size_t)sz * sz, 0.0);
+        for (int q = 0; q < sz; ++q) {
+          M[(size_t)q * sz + q] = A.diag[lo + q];
+          for (int k = A.off[lo + q]; k < A.off[lo + q + 1]; ++k) {
+            const int c2 = A.col[k] - lo;
+            if (c2 >= 0 && c2 < sz) M[(size_t)q * sz + c2] = A.val[k];
+          }
+        }
+        for (int j = 0; j < sz; ++j) {       // dense Cholesky, lower triangle in place
+          double d = M[(size_t)j * sz + j];
+          for (int k = 0; k < j; ++k) d -= M[(size_t)j * sz + k] * M[(size_t)j * sz + k];
+          d = std::sqrt(d);
+          M[(size_t)j * sz + j] = d;
+          for (int i2 = j + 1; i2 < sz; ++i2) {
+            double v = M[(size_t)i2 * sz + j];
+            for (int k = 0; k < j; ++k) v -= M[(size_t)i2 * sz + k] * M[(size_t)j * sz + k];
+            M[(size_t)i2 * sz + j] = v / d;
+          }
+        }
+      }
+    } else if (precond == 4) {
+      for (int q = 0; q < m; ++q) {          // Gershgorin bound of the largest eigenvalue
+        double s2 = A.diag[q];
+        for (int k = A.off[q]; k < A.off[q + 1]; ++k) s2 += std::fabs(A.val[k]);
+        lmax = std::max(lmax, s2);
+      }
+    }
+    auto apply_M = [&](const std::vector<double>& rin, std::vector<double>& zout) {
+      if (precond == 1) { for (int q = 0; q < m; ++q) zout[q] = rin[q] / A.diag[q]; }
+      else if (precond == 2) {
+        for (size_t bq = 0; bq + 1 < blk_off.size(); ++bq) {
+          const int lo = blk_off[bq], sz = blk_off[bq + 1] - lo;
+          const std::vector<double>& M = blkL[bq];
+          for (int i2 = 0; i2 < sz; ++i2) { double v = rin[lo + i2]; for (int k = 0; k < i2; ++k) v -= M[(size_t)i2 * sz + k] * zout[lo + k]; zout[lo + i2] = v / M[(size_t)i2 * sz + i2]; }
+          for (int i2 = sz - 1; i2 >= 0; --i2) { double v = zout[lo + i2]; for (int k = i2 + 1; k < sz; ++k) v -= M[(size_t)k * sz + i2] * zout[lo + k]; zout[lo + i2] = v / M[(size_t)i2 * sz + i2]; }
+        }
+      } else if (precond == 3) {
+        // L y = r (forward), L^T z = y (backward, column-oriented)
+        for (int q = 0; q < m; ++q) {
+          double v = rin[q];
+          for (int a = A.off[q]; a < A.off[q + 1] && A.col[a] < q; ++a) v -= Lv[a] * zout[A.col[a]];
+          zout[q] = v / Ld[q];
+        }
+        for (int q = m - 1; q >= 0; --q) {
+          zout[q] /= Ld[q];
+          const double zq = zout[q];
+          for (int a = A.off[q]; a < A.off[q + 1] && A.col[a] < q; ++a) zout[A.col[a]] -= Lv[a] * zq;
+        }
+      } else if (precond == 4) {
+        // `degree` steps of the Chebyshev iteration for A z = r from z = 0 on [lmax/ratio, lmax]
+        const double lmin = lmax / ratio, theta = 0.5 * (lmax + lmin), delta = 0.5 * (lmax - lmin);
+        std::vector<double> res(rin), d(m), t(m);
+        double sigma = theta / delta, rho_c = 1.0 / sigma;
+        for (int q = 0; q < m; ++q) { d[q] = res[q] / theta; zout[q] = 0.0; }
+        for (int it = 0; it < degree; ++it) {
+          for (int q = 0; q < m; ++q) zout[q] += d[q];
+          if (it + 1 == degree) break;
+          csr_apply(A, d, t);
+          for (int q = 0; q < m; ++q) res[q] -= t[q];
+          const double rho_n = 1.0 / (2.0 * sigma - rho_c);
+          for (int q = 0; q < m; ++q) d[q] = rho_n * rho_c * d[q] + 2.0 * rho_n / delta * res[q];
+          rho_c = rho_n;
+        }
+      } else zout = rin;
+    };
+    double bb = 0.0;
+    for (int q = 0; q < m; ++q) { r[q] = b[q]; bb += b[q] * b[q]; }
+    pcg_iters = 0; pcg_relres = 0.0;
+    std::vector<double>& xs = f[17];
+    for (int i = 0; i < n; ++i) xs[i] = 0.0;
+    if (bb == 0.0) return 0;
+    apply_M(r, z);
+    p = z;
+    double rz = 0.0;
+    for (int q = 0; q < m; ++q) rz += r[q] * z[q];
+    int it; bool conv = false; double rr = bb;
+    for (it = 1; it <= maxit; ++it) {
+      csr_apply(A, p, Ap);
+      double pAp = 0.0;
+      for (int q = 0; q < m; ++q) pAp += p[q] * Ap[q];
+      const double alpha = rz / pAp;
+      rr = 0.0;
+      for (int q = 0; q < m; ++q) { x[q] += alpha * p[q]; r[q] -= alpha * Ap[q]; rr += r[q] * r[q]; }
+      if (rr <= rtol * rtol * bb) { conv = true; break; }
+      apply_M(r, z);
+      double rz2 = 0.0;
+      for (int q = 0; q < m; ++q) rz2 += r[q] * z[q];
+      const double beta = rz2 / rz;
+      for (int q = 0; q < m; ++q) p[q] = z[q] + beta * p[q];
+      rz = rz2;
+    }
+    pcg_iters = conv ? it : maxit;
+    pcg_relres = std::sqrt(rr / bb);
+    for (int q = 0; q < m; ++q) xs[A.slot[q]] = x[q];
+    return conv ? pcg_iters : -pcg_iters;
+  }
+
   // step 7b (whole) incl. 7b.5 (Q4 clamp).
   int pressure_ppe() {
     ppe_flags();
@@ -775,6 +955,9 @@ int orc_ppe_flags(void* h) { ((Orc*)h)->ppe_flags(); return 0; }
 int orc_ppe_rhs(void* h) { ((Orc*)h)->ppe_rhs(); return 0; }
 int orc_ppe_apply(void* h, const double* xin, double* yout) { ((Orc*)h)->ppe_apply(xin, yout); return 0; }
 int orc_ppe_solve(void* h, double rtol, int maxit) { return ((Orc*)h)->ppe_solve(rtol, maxit); }
+int orc_ppe_solve_pcg(void* h, double rtol, int maxit, int precond, int degree, double ratio) {
+  return ((Orc*)h)->ppe_solve_pcg(rtol, maxit, precond, degree, ratio);
+}
 int orc_morton3(int cx, int cy, int cz) { return Orc::morton3(cx, cy, cz); }
 int orc_pressure_ppe(void* h) { return ((Orc*)h)->pressure_ppe(); }
 void orc_smooth_density(void* h) { ((Orc*)h)->smooth_density(); }

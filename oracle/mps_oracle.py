@@ -51,6 +51,7 @@ def lib():
         L.orc_ppe_solve.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.orc_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_morton3.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.orc_ppe_solve_pcg.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_int, C.c_double]
         L.orc_lattice_constants.argtypes = [C.c_int, C.c_double, C.c_double, _dp]
         L.orc_lattice_constants_k.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int, _dp]
         L.orc_eos.restype = C.c_double
@@ -195,6 +196,11 @@ class Oracle:
 
     def ppe_solve(self, rtol: float, maxit: int) -> int:
         return int(self.L.orc_ppe_solve(self.h, rtol, maxit))
+
+    def ppe_solve_pcg(self, rtol: float, maxit: int, precond: int, degree: int = 0, ratio: float = 30.0) -> int:
+        """Preconditioned CG on the assembled rows (needs ppe_flags + ppe_rhs): precond 0 none, 1 Jacobi,
+        2 cell-block Jacobi, 3 IC(0), 4 Chebyshev polynomial (degree, lmax/lmin ratio).  Returns iterations."""
+        return int(self.L.orc_ppe_solve_pcg(self.h, rtol, maxit, precond, degree, ratio))
 
     def step(self, nsteps: int = 1, route: int = 0) -> int:
         return int(self.L.orc_step(self.h, nsteps, route))

@@ -25,6 +25,38 @@ __global__ void k_load(int n, const double* __restrict__ x, const double* __rest
   oid[i] = (uint32_t)i;
 }
 
+// ------------------------------------------------------- Morton key (key_mode 1) ---
+// bit k of c_x -> bit 3k, c_y -> bit 3k+1, c_z -> bit 3k+2, k = 0..9 (the "3 x 10-bit interleave").
+__device__ __forceinline__ uint32_t dilate3(uint32_t v) {
+  v &= 0x3ffu;
+  v = (v | (v << 16)) & 0x030000ffu;
+  v = (v | (v << 8)) & 0x0300f00fu;
+  v = (v | (v << 4)) & 0x030c30c3u;
+  v = (v | (v << 2)) & 0x09249249u;
+  return v;
+}
+__device__ __forceinline__ uint32_t compact3(uint32_t v) {
+  v &= 0x09249249u;
+  v = (v | (v >> 2)) & 0x030c30c3u;
+  v = (v | (v >> 4)) & 0x0300f00fu;
+  v = (v | (v >> 8)) & 0x030000ffu;
+  v = (v | (v >> 16)) & 0x3ffu;
+  return v;
+}
+__device__ __forceinline__ uint32_t cell_key(const KConst& kc, int cx, int cy, int cz) {
+  if (kc.key_mode == 1) return dilate3((uint32_t)cx) | (dilate3((uint32_t)cy) << 1) | (dilate3((uint32_t)cz) << 2);
+  return (uint32_t)(cx + kc.nx * (cy + kc.ny * cz));
+}
+__device__ __forceinline__ void key_cell(const KConst& kc, uint32_t k, int& cx, int& cy, int& cz) {
+  if (kc.key_mode == 1) {
+    cx = (int)compact3(k); cy = (int)compact3(k >> 1); cz = (int)compact3(k >> 2);
+  } else {
+    cx = (int)(k % (uint32_t)kc.nx);
+    cy = (int)((k / (uint32_t)kc.nx) % (uint32_t)kc.ny);
+    cz = (int)(k / ((uint32_t)kc.nx * (uint32_t)kc.ny));
+  }
+}
+
 // ---------------------------------------------------------------- S1: keys ---
 // c_a = floor((x_a - min_a) * inv_h); key = c_x + n_x (c_y + n_y c_z); particles
 // outside the grid (or non-finite) become GHOST with key = n_cells.  The rank
@@ -51,7 +83,7 @@ __global__ void k_keys(KConst kc, const double4* __restrict__ pos4, uint32_t* __
       if (!ghost) tp[i] = (t & ~0xffu) | MPS_GHOST;
       key = (uint32_t)kc.ncells;
     } else {
-      key = (uint32_t)((int)fx + kc.nx * ((int)fy + kc.ny * (int)fz));
+      key = cell_key(kc, (int)fx, (int)fy, (int)fz);
     }
     key_tmp[i] = key;
   }
@@ -381,6 +413,140 @@ k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
   }
 }
 
+
+// --------------------------------- S3: the row builder (lanes on candidates) ---
+// One warp builds the rows of four consecutive slots (almost always one cell): the 32 lanes load 32
+// candidates j of a cell run as coalesced records and test them against each of the four particles,
+// so one candidate load serves four rows.  A trip costs, per particle, the exact test of reading Q2
+// (8 fp64 operations + 2 compares), two ballots and the stores of the hits: the lane that holds hit
+// number k of the trip writes entry nf + k of the front part (r < re_n) or entry nb + k of the back
+// part (back_slot), so rows come out in ascending slot order with no per-hit loop.  Linear key: the
+// candidates of a (dy, dz) row of cells are one contiguous range; Morton key: one range per cell.
+// mode: ROWS_FLUID_ONLY (rows of fluid particles only), ROWS_RN_ONLY (front part only, R_n cells).
+constexpr int LEAN_TPB = 256;
+constexpr int LEAN_PPW = 4;
+
+// rare path: the trip's hits do not all fit; keep what fits, in order
+__device__ __noinline__ void row_append_overflow(uint32_t* row, int stride, uint32_t cap, uint32_t lt_mask,
+                                                 bool in_n, bool in_o, uint32_t e, uint32_t& nf, uint32_t& nb) {
+  const uint32_t m_n = __ballot_sync(0xffffffffu, in_n);
+  const uint32_t m_o = __ballot_sync(0xffffffffu, in_o);
+  const uint32_t add_n = (uint32_t)__popc(m_n), add_o = (uint32_t)__popc(m_o);
+  const uint32_t pn = (uint32_t)__popc(m_n & lt_mask), po = (uint32_t)__popc(m_o & lt_mask);
+  const uint32_t room = cap - (nf + nb);
+  if (in_n && pn < room) row[nf + pn] = e;
+  const uint32_t took_n = add_n < room ? add_n : room;
+  const uint32_t room_o = room - took_n;
+  if (in_o && po < room_o) row[back_slot(stride, nb + po)] = e;
+  nf += took_n;
+  nb += add_o < room_o ? add_o : room_o;
+}
+
+__global__ void __launch_bounds__(LEAN_TPB)
+k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
+             const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
+             uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
+             DevFlags* __restrict__ flags, int mode) {
+  const int lane = threadIdx.x & 31;
+  const int warp = (blockIdx.x * LEAN_TPB + threadIdx.x) >> 5;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  const int i0 = warp * LEAN_PPW;
+  if (i0 >= kc.n) return;
+  const bool rn_only = (mode & ROWS_RN_ONLY) != 0;
+  const int R = rn_only ? kc.R_n : kc.R_lap, S = kc.stride;
+  const double re_out2 = rn_only ? kc.re_n2 : kc.re_lap2;
+  const uint32_t cap = (uint32_t)kc.cap;
+  // the four particles: key, wanted?, position, row
+  uint32_t kk[LEAN_PPW], nf[LEAN_PPW], nb[LEAN_PPW];
+  bool want[LEAN_PPW];
+  double px[LEAN_PPW], py[LEAN_PPW], pz[LEAN_PPW];
+#pragma unroll
+  for (int t = 0; t < LEAN_PPW; ++t) {
+    const int i = i0 + t;
+    const bool in = i < kc.n;
+    kk[t] = in ? key[i] : 0xffffffffu;
+    want[t] = in && kk[t] < (uint32_t)kc.ncells &&
+              !((mode & ROWS_FLUID_ONLY) && (ent[i] & (NB_DUMMY | NB_WALL)));
+    const double4 q = pos4[in ? i : i0];
+    px[t] = q.x; py[t] = q.y; pz[t] = q.z;
+    nf[t] = 0; nb[t] = 0;
+  }
+  bool coincident = false, overflow = false;
+  // particles of one cell share the candidate scan; a warp that straddles cells takes them in turns
+  for (int t0 = 0; t0 < LEAN_PPW;) {
+    int t1 = t0 + 1;
+    while (t1 < LEAN_PPW && kk[t1] == kk[t0]) ++t1;
+    bool act[LEAN_PPW];
+    bool any = false;
+#pragma unroll
+    for (int t = 0; t < LEAN_PPW; ++t) { act[t] = t >= t0 && t < t1 && want[t]; any = any || act[t]; }
+    if (any) {
+      int cx, cy, cz;
+      key_cell(kc, kk[t0], cx, cy, cz);
+      const int x_lo = max(cx - R, 0), x_hi = min(cx + R, kc.nx - 1);
+      const int seg = kc.key_mode == 1 ? 1 : x_hi - x_lo + 1;  // cells per contiguous candidate range
+      for (int dz = -R; dz <= R; ++dz) {
+        const int z2 = cz + dz;
+        if (z2 < 0 || z2 >= kc.nz) continue;
+        for (int dy = -R; dy <= R; ++dy) {
+          const int y2 = cy + dy;
+          if (y2 < 0 || y2 >= kc.ny) continue;
+          for (int x2 = x_lo; x2 <= x_hi; x2 += seg) {
+            const uint32_t js = cell_start[cell_key(kc, x2, y2, z2)];
+            const uint32_t je = cell_start[cell_key(kc, x2 + seg - 1, y2, z2) + 1u];
+            for (uint32_t j0 = js; j0 < je; j0 += 32) {
+              const uint32_t j = j0 + (uint32_t)lane;
+              const bool valid = j < je;
+              const double4 q = pos4[valid ? j : js];
+              const uint32_t e = ent[valid ? j : js];
+#pragma unroll
+              for (int t = 0; t < LEAN_PPW; ++t) {
+                if (!act[t]) continue;  // warp-uniform
+                const double dx = __dsub_rn(q.x, px[t]), dy_ = __dsub_rn(q.y, py[t]), dz_ = __dsub_rn(q.z, pz[t]);
+                const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
+                const bool in_lap = valid && (r2 < re_out2);
+                uint32_t m_lap = __ballot_sync(0xffffffffu, in_lap);
+                // the particle itself (r2 = 0) sits in lane i - j0 of its own trip
+                const uint32_t self = (uint32_t)(i0 + t) - j0;
+                if (self < 32u) m_lap &= ~(1u << self);
+                if (m_lap == 0u) continue;
+                const bool hit = (m_lap >> lane) & 1u;
+                const bool in_n = hit && (rn_only || r2 < kc.re_n2);
+                if (hit && __double2hiint(r2) == 0) coincident = true;  // r = 0 (or denormal): Eq. 3 is infinite
+                const uint32_t m_n = __ballot_sync(0xffffffffu, in_n);
+                const uint32_t m_o = m_lap & ~m_n;
+                uint32_t* row = nbr + (size_t)(i0 + t) * (size_t)S;
+                if (nf[t] + nb[t] + (uint32_t)__popc(m_lap) <= cap) {
+                  if (in_n) row[nf[t] + (uint32_t)__popc(m_n & lt_mask)] = e;
+                  else if (hit) row[back_slot(S, nb[t] + (uint32_t)__popc(m_o & lt_mask))] = e;
+                  nf[t] += (uint32_t)__popc(m_n);
+                  nb[t] += (uint32_t)__popc(m_o);
+                } else {
+                  overflow = true;
+                  row_append_overflow(row, S, cap, lt_mask, in_n, hit && !in_n, e, nf[t], nb[t]);
+                }
+              }
+            }
+          }
+        }
+      }
+    }
+    t0 = t1;
+  }
+  int warp_max = 0;
+#pragma unroll
+  for (int t = 0; t < LEAN_PPW; ++t) {
+    if (i0 + t < kc.n && lane == 0) { cn[i0 + t] = nf[t]; co[i0 + t] = nb[t]; }
+    warp_max = max(warp_max, (int)(nf[t] + nb[t]));
+  }
+  coincident = __any_sync(0xffffffffu, coincident);
+  if (lane == 0) {
+    if (overflow) flags->overflow = 1;
+    if (coincident) flags->nonfinite = 1;
+    if (warp_max > *(volatile int*)&flags->max_row) atomicMax(&flags->max_row, warp_max);
+  }
+}
+
 // ------------------------------------ S3, cell_div = 1: one warp per cell ---
 // The 32 lanes hold up to 32 particles i of one cell and walk the candidates j of
 // the (2R+1)^2 cell runs in lock-step, so every candidate is ONE broadcast load
@@ -403,7 +569,8 @@ __global__ void __launch_bounds__(CELL_TPB, 4)
 k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
                   const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
                   uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags,
-                  int fluid_only) {
+                  int mode) {
+  const bool fluid_only = (mode & ROWS_FLUID_ONLY) != 0, rn_only = (mode & ROWS_RN_ONLY) != 0;
   __shared__ uint32_t buf[2][CELL_WARPS][8][32];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarp = blockIdx.x * CELL_WARPS + wid;
@@ -472,6 +639,7 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
             uint32_t keep = cnt == 32u ? 0xffffffffu : ((1u << cnt) - 1u);
             if (i - j0 < 32u) keep &= ~(1u << (i - j0));  // j == i
             m_lap = act ? (m_lap & keep) : 0u;
+            if (rn_only) m_lap &= m_n;  // the explicit route needs only the re_n part at r*
             // capacity: keep the first hits that fit (ascending j), flag the rest
             if (nf + nb + (uint32_t)__popc(m_lap) > cap) {
               overflow = 1;
@@ -663,8 +831,8 @@ int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const doub
   return MPS_OK;
 }
 
-int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
-  const int fo = fluid_rows_only ? 1 : 0;
+int mpsk_bin(mps_ctx* c, int rows_mode) {
+  const int fo = (rows_mode & ROWS_FLUID_ONLY) ? 1 : 0;
   const int n = (int)c->n;
   const int nc = c->kc.ncells;
   const int cur = c->cur, nxt = cur ^ 1;
@@ -683,9 +851,12 @@ int mpsk_bin(mps_ctx* c, bool fluid_rows_only) {
   c->cur = nxt;
   c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
   c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;
-  if (c->prm.cell_div == 1 && !c->rows_by_warp) {
+  if (c->rows_builder == 0) {
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (LEAN_TPB / 32) * LEAN_PPW), LEAN_TPB, c->kc, c->pos4[nxt],
+               c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode);
+  } else if (c->prm.cell_div == 1 && c->rows_builder == 2) {
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, c->kc, c->pos4[nxt],
-               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
+               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode);
   } else {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc,

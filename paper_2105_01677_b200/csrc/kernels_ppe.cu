@@ -32,6 +32,11 @@
 namespace {
 
 constexpr int PPE_ILP = 4;   // independent neighbour gathers in flight per lane
+// Streamed entries of the assembled operator in flight per lane: the loop is bound by HBM latency x
+// bandwidth, so one 1024-thread block per SM keeps 1024 x 8 x 12 B = 96 KB of matrix in flight
+// (measured at 1.44M rows: 315 ps per row per iteration with 4, 265 with 8; two blocks per SM at 32
+// registers spill and are slower, 303-330)
+constexpr int ASM_ILP = 8;
 constexpr int CG_TPB = 1024;
 constexpr int L = 8;         // lanes per row
 constexpr int GPW = 32 / L;  // row groups per warp
@@ -292,21 +297,21 @@ __device__ __forceinline__ double asm_row(const KConst& kc, const PpeArgs& a, co
   const double* vrow = a.mval + (size_t)g * (size_t)kc.stride;
   const uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
   double s0 = 0.0, s1 = 0.0;
-  for (uint32_t k = sub; k < n; k += PPE_ILP * L) {
-    double c[PPE_ILP];
-    uint32_t j[PPE_ILP];
+  for (uint32_t k = sub; k < n; k += ASM_ILP * L) {
+    double c[ASM_ILP];
+    uint32_t j[ASM_ILP];
 #pragma unroll
-    for (int u = 0; u < PPE_ILP; ++u) {
+    for (int u = 0; u < ASM_ILP; ++u) {
       const uint32_t kk = k + (uint32_t)(u * L);
       const bool in = kk < n;
       c[u] = in ? __ldcs(vrow + kk) : 0.0;
       j[u] = in ? __ldcs(crow + kk) : (uint32_t)g;
     }
-    double vj[PPE_ILP];
+    double vj[ASM_ILP];
 #pragma unroll
-    for (int u = 0; u < PPE_ILP; ++u) vj[u] = v[j[u]];
+    for (int u = 0; u < ASM_ILP; ++u) vj[u] = v[j[u]];
 #pragma unroll
-    for (int u = 0; u < PPE_ILP; u += 2) {
+    for (int u = 0; u < ASM_ILP; u += 2) {
       s0 = fma(c[u], vg - vj[u], s0);
       s1 = fma(c[u + 1], vg - vj[u + 1], s1);
     }
@@ -697,7 +702,7 @@ int mpsk_ppe_plan(mps_ctx* c) {
   else if (c->cg_tex) per_sm = tp ? cg_blocks_per_sm<true, false, true>() : cg_blocks_per_sm<false, false, true>();
   else per_sm = tp ? cg_blocks_per_sm<true, false, false>() : cg_blocks_per_sm<false, false, false>();
   if (per_sm < 1) return MPS_ERR_CUDA;
-  c->cg_grid = c->sm_count;  // one 1024-thread block per SM: fewest barrier arrivals
+  c->cg_grid = c->sm_count;  // one 1024-thread block per SM
   c->cg_lanes = L;
   const char* to = getenv("MPS_B200_CG_TIMEOUT_CYCLES");  // documented in include/mps_b200.h
   if (to) c->cg_timeout_cycles = atoll(to);

@@ -87,7 +87,7 @@ static int check_params(const mps_params* p, int64_t n) {
     return fail(nullptr, MPS_ERR_ARG, "l0, re_n, re_lap and dt must be positive");
   if (p->re_grad != p->re_n) return fail(nullptr, MPS_ERR_ARG, "re_grad must equal re_n");
   if (p->re_lap < p->re_n) return fail(nullptr, MPS_ERR_ARG, "re_lap must be >= re_n");
-  if (p->key_mode != 0) return fail(nullptr, MPS_ERR_ARG, "key_mode 0 (linear) is the only mode");
+  if (p->key_mode < 0 || p->key_mode > 1) return fail(nullptr, MPS_ERR_ARG, "key_mode must be 0 (linear) or 1 (Morton)");
   if (p->cell_div < 1 || p->cell_div > 3) return fail(nullptr, MPS_ERR_ARG, "cell_div must be 1..3");
   if (p->n_phases < 1 || p->n_phases > 2) return fail(nullptr, MPS_ERR_ARG, "n_phases must be 1 or 2");
   if (p->max_neighbours < 1 || p->max_neighbours > 4096)
@@ -169,12 +169,22 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     if (nc[a] < 1) nc[a] = 1;
     ncells *= nc[a];
   }
-  if (ncells > (int64_t)1 << 30) {
+  k.key_mode = prm->key_mode;
+  if (prm->key_mode == 1) {  // Morton keys live in [0, 8^bits), bits = smallest with 2^bits >= every n_a
+    int bits = 0;
+    while ((1 << bits) < std::max(nc[0], std::max(nc[1], nc[2]))) ++bits;
+    ncells = bits > 10 ? ((int64_t)1 << 31) : ((int64_t)1 << (3 * bits));
+  }
+  if (ncells >= (int64_t)1 << 30) {
     delete c;
-    return fail(nullptr, MPS_ERR_ARG, "grid has more than 2^30 cells");
+    return fail(nullptr, MPS_ERR_ARG, "grid has 2^30 cells or more (Morton: more than 512 cells along an axis)");
   }
   k.nx = nc[0]; k.ny = nc[1]; k.nz = nc[2]; k.ncells = (int)ncells;
-  k.R_lap = (int)ceil(prm->re_lap * k.inv_h);
+  // cells to scan on each side: ceil(re / h), guarded against re * (1/h) rounding just above an
+  // integer (h = re_lap / cell_div gives 3.0000000000000004 for some l0): the scan only needs to be a
+  // superset of the radius, and is one with the integer below
+  k.R_lap = std::max(1, (int)ceil(prm->re_lap * k.inv_h - 1e-9));
+  k.R_n = std::max(1, (int)ceil(prm->re_n * k.inv_h - 1e-9));
   k.cap = prm->max_neighbours;
   k.stride = (k.cap + 14 + 7) / 8 * 8;
   k.grad_variant = prm->grad_variant; k.clamp_negative_p = prm->clamp_negative_p;
@@ -217,10 +227,14 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     return MPS_ERR_CUDA;
   }
   {
+    // Row builder: 2 = one warp per cell (cell_div 1, large scenes), 1 = one warp per particle (few
+    // occupied cells cannot fill the GPU with one warp per cell: measured crossover between 89 k and
+    // 438 k particles), 0 = k_build_rows (any key, any cell size; the only one that walks Morton
+    // keys).  MPS_B200_ROWS=lean|warp|cell overrides the choice (tests run every builder).
     const char* rw = getenv("MPS_B200_ROWS");
-    // few occupied cells cannot fill the GPU with one warp per cell: small scenes use one
-    // warp per particle (measured crossover between scene 2, 89 k, and scene 3, 438 k)
-    c->rows_by_warp = rw ? !strcmp(rw, "warp") : (n < 200000);
+    c->rows_builder = (n >= 200000 && prm->cell_div == 1) ? 2 : 1;
+    if (rw) c->rows_builder = !strcmp(rw, "warp") ? 1 : !strcmp(rw, "cell") ? 2 : 0;
+    if (prm->key_mode == 1) c->rows_builder = 0;
   }
   {
     // texture views of the two position buffers (MPS_B200_CG_TEX=0 switches them off)
@@ -486,7 +500,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       ++c->reuse_count;
     } else {
       // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
-      mpsk_bin(c, /*fluid_rows_only=*/!ecs);
+      mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY);
     }
     if (ecs) {
       mpsk_density(c);
@@ -494,7 +508,8 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     }
     mpsk_viscosity(c);
     mpsk_predict(c);
-    if (K == 1) mpsk_bin(c);
+    // the explicit route needs only the re_n part at r* (density, p-hat, gradient)
+    if (K == 1) mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
     mpsk_density(c);
     if (hs) mpsk_dndt(c, 0);
     if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);

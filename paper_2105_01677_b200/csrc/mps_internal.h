@@ -76,6 +76,8 @@ struct KConst {  // by-value kernel parameter
   double dmin[3], inv_h;
   int nx, ny, nz, ncells;
   int R_lap;  // cells to each side for re_lap
+  int R_n;    // ... and for re_n
+  int key_mode;  // 0: key = c_x + n_x (c_y + n_y c_z); 1: Morton (3 x 10-bit interleave), ncells = 8^bits
   int cap;    // row capacity (max_neighbours)
   int stride; // row stride in entries (cap + 14 rounded up to a multiple of 8)
   int grad_variant, clamp_negative_p, rho_pair_mean, nu_pair_mean;
@@ -101,7 +103,8 @@ struct mps_ctx {
   uint32_t* tp[2] = {nullptr, nullptr};
   uint32_t* oid[2] = {nullptr, nullptr};
   uint32_t* ent = nullptr;         // per slot: own index | NB_* flags (what a neighbour row stores)
-  bool rows_by_warp = false;       // warp-per-particle row builder (small scenes; MPS_B200_ROWS=warp|cell overrides)
+  int rows_builder = 0;            // 0: k_build_rows (lanes on candidates, four particles per warp); 1 / 2: the
+                                   // round-1 builders, kept for comparison (MPS_B200_ROWS=lean|warp|cell)
   int cur = 0;
   // bin scratch
   uint32_t* key = nullptr;         // per slot (after bin: key of the slot)
@@ -193,9 +196,12 @@ void mps_timer_drain(mps_ctx* c);
 static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // ---- stage launchers (defined in the .cu files) -----------------------------------
-// keys, counting sort, reorder, neighbour rows (fluid_rows_only: rows of FLUID particles only,
-// all a viscosity sweep needs; used for the first bin of mps_step)
-int mpsk_bin(mps_ctx* c, bool fluid_rows_only = false);
+// keys, counting sort, reorder, neighbour rows
+// rows_mode bit 0: rows of FLUID particles only (all a viscosity sweep needs); bit 1: the re_n part only
+// (all the explicit route needs at r*)
+#define ROWS_FLUID_ONLY 1
+#define ROWS_RN_ONLY 2
+int mpsk_bin(mps_ctx* c, int rows_mode = 0);
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
                          uint32_t* tmp);
 int mpsk_density(mps_ctx* c);

@@ -51,16 +51,17 @@ def inject(g, o, names):
 
 
 # ---------------------------------------------------------------- S1, S2: bin ---
+@pytest.mark.parametrize("key_mode", [0, 1])   # linear x-fastest key / Morton key
 @pytest.mark.parametrize("cell_div", [1, 2, 3])
 @pytest.mark.parametrize("scene", ["tank", "config1"])
-def test_bin_is_bit_exact(B, O, scene, cell_div):
+def test_bin_is_bit_exact(B, O, scene, cell_div, key_mode):
     s = scenes.small_tank(shuffle=True) if scene == "tank" else scenes.make_scene(1, shuffle=True)
     s.x[5] = 10.0            # outside the domain -> GHOST
     s.y[17] = float("nan")   # non-finite -> GHOST + error flag
     s.z[40] = -1.0
-    o = O.Oracle(s, cell_div=cell_div)
+    o = O.Oracle(s, cell_div=cell_div, key_mode=key_mode)
     key, perm, cs = o.bin()
-    g = B.Mps(s, cell_div=cell_div)
+    g = B.Mps(s, cell_div=cell_div, key_mode=key_mode)
     g.bin()
     assert g.grid() == o.grid()
     assert np.array_equal(g.get("key"), key)
@@ -92,21 +93,22 @@ def test_bin_after_motion_matches_oracle(B, O):
 
 
 # ----------------------------------------------------------- S3: neighbour sets ---
-@pytest.mark.parametrize("rows", ["warp", "cell"])
-@pytest.mark.parametrize("cell_div", [1, 2])
+@pytest.mark.parametrize("rows", ["lean", "morton", "warp", "cell"])
+@pytest.mark.parametrize("cell_div", [1, 2, 3])
 @pytest.mark.parametrize("scene", ["tank_moved", "config1", "cloud"])
 def test_neighbour_sets_are_bit_exact(B, O, scene, cell_div, rows, monkeypatch):
-    # both row builders (warp per particle / warp per cell; the library picks by size)
-    monkeypatch.setenv("MPS_B200_ROWS", rows)
+    # the row builder (lanes on candidates) with either key, and the two round-1 builders
+    monkeypatch.setenv("MPS_B200_ROWS", "lean" if rows == "morton" else rows)
+    km = 1 if rows == "morton" else 0
     if scene == "cloud":
         s = scenes.random_cloud(3000, 10 * 0.031, seed=3)
         s.params.update(l0=0.01, re_n=0.021, re_lap=0.031)
         o = O.Oracle(s, cell_div=cell_div)
-        g = B.Mps(s, cell_div=cell_div)
+        g = B.Mps(s, cell_div=cell_div, key_mode=km)
     else:
         s = scenes.small_tank(shuffle=True) if scene == "tank_moved" else scenes.make_scene(1, shuffle=True)
         o = moved_state(O, s, 2, cell_div=cell_div)
-        g = B.Mps(s, cell_div=cell_div)
+        g = B.Mps(s, cell_div=cell_div, key_mode=km)
         inject(g, o, ("x", "y", "z"))
     g.bin()
     for rid, re in ((B.RADIUS_N, s.params["re_n"]), (B.RADIUS_LAP, s.params["re_lap"])):
@@ -330,11 +332,11 @@ def _trajectory(B, O, s, nsteps, route, **over):
     return d.max() / L, d.max() / s.params["l0"], moved / s.params["l0"], g, o
 
 
-@pytest.mark.parametrize("rows", ["warp", "cell"])
+@pytest.mark.parametrize("rows", ["lean", "morton", "warp", "cell"])
 def test_trajectory_config1_explicit_20_steps(B, O, rows, monkeypatch):
-    monkeypatch.setenv("MPS_B200_ROWS", rows)
+    monkeypatch.setenv("MPS_B200_ROWS", "lean" if rows == "morton" else rows)
     s = scenes.make_scene(1)
-    eL, el0, moved, g, o = _trajectory(B, O, s, 20, 0)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, 0, key_mode=1 if rows == "morton" else 0)
     print(f"config 1, 20 explicit steps: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}; max displacement {moved:.2f} l0")
     assert moved > 0.05
     assert eL <= 1e-7
@@ -361,11 +363,44 @@ def test_two_phase_smagorinsky_ppe_steps(B, O):
     assert eL <= 1e-7
 
 
-def test_config2_ppe_two_steps(B, O):
+# ---- BASELINE.json configs at full size and (for config 2) full length: both sides start from the
+# same seeded scene and step on their own; bar: max |r_gpu - r_oracle| <= 1e-7 x the longest side.
+def test_config2_ppe_full_20_steps(B, O):
     s = scenes.make_scene(2)
-    eL, el0, moved, g, o = _trajectory(B, O, s, 2, 1)
-    print(f"config 2 (N={s.n}), 2 PPE steps: max |dr|/L = {eL:.2e}; cg iters {g.stats()['cg_iters']} vs {o.stats()['cg_iters']}")
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, 1)
+    print(f"config 2 (N={s.n}), 20 PPE steps: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}, moved {moved:.3f} l0; "
+          f"cg iters last step {g.stats()['cg_iters']} vs {o.stats()['cg_iters']}")
+    assert eL <= 1e-7 and moved > 0.01
+    assert abs(g.stats()["cg_iters"] - o.stats()["cg_iters"]) <= 3
+
+
+@pytest.mark.parametrize("route,variant,nsteps,op,key_mode", [
+    (0, 2, 10, 1, 0), (0, 1, 10, 1, 1),          # explicit route, (p_i + p_j) and Eq. 14 as printed
+    (1, 2, 10, 1, 0), (1, 1, 4, 0, 1),           # PPE route: assembled operator / matrix-free + Morton key
+])
+def test_config3_trajectories(B, O, route, variant, nsteps, op, key_mode):
+    s = scenes.make_scene(3)
+    eL, el0, moved, g, o = _trajectory(B, O, s, nsteps, route, grad_variant=variant, ppe_operator=op,
+                                       key_mode=key_mode)
+    print(f"config 3 (N={s.n}), {nsteps} steps, route {route}, variant {variant}, operator {op}, key {key_mode}: "
+          f"max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}, moved {moved:.3f} l0")
+    assert eL <= 1e-7 and moved > 0.005
+
+
+def test_config4_two_phase_ppe_5_steps(B, O):
+    s = scenes.make_scene(4)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 5, 1)
+    print(f"config 4 (N={s.n}), 5 PPE steps (two-phase, Cs 0.12): max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}, "
+          f"moved {moved:.4f} l0; cg iters {g.stats()['cg_iters']} vs {o.stats()['cg_iters']}")
     assert eL <= 1e-7
+    assert relerr(g.get("nut"), o.get("nut"), 1e-30) <= 1e-6
+
+
+def test_config5_250k_explicit_10_steps(B, O):
+    s = scenes.make_scene(5, sweep_index=1)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 10, 0)
+    print(f"config 5[1] (N={s.n}), 10 explicit steps: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}, moved {moved:.3f} l0")
+    assert eL <= 1e-7 and moved > 0.005
 
 
 def test_step_host_equals_ctx_path(B, O):
@@ -552,7 +587,7 @@ def test_trajectory_small_tank_hs_hl_ecs(B, O, src, lap):
 
 
 # ----------------------------------------------------- NEXT-3 (part): 2D mode ---
-@pytest.mark.parametrize("rows", ["warp", "cell"])
+@pytest.mark.parametrize("rows", ["lean", "warp", "cell"])
 def test_2d_bin_neighbours_and_fields(B, O, rows, monkeypatch):
     monkeypatch.setenv("MPS_B200_ROWS", rows)
     s = scenes.dam_break_2d(0.01, (60, 40), (20, 30), seed=9, shuffle=True)
@@ -609,7 +644,7 @@ def test_eq4_kernel_fields_and_trajectory(B, O):
 
 # -------------------------------------- NEXT-3 (part): neighbour-list reuse ---
 @pytest.mark.parametrize("route", [0, 1])
-@pytest.mark.parametrize("rows", ["warp", "cell"])
+@pytest.mark.parametrize("rows", ["lean", "warp", "cell"])
 def test_list_reuse_every_four_steps(B, O, route, rows, monkeypatch):
     monkeypatch.setenv("MPS_B200_ROWS", rows)
     s = scenes.small_tank(shuffle=True)
@@ -687,3 +722,27 @@ def test_max_size_8m_sampled(B, O):
         assert abs(n[i] - (rn / np.sqrt(r2[mn]) - 1.0).sum()) <= 1e-10 * 14.4
     g.step(1, 0)                     # one whole explicit step at this size
     assert g.stats()["device_error"] == 0 and np.isfinite(g.get("p")).all()
+
+
+# --------------- NEXT-3: the paper's water-drop test (Table 1) on the GPU ---
+def test_water_drop_trajectory_and_invariant(B, O):
+    s = scenes.water_drop()
+    over = dict(c0=2000.0)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 100, 0, **over)
+    print(f"water drop, 100 explicit steps (2D, Eq. 4, re = 3 l0): max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
+    assert eL <= 1e-7 and moved > 1.0
+    # the whole run on the GPU: ab constant while b doubles (the paper's criterion; the oracle pin
+    # test_water_drop_ab_invariant_and_doubling_time states theory and measured figures)
+    ax = lambda x, y: (2.0 * np.sqrt((x * x).mean()), 2.0 * np.sqrt((y * y).mean()))
+    a0, b0 = ax(s.x, s.y)
+    k, worst = 100, 0.0
+    while True:
+        g.step(10, 0)
+        k += 10
+        a, b = ax(g.get("x"), g.get("y"))
+        worst = max(worst, abs(a * b - a0 * b0) / (a0 * b0))
+        if b >= 2.0 * b0 or k >= 2000:
+            break
+    print(f"  GPU: b doubled after {k} steps, worst ab error {100 * worst:.2f} %")
+    assert abs(k * 1e-5 - 8.005e-3) <= 0.06 * 8.005e-3 and worst <= 0.035
+    assert g.stats()["n_ghost"] == 0

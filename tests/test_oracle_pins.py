@@ -1025,3 +1025,78 @@ def test_morton_key_table_and_sort_invariants():
     lin2.step(3, 1); mor2.step(3, 1)
     for k in ("x", "y", "z"):               # only the order of additions inside a sum differs
         assert np.abs(lin2.get(k) - mor2.get(k)).max() <= 1e-12 * 0.12
+
+
+# ---- NEXT-4: preconditioned CG (P:176 ICCG) against the dense solve and against plain CG ----
+@pytest.mark.parametrize("precond,degree", [(0, 0), (1, 0), (2, 0), (3, 0), (4, 3)])
+def test_pcg_equals_dense_solve(precond, degree):
+    # 0 none, 1 Jacobi, 2 block Jacobi on the grid cells, 3 incomplete Cholesky IC(0) -- the paper's
+    # ICCG -- 4 Chebyshev polynomial.  Each must reach THE solution of A x = b (textbook LAPACK solve of
+    # the matrix assembled in numpy from Listing 2's rule), whatever M is.
+    s = scenes.small_tank(shuffle=True)
+    o = O.Oracle(s)
+    o.step(2, 0)
+    o.viscosity(); o.predict(); o.density(); o.ppe_flags(); o.ppe_rhs()
+    A, rows = _dense_A(o, s)
+    b = o.get("b")[rows]
+    xd = np.linalg.solve(A, b)
+    it = o.ppe_solve_pcg(1e-12, 5000, precond, degree, 30.0)
+    assert it > 0
+    xp = o.get("xcg")
+    assert (xp[o.get("bc") != 0] == 0).all()
+    assert np.linalg.norm(xp[rows] - xd) <= 1e-9 * np.linalg.norm(xd)
+    # at the default tolerance: the stated residual bound, and fewer iterations than plain CG for IC(0)
+    it8 = o.ppe_solve_pcg(1e-8, 5000, precond, degree, 30.0)
+    x8 = o.get("xcg")[rows]
+    assert np.linalg.norm(b - A @ x8) <= 1.5e-8 * np.linalg.norm(b)
+    it_cg = o.ppe_solve(1e-8, 5000)
+    if precond == 0:
+        assert it8 == it_cg                # the CSR path and the matrix-free path are the same iteration
+    if precond == 3:
+        assert it8 <= 0.5 * it_cg          # what the paper's preconditioner buys (measured: 21 -> 7)
+    if precond in (1, 2):
+        assert it8 <= it_cg
+
+
+# ---- NEXT-3: the paper's water-drop test (section 5.1, Table 1) ----
+def _drop_axes(x, y):
+    # semi-axes from second moments: a uniform ellipse has <x^2> = a^2 / 4 (robust against the few
+    # stray surface particles that the maximum extent follows)
+    return 2.0 * math.sqrt(float((x * x).mean())), 2.0 * math.sqrt(float((y * y).mean()))
+
+
+def test_water_drop_ab_invariant_and_doubling_time():
+    # An incompressible drop with u = (-A x, A y) stays an ellipse with a b = R^2 (the paper's
+    # criterion, after Monaghan [47]), and Euler's equations with p = 0 on the boundary give
+    # A' = A^2 (a^2 - b^2)/(a^2 + b^2), so with s = b/R: A = A0 s sqrt(2/(1 + s^4)) and b doubles at
+    # t2 = (1/(A0 sqrt 2)) int_1^2 sqrt(1 + s^4)/s^2 ds = 8.005e-3 s for A0 = 100 1/s.  The paper reports
+    # ab constant within 0.26 % with its (unstated) default configuration; with this build's readings
+    # (no surface or collision treatment, Q11; explicit route with Eq. 4 and c0 = 2000 m/s, Mach 0.09)
+    # the measured figures are ab within 2.7 % and t2 = 8.3e-3 s.
+    s = scenes.water_drop()
+    assert s.n == 1257
+    sN = np.linspace(1.0, 2.0, 20001)
+    f = np.sqrt(1.0 + sN ** 4) / sN ** 2
+    t2 = float(((f[1:] + f[:-1]) * 0.5 * np.diff(sN)).sum()) / (100.0 * math.sqrt(2.0))
+    assert abs(t2 - 8.005e-3) < 2e-6
+    o = O.Oracle(s, c0=2000.0)
+    a0, b0 = _drop_axes(s.x, s.y)
+    assert a0 * b0 == pytest.approx(0.875 ** 2, rel=5e-3)     # Table 1: ab(0) = 0.766
+    k, worst = 0, 0.0
+    while True:
+        o.step(10, 0)
+        k += 10
+        a, b = _drop_axes(o.get("x"), o.get("y"))
+        worst = max(worst, abs(a * b - a0 * b0) / (a0 * b0))
+        if b >= 2.0 * b0 or k >= 2000:
+            break
+    t_double = k * s.params["dt"]
+    print(f"water drop: b doubled after {k} steps (t = {t_double:.2e} s, theory {t2:.2e}); "
+          f"ab error at the end {100 * abs(a * b - a0 * b0) / (a0 * b0):.2f} %, worst {100 * worst:.2f} % (paper: 0.26 %)")
+    assert o.stats()["n_ghost"] == 0
+    assert abs(t_double - t2) <= 0.06 * t2                 # measured 8.3e-3 vs 8.005e-3
+    assert worst <= 0.035                                   # measured 2.7 %
+    # the field stays close to the linear one: v / y = A(t) with A(t2) = A0 * 2 sqrt(2/17)
+    y, v = o.get("y"), o.get("v")
+    A_fit = float((y * v).sum() / (y * y).sum())
+    assert A_fit == pytest.approx(100.0 * 2.0 * math.sqrt(2.0 / 17.0), rel=0.08)
