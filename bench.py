@@ -7,7 +7,9 @@
 One "step" is one pass of the whole hot path (SURVEY.md 8(a) rows S1-S11:
 bin, viscosity, predictor, bin, density, pressure, gradient, corrector) over
 all particles of one seeded synthetic dam-break scene.  Default workload:
-BASELINE.json configs[1] (scene 2: 89,228 particles, semi-implicit PPE route).
+BASELINE.json configs[4] at its 2M point (scene 5[3]: 1,994,776 particles), semi-implicit
+PPE route; the explicit route of the same scene is measured too and reported under
+"routes".  --config 2 gives BASELINE configs[1] (89,228 particles).
 
 Prints ONE JSON line (rank 0).  Keys beyond the base contract:
   roofline      dominant kernel: algorithmic bytes per launch / CUDA-event time
@@ -45,9 +47,10 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="scene 1..5 (SURVEY.md 8(d)); default 2 = BASELINE configs[1]; 6 = paper-shaped 2D dam break")
-    ap.add_argument("--sweep-index", type=int, default=0, help="size index 0..4 of scene 5")
-    ap.add_argument("--route", default=None, choices=[None, "explicit", "ppe"])
+    ap.add_argument("--config", type=int, default=5, help="scene 1..5 (SURVEY.md 8(d)); default 5 = BASELINE configs[4], the throughput sweep; 6 = paper-shaped 2D dam break")
+    ap.add_argument("--sweep-index", type=int, default=3, help="size index 0..4 of scene 5 (default 3: N = 1,994,776)")
+    ap.add_argument("--route", default=None, choices=[None, "explicit", "ppe"], help="default: ppe for scene 5, else the scene's own")
+    ap.add_argument("--no-other-route", action="store_true", help="do not measure the other pressure route of the scene")
     ap.add_argument("--rebin-every", type=int, default=1,
                     help="K > 1: the paper's neighbour-list reuse (PAPER.md:433), NOT the BASELINE workload")
     ap.add_argument("--ppe-operator", type=int, default=None, choices=[0, 1],
@@ -81,7 +84,7 @@ def make_scene(args, rank=0):
     from paper_2105_01677_b200 import scenes
     seed = scenes.BASE_SEED + args.config + (args.sweep_index if args.config >= 5 else 0) + 1000 * rank
     s = scenes.make_scene(args.config, seed=seed, sweep_index=args.sweep_index)
-    route = s.route if args.route is None else {"explicit": 0, "ppe": 1}[args.route]
+    route = (1 if args.config == 5 else s.route) if args.route is None else {"explicit": 0, "ppe": 1}[args.route]
     if getattr(args, "ppe_operator", None) is not None:
         s.params["ppe_operator"] = int(args.ppe_operator)
     if getattr(args, "warm_start", False):
@@ -245,6 +248,190 @@ def cpu_baseline(scene, route, budget_s=12.0, max_steps=5):
             "host_cores_present": os.cpu_count()}
 
 
+def neighbour_statistics(np, B, g, scene, route):
+    """Mean neighbour counts, PPE rows and the candidate tests of one row build (for the byte / ALU models)."""
+    bc = g.get("bc") if route == 1 else None
+    typ = g.get("type")
+    g.bin()
+    cl = g.neighbour_counts(B.RADIUS_LAP).astype(np.float64)
+    cn = g.neighbour_counts(B.RADIUS_N).astype(np.float64)
+    rows = int((bc == 0).sum()) if bc is not None else 0
+    # candidates the row builder tests: the particles of the (2R+1)^3 cells around each particle's cell
+    p = scene.params
+    h = max(p["re_n"], p["re_lap"]) / p["cell_div"]
+    nx_, ny_, nz_, _ = g.grid()
+    R_ = int(np.ceil(p["re_lap"] / h - 1e-9))
+    live = typ != 3
+    cx = np.floor((g.get("x")[live] - p["domain_min"][0]) / h).astype(np.int64).clip(0, nx_ - 1)
+    cy = np.floor((g.get("y")[live] - p["domain_min"][1]) / h).astype(np.int64).clip(0, ny_ - 1)
+    cz = np.floor((g.get("z")[live] - p["domain_min"][2]) / h).astype(np.int64).clip(0, nz_ - 1)
+    lin = cx + nx_ * (cy + ny_ * cz)
+    cnt = np.bincount(lin, minlength=nx_ * ny_ * nz_).reshape(nz_, ny_, nx_)
+    fl_cnt = np.bincount(lin[typ[live] == 0], minlength=nx_ * ny_ * nz_).reshape(nz_, ny_, nx_)
+    pad = np.pad(cnt, R_)
+    cand = np.zeros_like(cnt)
+    for dz in range(2 * R_ + 1):
+        for dy in range(2 * R_ + 1):
+            for dx in range(2 * R_ + 1):
+                cand += pad[dz:dz + nz_, dy:dy + ny_, dx:dx + nx_]
+    return {"kl": float(cl.mean()), "kn": float(cn.mean()), "rows": rows,
+            "klr": float(cl[bc == 0].mean()) if rows else 0.0,
+            "tests_all": float((cnt * cand).sum()), "tests_fluid": float((fl_cnt * cand).sum())}
+
+
+def load_traffic():
+    """dram bytes per use of the dominant kernels, written from the committed ncu captures by
+    `python -m paper_2105_01677_b200.ncu_summary` (profiles/r02_traffic.json)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K, W, sample_clocks):
+    """One route of one scene: the device-resident timed steps, then an instrumented replay of the
+    same steps with per-kernel CUDA events, and the roofline of the dominant kernel."""
+    g = B.Mps(scene, device=str(dev))
+    clocks = None
+    if sample_clocks:
+        try:
+            gpu_id = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+        except Exception:
+            gpu_id = str(dev.index)
+        # the sampler runs over warm-up and timed steps: the timed region alone can be shorter than
+        # nvidia-smi's start-up, and both are the same load
+        sampler = ClockSampler(gpu_id)
+        sampler.start()
+    g.step(max(W, 3), route)
+    if sample_clocks:
+        t_end = time.perf_counter() + 0.5
+        while time.perf_counter() < t_end and len(sampler.rows) < 3:
+            g.step(1, route)           # untimed: keep the GPU under load until the sampler reports
+    l0 = g.launch_count()
+    st0 = g.stats()
+    ms_rank = timed_steps(torch, world, g, route, K, flush, stream)
+    launches = g.launch_count() - l0
+    if sample_clocks:
+        clocks = sampler.stop()
+    ms_total = barrier_and_max(world, ms_rank, dev)
+    stats = g.stats()
+    cg_iters = stats["cg_iters_total"] - st0["cg_iters_total"]
+    cg_loop_ms = stats["cg_loop_ms_total"] - st0["cg_loop_ms_total"]  # device-timed (%globaltimer) CG loops
+    n_all = all_sum(world, scene.n, dev)
+    value = n_all * K / (ms_total * 1e-3)
+    ns = neighbour_statistics(np, B, g, scene, route)
+    g.close()
+    N, rows, kn, kl, klr = scene.n, ns["rows"], ns["kn"], ns["kl"], ns["klr"]
+    asm = int(scene.params.get("ppe_operator", 1)) == 1
+    out = {"value": value, "ms_per_step": ms_total / K, "gpu_launches": int(launches), "clocks": clocks,
+           "fluid_particle_steps_per_sec": value * scene.n_fluid / scene.n,
+           "units": {"N": N, "ppe_rows": rows, "mean_k_re_n": kn, "mean_k_re_lap": kl, "mean_k_re_lap_rows": klr}}
+    cg = None
+    if route == 1:
+        nnz = int(stats["cg_nnz"]) if asm else None
+        # bytes one CG iteration must move: the operator application plus the vector updates (the
+        # device-timed loop covers both).  Assembled: 12 B per stored pair + per row count, diagonal term,
+        # r_g and w_g; matrix-free: 4 B per listed pair + position, r_i, bc, w_i (SURVEY.md 8(d))
+        per_iter = (12.0 * nnz + rows * (4 + 8 + 8 + 8) if asm else rows * (4.0 * klr + 24 + 8 + 1 + 8)) + rows * 72.0
+        cg = {"operator": "assembled once per solve (ppe_operator 1)" if asm else "matrix-free (ppe_operator 0)",
+              "rows": rows, "nnz": nnz, "iters_per_step": cg_iters / K, "iters_per_sec": cg_iters / (ms_total * 1e-3),
+              "loop_ms_per_step": cg_loop_ms / K, "setup_ms_last_solve": stats["cg_setup_ms"],
+              "us_per_iteration": 1e3 * cg_loop_ms / max(cg_iters, 1),
+              "ps_per_row_per_iteration": 1e9 * cg_loop_ms / max(cg_iters, 1) / max(rows, 1),
+              "algorithmic_bytes_per_iteration": per_iter,
+              "algorithmic_gbs": per_iter * cg_iters / (cg_loop_ms * 1e-3) / 1e9 if cg_loop_ms > 0 else None,
+              "timing": "%globaltimer of block 0 inside k_ppe_cg around the iteration loop"}
+        out["cg"] = cg
+    if args.no_replay:
+        out.update({"kernels": {}, "roofline": None})
+        return out
+
+    # ---- instrumented replay of the same steps: per-kernel CUDA-event times ------------------
+    g = B.Mps(scene, device=str(dev))
+    g.step(W, route)
+    g.timers_enable((1 << len(B.TIMERS)) - 1)
+    ms_replay = timed_steps(torch, 1, g, route, K, flush, stream)
+    tm = g.timers_read()
+    g.timers_enable(0)
+    g.close()
+    peak, peak_src = peaks()
+    n_bins = tm["bin_list"][1]          # one row-builder launch per bin (2 per step; fewer with list reuse)
+    kernels = {}
+    for cat, (ms, ln) in tm.items():
+        if ln == 0:
+            continue
+        ab = algorithmic_bytes(cat, N, rows, kn, kl, klr)
+        # categories with several kernels per use: bytes are per use, not per launch
+        uses = {"bin_sort": n_bins, "bin_list": n_bins, "viscosity": K, "gradient": K, "ppe_setup": K}.get(cat, ln)
+        kernels[cat] = {"ms_per_step": ms / K, "launches_per_step": ln / K, "us_per_launch": 1e3 * ms / ln,
+                        "algorithmic_gbs": (ab * uses / (ms * 1e-3) / 1e9) if (ab and ms > 0 and cat != "cg_spmv") else None}
+    top = max(kernels, key=lambda c: kernels[c]["ms_per_step"])
+    ms_top, ln_top = tm[top]
+    tag = f"scene{args.config}" + (f"[{args.sweep_index}]" if args.config >= 5 else "")
+    traffic = load_traffic().get(f"{tag}:{ROUTE_NAME[route]}:{top}" + (":asm" if (top == "cg_spmv" and asm) else ""))
+    roof = {"kernel": top, "share_of_step": (ms_top / K) / (ms_replay / K), "ms_per_step_instrumented": ms_replay / K,
+            "peak_source": peak_src}
+    if top == "cg_spmv" and cg:
+        # one launch of k_ppe_cg is a whole solve; the unit of the roofline is one CG iteration
+        # (operator application + vector updates), timed on the device inside the kernel
+        ach = cg["algorithmic_gbs"]
+        tr = traffic["dram_bytes_per_use"] if traffic else None
+        l2_resident = tr is not None and tr < 0.5 * cg["algorithmic_bytes_per_iteration"]
+        roof.update({"per": "CG iteration (operator application + vector updates) inside k_ppe_cg",
+                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                     "traffic": tr, "traffic_source": traffic.get("source") if traffic else None,
+                     "algorithmic_bytes_per_use": cg["algorithmic_bytes_per_iteration"], "uses": cg_iters,
+                     "us_per_use": cg["us_per_iteration"], "launches": ln_top,
+                     "bound": ("L2-resident: the iteration's data stay in the 126 MB L2, the HBM fraction is not a "
+                               "roofline here; grid barriers and L2 latency bind") if l2_resident else
+                              ("hbm" if asm else "l1-gather (one 32-byte record gather per pair; no unit saturated "
+                                                 "in ncu, HBM fraction reported against the measured copy peak)")})
+    elif top == "bin_list":
+        # the row builder is bound by the fp64 pipe / instruction issue, not by HBM: report it against
+        # the fp64 pipe (DESIGN.md section 7: 148 SMs x 64 lanes x 1.965 GHz; 10 fp64-pipe instructions
+        # per candidate: 3 sub, 3 mul, 2 add, 2 compares)
+        ab = algorithmic_bytes(top, N, rows, kn, kl, klr)
+        reuse = int(scene.params.get("rebin_every", 1))
+        tests = n_bins * ns["tests_all"] if reuse > 1 else K * (ns["tests_all"] + ns["tests_fluid"])
+        a_alu = tests * 10.0 / (ms_top * 1e-3) / 1e12
+        hbm = ab * n_bins / (ms_top * 1e-3) / 1e9
+        roof.update({"per": "row build (one per bin)", "bound": "alu", "achieved": a_alu, "peak": 18.61,
+                     "unit": "T fp64-pipe instructions/s", "frac": a_alu / 18.61,
+                     "peak_source": "148 SMs x 64 fp64 lanes x 1.965 GHz (measured 18.5 T DADD/DMUL per s)",
+                     "hbm_achieved_gbs": hbm, "hbm_frac": hbm / peak, "candidate_tests_per_step": tests / K,
+                     "traffic": traffic["dram_bytes_per_use"] if traffic else None, "uses": n_bins,
+                     "us_per_use": 1e3 * ms_top / max(n_bins, 1), "launches": ln_top})
+    else:
+        ab = algorithmic_bytes(top, N, rows, kn, kl, klr)
+        uses = {"viscosity": K, "gradient": K, "ppe_setup": K}.get(top, ln_top)
+        ach = ab * uses / (ms_top * 1e-3) / 1e9
+        roof.update({"per": "use", "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                     "traffic": traffic["dram_bytes_per_use"] if traffic else None, "uses": uses,
+                     "us_per_use": 1e3 * ms_top / max(uses, 1), "launches": ln_top})
+    out.update({"kernels": kernels, "roofline": roof})
+    return out
+
+
+def sample_scene(args, full):
+    """A bounded sample of the workload for the CPU oracle (it needs minutes per step at 1M+ particles):
+    the same shape, parameters and route at a size one oracle step finishes in seconds."""
+    from paper_2105_01677_b200 import scenes
+    if full.n <= 120000:
+        return full, "the whole scene"
+    if args.config == 5:
+        s = scenes.make_scene(5, seed=scenes.BASE_SEED + 5, sweep_index=0)
+        what = f"scene5[0]: the same dam-break shape, parameters and route at N={s.n} (fluid {s.n_fluid}) instead of N={full.n}"
+    else:
+        l0 = 2.0 * full.params["l0"]
+        geo = {3: ((100, 25, 50), (50, 25, 25))}.get(args.config, ((40, 20, 30), (20, 20, 10)))
+        s = scenes.dam_break(l0, geo[0], geo[1], scenes.BASE_SEED + args.config, "reference_sample")
+        what = f"same tank and parameters at 2x spacing: N={s.n} (fluid {s.n_fluid}) instead of N={full.n}"
+    for k in ("grad_variant", "n_phases", "rho", "nu", "cs", "rho_pair_mean", "nu_pair_mean"):
+        s.params[k] = full.params[k]
+    return s, what
+
+
 def run_b200(args):
     import numpy as np
     import torch
@@ -264,125 +451,17 @@ def run_b200(args):
     K, W = args.steps, max(args.warmup, 3)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
-    try:
-        gpu_id = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
-    except Exception:
-        gpu_id = str(dev.index)
 
-    # ---- device-resident arm: the headline value -------------------------------------
-    g = B.Mps(scene, device=str(dev))
-    # the sampler runs over warm-up and timed steps: the timed region alone (tens of ms) is
-    # shorter than nvidia-smi's start-up, and both are the same load
-    sampler = ClockSampler(gpu_id)
-    sampler.start()
-    g.step(max(W, 3), route)
-    t_end = time.perf_counter() + 0.5
-    while time.perf_counter() < t_end and len(sampler.rows) < 3:
-        g.step(1, route)               # untimed: keep the GPU under load until the sampler reports
-    l0 = g.launch_count()
-    st0 = g.stats()
-    cg_before, loop_before = st0["cg_iters_total"], st0["cg_loop_ms_total"]
-    ms_rank = timed_steps(torch, world, g, route, K, flush, stream)
-    launches = g.launch_count() - l0
-    clocks = sampler.stop()
-    ms_total = barrier_and_max(world, ms_rank, dev)
-    stats = g.stats()
-    cg_timed_main = stats["cg_iters_total"] - cg_before
-    cg_loop_ms = stats["cg_loop_ms_total"] - loop_before   # device-timed (%globaltimer) CG loops of the timed steps
+    main = measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K, W, sample_clocks=True)
     n_all = all_sum(world, scene.n, dev)
-    value = n_all * K / (ms_total * 1e-3)
 
-    # neighbour statistics of the last state, for the algorithmic-byte model
-    bc = g.get("bc") if route == 1 else None
-    g.bin()
-    cl = g.neighbour_counts(B.RADIUS_LAP).astype(np.float64)
-    cn = g.neighbour_counts(B.RADIUS_N).astype(np.float64)
-    kl, kn = float(cl.mean()), float(cn.mean())
-    rows = int((bc == 0).sum()) if bc is not None else 0
-    klr = float(cl[bc == 0].mean()) if rows else 0.0
-    # candidates the row builder must test (27 cells around every particle), for its ALU roofline
-    nx_, ny_, nz_, ncell = g.grid()
-    cs = g.cell_start().astype(np.int64)
-    cnt = np.diff(cs[:ncell + 1]).reshape(nz_, ny_, nx_)
-    R_ = int(np.ceil(scene.params["re_lap"] / (max(scene.params["re_n"], scene.params["re_lap"]) / scene.params["cell_div"]) - 1e-12))
-    pad = np.pad(cnt, R_)
-    cand = np.zeros_like(cnt)
-    for dz in range(2 * R_ + 1):
-        for dy in range(2 * R_ + 1):
-            for dx in range(2 * R_ + 1):
-                cand += pad[dz:dz + nz_, dy:dy + ny_, dx:dx + nx_]
-    key_now = g.get("key"); typ_now = g.get("type")
-    live = key_now < ncell
-    fl_cnt = np.bincount(key_now[live & (typ_now == 0)], minlength=ncell).reshape(nz_, ny_, nx_)
-    tests_all = float((cnt * cand).sum())       # a bin that builds every row
-    tests_fluid = float((fl_cnt * cand).sum())  # the first bin of a step (fluid rows only)
-    g.close()
-
-    # ---- instrumented replay of the same steps: per-kernel CUDA-event times ------------
-    kernels, roof = {}, None
-    if not args.no_replay:
-        g = B.Mps(scene, device=str(dev))
-        g.step(W, route)
-        cg_before_replay = g.stats()["cg_iters_total"]
-        g.timers_enable((1 << len(B.TIMERS)) - 1)
-        ms_replay = timed_steps(torch, 1, g, route, K, flush, stream)
-        tm = g.timers_read()
-        g.timers_enable(0)
-        st_r = g.stats()
-        g.close()
-        # full operator applications / vector updates actually performed (launches issued after
-        # convergence return at once; their time stays in the category's total)
-        cg_iters_timed = st_r["cg_iters_total"] - cg_before_replay
-        cg_uses = {"cg_spmv": cg_iters_timed + K, "cg_update": cg_iters_timed}
-        peak, peak_src = peaks()
-        n_bins = tm["bin_list"][1]          # one row-builder launch per bin (2 per step; fewer with list reuse)
-        for cat, (ms, ln) in tm.items():
-            if ln == 0:
-                continue
-            ab = algorithmic_bytes(cat, scene.n, rows, kn, kl, klr)
-            # categories with several kernels per use: bytes are per use, not per launch
-            uses = {"bin_sort": n_bins, "bin_list": n_bins, "viscosity": K, "gradient": K,
-                    "ppe_setup": K, **cg_uses}.get(cat, ln)
-            kernels[cat] = {"ms_per_step": ms / K, "launches_per_step": ln / K,
-                            "us_per_launch": 1e3 * ms / ln,
-                            "algorithmic_gbs": (ab * uses / (ms * 1e-3) / 1e9) if (ab and ms > 0) else None}
-        top = max(kernels, key=lambda c: kernels[c]["ms_per_step"])
-        ab = algorithmic_bytes(top, scene.n, rows, kn, kl, klr)
-        ms, ln = tm[top]
-        uses = {"bin_sort": n_bins, "bin_list": n_bins, "viscosity": K, "gradient": K, "ppe_setup": K,
-                **cg_uses}.get(top, ln)
-        achieved = ab * uses / (ms * 1e-3) / 1e9
-        roof = {"kernel": top, "bound": "hbm", "per": "use (cg_spmv: one operator application; one k_ppe_cg launch runs a whole solve)",
-                "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, ROUTE_NAME[route], top)),
-                "peak_source": peak_src, "algorithmic_bytes_per_use": ab, "uses": uses,
-                "us_per_use": 1e3 * ms / max(uses, 1), "launches": ln,
-                "share_of_step": (ms / K) / (ms_replay / K),
-                "units": {"N": scene.n, "ppe_rows": rows, "mean_k_re_n": kn, "mean_k_re_lap": kl,
-                          "mean_k_re_lap_rows": klr},
-                "ms_per_step_instrumented": ms_replay / K}
-        if top == "bin_list":
-            # the row builder is bound by the fp64 pipe / instruction issue, not by HBM: report it
-            # against the fp64 pipe (148 SMs x 64 lanes x 1.965 GHz; 10 fp64-pipe
-            # instructions per candidate: 3 sub, 3 mul, 2 add, 2 compares)
-            reuse = int(scene.params.get("rebin_every", 1))
-            tests = n_bins * tests_all if reuse > 1 else K * (tests_all + tests_fluid)
-            a_alu = tests * 10.0 / (ms * 1e-3) / 1e12
-            roof.update({"bound": "alu", "hbm_achieved_gbs": roof["achieved"], "hbm_frac": roof["frac"],
-                         "achieved": a_alu, "peak": 18.61, "unit": "T fp64-pipe instructions/s",
-                         "frac": a_alu / 18.61, "peak_source": "148 SMs x 64 fp64 lanes x 1.965 GHz (measured 18.5 DADD/DMUL)",
-                         "candidate_tests_per_step": tests / K})
-        if top == "cg_spmv" and rows:
-            # the two on-chip ceilings of a list-driven sweep (profiles/r01_ceilings_microbench.md):
-            # 15 fp64 instructions per pair at 1.86e13/s, and the record gather at 30.8 SM-cycles
-            # per 32 pairs (texture + LSU split) on 148 SMs at 1.965 GHz
-            pairs = rows * klr
-            t_use = 1e-3 * ms / max(uses, 1)
-            roof["on_chip_ceilings"] = {
-                "fp64_pipe_frac": pairs * 15.0 / 1.86e13 / t_use,
-                "l1_gather_frac": pairs / 32.0 * 30.8 / (148 * 1.965e9) / t_use,
-                "note": "fractions of the time of one operator application that the fp64 pipe and the "
-                        "L1 record gather would need at their measured peaks; the gather binds"}
+    # the other pressure route of the same scene, in the same line (single GPU only)
+    other = None
+    if world == 1 and not args.no_other_route and args.rebin_every == 1:
+        r2 = 1 - route
+        o = measure_route(torch, np, B, args, scene, r2, 1, dev, stream, flush, K, W, sample_clocks=False)
+        other = {ROUTE_NAME[r2]: {k: o[k] for k in ("value", "ms_per_step", "gpu_launches", "roofline", "kernels")
+                                  if k in o} | ({"cg": o["cg"]} if "cg" in o else {})}
 
     # ---- end to end: pinned host buffers in, one step, host buffers out, every step ----
     e2e = None
@@ -424,74 +503,54 @@ def run_b200(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(scene, route)
+        smp, what = sample_scene(args, scene)
+        cpu = cpu_baseline(smp, route)
+        cpu["sample"] = what + "; " + cpu["sample"]
 
     if rank == 0:
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak",
+            "metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args, scene, route),
-                       "baseline_config": (f"BASELINE.json configs[{args.config - 1}]" if args.config <= 5 else
+                       "baseline_config": (f"BASELINE.json configs[{args.config - 1}]" + (f", size index {args.sweep_index} of its sweep" if args.config == 5 else "")
+                                           if args.config <= 5 else
                                            "none: the paper's own 2D dam-break shape (PAPER.md:397), context only"),
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+                       "options": {k: scene.params.get(k) for k in ("ppe_operator", "cg_warm_start", "key_mode", "cell_div", "rebin_every")},
                        "l2": "flushed before every timed step (256 MiB write, untimed)",
                        "timing": "CUDA events on the ctx stream around each mps_step(1), summed; max over ranks"},
-            "gpu_launches": int(launches), "clocks": clocks,
-            "cg_iters_per_step": cg_timed_main / K,
-            "fluid_particle_steps_per_sec": value * scene.n_fluid / scene.n,
-            "roofline": roof, "kernels": kernels, "e2e": e2e, "cpu_baseline": cpu,
+            "gpu_launches": main["gpu_launches"], "clocks": main["clocks"],
+            "fluid_particle_steps_per_sec": main["fluid_particle_steps_per_sec"],
+            "roofline": main["roofline"], "kernels": main["kernels"], "units": main["units"],
+            "e2e": e2e, "cpu_baseline": cpu,
         }
-        if route == 1:
-            out["cg_iters_per_sec"] = cg_timed_main / (ms_total * 1e-3)
-            out["cg"] = {"operator": {0: "matrix-free", 1: "assembled once per solve"}[int(scene.params.get("ppe_operator", 1))],
-                         "rows": int(stats["n_rows"]), "loop_ms_per_step": cg_loop_ms / K,
-                         "setup_ms_last_solve": stats["cg_setup_ms"],
-                         "us_per_iteration": 1e3 * cg_loop_ms / max(cg_timed_main, 1),
-                         "ps_per_row_per_iteration": 1e9 * cg_loop_ms / max(cg_timed_main, 1) / max(int(stats["n_rows"]), 1),
-                         "timing": "%globaltimer of block 0 inside k_ppe_cg around the iteration loop"}
+        if "cg" in main:
+            out["cg"] = main["cg"]
+            out["cg_iters_per_step"] = main["cg"]["iters_per_step"]
+            out["cg_iters_per_sec"] = main["cg"]["iters_per_sec"]
+        if other:
+            out["routes"] = other
         print(json.dumps(out))
     if world > 1:
         torch.distributed.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, copied by
-# hand from the ncu --set full capture summarised under profiles/ (key: scene, route, category).
-NCU_TRAFFIC = {
-    # profiles/r01d_scene2_scene3_ppe.md: per operator application (whole-solve DRAM bytes / applications)
-    (2, "ppe", "cg_spmv"): (20.16e6 + 0.38e6) / 53,
-    (3, "ppe", "cg_spmv"): (9.293e9 + 1.011e9) / 62,
-}
-
-
 def run_reference(args):
     """The reference arm of this tier: the CPU oracle, as it stands, on host cores.
 
-    Each timed "step" is one whole oracle step of a BOUNDED SAMPLE of the workload:
-    the same tank, parameters and route at twice the particle spacing (1/8 of the
-    fluid particles; for scene 2 this is scene 1's particle set), so that
-    --steps 20 --warmup 3 ends within a few minutes (a full scene-2 PPE step takes
-    the oracle about 15 s).  particle-steps/s is normalised by the particle count."""
+    Each timed "step" is one whole oracle step of a BOUNDED SAMPLE of the workload (sample_scene):
+    the same shape, parameters and route at a size where --steps 20 --warmup 5 ends within a few
+    minutes (one oracle PPE step of the 2M-particle default takes minutes).  particle-steps/s is
+    normalised by the sample's particle count."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from oracle import build as orc_build
     orc_build.build()
     from oracle import mps_oracle as O
-    from paper_2105_01677_b200 import scenes
     full, route = make_scene(args, 0)
-    if args.config in (1,):
-        sample, what = full, "the whole scene"
-    else:
-        l0 = 2.0 * full.params["l0"]
-        geo = {2: ((40, 20, 30), (20, 20, 10)), 3: ((100, 25, 50), (50, 25, 25))}.get(args.config)
-        if geo is None:
-            geo = ((40, 20, 30), (20, 20, 10))
-        sample = scenes.dam_break(l0, geo[0], geo[1], scenes.BASE_SEED + args.config, "reference_sample")
-        for k in ("grad_variant", "n_phases", "rho", "nu", "cs", "rho_pair_mean", "nu_pair_mean"):
-            sample.params[k] = full.params[k]
-        what = (f"same tank and parameters at 2x spacing: N={sample.n} "
-                f"(fluid {sample.n_fluid}) instead of N={full.n}")
+    sample, what = sample_scene(args, full)
     K, W = args.steps, args.warmup
     o = O.Oracle(sample)
     o.step(W, route)

@@ -19,6 +19,13 @@
  *    mps_sync, mps_get_stats, mps_pressure_ppe and mps_step.
  *  - A ctx is not thread-safe.  There is no CPU fallback: every call needs a
  *    CUDA device of compute capability 10.0 (B200).
+ *  - Every entry point that launches work opens an NVTX range of its own name.
+ *  - Environment variables read at mps_init (development switches; the defaults are what is
+ *    measured and tested): MPS_B200_ROWS=lean|warp|cell picks the neighbour-row builder (default: by
+ *    size and key_mode; all builders give identical rows), MPS_B200_CG_TEX=0 turns the texture path
+ *    of the matrix-free gathers off, MPS_B200_CG_TIMEOUT_CYCLES=<n> sets the spin limit of the
+ *    grid barrier inside the persistent CG kernel (default 4e9 SM cycles, 0 = no limit; raise it
+ *    or set 0 under compute-sanitizer or a debugger).
  */
 #ifndef MPS_B200_H
 #define MPS_B200_H
@@ -80,7 +87,10 @@ typedef struct mps_params {
   int32_t clamp_negative_p; /* (1) p < 0 -> 0 after either pressure route; Q4 */
   int32_t rho_pair_mean;    /* 0 arithmetic (default), 1 harmonic; Q6 */
   int32_t nu_pair_mean;     /* 1 harmonic (default), 0 arithmetic; Q9 */
-  int32_t key_mode;         /* 0: linear x-fastest cell key (the only mode supported) */
+  int32_t key_mode;         /* (0) 0: linear cell key c_x + n_x (c_y + n_y c_z); 1: Morton key, bit k of c_x, c_y, c_z
+                               at bits 3k, 3k+1, 3k+2 (3 x 10-bit interleave; at most 512 cells per axis): the key
+                               space then has 8^bits entries, bits = ceil(log2(max n_a)), ghosts get 8^bits, and
+                               mps_get_grid / mps_get_cell_start report that size */
   int32_t cell_div;         /* (1) cell side h = max(re_n, re_lap) / cell_div; 1..3 */
   int32_t max_neighbours;   /* (300) P:286; capacity of one neighbour row */
   int32_t ppe_source;       /* (0) 0: Eq. 8; 1: higher-order source, Eq. 15 (MPS-HS); 2: HS plus the
@@ -137,6 +147,7 @@ typedef struct mps_stats {
                                compaction and (ppe_operator 1) assembly ... */
   double cg_loop_ms;        /* ... and the CG iterations alone */
   double cg_loop_ms_total;  /* cg_loop_ms summed over the life of the ctx */
+  int64_t cg_nnz;           /* ppe_operator 1: off-diagonal entries of the matrix assembled by the last solve */
 } mps_stats;
 
 /* mps_init: create a ctx and copy n particles in (device pointers, caller's
@@ -261,7 +272,8 @@ int mps_ppe_apply(mps_ctx* ctx, const double* x, double* y, int32_t order);
 int mps_get_constants(mps_ctx* ctx, double* out);
 int mps_get_stats(mps_ctx* ctx, mps_stats* out);
 int mps_sync(mps_ctx* ctx);
-/* Per-kernel CUDA-event timing for bench.py: mps_timers_enable(ctx, mask) with
+/* Per-kernel CUDA-event timing for bench.py (the one call that allocates after mps_init: the first
+ * mps_timers_enable with a non-zero mask creates a pool of 8192 CUDA events): mps_timers_enable(ctx, mask) with
  * bit k of mask set times every launch of category k with a CUDA-event pair on
  * the ctx's stream (mask 0 switches timing off); mps_timers_read returns the
  * accumulated milliseconds and launch counts (HOST arrays of MPS_NUM_TIMERS). */

@@ -43,9 +43,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 def build_peaks() -> str:
-    """The stand-alone ceilings micro-benchmark (csrc/peaks.cu) -> ./mps_peaks."""
+    """The stand-alone ceilings micro-benchmark (microbench/peaks.cu, measurement tooling that is not
+    part of libmps_b200.so; profiles/r01_ceilings_microbench.md) -> ./mps_peaks."""
     exe = os.path.join(HERE, "mps_peaks")
-    src = os.path.join(CSRC, "peaks.cu")
+    src = os.path.join(HERE, "microbench", "peaks.cu")
     if _stale(exe, [src]):
         subprocess.check_call([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo",
                                "-std=c++17", "-o", exe, src])

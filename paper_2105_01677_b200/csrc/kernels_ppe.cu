@@ -233,8 +233,8 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 // ELL row g; neighbours on the free surface (p = 0) only add to the diagonal term.
 // Every lane of the warp must come through here with a warp-uniform trip count m_max.
 template <bool TWO_PHASE>
-__device__ __forceinline__ void assemble_row(const KConst& kc, const PpeArgs& a, int g, int i, int sub,
-                                             int grp, bool live, uint32_t m_max) {
+__device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs& a, int g, int i, int sub,
+                                                 int grp, bool live, uint32_t m_max) {
   const double4 pi = a.pos4[i];
   const uint32_t* row = row_ptr(a.nbr, kc.stride, i);
   const uint32_t nf = live ? a.cn[i] : 0u;
@@ -285,6 +285,7 @@ __device__ __forceinline__ void assemble_row(const KConst& kc, const PpeArgs& a,
     a.mcnt[g] = cnt;
     a.mdex[g] = dex + kc.compress_dt2;
   }
+  return cnt;
 }
 
 // ---- one row of y = A v with the assembled operator -------------------------------------
@@ -329,7 +330,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
   const int nb = (int)gridDim.x, bid = (int)blockIdx.x;
   unsigned int gen = 0;
   unsigned long long t_start = 0, t_loop = 0;
-  if (bid == 0 && tid == 0) t_start = global_ns();
+  if (bid == 0 && tid == 0) { t_start = global_ns(); a.cg->nnz = 0ull; }
 
   // -- S8b-1, S8b-2: flags and right-hand side over this block's contiguous chunk --------
   const int chunk = (kc.n + nb - 1) / nb;
@@ -450,20 +451,24 @@ k_ppe_cg(KConst kc, PpeArgs a) {
 
   // -- ppe_operator 1: assemble the rows, set up the compact vectors ------------------------
   if (ASM) {
+    uint32_t nnz = 0;
     for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
       const int g = sc * (SCW * GPW) + g_in_sc;
       const bool live = g < n_rows;
       const int i = live ? (int)a.rows[g] : 0;
       uint32_t m = live ? a.cn[i] + a.co[i] : 0u;
       m = __reduce_max_sync(0xffffffffu, m);
-      assemble_row<TWO_PHASE>(kc, a, live ? g : 0, i, sub, grp, live, m);
+      const uint32_t cnt = assemble_row<TWO_PHASE>(kc, a, live ? g : 0, i, sub, grp, live, m);
       if (live && sub == 0) {
+        nnz += cnt;
         a.xc[g] = a.x[i];
         a.rc[g] = a.b[i];
         a.pv[g] = 0.0;
         a.sv[g] = 0.0;
       }
     }
+    nnz = __reduce_add_sync(0xffffffffu, nnz);
+    if (lane == 0 && nnz) atomicAdd(&a.cg->nnz, (unsigned long long)nnz);
     if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
   }
   // -- warm start: r0 = b - A x0 ---------------------------------------------------------------
@@ -733,6 +738,7 @@ int mpsk_ppe_read_stats(mps_ctx* c) {
   c->stats.cg_setup_ms = 1e-6 * (double)s.t_setup_ns;
   c->stats.cg_loop_ms = 1e-6 * (double)s.t_loop_ns;
   c->stats.cg_loop_ms_total = 1e-6 * (double)s.t_loop_ns_total;
+  c->stats.cg_nnz = (int64_t)s.nnz;
   const bool noconv = s.noconv_total > c->noconv_seen;
   c->noconv_seen = s.noconv_total;
   if (noconv) {

@@ -7,9 +7,18 @@
 #include <algorithm>
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>  // header-only: ranges show up when a profiler is attached, cost nothing otherwise
+
 #include "mps_internal.h"
 
 static std::string g_init_error;
+
+// one NVTX range per ABI call
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
+#define MPS_RANGE() NvtxRange nvtx_range_(__func__)
 
 #define CK(call)                                                                 \
   do {                                                                           \
@@ -349,6 +358,7 @@ const char* mps_last_error(mps_ctx* c) { return c ? c->err.c_str() : g_init_erro
 int mps_init(mps_ctx** out, const mps_params* prm, int64_t n, const double* x, const double* y,
              const double* z, const double* u, const double* v, const double* w, const int32_t* type,
              const int32_t* phase, void* stream) {
+  MPS_RANGE();
   if (!x || !y || !z || !u || !v || !w || !type || !phase)
     return fail(nullptr, MPS_ERR_ARG, "a particle array pointer is NULL");
   int rc = create_ctx(out, prm, n, stream);
@@ -369,6 +379,7 @@ int mps_init(mps_ctx** out, const mps_params* prm, int64_t n, const double* x, c
 int mps_init_host(mps_ctx** out, const mps_params* prm, int64_t n, const double* x, const double* y,
                   const double* z, const double* u, const double* v, const double* w,
                   const int32_t* type, const int32_t* phase, void* stream) {
+  MPS_RANGE();
   if (!x || !y || !z || !u || !v || !w || !type || !phase)
     return fail(nullptr, MPS_ERR_ARG, "a particle array pointer is NULL");
   int rc = create_ctx(out, prm, n, stream);
@@ -396,6 +407,7 @@ int mps_init_host(mps_ctx** out, const mps_params* prm, int64_t n, const double*
 }
 
 int mps_destroy(mps_ctx* c) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   cudaStreamSynchronize(c->stream);
   free_all(c);
@@ -404,6 +416,7 @@ int mps_destroy(mps_ctx* c) {
 }
 
 int mps_bin(mps_ctx* c) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   mpsk_bin(c);
   CK(cudaGetLastError());
@@ -417,42 +430,49 @@ int mps_bin(mps_ctx* c) {
   } while (0)
 
 int mps_density(mps_ctx* c) {
+  MPS_RANGE();
   NEED_BIN(c);
   mpsk_density(c);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_smooth_density(mps_ctx* c) {
+  MPS_RANGE();
   NEED_BIN(c);
   mpsk_smooth_density(c);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_dndt(mps_ctx* c, int32_t keep) {
+  MPS_RANGE();
   NEED_BIN(c);
   mpsk_dndt(c, keep ? 1 : 0);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_viscosity(mps_ctx* c) {
+  MPS_RANGE();
   NEED_BIN(c);
   mpsk_viscosity(c);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_predict(mps_ctx* c) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   mpsk_predict(c);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_pressure_explicit(mps_ctx* c) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   mpsk_pressure_explicit(c);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_pressure_ppe(mps_ctx* c, int32_t* iters_out, double* relres_out) {
+  MPS_RANGE();
   NEED_BIN(c);
   int rc = mpsk_pressure_ppe(c);
   if (iters_out) *iters_out = c->stats.cg_iters;
@@ -463,12 +483,14 @@ int mps_pressure_ppe(mps_ctx* c, int32_t* iters_out, double* relres_out) {
   return rc;
 }
 int mps_gradient(mps_ctx* c) {
+  MPS_RANGE();
   NEED_BIN(c);
   mpsk_gradient(c);
   CK(cudaGetLastError());
   return MPS_OK;
 }
 int mps_correct(mps_ctx* c) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   mpsk_correct(c);
   CK(cudaGetLastError());
@@ -476,6 +498,7 @@ int mps_correct(mps_ctx* c) {
 }
 
 int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   if (nsteps < 0 || (route != MPS_ROUTE_EXPLICIT && route != MPS_ROUTE_PPE))
     return fail(c, MPS_ERR_ARG, "bad nsteps or pressure_route");
@@ -536,6 +559,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
 int mps_step_host(const mps_params* prm, int64_t n, double* x, double* y, double* z, double* u,
                   double* v, double* w, const int32_t* type, const int32_t* phase, double* p_out,
                   int32_t nsteps, int32_t route, mps_stats* stats_out, void* stream) {
+  MPS_RANGE();
   mps_ctx* c = nullptr;
   int rc = mps_init_host(&c, prm, n, x, y, z, u, v, w, type, phase, stream);
   if (rc) return rc;
@@ -566,6 +590,7 @@ int mps_step_host(const mps_params* prm, int64_t n, double* x, double* y, double
 
 int mps_upload_host(mps_ctx* c, const double* x, const double* y, const double* z, const double* u,
                     const double* v, const double* w, const int32_t* type, const int32_t* phase) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   if (!x || !y || !z || !u || !v || !w || !type || !phase)
     return fail(c, MPS_ERR_ARG, "a particle array pointer is NULL");
@@ -590,6 +615,7 @@ int mps_upload_host(mps_ctx* c, const double* x, const double* y, const double* 
 
 int mps_download_host(mps_ctx* c, double* x, double* y, double* z, double* u, double* v, double* w,
                       double* p) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   double* host[7] = {x, y, z, u, v, w, p};
   const int fields[7] = {MPS_F_X, MPS_F_Y, MPS_F_Z, MPS_F_U, MPS_F_V, MPS_F_W, MPS_F_P};
@@ -603,6 +629,7 @@ int mps_download_host(mps_ctx* c, double* x, double* y, double* z, double* u, do
 }
 
 int mps_get_field(mps_ctx* c, int32_t field, void* dst, int32_t order) {
+  MPS_RANGE();
   if (!c || !dst) return MPS_ERR_ARG;
   if (order != MPS_ORDER_ORIGINAL && order != MPS_ORDER_SORTED) return fail(c, MPS_ERR_ARG, "bad order");
   int rc = mpsk_get_field(c, field, dst, order);
@@ -611,6 +638,7 @@ int mps_get_field(mps_ctx* c, int32_t field, void* dst, int32_t order) {
   return MPS_OK;
 }
 int mps_set_field(mps_ctx* c, int32_t field, const void* src, int32_t order) {
+  MPS_RANGE();
   if (!c || !src) return MPS_ERR_ARG;
   if (order != MPS_ORDER_ORIGINAL && order != MPS_ORDER_SORTED) return fail(c, MPS_ERR_ARG, "bad order");
   int rc = mpsk_set_field(c, field, src, order);
@@ -636,6 +664,7 @@ int mps_get_cell_start(mps_ctx* c, uint32_t* dst) {
 }
 int mps_get_neighbours(mps_ctx* c, int32_t radius_id, uint32_t* counts, uint32_t* idx, int64_t cap,
                        int64_t* total) {
+  MPS_RANGE();
   NEED_BIN(c);
   if (!counts || (radius_id != MPS_RADIUS_N && radius_id != MPS_RADIUS_LAP)) return MPS_ERR_ARG;
   int rc = mpsk_get_neighbours(c, radius_id, counts, idx, cap, total);
@@ -643,6 +672,7 @@ int mps_get_neighbours(mps_ctx* c, int32_t radius_id, uint32_t* counts, uint32_t
   return rc;
 }
 int mps_ppe_apply(mps_ctx* c, const double* x, double* y, int32_t order) {
+  MPS_RANGE();
   NEED_BIN(c);
   if (!x || !y) return MPS_ERR_ARG;
   if (!c->ppe_ready) return fail(c, MPS_ERR_ORDER, "mps_ppe_apply needs mps_pressure_ppe first");
@@ -657,12 +687,14 @@ int mps_get_constants(mps_ctx* c, double* out) {
   return MPS_OK;
 }
 int mps_get_stats(mps_ctx* c, mps_stats* out) {
+  MPS_RANGE();
   if (!c || !out) return MPS_ERR_ARG;
   int rc = read_flags(c);
   *out = c->stats;
   return rc == MPS_ERR_CUDA ? rc : MPS_OK;
 }
 int mps_sync(mps_ctx* c) {
+  MPS_RANGE();
   if (!c) return MPS_ERR_ARG;
   return read_flags(c);
 }

@@ -45,6 +45,7 @@ struct CgScalars {  // what the persistent CG kernel reports at exit (block 0)
   long long iters_total;        // iterations since the ctx was made
   unsigned long long t_setup_ns, t_loop_ns;  // %globaltimer of block 0: setup (+ assembly) and the CG loop
   unsigned long long t_loop_ns_total;
+  unsigned long long nnz;       // entries of the assembled operator (ppe_operator 1)
 };
 
 // Grid-wide barrier state of the persistent CG kernel (zeroed before every launch).
