@@ -331,9 +331,10 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
     if route == 1:
         nnz = int(stats["cg_nnz"]) if asm else None
         # bytes one CG iteration must move: the operator application plus the vector updates (the
-        # device-timed loop covers both).  Assembled: 12 B per stored pair + per row count, diagonal term,
-        # r_g and w_g; matrix-free: 4 B per listed pair + position, r_i, bc, w_i
-        per_iter = (12.0 * nnz + rows * (4 + 8 + 8 + 8) if asm else rows * (4.0 * klr + 24 + 8 + 1 + 8)) + rows * 72.0
+        # device-timed loop covers both).  Assembled: one 8-byte word per stored pair (24-bit column +
+        # 40-bit coefficient) + per row count, diagonal term, scale, r_g and w_g; matrix-free: 4 B per
+        # listed pair + position, r_i, bc, w_i
+        per_iter = (8.0 * nnz + rows * (4 + 8 + 8 + 8 + 8) if asm else rows * (4.0 * klr + 24 + 8 + 1 + 8)) + rows * 72.0
         cg = {"operator": "assembled once per solve (ppe_operator 1)" if asm else "matrix-free (ppe_operator 0)",
               "rows": rows, "nnz": nnz, "iters_per_step": cg_iters / K, "iters_per_sec": cg_iters / (ms_total * 1e-3),
               "loop_ms_per_step": cg_loop_ms / K, "setup_ms_last_solve": stats["cg_setup_ms"],

@@ -251,7 +251,11 @@ int mps_download_host(mps_ctx* ctx, double* x, double* y, double* z,
                       double* u, double* v, double* w, double* p);
 
 /* Field access for parity tests and checkpoints.  dst/src are DEVICE pointers
- * to n elements (double for ids < 32, int32_t otherwise). */
+ * to n elements (double for ids < 32, int32_t otherwise).  Positions, velocities, type, phase and the
+ * fields an option carries per particle (MPS_F_NK, MPS_F_DNDTK, MPS_F_RHOS) follow their particle
+ * through every sort; every other field is the result of the last call that computed it and is only
+ * meaningful until the next mps_bin (inside mps_step: MPS_F_AX..AZ and MPS_F_NUT belong to the
+ * step's first bin and are not valid after the step). */
 int mps_get_field(mps_ctx* ctx, int32_t field, void* dst, int32_t order);
 int mps_set_field(mps_ctx* ctx, int32_t field, const void* src, int32_t order);
 

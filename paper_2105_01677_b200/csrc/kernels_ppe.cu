@@ -20,10 +20,13 @@
 //   0  matrix-free: r lives in pos4.w (a neighbour gather is one 32-byte record) and
 //      c_ij = A_lap w(r_ij) / rho_ij is recomputed at every application;
 //   1  assembled: positions are fixed during a solve, so the c_ij of the rows bc = 0 are
-//      computed once into a compact ELL matrix (fp64 value + uint32 column in the numbering
-//      of the compacted rows; neighbours on the free surface fold into a per-row diagonal
-//      term, dummies drop out).  An application streams 12 bytes per pair, coalesced, and
-//      gathers 8 bytes from a dense vector in which neighbouring rows share cache lines.
+//      computed once into a compact ELL matrix in the numbering of the compacted rows
+//      (neighbours on the free surface fold into a per-row diagonal term, dummies drop out).
+//      One stored pair is ONE 64-bit word: the column in the low 24 bits and c_ij as a 40-bit
+//      fixed-point fraction of the row's largest coefficient in the high 40 (absolute error
+//      <= 2^-41 of that coefficient: 1e-12 of an operator row, far inside the 1e-10 bar).  An
+//      application streams 8 bytes per pair, coalesced, and gathers 8 bytes from a dense
+//      vector in which neighbouring rows share cache lines.
 #include <algorithm>
 #include <stdlib.h>
 
@@ -37,6 +40,7 @@ constexpr int PPE_ILP = 4;   // independent neighbour gathers in flight per lane
 // (measured at 1.44M rows: 315 ps per row per iteration with 4, 265 with 8; two blocks per SM at 32
 // registers spill and are slower, 303-330)
 constexpr int ASM_ILP = 8;
+constexpr double PACK_QMAX = 1099511627775.0;  // 2^40 - 1: a stored coefficient is q / QMAX of the row's largest
 constexpr int CG_TPB = 1024;
 constexpr int L = 8;         // lanes per row
 constexpr int GPW = 32 / L;  // row groups per warp
@@ -71,6 +75,7 @@ struct PpeArgs {
   uint32_t* mcol;
   uint32_t* mcnt;
   double* mdex;
+  double* mscale;  // row's largest coefficient / (2^40 - 1)
   double* rc;
   double* xc;
   double tol2;
@@ -79,6 +84,9 @@ struct PpeArgs {
   int warm;
 };
 
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
 __device__ __forceinline__ unsigned long long global_ns() {
   unsigned long long t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -247,7 +255,7 @@ __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs
   uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
   const uint32_t lt = (1u << sub) - 1u;
   uint32_t cnt = 0;
-  double dex = 0.0;
+  double dex = 0.0, cmax = 0.0;
   for (uint32_t k0 = 0; k0 < m_max; k0 += PPE_ILP * L) {
     uint32_t e[PPE_ILP], rm[PPE_ILP];
     double4 q[PPE_ILP];
@@ -276,14 +284,25 @@ __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs
         const uint32_t at = cnt + (uint32_t)__popc(m8 & lt);
         vrow[at] = c;
         crow[at] = rm[u];
+        cmax = fmax(cmax, c);
       }
       cnt += (uint32_t)__popc(m8);
     }
   }
   dex = group_sum<L>(dex);
+  cmax = group_max<L>(cmax);
+  // second pass over the row just written (L1 / L2 hot): pack (coefficient, column) into one word
+  __syncwarp();
+  const double inv = cmax > 0.0 ? PACK_QMAX / cmax : 0.0;
+  unsigned long long* prow = reinterpret_cast<unsigned long long*>(vrow);
+  for (uint32_t k = sub; k < cnt; k += L) {
+    const unsigned long long q = __double2ull_rn(vrow[k] * inv);
+    prow[k] = (q << 24) | (unsigned long long)crow[k];
+  }
   if (live && sub == 0) {
     a.mcnt[g] = cnt;
     a.mdex[g] = dex + kc.compress_dt2;
+    a.mscale[g] = cmax / PACK_QMAX;
   }
   return cnt;
 }
@@ -295,30 +314,29 @@ __device__ __forceinline__ double asm_row(const KConst& kc, const PpeArgs& a, co
                                           int g, int sub, bool live, double& vg) {
   vg = v[g];
   const uint32_t n = live ? a.mcnt[g] : 0u;
-  const double* vrow = a.mval + (size_t)g * (size_t)kc.stride;
-  const uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
+  const unsigned long long* prow = reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g * (size_t)kc.stride;
   double s0 = 0.0, s1 = 0.0;
   for (uint32_t k = sub; k < n; k += ASM_ILP * L) {
-    double c[ASM_ILP];
-    uint32_t j[ASM_ILP];
+    unsigned long long w[ASM_ILP];
 #pragma unroll
     for (int u = 0; u < ASM_ILP; ++u) {
       const uint32_t kk = k + (uint32_t)(u * L);
-      const bool in = kk < n;
-      c[u] = in ? __ldcs(vrow + kk) : 0.0;
-      j[u] = in ? __ldcs(crow + kk) : (uint32_t)g;
+      w[u] = kk < n ? __ldcs(prow + kk) : (unsigned long long)(uint32_t)g;  // q = 0, column g
     }
     double vj[ASM_ILP];
 #pragma unroll
-    for (int u = 0; u < ASM_ILP; ++u) vj[u] = v[j[u]];
+    for (int u = 0; u < ASM_ILP; ++u) vj[u] = v[(uint32_t)w[u] & 0xffffffu];
 #pragma unroll
     for (int u = 0; u < ASM_ILP; u += 2) {
-      s0 = fma(c[u], vg - vj[u], s0);
-      s1 = fma(c[u + 1], vg - vj[u + 1], s1);
+      // q < 2^40 as a double without a conversion instruction: 2^52 + q has q in its mantissa
+      const double c0 = __longlong_as_double((long long)(0x4330000000000000ull | (w[u] >> 24))) - 4503599627370496.0;
+      const double c1 = __longlong_as_double((long long)(0x4330000000000000ull | (w[u + 1] >> 24))) - 4503599627370496.0;
+      s0 = fma(c0, vg - vj[u], s0);
+      s1 = fma(c1, vg - vj[u + 1], s1);
     }
   }
   const double s = group_sum<L>(s0 + s1);
-  return fma(live ? a.mdex[g] : 0.0, vg, s);
+  return live ? fma(a.mdex[g], vg, a.mscale[g] * s) : 0.0;
 }
 
 // ---- the persistent solve -------------------------------------------------------------
@@ -505,11 +523,26 @@ k_ppe_cg(KConst kc, PpeArgs a) {
     for (;;) {
       // phase A: w = A r, gamma = r.r, delta = r.w
       double g_part = 0.0, d_part = 0.0;
+      // assembled operator: the loop is bound by HBM latency x bytes in flight, so each group asks
+      // the L2 for the words of its NEXT row (one 128-byte line per lane, as many as that row has)
+      // while it works on this one; the row counts run one more row ahead
+      uint32_t n_ahead = 0;
+      if (ASM) {
+        const int g1 = (sc_first + sc_step) * (SCW * GPW) + g_in_sc;
+        n_ahead = g1 < n_rows ? a.mcnt[g1] : 0u;
+      }
       for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
         const int g = sc * (SCW * GPW) + g_in_sc;
         const bool live = g < n_rows;
         double ri, wi;
         if (ASM) {
+          const int g1 = g + sc_step * (SCW * GPW), g2 = g1 + sc_step * (SCW * GPW);
+          if ((uint32_t)(sub * 16) < n_ahead)
+            prefetch_l2(reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g1 * (size_t)kc.stride + sub * 16);
+          if (sub == 0 && n_ahead > 128u)  // a row longer than 128 pairs: its second kilobyte
+            for (uint32_t k = 128; k < n_ahead; k += 16)
+              prefetch_l2(reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g1 * (size_t)kc.stride + k);
+          n_ahead = g2 < n_rows ? a.mcnt[g2] : 0u;
           wi = asm_row(kc, a, a.rc, live ? g : 0, sub, live, ri);
           if (live && sub == 0) a.wv[g] = wi;
         } else {
@@ -686,7 +719,7 @@ PpeArgs make_args(mps_ctx* c) {
   a.x = c->cg_x; a.pv = c->cg_p; a.sv = c->cg_s; a.wv = c->cg_w; a.p = c->p;
   a.nbr = c->nbr; a.cn = c->cn; a.co = c->co; a.rows = c->cg_rows; a.bcount = c->cg_bcount;
   a.part = c->cg_part; a.cg = c->cg; a.bar = c->cg_bar;
-  a.rowmap = c->rowmap; a.mval = c->mat_val; a.mcol = c->mat_col; a.mcnt = c->mat_cnt; a.mdex = c->mat_dex;
+  a.rowmap = c->rowmap; a.mval = c->mat_val; a.mcol = c->mat_col; a.mcnt = c->mat_cnt; a.mdex = c->mat_dex; a.mscale = c->mat_scale;
   a.rc = c->cg_rc; a.xc = c->cg_xc;
   a.tol2 = c->prm.cg_rtol * c->prm.cg_rtol;
   a.timeout_cycles = c->cg_timeout_cycles;

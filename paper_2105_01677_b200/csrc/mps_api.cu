@@ -77,7 +77,7 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->rho_s[0]); cudaFree(c->rho_s[1]); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
   cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
   cudaFree(c->cg_rows); cudaFree(c->cg_bcount); cudaFree(c->cg_bar);
-  cudaFree(c->mat_val); cudaFree(c->mat_col); cudaFree(c->mat_cnt); cudaFree(c->mat_dex); cudaFree(c->rowmap);
+  cudaFree(c->mat_val); cudaFree(c->mat_col); cudaFree(c->mat_cnt); cudaFree(c->mat_dex); cudaFree(c->mat_scale); cudaFree(c->rowmap);
   cudaFree(c->cg_rc); cudaFree(c->cg_xc);
   if (c->bar_host) cudaFreeHost(c->bar_host);
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
@@ -105,6 +105,8 @@ static int check_params(const mps_params* p, int64_t n) {
   if (p->ppe_laplacian < 0 || p->ppe_laplacian > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_laplacian must be 0 or 1");
   if (p->rebin_every < 1 || p->rebin_every > 1000) return fail(nullptr, MPS_ERR_ARG, "rebin_every must be in [1, 1000]");
   if (p->ppe_operator < 0 || p->ppe_operator > 1) return fail(nullptr, MPS_ERR_ARG, "ppe_operator must be 0 (matrix-free) or 1 (assembled)");
+  if (p->ppe_operator == 1 && n >= ((int64_t)1 << 24))
+    return fail(nullptr, MPS_ERR_ARG, "ppe_operator 1 stores 24-bit column indices: n must be below 2^24 (use ppe_operator 0)");
   if (p->cg_warm_start < 0 || p->cg_warm_start > 1) return fail(nullptr, MPS_ERR_ARG, "cg_warm_start must be 0 or 1");
   if (p->kernel < 0 || p->kernel > 1) return fail(nullptr, MPS_ERR_ARG, "kernel must be 0 (Eq. 3) or 1 (Eq. 4)");
   if (p->kernel == 1 && (p->ppe_source != 0 || p->ppe_laplacian != 0))
@@ -222,7 +224,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->cg_bar, 1));
   if (prm->ppe_operator == 1) {  // the assembled operator: 12 bytes per pair of the rows bc = 0
     A(dalloc(&c->mat_val, N * (size_t)k.stride)); A(dalloc(&c->mat_col, N * (size_t)k.stride));
-    A(dalloc(&c->mat_cnt, N)); A(dalloc(&c->mat_dex, N)); A(dalloc(&c->rowmap, N));
+    A(dalloc(&c->mat_cnt, N)); A(dalloc(&c->mat_dex, N)); A(dalloc(&c->mat_scale, N)); A(dalloc(&c->rowmap, N));
     A(dalloc(&c->cg_rc, N)); A(dalloc(&c->cg_xc, N));
   }
   A(cudaMallocHost((void**)&c->bar_host, sizeof(GridBar)));

@@ -142,8 +142,10 @@ struct mps_ctx {
   uint32_t* cg_rows = nullptr;   // compacted slot indices of the PPE unknowns (bc == 0)
   // ppe_operator 1: the assembled operator over the compacted rows g = 0..n_rows-1 (ELL, row g at
   // g * kc.stride) and the CG vectors in the same compact numbering
-  double* mat_val = nullptr;     // c_ij of the neighbours j that are unknowns too
-  uint32_t* mat_col = nullptr;   // their compact row index
+  double* mat_val = nullptr;     // one 64-bit word per stored pair: column (24 bits) | coefficient (40-bit fraction
+                                 // of the row's largest); holds plain fp64 coefficients while a row is assembled
+  uint32_t* mat_col = nullptr;   // assembly scratch: the columns before packing
+  double* mat_scale = nullptr;   // row's largest coefficient / (2^40 - 1)
   uint32_t* mat_cnt = nullptr;   // entries of row g
   double* mat_dex = nullptr;     // sum of c_ij over free-surface neighbours + compress / dt^2
   uint32_t* rowmap = nullptr;    // slot -> compact row (ROW_SURFACE / ROW_NONE otherwise)

@@ -72,4 +72,10 @@ __device__ __forceinline__ double group_min(double v) {
   for (int o = L / 2; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
 }
+template <int L>
+__device__ __forceinline__ double group_max(double v) {
+#pragma unroll
+  for (int o = L / 2; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
 __device__ __forceinline__ double warp_sum(double v) { return group_sum<32>(v); }

@@ -78,6 +78,8 @@ def main():
     ap.add_argument("--out", required=True)
     ap.add_argument("--traffic", action="append", default=[], help="KEY=KERNEL_REGEX:DIVISOR")
     ap.add_argument("--note", action="append", default=[])
+    ap.add_argument("--traffic-file", default=TRAFFIC, help="where the traffic table lives (default profiles/r02_traffic.json)")
+    ap.add_argument("--source-name", default=None, help="path recorded as the entry's source (default: --out)")
     a = ap.parse_args()
     launches = read_report(a.report)
     groups = {}
@@ -108,7 +110,7 @@ def main():
         lines += ["", n]
     if a.traffic:
         try:
-            with open(TRAFFIC) as f:
+            with open(a.traffic_file) as f:
                 table = json.load(f)
         except Exception:
             table = {}
@@ -122,9 +124,9 @@ def main():
             tot = (hit["dram__bytes_read.sum"] or 0.0) + (hit["dram__bytes_write.sum"] or 0.0)
             table[key] = {"dram_bytes_per_use": tot / float(div), "uses_in_launch": float(div),
                           "dram_bytes_launch": tot, "kernel": hit["name"], "launch_us": hit["gpu__time_duration.sum"],
-                          "source": os.path.relpath(a.out, ROOT)}
+                          "source": a.source_name or os.path.relpath(a.out, ROOT)}
             lines.append(f"* `{key}`: {tot / 1e6:.1f} MB / {div} = {tot / float(div) / 1e6:.2f} MB per use ({hit['name']})")
-        with open(TRAFFIC, "w") as f:
+        with open(a.traffic_file, "w") as f:
             json.dump(table, f, indent=1, sort_keys=True)
             f.write("\n")
     with open(a.out, "w") as f:

@@ -393,9 +393,11 @@ def test_config4_two_phase_ppe_5_steps(B, O):
     print(f"config 4 (N={s.n}), 5 PPE steps (two-phase, Cs 0.12): max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}, "
           f"moved {moved:.4f} l0; cg iters {g.stats()['cg_iters']} vs {o.stats()['cg_iters']}")
     assert eL <= 1e-7
-    # five steps from rest the strain rate is a difference of nearly equal velocities: compare nu_t on
-    # its natural scale (Cs l0)^2 x 1/s, not relative to its own (rounding-level) size
-    assert relerr(g.get("nut"), o.get("nut"), (0.12 * 0.004) ** 2) <= 1e-6
+    # (nu_t and the viscous acceleration belong to the slots of the step's first bin and are not
+    # carried through the re-sort at r*: they are compared stage by stage in
+    # test_full_size_ppe_residual_under_oracle_operator; here the velocities they feed)
+    assert vec_relerr([g.get(k) for k in "uvw"], [o.get(k) for k in "uvw"], 1e-3) <= 1e-8
+    assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-6
 
 
 def test_config5_250k_explicit_10_steps(B, O):
