@@ -217,8 +217,10 @@ def timed_steps(torch, world, g, route, K, flush, stream):
     if world > 1:
         torch.distributed.barrier()
     torch.cuda.synchronize()
+    stream = g.stream                      # the ctx's own stream: flush, events and kernels in one queue
     for k in range(K):
-        flush.zero_()
+        with torch.cuda.stream(stream):
+            flush.zero_()
         ev0[k].record(stream)
         g.step(1, route)
         ev1[k].record(stream)
@@ -489,10 +491,11 @@ def run_b200(args):
         if world > 1:
             torch.distributed.barrier()
         for k in range(K):
-            flush.zero_()
-            e0[k].record(stream)
+            with torch.cuda.stream(g.stream):
+                flush.zero_()
+            e0[k].record(g.stream)
             one()
-            e1[k].record(stream)
+            e1[k].record(g.stream)
         torch.cuda.synchronize()
         ms_e = barrier_and_max(world, sum(a.elapsed_time(b) for a, b in zip(e0, e1)), dev)
         g.close()

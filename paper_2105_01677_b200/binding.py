@@ -173,7 +173,10 @@ class Mps:
         self.params = p
         self._prm = make_params(p)
         self.n = int(arrays["x"].shape[0])
-        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        # a stream of the ctx's own by default: the legacy default stream cannot be captured, and
+        # mps_step replays its launch sequence from CUDA graphs.  Every method below orders the ctx
+        # stream against torch's current stream where data changes hands.
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
         with torch.cuda.device(self.device):
             dev = {}
             for k in ("x", "y", "z", "u", "v", "w"):

@@ -84,6 +84,7 @@ static void free_all(mps_ctx* c) {
   if (c->cg_host) cudaFreeHost(c->cg_host);
   if (c->flags_host) cudaFreeHost(c->flags_host);
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+  for (auto& r : c->seg) for (auto& p : r) for (auto& g : p) if (g.exec) cudaGraphExecDestroy(g.exec);
 }
 
 static int check_params(const mps_params* p, int64_t n) {
@@ -351,6 +352,64 @@ void mps_timer_drain(mps_ctx* c) {
   c->ev_used = 0;
 }
 
+// ---- mps_step segments as CUDA graphs ----------------------------------------------
+// The launch sequence of a step is fixed by (route, which of the two particle buffers is
+// current, segment), so it is captured once and replayed: a step of a small scene is bound by
+// the host's launch rate (about twenty launches and memsets of a few microseconds each), a graph
+// launch costs one.  The body runs for real when capture is not possible (legacy default stream,
+// timers on) and mutates the same host state either way.
+struct HostState {
+  int cur; bool binned, ppe_ready, posw_is_p; cudaTextureObject_t pos_tex, vel_tex;
+  int64_t launches; int64_t t_launches[MPS_NUM_TIMERS];
+};
+static HostState save_state(const mps_ctx* c) {
+  HostState h{c->cur, c->binned, c->ppe_ready, c->posw_is_p, c->kc.pos_tex, c->kc.vel_tex, c->launches, {0}};
+  for (int k = 0; k < MPS_NUM_TIMERS; ++k) h.t_launches[k] = c->t_launches[k];
+  return h;
+}
+static void restore_state(mps_ctx* c, const HostState& h) {
+  c->cur = h.cur; c->binned = h.binned; c->ppe_ready = h.ppe_ready; c->posw_is_p = h.posw_is_p;
+  c->kc.pos_tex = h.pos_tex; c->kc.vel_tex = h.vel_tex; c->launches = h.launches;
+  for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] = h.t_launches[k];
+}
+template <class F>
+static void run_segment(mps_ctx* c, int route, int which, F&& body) {
+  if (!c->graphs_ok || c->timer_mask != 0 || c->stream == nullptr) { body(); return; }
+  StepSeg& g = c->seg[route][c->cur][which];
+  if (!g.exec) {
+    const HostState before = save_state(c);
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      cudaGetLastError();
+      c->graphs_ok = false;
+      body();
+      return;
+    }
+    body();
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (e == cudaSuccess && graph) e = cudaGraphInstantiate(&g.exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e != cudaSuccess || !g.exec) {  // not capturable here: run the launches for real from now on
+      cudaGetLastError();
+      g.exec = nullptr;
+      c->graphs_ok = false;
+      restore_state(c, before);
+      body();
+      return;
+    }
+    g.cur_after = c->cur; g.binned = c->binned; g.ppe_ready = c->ppe_ready; g.posw_is_p = c->posw_is_p;
+    g.pos_tex = c->kc.pos_tex; g.vel_tex = c->kc.vel_tex;
+    g.launches = c->launches - before.launches;
+    for (int k = 0; k < MPS_NUM_TIMERS; ++k) g.t_launches[k] = c->t_launches[k] - before.t_launches[k];
+  } else {
+    c->cur = g.cur_after; c->binned = g.binned; c->ppe_ready = g.ppe_ready; c->posw_is_p = g.posw_is_p;
+    c->kc.pos_tex = g.pos_tex; c->kc.vel_tex = g.vel_tex;
+    c->launches += g.launches;
+    for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] += g.t_launches[k];
+  }
+  cudaGraphLaunch(g.exec, c->stream);
+}
+
 extern "C" {
 
 const char* mps_version(void) { return "mps_b200 0.1 (sm_100a)"; }
@@ -523,27 +582,35 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       }
       c->kc.stale = 1;
       ++c->reuse_count;
-    } else {
+    }
+    // everything up to the pressure: one replayable segment (list reuse changes the sequence from
+    // step to step and runs its launches directly)
+    auto pre = [&]() {
       // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
-      mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY);
-    }
-    if (ecs) {
+      if (K == 1) mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY);
+      if (ecs) {
+        mpsk_density(c);
+        mpsk_dndt(c, 1);
+      }
+      mpsk_viscosity(c);
+      mpsk_predict(c);
+      // the explicit route needs only the re_n part at r* (density, p-hat, gradient)
+      if (K == 1) mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
       mpsk_density(c);
-      mpsk_dndt(c, 1);
-    }
-    mpsk_viscosity(c);
-    mpsk_predict(c);
-    // the explicit route needs only the re_n part at r* (density, p-hat, gradient)
-    if (K == 1) mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
-    mpsk_density(c);
-    if (hs) mpsk_dndt(c, 0);
-    if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
-    else {
+      if (hs) mpsk_dndt(c, 0);
+      if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
+    };
+    auto post = [&]() {
+      mpsk_gradient(c);
+      mpsk_correct(c);
+    };
+    if (K > 1) pre(); else run_segment(c, route, 0, pre);
+    if (route == MPS_ROUTE_PPE) {
+      // the solve is a cooperative launch of its own, between the two segments
       int rc = mpsk_pressure_ppe(c, /*sync=*/false);  // statistics are read once, after the last step
       if (rc == MPS_ERR_CUDA) return rc;
     }
-    mpsk_gradient(c);
-    mpsk_correct(c);
+    if (K > 1) post(); else run_segment(c, route, 1, post);
     c->stats.steps_total++;
   }
   c->kc.stale = 0;  // API-level sweeps always run on exact rows (they need mps_bin first)

@@ -88,6 +88,17 @@ struct KConst {  // by-value kernel parameter
   cudaTextureObject_t pos_tex, vel_tex;
 };
 
+// One captured segment of mps_step (a CUDA graph of its kernel launches and memsets) and the host
+// state the segment leaves behind, so that a replay can skip the launch code.
+struct StepSeg {
+  cudaGraphExec_t exec = nullptr;
+  int cur_after = 0;
+  bool binned = false, ppe_ready = false, posw_is_p = false;
+  cudaTextureObject_t pos_tex = 0, vel_tex = 0;
+  int64_t launches = 0;
+  int64_t t_launches[MPS_NUM_TIMERS] = {0};
+};
+
 struct mps_ctx {
   mps_params prm;
   KConst kc;
@@ -180,6 +191,10 @@ struct mps_ctx {
   std::vector<int> ev_cat;
   size_t ev_used = 0;
   int sm_count = 148;
+  // mps_step replays its launch sequence from CUDA graphs (one per route, buffer parity and segment)
+  // when the ctx has a capturable stream (not the legacy default stream) and timers are off
+  StepSeg seg[2][2][2];
+  bool graphs_ok = true;
 };
 
 // ---- launch helper: counts launches, optional CUDA-event timing ------------------
