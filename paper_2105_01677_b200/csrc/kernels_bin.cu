@@ -559,8 +559,12 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
 // Measured and rejected in round 2: whole rows staged in shared memory
 // and copied out coalesced (fewer instructions but 12 instead of 20 warps per SM: 6.1 vs 4.9 ms
 // per step at 2M particles), 16-entry rings drained once per 32-candidate chunk (4.7 vs 4.2 ms),
-// cells handed out through an atomic counter (2.2 vs 1.2 ms at 438k: the warps of a block share
-// the candidates of neighbouring cells in L1).
+// cells handed out through an atomic counter, grid-wide (2.2 vs 1.2 ms at 438k: the warps of a
+// block share the candidates of neighbouring cells in L1) or per block of 24 cells (1.4 vs 1.05 ms
+// at 438k, no change at 2M), and a tests-only kernel writing hit masks followed by a warp-per-row
+// expansion (1.7 + 1.8 ms per bin at 2M against 2.5 ms: the tests alone take 1.7 ms at 58 % of the
+// fp64 pipe, so the appends cost about a third of this kernel, not the half their instruction
+// count suggests).
 constexpr int CELL_TPB = 256;
 constexpr int CELL_WARPS = CELL_TPB / 32;
 constexpr int CELL_BATCH = 8;  // candidates tested per lane before the hits are appended

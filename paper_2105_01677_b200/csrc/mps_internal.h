@@ -115,8 +115,8 @@ struct mps_ctx {
   uint32_t* tp[2] = {nullptr, nullptr};
   uint32_t* oid[2] = {nullptr, nullptr};
   uint32_t* ent = nullptr;         // per slot: own index | NB_* flags (what a neighbour row stores)
-  int rows_builder = 0;            // 0: k_build_rows (lanes on candidates, four particles per warp); 1 / 2: the
-                                   // round-1 builders, kept for comparison (MPS_B200_ROWS=lean|warp|cell)
+  int rows_builder = 0;            // 0: k_build_rows (lanes on candidates, four particles per warp, any key); 1: one
+                                   // warp per particle; 2: one warp per cell (MPS_B200_ROWS=lean|warp|cell)
   int cur = 0;
   // bin scratch
   uint32_t* key = nullptr;         // per slot (after bin: key of the slot)
