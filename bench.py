@@ -396,7 +396,9 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
         # per candidate: 3 sub, 3 mul, 2 add, 2 compares)
         ab = algorithmic_bytes(top, N, rows, kn, kl, klr)
         reuse = int(scene.params.get("rebin_every", 1))
-        tests = n_bins * ns["tests_all"] if reuse > 1 else K * (ns["tests_all"] + ns["tests_fluid"])
+        # one full scan per step when mps_step carries its rows across the corrector, else a fluid-only
+        # scan at r^k and a full one at r*
+        tests = n_bins * ns["tests_all"] if (reuse > 1 or n_bins <= K) else K * (ns["tests_all"] + ns["tests_fluid"])
         a_alu = tests * 10.0 / (ms_top * 1e-3) / 1e12
         hbm = ab * n_bins / (ms_top * 1e-3) / 1e9
         roof.update({"per": "row build (one per bin)", "bound": "alu", "achieved": a_alu, "peak": 18.61,

@@ -25,7 +25,8 @@
  *    size and key_mode; all builders give identical rows), MPS_B200_CG_TEX=0 turns the texture path
  *    of the matrix-free gathers off, MPS_B200_CG_TIMEOUT_CYCLES=<n> sets the spin limit of the
  *    grid barrier inside the persistent CG kernel (default 4e9 SM cycles, 0 = no limit; raise it
- *    or set 0 under compute-sanitizer or a debugger).
+ *    or set 0 under compute-sanitizer or a debugger), MPS_B200_CARRY=0 makes mps_step bin twice per
+ *    step instead of carrying the rows of its one bin across the corrector (see mps_step).
  */
 #ifndef MPS_B200_H
 #define MPS_B200_H
@@ -227,8 +228,15 @@ int mps_gradient(mps_ctx* ctx);
 int mps_correct(mps_ctx* ctx);
 
 /* mps_step: nsteps times { bin, [ppe_source 2: density, dndt(keep)], viscosity, predict, bin,
- * density, [ppe_source >= 1: dndt], pressure (route), gradient, correct }.  No host synchronisation inside except the CG
- * convergence poll of the PPE route.  Returns the first error met. */
+ * density, [ppe_source >= 1: dndt], pressure (route), gradient, correct }.  Every sweep sees the exact
+ * neighbour set of the positions it works at (Q7).  How the library gets there (Q26): the bin at r* runs
+ * on an internal grid whose cells are 1/256 larger than mps_bin's and builds rows with a margin of 0.8 of
+ * that slack; every sweep re-tests r2 < re^2 with the rounding of Q2, so the sets are exact, and the same
+ * rows serve the first sweeps of the NEXT step at r^(k+1) when the corrector moved no particle by more
+ * than 0.45 margins and none left the domain (checked on the device; one 4-byte read-back per step) --
+ * otherwise, and in the first step, that step bins at r^k as written above.  GHOST decisions always use
+ * mps_bin's grid.  The launches of a step are replayed from CUDA graphs when the ctx has its own stream.
+ * Returns the first error met. */
 int mps_step(mps_ctx* ctx, int32_t nsteps, int32_t pressure_route);
 
 /* mps_step_host: the end-to-end call on HOST buffers: init from host arrays,

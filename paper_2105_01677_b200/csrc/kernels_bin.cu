@@ -75,11 +75,15 @@ __global__ void k_keys(KConst kc, const double4* __restrict__ pos4, uint32_t* __
     uint32_t t = tp[i];
     bool ghost = (t & 0xff) == MPS_GHOST;
     // (x - min) * inv_h: a subtraction then a multiplication, each rounded (no FMA possible)
-    double fx = floor(__dmul_rn(__dsub_rn(q.x, kc.dmin[0]), kc.inv_h));
-    double fy = floor(__dmul_rn(__dsub_rn(q.y, kc.dmin[1]), kc.inv_h));
-    double fz = floor(__dmul_rn(__dsub_rn(q.z, kc.dmin[2]), kc.inv_h));
-    bool in = (fx >= 0.0 && fx < (double)kc.nx) && (fy >= 0.0 && fy < (double)kc.ny) &&
-              (fz >= 0.0 && fz < (double)kc.nz);
+    const double sx = __dsub_rn(q.x, kc.dmin[0]), sy = __dsub_rn(q.y, kc.dmin[1]), sz = __dsub_rn(q.z, kc.dmin[2]);
+    // in or out of the domain: always on the contract's grid (B1)
+    const double gx = floor(__dmul_rn(sx, kc.inv_h_dom)), gy = floor(__dmul_rn(sy, kc.inv_h_dom));
+    const double gz = floor(__dmul_rn(sz, kc.inv_h_dom));
+    bool in = (gx >= 0.0 && gx < (double)kc.nx_dom) && (gy >= 0.0 && gy < (double)kc.ny_dom) &&
+              (gz >= 0.0 && gz < (double)kc.nz_dom);
+    // the cell that holds the particle (the same grid, except for the internal bin of mps_step)
+    double fx = floor(__dmul_rn(sx, kc.inv_h)), fy = floor(__dmul_rn(sy, kc.inv_h)), fz = floor(__dmul_rn(sz, kc.inv_h));
+    fx = fmin(fx, (double)(kc.nx - 1)); fy = fmin(fy, (double)(kc.ny - 1)); fz = fmin(fz, (double)(kc.nz - 1));
     if (!ghost && !(isfinite(q.x) && isfinite(q.y) && isfinite(q.z))) flags->nonfinite = 1;
     if (ghost || !in) {
       if (!ghost) tp[i] = (t & ~0xffu) | MPS_GHOST;
@@ -205,7 +209,10 @@ __global__ void k_scatter(int n, const uint32_t* __restrict__ key_tmp, const uin
                           uint32_t* __restrict__ tmp_src, uint32_t* __restrict__ tmp_oid,
                           uint32_t* __restrict__ key, int ncells, DevFlags* __restrict__ flags) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i == 0) flags->n_ghost = n - (int)cell_start[ncells];  // ghosts sit behind the last cell
+  if (i == 0) {
+    flags->n_ghost = n - (int)cell_start[ncells];  // ghosts sit behind the last cell
+    flags->carry_bad = 0;                          // raised again by this step's corrector if need be
+  }
   if (i >= n) return;
   uint32_t k = key_tmp[i];
   uint32_t dst = cell_start[k] + rank[i];
@@ -460,15 +467,16 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
   const uint32_t cap = (uint32_t)kc.cap;
   // the four particles: key, wanted?, position, row
   uint32_t kk[LEAN_PPW], nf[LEAN_PPW], nb[LEAN_PPW];
-  bool want[LEAN_PPW];
+  bool want[LEAN_PPW], back_skip[LEAN_PPW];
   double px[LEAN_PPW], py[LEAN_PPW], pz[LEAN_PPW];
 #pragma unroll
   for (int t = 0; t < LEAN_PPW; ++t) {
     const int i = i0 + t;
     const bool in = i < kc.n;
     kk[t] = in ? key[i] : 0xffffffffu;
-    want[t] = in && kk[t] < (uint32_t)kc.ncells &&
-              !((mode & ROWS_FLUID_ONLY) && (ent[i] & (NB_DUMMY | NB_WALL)));
+    const bool solid = in && (ent[i] & (NB_DUMMY | NB_WALL));
+    want[t] = in && kk[t] < (uint32_t)kc.ncells && !((mode & ROWS_FLUID_ONLY) && solid);
+    back_skip[t] = (mode & ROWS_BACK_FLUID) && solid;
     const double4 q = pos4[in ? i : i0];
     px[t] = q.x; py[t] = q.y; pz[t] = q.z;
     nf[t] = 0; nb[t] = 0;
@@ -512,10 +520,15 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
                 const uint32_t self = (uint32_t)(i0 + t) - j0;
                 if (self < 32u) m_lap &= ~(1u << self);
                 if (m_lap == 0u) continue;
-                const bool hit = (m_lap >> lane) & 1u;
+                bool hit = (m_lap >> lane) & 1u;
                 const bool in_n = hit && (rn_only || r2 < kc.re_n2);
                 if (hit && __double2hiint(r2) == 0) coincident = true;  // r = 0 (or denormal): Eq. 3 is infinite
                 const uint32_t m_n = __ballot_sync(0xffffffffu, in_n);
+                if (back_skip[t]) {  // ROWS_BACK_FLUID: a wall or dummy row keeps its re_n part only (warp-uniform)
+                  m_lap = m_n;
+                  hit = in_n;
+                  if (m_lap == 0u) continue;
+                }
                 const uint32_t m_o = m_lap & ~m_n;
                 uint32_t* row = nbr + (size_t)(i0 + t) * (size_t)S;
                 if (nf[t] + nb[t] + (uint32_t)__popc(m_lap) <= cap) {
@@ -617,6 +630,7 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
       const uint32_t ii = act ? i : ps;
       const double4 pi = pos4[ii];
       uint32_t* row = nbr + (size_t)ii * (size_t)S;
+      const bool back_skip = (mode & ROWS_BACK_FLUID) && (ent[ii] & (NB_DUMMY | NB_WALL));
       uint32_t nf = 0, nb = 0;
       for (int dz = -R; dz <= R; ++dz) {
         const int z2 = cz + dz;
@@ -650,7 +664,7 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
             uint32_t keep = cnt == 32u ? 0xffffffffu : ((1u << cnt) - 1u);
             if (i - j0 < 32u) keep &= ~(1u << (i - j0));  // j == i
             m_lap = act ? (m_lap & keep) : 0u;
-            if (rn_only) m_lap &= m_n;  // the explicit route needs only the re_n part at r*
+            if (rn_only || back_skip) m_lap &= m_n;  // only the re_n part is wanted (for this row)
             // capacity: keep the first hits that fit (ascending j), flag the rest
             if (nf + nb + (uint32_t)__popc(m_lap) > cap) {
               overflow = 1;
@@ -842,14 +856,15 @@ int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const doub
   return MPS_OK;
 }
 
-int mpsk_bin(mps_ctx* c, int rows_mode) {
+int mpsk_bin(mps_ctx* c, int rows_mode, bool step_grid) {
   const int fo = (rows_mode & ROWS_FLUID_ONLY) ? 1 : 0;
   const int n = (int)c->n;
-  const int nc = c->kc.ncells;
+  const KConst& kg = step_grid ? c->kc_step : c->kc;
+  const int nc = kg.ncells;
   const int cur = c->cur, nxt = cur ^ 1;
   cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * (nc + 2), c->stream);
   cudaMemsetAsync(&c->flags->max_row, 0, sizeof(int), c->stream);
-  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_keys, div_up(n, TPB), TPB, c->kc, c->pos4[cur], c->tp[cur],
+  MPS_LAUNCH(c, MPS_T_BIN_SORT, k_keys, div_up(n, TPB), TPB, kg, c->pos4[cur], c->tp[cur],
              c->key_tmp, c->rank, c->cell_count, c->flags);
   mpsk_exclusive_scan(c, MPS_T_BIN_SORT, c->cell_count, c->cell_start, nc + 2, c->scan_tmp);
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_scatter, div_up(n, TPB), TPB, n, c->key_tmp, c->rank,
@@ -862,15 +877,16 @@ int mpsk_bin(mps_ctx* c, int rows_mode) {
   c->cur = nxt;
   c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
   c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;
+  c->carry_valid = false;
   if (c->rows_builder == 0) {
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (LEAN_TPB / 32) * LEAN_PPW), LEAN_TPB, c->kc, c->pos4[nxt],
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (LEAN_TPB / 32) * LEAN_PPW), LEAN_TPB, kg, c->pos4[nxt],
                c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode);
   } else if (c->prm.cell_div == 1 && c->rows_builder == 2) {
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, c->kc, c->pos4[nxt],
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, kg, c->pos4[nxt],
                c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode);
   } else {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, c->kc,
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, kg,
                c->pos4[nxt], c->tp[nxt], c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
   }
   c->binned = true;

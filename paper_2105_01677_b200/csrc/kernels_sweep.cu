@@ -352,8 +352,12 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
 
 // --------------------------------------------------------------- S11 corrector ---
 // u = u* - (dt / rho_i) G; r = r* + dt (u - u*); fluid only (Q8).
+// flags != NULL (mps_step carrying rows into the next step): raise carry_bad when a particle moved by
+// more than the rows' margin allows, left the domain (the next BIN would make it a GHOST) or became
+// non-finite -- the next step then bins at r^k as the definition says instead of reusing the rows.
 __global__ void k_correct(KConst kc, double4* __restrict__ pos4, double4* __restrict__ vel4,
-                          const double4* __restrict__ grad4, const uint32_t* __restrict__ tp) {
+                          const double4* __restrict__ grad4, const uint32_t* __restrict__ tp,
+                          DevFlags* __restrict__ flags) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= kc.n) return;
   uint32_t t = tp[i];
@@ -363,9 +367,18 @@ __global__ void k_correct(KConst kc, double4* __restrict__ pos4, double4* __rest
   double ux = __dsub_rn(v.x, __dmul_rn(s, gq.x));
   double uy = __dsub_rn(v.y, __dmul_rn(s, gq.y));
   double uz = __dsub_rn(v.z, __dmul_rn(s, gq.z));
-  r.x = __dadd_rn(r.x, __dmul_rn(kc.dt, __dsub_rn(ux, v.x)));
-  r.y = __dadd_rn(r.y, __dmul_rn(kc.dt, __dsub_rn(uy, v.y)));
-  r.z = __dadd_rn(r.z, __dmul_rn(kc.dt, __dsub_rn(uz, v.z)));
+  const double ex = __dmul_rn(kc.dt, __dsub_rn(ux, v.x)), ey = __dmul_rn(kc.dt, __dsub_rn(uy, v.y));
+  const double ez = __dmul_rn(kc.dt, __dsub_rn(uz, v.z));
+  r.x = __dadd_rn(r.x, ex);
+  r.y = __dadd_rn(r.y, ey);
+  r.z = __dadd_rn(r.z, ez);
+  if (flags) {
+    const double gx = floor((r.x - kc.dmin[0]) * kc.inv_h_dom), gy = floor((r.y - kc.dmin[1]) * kc.inv_h_dom);
+    const double gz = floor((r.z - kc.dmin[2]) * kc.inv_h_dom);
+    const bool in = (gx >= 0.0 && gx < (double)kc.nx_dom) && (gy >= 0.0 && gy < (double)kc.ny_dom) &&
+                    (gz >= 0.0 && gz < (double)kc.nz_dom);
+    if (!(ex * ex + ey * ey + ez * ez <= kc.carry_d2) || !in) flags->carry_bad = 1;  // NaN fails both tests
+  }
   v.x = ux; v.y = uy; v.z = uz;
   vel4[i] = v;
   pos4[i] = r;
@@ -421,6 +434,7 @@ int mpsk_predict(mps_ctx* c) {
   MPS_LAUNCH(c, MPS_T_PREDICT, k_predict, div_up(n, 256), 256, c->kc, c->pos4[cur], c->vel4[cur],
              c->acc4, c->tp[cur]);
   c->binned = false;
+  c->carry_valid = false;
   c->ppe_ready = false;
   return MPS_OK;
 }
@@ -471,8 +485,9 @@ int mpsk_correct(mps_ctx* c) {
   int n = (int)c->n;
   int cur = c->cur;
   MPS_LAUNCH(c, MPS_T_CORRECT, k_correct, div_up(n, 256), 256, c->kc, c->pos4[cur], c->vel4[cur],
-             c->grad4, c->tp[cur]);
+             c->grad4, c->tp[cur], c->carry_rows ? c->flags : nullptr);
   c->binned = false;
+  c->carry_valid = false;  // mps_step sets it again once its own corrector has run
   c->ppe_ready = false;
   return MPS_OK;
 }

@@ -202,6 +202,43 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.grad_variant = prm->grad_variant; k.clamp_negative_p = prm->clamp_negative_p;
   k.rho_pair_mean = prm->rho_pair_mean; k.nu_pair_mean = prm->nu_pair_mean;
   k.n = (int)n;
+  k.inv_h_dom = k.inv_h; k.nx_dom = k.nx; k.ny_dom = k.ny; k.nz_dom = k.nz;
+  k.carry_d2 = 0.0;
+  {
+    // mps_step's own bin (Q26): cells 1/256 larger than the contract's, rows built with a margin of 0.8 of
+    // that slack on both radii.  A 27-cell scan still finds every pair inside the enlarged radius, and
+    // the rows stay exact supersets at r^(k+1) as long as no particle moves by more than 0.45 margins in
+    // the corrector -- which k_correct checks.  GHOST decisions stay on the contract's grid.
+    KConst& s = c->kc_step;
+    s = k;
+    const double hs = c->h * (1.0 + 1.0 / 256.0);
+    const double margin = 0.8 * (hs - c->h) * prm->cell_div;  // slack per radius: cell_div cells cover re_lap
+    s.inv_h = 1.0 / hs;
+    int64_t ncs = 1;
+    int ns[3];
+    for (int a = 0; a < 3; ++a) {
+      ns[a] = std::max(1, (int)ceil(nc[a] * c->h * s.inv_h));  // covers the contract grid's extent
+      ncs *= ns[a];
+    }
+    s.nx = ns[0]; s.ny = ns[1]; s.nz = ns[2];
+    if (prm->key_mode == 1) {
+      int bits = 0;
+      while ((1 << bits) < std::max(ns[0], std::max(ns[1], ns[2]))) ++bits;
+      ncs = (int64_t)1 << (3 * bits);
+    }
+    s.ncells = (int)ncs;
+    s.re_lap2 = (prm->re_lap + margin) * (prm->re_lap + margin);
+    s.re_n2 = (prm->re_n + margin) * (prm->re_n + margin);
+    s.R_lap = std::max(1, (int)ceil((prm->re_lap + margin) * s.inv_h - 1e-9));
+    s.R_n = std::max(1, (int)ceil((prm->re_n + margin) * s.inv_h - 1e-9));
+    k.carry_d2 = s.carry_d2 = (0.45 * margin) * (0.45 * margin);
+    // one bin per step with rows carried across the corrector (off with list reuse, which has its own
+    // schedule, and for small scenes, where the per-step read-back of the validity flag costs more than
+    // the second bin: measured 0.166 vs 0.179 ms per step at 19k particles, 1.10 vs 1.01 at 89k;
+    // MPS_B200_CARRY=0 / 1 forces the two bins per step of reading Q7 as literally stated / the carry)
+    const char* cr = getenv("MPS_B200_CARRY");
+    c->carry_rows = prm->rebin_every == 1 && ncs <= ncells && s.R_lap == k.R_lap && (cr ? atoi(cr) != 0 : n >= 32768);
+  }
 
   // every buffer any later call needs
   cudaError_t e = cudaSuccess;
@@ -359,16 +396,16 @@ void mps_timer_drain(mps_ctx* c) {
 // launch costs one.  The body runs for real when capture is not possible (legacy default stream,
 // timers on) and mutates the same host state either way.
 struct HostState {
-  int cur; bool binned, ppe_ready, posw_is_p; cudaTextureObject_t pos_tex, vel_tex;
+  int cur, stale; bool binned, ppe_ready, posw_is_p; cudaTextureObject_t pos_tex, vel_tex;
   int64_t launches; int64_t t_launches[MPS_NUM_TIMERS];
 };
 static HostState save_state(const mps_ctx* c) {
-  HostState h{c->cur, c->binned, c->ppe_ready, c->posw_is_p, c->kc.pos_tex, c->kc.vel_tex, c->launches, {0}};
+  HostState h{c->cur, c->kc.stale, c->binned, c->ppe_ready, c->posw_is_p, c->kc.pos_tex, c->kc.vel_tex, c->launches, {0}};
   for (int k = 0; k < MPS_NUM_TIMERS; ++k) h.t_launches[k] = c->t_launches[k];
   return h;
 }
 static void restore_state(mps_ctx* c, const HostState& h) {
-  c->cur = h.cur; c->binned = h.binned; c->ppe_ready = h.ppe_ready; c->posw_is_p = h.posw_is_p;
+  c->cur = h.cur; c->kc.stale = h.stale; c->binned = h.binned; c->ppe_ready = h.ppe_ready; c->posw_is_p = h.posw_is_p;
   c->kc.pos_tex = h.pos_tex; c->kc.vel_tex = h.vel_tex; c->launches = h.launches;
   for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] = h.t_launches[k];
 }
@@ -397,12 +434,12 @@ static void run_segment(mps_ctx* c, int route, int which, F&& body) {
       body();
       return;
     }
-    g.cur_after = c->cur; g.binned = c->binned; g.ppe_ready = c->ppe_ready; g.posw_is_p = c->posw_is_p;
+    g.cur_after = c->cur; g.stale = c->kc.stale; g.binned = c->binned; g.ppe_ready = c->ppe_ready; g.posw_is_p = c->posw_is_p;
     g.pos_tex = c->kc.pos_tex; g.vel_tex = c->kc.vel_tex;
     g.launches = c->launches - before.launches;
     for (int k = 0; k < MPS_NUM_TIMERS; ++k) g.t_launches[k] = c->t_launches[k] - before.t_launches[k];
   } else {
-    c->cur = g.cur_after; c->binned = g.binned; c->ppe_ready = g.ppe_ready; c->posw_is_p = g.posw_is_p;
+    c->cur = g.cur_after; c->kc.stale = g.stale; c->binned = g.binned; c->ppe_ready = g.ppe_ready; c->posw_is_p = g.posw_is_p;
     c->kc.pos_tex = g.pos_tex; c->kc.vel_tex = g.vel_tex;
     c->launches += g.launches;
     for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] += g.t_launches[k];
@@ -583,19 +620,40 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       c->kc.stale = 1;
       ++c->reuse_count;
     }
+    // Rows carried over from the last step's bin at r* (margin rows, Q26)?  Only if that step's
+    // corrector left them exact supersets: one small read-back per step.
+    bool carried = false;
+    if (c->carry_rows && c->carry_valid) {
+      CK(cudaMemcpyAsync(&c->flags_host->carry_bad, &c->flags->carry_bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+      CK(cudaStreamSynchronize(c->stream));
+      carried = c->flags_host->carry_bad == 0;
+    }
+    const bool carry = c->carry_rows;
     // everything up to the pressure: one replayable segment (list reuse changes the sequence from
     // step to step and runs its launches directly)
     auto pre = [&]() {
-      // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
-      if (K == 1) mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY);
+      if (K == 1) {
+        if (carried) c->kc.stale = 1;  // the rows are supersets: every sweep re-tests the distance (exact)
+        // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
+        else { c->kc.stale = 0; mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY); }
+      }
       if (ecs) {
         mpsk_density(c);
         mpsk_dndt(c, 1);
       }
       mpsk_viscosity(c);
       mpsk_predict(c);
-      // the explicit route needs only the re_n part at r* (density, p-hat, gradient)
-      if (K == 1) mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
+      if (K == 1) {
+        if (carry) {
+          // the step's one full bin: on the internal grid, with margin rows that the next step's first
+          // sweeps reuse; the explicit route needs the re_lap part for fluid rows only (next viscosity)
+          mpsk_bin(c, route == MPS_ROUTE_EXPLICIT && !ecs ? ROWS_BACK_FLUID : 0, /*step_grid=*/true);
+          c->kc.stale = 1;
+        } else {
+          // the explicit route needs only the re_n part at r* (density, p-hat, gradient)
+          mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
+        }
+      }
       mpsk_density(c);
       if (hs) mpsk_dndt(c, 0);
       if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
@@ -604,13 +662,14 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       mpsk_gradient(c);
       mpsk_correct(c);
     };
-    if (K > 1) pre(); else run_segment(c, route, 0, pre);
+    if (K > 1) pre(); else run_segment(c, route, carried ? 2 : 0, pre);
     if (route == MPS_ROUTE_PPE) {
       // the solve is a cooperative launch of its own, between the two segments
       int rc = mpsk_pressure_ppe(c, /*sync=*/false);  // statistics are read once, after the last step
       if (rc == MPS_ERR_CUDA) return rc;
     }
     if (K > 1) post(); else run_segment(c, route, 1, post);
+    c->carry_valid = carry && K == 1;
     c->stats.steps_total++;
   }
   c->kc.stale = 0;  // API-level sweeps always run on exact rows (they need mps_bin first)
@@ -678,6 +737,7 @@ int mps_upload_host(mps_ctx* c, const double* x, const double* y, const double* 
   c->binned = false;
   c->ppe_ready = false;
   c->reuse_count = 0;  // new particle order: the stored rows are void
+  c->carry_valid = false;
   c->rho_s_ready = false;
   return MPS_OK;
 }
@@ -711,6 +771,7 @@ int mps_set_field(mps_ctx* c, int32_t field, const void* src, int32_t order) {
   if (!c || !src) return MPS_ERR_ARG;
   if (order != MPS_ORDER_ORIGINAL && order != MPS_ORDER_SORTED) return fail(c, MPS_ERR_ARG, "bad order");
   int rc = mpsk_set_field(c, field, src, order);
+  c->carry_valid = false;
   if (rc) return fail(c, rc, "unknown or read-only field id");
   CK(cudaGetLastError());
   return MPS_OK;

@@ -59,6 +59,9 @@ struct DevFlags {
   int nonfinite;      // NaN/Inf position or coincident pair
   int max_row;        // largest r_lap row
   int n_ghost;
+  int carry_bad;      // the last corrector moved a particle too far (or out of the domain) for the rows
+                      // of the step's bin to serve the next step's first sweeps: that step bins again
+  int pad;
 };
 
 struct KConst {  // by-value kernel parameter
@@ -76,6 +79,11 @@ struct KConst {  // by-value kernel parameter
   double inv_re_n, inv_re_lap;
   double dmin[3], inv_h;
   int nx, ny, nz, ncells;
+  // the grid that decides which particles are GHOST (always the contract's grid, h = max r_e / cell_div;
+  // equal to the fields above except in kc_step, whose cells are a little larger)
+  double inv_h_dom;
+  int nx_dom, ny_dom, nz_dom;
+  double carry_d2;  // (0.45 x row margin)^2: the corrector displacement up to which carried rows stay exact
   int R_lap;  // cells to each side for re_lap
   int R_n;    // ... and for re_n
   int key_mode;  // 0: key = c_x + n_x (c_y + n_y c_z); 1: Morton (3 x 10-bit interleave), ncells = 8^bits
@@ -92,7 +100,7 @@ struct KConst {  // by-value kernel parameter
 // state the segment leaves behind, so that a replay can skip the launch code.
 struct StepSeg {
   cudaGraphExec_t exec = nullptr;
-  int cur_after = 0;
+  int cur_after = 0, stale = 0;
   bool binned = false, ppe_ready = false, posw_is_p = false;
   cudaTextureObject_t pos_tex = 0, vel_tex = 0;
   int64_t launches = 0;
@@ -102,6 +110,9 @@ struct StepSeg {
 struct mps_ctx {
   mps_params prm;
   KConst kc;
+  KConst kc_step;   // kc with the internal grid and the margin radii of mps_step's bin (mps_api.cu)
+  bool carry_rows = false;   // mps_step keeps one bin per step and carries its rows into the next step
+  bool carry_valid = false;  // the rows in nbr are margin rows built at the r* of the last step
   int64_t n = 0;
   int64_t n_pad = 0;  // n rounded up to 32
   cudaStream_t stream = nullptr;
@@ -193,7 +204,7 @@ struct mps_ctx {
   int sm_count = 148;
   // mps_step replays its launch sequence from CUDA graphs (one per route, buffer parity and segment)
   // when the ctx has a capturable stream (not the legacy default stream) and timers are off
-  StepSeg seg[2][2][2];
+  StepSeg seg[2][2][4];   // [route][buffer parity][segment: 0 pre (with first bin), 1 post, 2 pre (carried rows)]
   bool graphs_ok = true;
 };
 
@@ -219,7 +230,10 @@ static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); 
 // (all the explicit route needs at r*)
 #define ROWS_FLUID_ONLY 1
 #define ROWS_RN_ONLY 2
-int mpsk_bin(mps_ctx* c, int rows_mode = 0);
+#define ROWS_BACK_FLUID 4   // the re_n part of every row, the rest of the re_lap part for FLUID rows only
+// step_grid: bin on the ctx's internal grid of mps_step (cells 1/256 larger than the contract's) and build
+// rows with a margin (kc_step), so that they stay exact supersets across the corrector
+int mpsk_bin(mps_ctx* c, int rows_mode = 0, bool step_grid = false);
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
                          uint32_t* tmp);
 int mpsk_density(mps_ctx* c);
