@@ -149,6 +149,8 @@ typedef struct mps_stats {
   double cg_loop_ms;        /* ... and the CG iterations alone */
   double cg_loop_ms_total;  /* cg_loop_ms summed over the life of the ctx */
   int64_t cg_nnz;           /* ppe_operator 1: off-diagonal entries of the matrix assembled by the last solve */
+  int64_t bins_total;       /* bins (sort + neighbour rows) run over the life of the ctx: mps_step takes one
+                               per step when it carries its rows across the corrector, two otherwise */
 } mps_stats;
 
 /* mps_init: create a ctx and copy n particles in (device pointers, caller's

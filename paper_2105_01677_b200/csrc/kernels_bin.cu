@@ -892,6 +892,7 @@ int mpsk_bin(mps_ctx* c, int rows_mode, bool step_grid) {
   c->binned = true;
   c->ppe_ready = false;
   c->posw_is_p = false;
+  c->bins_run++;
   return MPS_OK;
 }
 

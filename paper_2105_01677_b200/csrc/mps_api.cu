@@ -365,6 +365,7 @@ static int read_flags(mps_ctx* c) {
     c->err = "a particle has more than max_neighbours neighbours";
   }
   c->stats.device_error = c->sticky_error;
+  c->stats.bins_total = c->bins_run;
   return c->sticky_error;
 }
 
@@ -397,16 +398,16 @@ void mps_timer_drain(mps_ctx* c) {
 // timers on) and mutates the same host state either way.
 struct HostState {
   int cur, stale; bool binned, ppe_ready, posw_is_p; cudaTextureObject_t pos_tex, vel_tex;
-  int64_t launches; int64_t t_launches[MPS_NUM_TIMERS];
+  int64_t launches, bins; int64_t t_launches[MPS_NUM_TIMERS];
 };
 static HostState save_state(const mps_ctx* c) {
-  HostState h{c->cur, c->kc.stale, c->binned, c->ppe_ready, c->posw_is_p, c->kc.pos_tex, c->kc.vel_tex, c->launches, {0}};
+  HostState h{c->cur, c->kc.stale, c->binned, c->ppe_ready, c->posw_is_p, c->kc.pos_tex, c->kc.vel_tex, c->launches, c->bins_run, {0}};
   for (int k = 0; k < MPS_NUM_TIMERS; ++k) h.t_launches[k] = c->t_launches[k];
   return h;
 }
 static void restore_state(mps_ctx* c, const HostState& h) {
   c->cur = h.cur; c->kc.stale = h.stale; c->binned = h.binned; c->ppe_ready = h.ppe_ready; c->posw_is_p = h.posw_is_p;
-  c->kc.pos_tex = h.pos_tex; c->kc.vel_tex = h.vel_tex; c->launches = h.launches;
+  c->kc.pos_tex = h.pos_tex; c->kc.vel_tex = h.vel_tex; c->launches = h.launches; c->bins_run = h.bins;
   for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] = h.t_launches[k];
 }
 template <class F>
@@ -437,11 +438,13 @@ static void run_segment(mps_ctx* c, int route, int which, F&& body) {
     g.cur_after = c->cur; g.stale = c->kc.stale; g.binned = c->binned; g.ppe_ready = c->ppe_ready; g.posw_is_p = c->posw_is_p;
     g.pos_tex = c->kc.pos_tex; g.vel_tex = c->kc.vel_tex;
     g.launches = c->launches - before.launches;
+    g.bins = c->bins_run - before.bins;
     for (int k = 0; k < MPS_NUM_TIMERS; ++k) g.t_launches[k] = c->t_launches[k] - before.t_launches[k];
   } else {
     c->cur = g.cur_after; c->kc.stale = g.stale; c->binned = g.binned; c->ppe_ready = g.ppe_ready; c->posw_is_p = g.posw_is_p;
     c->kc.pos_tex = g.pos_tex; c->kc.vel_tex = g.vel_tex;
     c->launches += g.launches;
+    c->bins_run += g.bins;
     for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] += g.t_launches[k];
   }
   cudaGraphLaunch(g.exec, c->stream);

@@ -104,6 +104,7 @@ struct StepSeg {
   bool binned = false, ppe_ready = false, posw_is_p = false;
   cudaTextureObject_t pos_tex = 0, vel_tex = 0;
   int64_t launches = 0;
+  int64_t bins = 0;
   int64_t t_launches[MPS_NUM_TIMERS] = {0};
 };
 
@@ -194,6 +195,7 @@ struct mps_ctx {
   mps_stats stats{};
   std::string err;
   int64_t launches = 0;
+  int64_t bins_run = 0;
   // timers
   uint32_t timer_mask = 0;  // bit k: time category k with CUDA events
   double t_ms[MPS_NUM_TIMERS] = {0};

@@ -750,3 +750,37 @@ def test_water_drop_trajectory_and_invariant(B, O):
     print(f"  GPU: b doubled after {k} steps, worst ab error {100 * worst:.2f} %")
     assert abs(k * 1e-5 - 8.005e-3) <= 0.06 * 8.005e-3 and worst <= 0.035
     assert g.stats()["n_ghost"] == 0
+
+
+# ---- one bin per step: rows carried across the corrector (reading Q26) ----
+@pytest.mark.parametrize("route", [0, 1])
+@pytest.mark.parametrize("carry", ["1", "0"])
+def test_row_carry_on_and_off_give_the_oracle_trajectory(B, O, route, carry, monkeypatch):
+    """MPS_B200_CARRY=1 forces the carry on a small scene (default: only from 32k particles), =0 the two
+    bins per step of Q7 as literally stated.  Both must follow the oracle; the bin count tells which ran."""
+    monkeypatch.setenv("MPS_B200_CARRY", carry)
+    s = scenes.small_tank(shuffle=True)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, route, cs=0.12)
+    bins = g.stats()["bins_total"]
+    print(f"carry={carry} route={route}: max |dr|/L = {eL:.2e}, bins in 20 steps {bins}")
+    assert eL <= 1e-7
+    assert bins == (21 if carry == "1" else 40)     # 2 in the first step, then 1 per step | 2 per step
+    assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-6
+
+
+@pytest.mark.parametrize("route", [0, 1])
+def test_row_carry_falls_back_when_the_corrector_moves_too_far(B, O, route, monkeypatch):
+    """A corrector displacement beyond the rows' margin (0.45 x 0.8 x re_lap / 256 = 0.0044 l0) must send
+    the next step back to a bin at r^k.  Random velocities of 0.4 m/s compress the small tank enough
+    (pressures of 5-13 kPa) that most steps fall back, and the trajectory still follows the oracle."""
+    monkeypatch.setenv("MPS_B200_CARRY", "1")
+    s = scenes.small_tank(shuffle=True)
+    rng = np.random.default_rng(3)
+    fl = s.type == scenes.FLUID
+    for k in "uvw":
+        getattr(s, k)[fl] = 0.4 * rng.standard_normal(fl.sum())
+    eL, el0, moved, g, o = _trajectory(B, O, s, 12, route)
+    bins = g.stats()["bins_total"]
+    print(f"carry with fallback, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0, bins in 12 steps {bins}")
+    assert eL <= 1e-7 and moved > 0.3
+    assert 13 < bins <= 24                       # more than one per step: the fallback ran
