@@ -57,6 +57,11 @@ def parse_args():
                     help="0 matrix-free, 1 assembled once per solve (library default)")
     ap.add_argument("--warm-start", action="store_true", help="cg_warm_start = 1")
     ap.add_argument("--key-mode", type=int, default=None, choices=[0, 1], help="0 linear cell key, 1 Morton")
+    ap.add_argument("--row-skin", type=float, default=None,
+                    help="Verlet skin of mps_step's rows in units of l0 (library default 0.2; < 0: two bins per step)")
+    ap.add_argument("--pre-steps", type=int, default=0,
+                    help="untimed steps before the warm-up (0: the timed window starts W steps from rest, as BASELINE.json's "
+                         "workloads do; e.g. 400 puts it in the developed dam-break flow)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-replay", action="store_true", help="skip the instrumented per-kernel replay")
@@ -94,6 +99,8 @@ def make_scene(args, rank=0):
     if getattr(args, "rebin_every", 1) > 1:
         s.params["rebin_every"] = int(args.rebin_every)
         s.name += f"_reuse{args.rebin_every}"
+    if getattr(args, "row_skin", None) is not None:
+        s.params["row_skin"] = float(args.row_skin)
     return s, route
 
 
@@ -305,6 +312,8 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
         # nvidia-smi's start-up, and both are the same load
         sampler = ClockSampler(gpu_id)
         sampler.start()
+    if getattr(args, "pre_steps", 0) > 0:
+        g.step(int(args.pre_steps), route)
     g.step(max(W, 3), route)
     if sample_clocks:
         t_end = time.perf_counter() + 0.5
@@ -327,6 +336,7 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
     N, rows, kn, kl, klr = scene.n, ns["rows"], ns["kn"], ns["kl"], ns["klr"]
     asm = int(scene.params.get("ppe_operator", 1)) == 1
     out = {"value": value, "ms_per_step": ms_total / K, "gpu_launches": int(launches), "clocks": clocks,
+           "bins_per_step": (stats["bins_total"] - st0["bins_total"]) / K,
            "fluid_particle_steps_per_sec": value * scene.n_fluid / scene.n,
            "units": {"N": N, "ppe_rows": rows, "mean_k_re_n": kn, "mean_k_re_lap": kl, "mean_k_re_lap_rows": klr}}
     cg = None
@@ -352,14 +362,17 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
 
     # ---- instrumented replay of the same steps: per-kernel CUDA-event times ------------------
     g = B.Mps(scene, device=str(dev))
-    g.step(W, route)
+    g.step(W + int(getattr(args, "pre_steps", 0)), route)
+    bins0 = g.stats()["bins_total"]
     g.timers_enable((1 << len(B.TIMERS)) - 1)
     ms_replay = timed_steps(torch, 1, g, route, K, flush, stream)
     tm = g.timers_read()
     g.timers_enable(0)
+    # bins that ran (with a skin the bin kernels are launched twice per step and return at once unless the
+    # device flag is up: the launch count is not the bin count)
+    n_bins = max(int(g.stats()["bins_total"] - bins0), 1)
     g.close()
     peak, peak_src = peaks()
-    n_bins = tm["bin_list"][1]          # one row-builder launch per bin (2 per step; fewer with list reuse)
     kernels = {}
     for cat, (ms, ln) in tm.items():
         if ln == 0:
@@ -523,10 +536,11 @@ def run_b200(args):
                                            if args.config <= 5 else
                                            "none: the paper's own 2D dam-break shape (PAPER.md:397), context only"),
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
-                       "options": {k: scene.params.get(k) for k in ("ppe_operator", "cg_warm_start", "key_mode", "cell_div", "rebin_every")},
+                       "options": {k: scene.params.get(k) for k in ("ppe_operator", "cg_warm_start", "key_mode", "cell_div", "rebin_every", "row_skin")},
+                       "pre_steps": int(getattr(args, "pre_steps", 0)),
                        "l2": "flushed before every timed step (256 MiB write, untimed)",
                        "timing": "CUDA events on the ctx stream around each mps_step(1), summed; max over ranks"},
-            "gpu_launches": main["gpu_launches"], "clocks": main["clocks"],
+            "gpu_launches": main["gpu_launches"], "clocks": main["clocks"], "bins_per_step": main["bins_per_step"],
             "fluid_particle_steps_per_sec": main["fluid_particle_steps_per_sec"],
             "roofline": main["roofline"], "kernels": main["kernels"], "units": main["units"],
             "e2e": e2e, "cpu_baseline": cpu,

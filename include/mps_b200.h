@@ -26,7 +26,7 @@
  *    of the matrix-free gathers off, MPS_B200_CG_TIMEOUT_CYCLES=<n> sets the spin limit of the
  *    grid barrier inside the persistent CG kernel (default 4e9 SM cycles, 0 = no limit; raise it
  *    or set 0 under compute-sanitizer or a debugger), MPS_B200_CARRY=0 makes mps_step bin twice per
- *    step instead of carrying the rows of its one bin across the corrector (see mps_step).
+ *    step as if row_skin < 0 (see mps_step).
  */
 #ifndef MPS_B200_H
 #define MPS_B200_H
@@ -130,6 +130,12 @@ typedef struct mps_params {
   double n0_n;              /* 0 => lattice closed form (Q1) */
   double n0_lap;            /* 0 => lattice closed form */
   double lambda;            /* 0 => lattice closed form */
+  double row_skin;          /* Verlet skin of mps_step's neighbour rows in units of l0 (Q26): the rows are built
+                               with both radii enlarged by row_skin * l0 and serve every sweep -- each re-tests
+                               r2 < re^2 with the rounding of Q2, so the sets stay exact -- until some particle has
+                               moved by more than 0.45 skins since the build (checked on the device by the predictor
+                               and the corrector).  0 => the library's default (0.2); < 0 => no skin: mps_step
+                               bins at r^k and at r* in every step, as Q7 is literally stated */
 } mps_params;
 
 typedef struct mps_stats {
@@ -149,8 +155,8 @@ typedef struct mps_stats {
   double cg_loop_ms;        /* ... and the CG iterations alone */
   double cg_loop_ms_total;  /* cg_loop_ms summed over the life of the ctx */
   int64_t cg_nnz;           /* ppe_operator 1: off-diagonal entries of the matrix assembled by the last solve */
-  int64_t bins_total;       /* bins (sort + neighbour rows) run over the life of the ctx: mps_step takes one
-                               per step when it carries its rows across the corrector, two otherwise */
+  int64_t bins_total;       /* bins (sort + neighbour rows) run over the life of the ctx: two per step of mps_step
+                               without a skin; with one (row_skin), only when a particle has moved 0.45 skins */
 } mps_stats;
 
 /* mps_init: create a ctx and copy n particles in (device pointers, caller's
@@ -231,13 +237,16 @@ int mps_correct(mps_ctx* ctx);
 
 /* mps_step: nsteps times { bin, [ppe_source 2: density, dndt(keep)], viscosity, predict, bin,
  * density, [ppe_source >= 1: dndt], pressure (route), gradient, correct }.  Every sweep sees the exact
- * neighbour set of the positions it works at (Q7).  How the library gets there (Q26): the bin at r* runs
- * on an internal grid whose cells are 1/256 larger than mps_bin's and builds rows with a margin of 0.8 of
- * that slack; every sweep re-tests r2 < re^2 with the rounding of Q2, so the sets are exact, and the same
- * rows serve the first sweeps of the NEXT step at r^(k+1) when the corrector moved no particle by more
- * than 0.45 margins and none left the domain (checked on the device; one 4-byte read-back per step) --
- * otherwise, and in the first step, that step bins at r^k as written above.  GHOST decisions always use
- * mps_bin's grid.  The launches of a step are replayed from CUDA graphs when the ctx has its own stream.
+ * neighbour set of the positions it works at (Q7).  How the library gets there (Q26): a bin of mps_step
+ * runs on an internal grid with cells of (max re + skin) / cell_div and builds rows with both radii
+ * enlarged by the skin (row_skin * l0), and remembers the positions it was made at.  Every sweep re-tests
+ * r2 < re^2 with the rounding of Q2, so the sets are exact as long as no particle is further than 0.45
+ * skins from its position at the build.  The predictor and the corrector check exactly that for every
+ * particle they move (and that none left the domain or became non-finite) and raise a flag ON THE DEVICE;
+ * the kernels of the two bins of a step are always launched and return at once unless the flag is up, so
+ * the host never waits for the device inside mps_step.  GHOST decisions always use mps_bin's grid.
+ * The launches of a step are replayed from CUDA graphs when the ctx has its own stream.  With
+ * row_skin < 0 both bins run in every step on mps_bin's grid with the exact radii.
  * Returns the first error met. */
 int mps_step(mps_ctx* ctx, int32_t nsteps, int32_t pressure_route);
 
@@ -277,7 +286,9 @@ int mps_get_grid(mps_ctx* ctx, int32_t* grid);
 int mps_get_cell_start(mps_ctx* ctx, uint32_t* dst);
 /* Neighbour sets of the last mps_bin as CSR in ORIGINAL numbering, each row
  * ascending: counts[i] (DEVICE, n x uint32) and, if idx != NULL, the first cap
- * entries of the concatenated rows (DEVICE).  *total (HOST) = number of entries. */
+ * entries of the concatenated rows (DEVICE).  *total (HOST) = number of entries.
+ * After mps_step with a skin: the sets at the CURRENT positions as the next sweep would see them
+ * (the stored rows filtered by the re-test), provided the rows are still valid -- else MPS_ERR_ORDER. */
 int mps_get_neighbours(mps_ctx* ctx, int32_t radius_id, uint32_t* counts, uint32_t* idx,
                        int64_t cap, int64_t* total);
 /* y = A x with the operator and flags of the last mps_pressure_ppe (DEVICE, n doubles each). */

@@ -55,6 +55,7 @@ class MpsParams(C.Structure):
         ("ppe_relax", C.c_double), ("cg_rtol", C.c_double), ("cs", C.c_double),
         ("domain_min", C.c_double * 3), ("domain_max", C.c_double * 3),
         ("n0_n", C.c_double), ("n0_lap", C.c_double), ("lambda_", C.c_double),
+        ("row_skin", C.c_double),
     ]
 
 
@@ -96,6 +97,7 @@ def make_params(p: Dict[str, object]) -> MpsParams:
         setattr(s, k, float(p[k]))
     s.re_grad = float(p.get("re_grad", p["re_n"]))
     s.lambda_ = float(p["lam"])
+    s.row_skin = float(p.get("row_skin", 0.0))
     for k, m in (("g", 3), ("rho", 2), ("nu", 2), ("domain_min", 3), ("domain_max", 3)):
         arr = getattr(s, k)
         for i in range(m):

@@ -10,6 +10,10 @@ namespace {
 
 constexpr int TPB = 256;
 
+// A bin of mps_step with a skin is launched in every step and runs only when the device flag *go is up
+// (raised by the predictor or the corrector); go == NULL: run.  Uniform over the grid.
+__device__ __forceinline__ bool skipped(const int* go) { return go != nullptr && *(const volatile int*)go == 0; }
+
 // ---------------------------------------------------------------- load / io ---
 __global__ void k_load(int n, const double* __restrict__ x, const double* __restrict__ y,
                        const double* __restrict__ z, const double* __restrict__ u,
@@ -66,8 +70,10 @@ __device__ __forceinline__ void key_cell(const KConst& kc, uint32_t k, int& cx, 
 // canonical order (ascending original index) is restored in k_reorder.
 __global__ void k_keys(KConst kc, const double4* __restrict__ pos4, uint32_t* __restrict__ tp,
                        uint32_t* __restrict__ key_tmp, uint32_t* __restrict__ rank,
-                       uint32_t* __restrict__ cell_count, DevFlags* __restrict__ flags) {
+                       uint32_t* __restrict__ cell_count, DevFlags* __restrict__ flags, const int* go) {
+  if (skipped(go)) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (go && i == 0) atomicAdd(&flags->bins, 1);
   bool live = i < kc.n;
   uint32_t key = 0xffffffffu;
   if (live) {
@@ -136,7 +142,9 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
   return off + inc - v;
 }
 
-__global__ void k_scan_reduce(const uint32_t* __restrict__ in, int64_t n, uint32_t* __restrict__ tile_sum) {
+__global__ void k_scan_reduce(const uint32_t* __restrict__ in, int64_t n, uint32_t* __restrict__ tile_sum,
+                              const int* go) {
+  if (skipped(go)) return;
   int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
   uint32_t s = 0;
 #pragma unroll
@@ -148,7 +156,8 @@ __global__ void k_scan_reduce(const uint32_t* __restrict__ in, int64_t n, uint32
   block_exclusive_scan(s, &tot);
   if (threadIdx.x == 0) tile_sum[blockIdx.x] = tot;
 }
-__global__ void k_scan_spine(uint32_t* __restrict__ tile_sum, int ntiles) {
+__global__ void k_scan_spine(uint32_t* __restrict__ tile_sum, int ntiles, const int* go) {
+  if (skipped(go)) return;
   uint32_t carry = 0;
   for (int base = 0; base < ntiles; base += TPB) {
     int i = base + threadIdx.x;
@@ -160,7 +169,8 @@ __global__ void k_scan_spine(uint32_t* __restrict__ tile_sum, int ntiles) {
   }
 }
 __global__ void k_scan_apply(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int64_t n,
-                             const uint32_t* __restrict__ tile_off) {
+                             const uint32_t* __restrict__ tile_off, const int* go) {
+  if (skipped(go)) return;
   int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
   uint32_t v[SCAN_ITEMS];
   uint32_t s = 0;
@@ -181,7 +191,8 @@ __global__ void k_scan_apply(const uint32_t* __restrict__ in, uint32_t* __restri
 // Small inputs (a few tiles): the whole scan in ONE block, tile after tile with a running carry
 // -- one launch instead of three.
 __global__ void __launch_bounds__(TPB) k_scan_small(const uint32_t* __restrict__ in,
-                                                    uint32_t* __restrict__ out, int64_t n) {
+                                                    uint32_t* __restrict__ out, int64_t n, const int* go) {
+  if (skipped(go)) return;
   uint32_t carry = 0;
   for (int64_t tile = 0; tile < n; tile += SCAN_TILE) {
     const int64_t base = tile + (int64_t)threadIdx.x * SCAN_ITEMS;
@@ -207,11 +218,12 @@ __global__ void __launch_bounds__(TPB) k_scan_small(const uint32_t* __restrict__
 __global__ void k_scatter(int n, const uint32_t* __restrict__ key_tmp, const uint32_t* __restrict__ rank,
                           const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ oid,
                           uint32_t* __restrict__ tmp_src, uint32_t* __restrict__ tmp_oid,
-                          uint32_t* __restrict__ key, int ncells, DevFlags* __restrict__ flags) {
+                          uint32_t* __restrict__ key, int ncells, DevFlags* __restrict__ flags, const int* go) {
+  if (skipped(go)) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) {
     flags->n_ghost = n - (int)cell_start[ncells];  // ghosts sit behind the last cell
-    flags->carry_bad = 0;                          // raised again by this step's corrector if need be
+    if (go) flags->max_row = 0;                    // the row builder of this bin raises it again
   }
   if (i >= n) return;
   uint32_t k = key_tmp[i];
@@ -232,7 +244,8 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
                           uint32_t* __restrict__ tp_out, uint32_t* __restrict__ oid_out,
                           uint32_t* __restrict__ ent_out, const double2* __restrict__ keep_in,
                           double2* __restrict__ keep_out, const double* __restrict__ rs_in,
-                          double* __restrict__ rs_out, int carry_w) {
+                          double* __restrict__ rs_out, int carry_w, const int* go) {
+  if (skipped(go)) return;
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   uint32_t c = key[s];
@@ -255,6 +268,27 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
   // the neighbour-row entry that names this particle (flags of mps_internal.h)
   ent_out[f] = f | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
                ((tj & 0x100) ? NB_PHASE1 : 0u);
+}
+
+// The bin of mps_step with a skin leaves the sorted particles in the buffers they came from (so that no
+// pointer on the host depends on whether the bin ran) and records the positions the rows are built at.
+__global__ void k_commit(int n, const double4* __restrict__ pos_s, const double4* __restrict__ vel_s,
+                         const uint32_t* __restrict__ tp_s, const uint32_t* __restrict__ oid_s,
+                         const double2* __restrict__ keep_s, const double* __restrict__ rs_s,
+                         double4* __restrict__ pos, double4* __restrict__ vel, uint32_t* __restrict__ tp,
+                         uint32_t* __restrict__ oid, double2* __restrict__ keep, double* __restrict__ rs,
+                         double4* __restrict__ pos_ref, const int* go) {
+  if (skipped(go)) return;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double4 q = pos_s[i];
+  pos[i] = q;
+  pos_ref[i] = q;
+  vel[i] = vel_s[i];
+  tp[i] = tp_s[i];
+  oid[i] = oid_s[i];
+  if (keep) keep[i] = keep_s[i];
+  if (rs) rs[i] = rs_s[i];
 }
 
 // ------------------------------------------------ S3: neighbour rows (the sweep) ---
@@ -306,7 +340,9 @@ k_build_rows_warp(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
              const uint32_t* __restrict__ ent, const uint32_t* __restrict__ key,
              const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
              uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags,
-             int fluid_only) {
+             int mode, const int* go) {
+  if (skipped(go)) return;
+  const int fluid_only = mode & ROWS_FLUID_ONLY;
   const int lane = threadIdx.x & 31;
   const int warp = (blockIdx.x * ROWS_TPB + threadIdx.x) >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
@@ -455,7 +491,8 @@ __global__ void __launch_bounds__(LEAN_TPB)
 k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
              const uint32_t* __restrict__ key, const uint32_t* __restrict__ cell_start,
              uint32_t* __restrict__ nbr, uint32_t* __restrict__ cn, uint32_t* __restrict__ co,
-             DevFlags* __restrict__ flags, int mode) {
+             DevFlags* __restrict__ flags, int mode, const int* go) {
+  if (skipped(go)) return;
   const int lane = threadIdx.x & 31;
   const int warp = (blockIdx.x * LEAN_TPB + threadIdx.x) >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
@@ -593,7 +630,8 @@ __global__ void __launch_bounds__(CELL_TPB, 4)
 k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
                   const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
                   uint32_t* __restrict__ cn, uint32_t* __restrict__ co, DevFlags* __restrict__ flags,
-                  int mode) {
+                  int mode, const int* go) {
+  if (skipped(go)) return;
   const bool fluid_only = (mode & ROWS_FLUID_ONLY) != 0, rn_only = (mode & ROWS_RN_ONLY) != 0;
   __shared__ uint32_t buf[2][CELL_WARPS][8][32];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -811,6 +849,48 @@ __global__ void k_nb_counts(int n, int radius_id, const uint32_t* __restrict__ c
   if (i >= n) return;
   counts[oid[i]] = cn[i] + (radius_id == MPS_RADIUS_LAP ? co[i] : 0u);
 }
+// Skin rows (mps_step): the set a sweep sees is the stored row filtered by the re-test at the current
+// positions.  GHOST rows are empty.
+__device__ __forceinline__ bool nb_keep(const double4* pos4, int i, uint32_t e, double re2) {
+  return r2_exact(pos4[e & NB_INDEX], pos4[i]) < re2;
+}
+__global__ void k_nb_counts_skin(int n, int cap_row, double re2, int lap, const double4* __restrict__ pos4,
+                                 const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
+                                 const uint32_t* __restrict__ cn, const uint32_t* __restrict__ co,
+                                 const uint32_t* __restrict__ oid, uint32_t* __restrict__ counts) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t* row = nbr + (size_t)i * (size_t)cap_row;
+  const uint32_t nf = cn[i], m = nf + (lap ? co[i] : 0u);
+  uint32_t k_ = 0;
+  if ((tp[i] & 0xff) != MPS_GHOST)
+    for (uint32_t k = 0; k < m; ++k) {
+      const uint32_t e = (k < nf) ? row[k] : row[back_slot(cap_row, k - nf)];
+      if (nb_keep(pos4, i, e, re2)) ++k_;
+    }
+  counts[oid[i]] = k_;
+}
+__global__ void k_nb_fill_skin(int n, int cap_row, double re2, int lap, const double4* __restrict__ pos4,
+                               const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
+                               const uint32_t* __restrict__ cn, const uint32_t* __restrict__ co,
+                               const uint32_t* __restrict__ oid, const uint32_t* __restrict__ offs,
+                               uint32_t* __restrict__ idx, int64_t cap) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n || (tp[i] & 0xff) == MPS_GHOST) return;
+  const uint32_t* row = nbr + (size_t)i * (size_t)cap_row;
+  const uint32_t nf = cn[i], m = nf + (lap ? co[i] : 0u);
+  const int64_t base = offs[oid[i]];
+  int64_t w = base;
+  for (uint32_t k = 0; k < m; ++k) {
+    const uint32_t e = (k < nf) ? row[k] : row[back_slot(cap_row, k - nf)];
+    if (!nb_keep(pos4, i, e, re2)) continue;
+    if (w >= cap) return;  // caller's buffer too small: the row is cut
+    const uint32_t v = oid[e & NB_INDEX];
+    int64_t t = w++;
+    while (t > base && idx[t - 1] > v) { idx[t] = idx[t - 1]; --t; }
+    idx[t] = v;
+  }
+}
 __global__ void k_nb_fill(int n, int cap_row, int radius_id, const uint32_t* __restrict__ nbr,
                           const uint32_t* __restrict__ cn, const uint32_t* __restrict__ co,
                           const uint32_t* __restrict__ oid, const uint32_t* __restrict__ offs,
@@ -836,15 +916,15 @@ __global__ void k_nb_fill(int n, int cap_row, int radius_id, const uint32_t* __r
 
 // ============================================================ host launchers ===
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
-                         uint32_t* tmp) {
+                         uint32_t* tmp, const int* go) {
   int ntiles = div_up(n, SCAN_TILE);
   if (ntiles <= 16) {  // up to 32k entries: one block is faster than three launches
-    MPS_LAUNCH(c, cat, k_scan_small, 1, TPB, in, out, n);
+    MPS_LAUNCH(c, cat, k_scan_small, 1, TPB, in, out, n, go);
     return;
   }
-  MPS_LAUNCH(c, cat, k_scan_reduce, ntiles, TPB, in, n, tmp);
-  MPS_LAUNCH(c, cat, k_scan_spine, 1, TPB, tmp, ntiles);
-  MPS_LAUNCH(c, cat, k_scan_apply, ntiles, TPB, in, out, n, tmp);
+  MPS_LAUNCH(c, cat, k_scan_reduce, ntiles, TPB, in, n, tmp, go);
+  MPS_LAUNCH(c, cat, k_scan_spine, 1, TPB, tmp, ntiles, go);
+  MPS_LAUNCH(c, cat, k_scan_apply, ntiles, TPB, in, out, n, tmp, go);
 }
 
 int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const double* z,
@@ -856,43 +936,54 @@ int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const doub
   return MPS_OK;
 }
 
-int mpsk_bin(mps_ctx* c, int rows_mode, bool step_grid) {
-  const int fo = (rows_mode & ROWS_FLUID_ONLY) ? 1 : 0;
+int mpsk_bin(mps_ctx* c, int rows_mode, const int* go) {
   const int n = (int)c->n;
-  const KConst& kg = step_grid ? c->kc_step : c->kc;
+  const KConst& kg = go ? c->kc_step : c->kc;
   const int nc = kg.ncells;
   const int cur = c->cur, nxt = cur ^ 1;
   cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * (nc + 2), c->stream);
-  cudaMemsetAsync(&c->flags->max_row, 0, sizeof(int), c->stream);
+  if (!go) cudaMemsetAsync(&c->flags->max_row, 0, sizeof(int), c->stream);  // predicated: k_scatter does it
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_keys, div_up(n, TPB), TPB, kg, c->pos4[cur], c->tp[cur],
-             c->key_tmp, c->rank, c->cell_count, c->flags);
-  mpsk_exclusive_scan(c, MPS_T_BIN_SORT, c->cell_count, c->cell_start, nc + 2, c->scan_tmp);
+             c->key_tmp, c->rank, c->cell_count, c->flags, go);
+  mpsk_exclusive_scan(c, MPS_T_BIN_SORT, c->cell_count, c->cell_start, nc + 2, c->scan_tmp, go);
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_scatter, div_up(n, TPB), TPB, n, c->key_tmp, c->rank,
-             c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key, nc, c->flags);
+             c->cell_start, c->oid[cur], c->tmp_src, c->tmp_oid, c->key, nc, c->flags, go);
+  const bool keep = c->prm.ppe_source == 2, rs = c->prm.grad_variant == 3;
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_reorder, div_up(n, TPB), TPB, n, nc, c->key, c->cell_start,
              c->tmp_src, c->tmp_oid, c->pos4[cur], c->vel4[cur], c->tp[cur], c->pos4[nxt],
              c->vel4[nxt], c->tp[nxt], c->oid[nxt], c->ent,
-             c->prm.ppe_source == 2 ? c->keep2[cur] : nullptr, c->keep2[nxt],
-             c->prm.grad_variant == 3 ? c->rho_s[cur] : nullptr, c->rho_s[nxt], c->prm.cg_warm_start);
-  c->cur = nxt;
-  c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
-  c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;
-  c->carry_valid = false;
+             keep ? c->keep2[cur] : nullptr, c->keep2[nxt],
+             rs ? c->rho_s[cur] : nullptr, c->rho_s[nxt], go ? 1 : c->prm.cg_warm_start, go);
+  int at = nxt;
+  if (go) {
+    // back into the current buffers (the host cannot know whether this bin ran) + the build positions
+    MPS_LAUNCH(c, MPS_T_BIN_SORT, k_commit, div_up(n, TPB), TPB, n, c->pos4[nxt], c->vel4[nxt], c->tp[nxt],
+               c->oid[nxt], c->keep2[nxt], c->rho_s[nxt], c->pos4[cur], c->vel4[cur], c->tp[cur], c->oid[cur],
+               keep ? c->keep2[cur] : nullptr, rs ? c->rho_s[cur] : nullptr, c->pos_ref, go);
+    at = cur;
+  } else {
+    c->cur = nxt;
+    c->kc.pos_tex = c->cg_tex ? c->pos_tex[nxt] : 0;
+    c->kc.vel_tex = c->cg_tex ? c->vel_tex[nxt] : 0;
+    c->carry_valid = false;
+  }
   if (c->rows_builder == 0) {
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (LEAN_TPB / 32) * LEAN_PPW), LEAN_TPB, kg, c->pos4[nxt],
-               c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode);
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (LEAN_TPB / 32) * LEAN_PPW), LEAN_TPB, kg, c->pos4[at],
+               c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
   } else if (c->prm.cell_div == 1 && c->rows_builder == 2) {
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, kg, c->pos4[nxt],
-               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode);
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, kg, c->pos4[at],
+               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
   } else {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, kg,
-               c->pos4[nxt], c->tp[nxt], c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, fo);
+               c->pos4[at], c->tp[at], c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
   }
-  c->binned = true;
+  if (!go) {
+    c->binned = true;
+    c->bins_run++;
+  }
   c->ppe_ready = false;
   c->posw_is_p = false;
-  c->bins_run++;
   return MPS_OK;
 }
 
@@ -952,6 +1043,13 @@ int mpsk_get_neighbours(mps_ctx* c, int radius_id, uint32_t* counts, uint32_t* i
                         int64_t* total) {
   int n = (int)c->n;
   int cur = c->cur;
+  const bool skin = !c->binned;  // the caller has checked that the skin rows are valid
+  const double re2 = radius_id == MPS_RADIUS_LAP ? c->kc.re_lap2 : c->kc.re_n2;
+  const int lap = radius_id == MPS_RADIUS_LAP;
+  if (skin)
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_counts_skin, div_up(n, TPB), TPB, n, c->kc.stride, re2, lap, c->pos4[cur],
+               c->tp[cur], c->nbr, c->cn, c->co, c->oid[cur], counts);
+  else
   MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_counts, div_up(n, TPB), TPB, n, radius_id, c->cn, c->co,
              c->oid[cur], counts);
   // offsets in original order: scan into tmp_src (n entries; free between bins)
@@ -961,7 +1059,10 @@ int mpsk_get_neighbours(mps_ctx* c, int radius_id, uint32_t* counts, uint32_t* i
   cudaMemcpyAsync(&last_cnt, counts + (n - 1), 4, cudaMemcpyDeviceToHost, c->stream);
   cudaStreamSynchronize(c->stream);
   if (total) *total = (int64_t)last_off + last_cnt;
-  if (idx) {
+  if (idx && skin) {
+    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_fill_skin, div_up(n, TPB), TPB, n, c->kc.stride, re2, lap, c->pos4[cur],
+               c->tp[cur], c->nbr, c->cn, c->co, c->oid[cur], c->tmp_src, idx, cap);
+  } else if (idx) {
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_nb_fill, div_up(n, TPB), TPB, n, c->kc.stride, radius_id, c->nbr,
                c->cn, c->co, c->oid[cur], c->tmp_src, idx, cap);
   }

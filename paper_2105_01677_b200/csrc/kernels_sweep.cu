@@ -208,11 +208,26 @@ k_viscosity(KConst kc, const double4* __restrict__ pos4, const double4* __restri
   }
 }
 
+// Skin rows of mps_step (Q26): do they still cover position r of a particle whose rows were built at ref?
+// Yes while |r - ref| <= 0.45 skins, r is inside the domain (else the next BIN makes it a GHOST) and finite.
+__device__ __forceinline__ bool rows_cover(const KConst& kc, const double4& r, const double4& ref) {
+  const double ex = r.x - ref.x, ey = r.y - ref.y, ez = r.z - ref.z;
+  const double gx = floor((r.x - kc.dmin[0]) * kc.inv_h_dom), gy = floor((r.y - kc.dmin[1]) * kc.inv_h_dom);
+  const double gz = floor((r.z - kc.dmin[2]) * kc.inv_h_dom);
+  const bool in = (gx >= 0.0 && gx < (double)kc.nx_dom) && (gy >= 0.0 && gy < (double)kc.ny_dom) &&
+                  (gz >= 0.0 && gz < (double)kc.nz_dom);
+  return (ex * ex + ey * ey + ez * ez <= kc.carry_d2) && in;  // NaN fails the first test
+}
+
 // -------------------------------------------------------------- S7 predictor ---
 // u* = u + dt a; r* = r + dt u*; fluid only (Q8).
+// flags != NULL (mps_step with a skin): lower need_k (the bin at r^k, if any, has run) and raise need_star
+// when the rows do not cover some r*: the predicated bin that follows then runs.
 __global__ void k_predict(KConst kc, double4* __restrict__ pos4, double4* __restrict__ vel4,
-                          const double4* __restrict__ acc4, const uint32_t* __restrict__ tp) {
+                          const double4* __restrict__ acc4, const uint32_t* __restrict__ tp,
+                          const double4* __restrict__ pos_ref, DevFlags* __restrict__ flags) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (flags && i == 0) flags->need_k = 0;
   if (i >= kc.n) return;
   if ((tp[i] & 0xff) != MPS_FLUID) return;
   double4 v = vel4[i], a = acc4[i], r = pos4[i];
@@ -224,6 +239,7 @@ __global__ void k_predict(KConst kc, double4* __restrict__ pos4, double4* __rest
   r.z = __dadd_rn(r.z, __dmul_rn(kc.dt, v.z));
   vel4[i] = v;
   pos4[i] = r;
+  if (flags && !rows_cover(kc, r, pos_ref[i])) flags->need_star = 1;
 }
 
 // ----------------------------------------------------- S8a equation of state ---
@@ -352,13 +368,13 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
 
 // --------------------------------------------------------------- S11 corrector ---
 // u = u* - (dt / rho_i) G; r = r* + dt (u - u*); fluid only (Q8).
-// flags != NULL (mps_step carrying rows into the next step): raise carry_bad when a particle moved by
-// more than the rows' margin allows, left the domain (the next BIN would make it a GHOST) or became
-// non-finite -- the next step then bins at r^k as the definition says instead of reusing the rows.
+// flags != NULL (mps_step with a skin): lower need_star and raise need_k when the rows do not cover some
+// r^(k+1): the predicated bin at the start of the next step then runs.
 __global__ void k_correct(KConst kc, double4* __restrict__ pos4, double4* __restrict__ vel4,
                           const double4* __restrict__ grad4, const uint32_t* __restrict__ tp,
-                          DevFlags* __restrict__ flags) {
+                          const double4* __restrict__ pos_ref, DevFlags* __restrict__ flags) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (flags && i == 0) flags->need_star = 0;
   if (i >= kc.n) return;
   uint32_t t = tp[i];
   if ((t & 0xff) != MPS_FLUID) return;
@@ -372,13 +388,7 @@ __global__ void k_correct(KConst kc, double4* __restrict__ pos4, double4* __rest
   r.x = __dadd_rn(r.x, ex);
   r.y = __dadd_rn(r.y, ey);
   r.z = __dadd_rn(r.z, ez);
-  if (flags) {
-    const double gx = floor((r.x - kc.dmin[0]) * kc.inv_h_dom), gy = floor((r.y - kc.dmin[1]) * kc.inv_h_dom);
-    const double gz = floor((r.z - kc.dmin[2]) * kc.inv_h_dom);
-    const bool in = (gx >= 0.0 && gx < (double)kc.nx_dom) && (gy >= 0.0 && gy < (double)kc.ny_dom) &&
-                    (gz >= 0.0 && gz < (double)kc.nz_dom);
-    if (!(ex * ex + ey * ey + ez * ez <= kc.carry_d2) || !in) flags->carry_bad = 1;  // NaN fails both tests
-  }
+  if (flags && !rows_cover(kc, r, pos_ref[i])) flags->need_k = 1;
   v.x = ux; v.y = uy; v.z = uz;
   vel4[i] = v;
   pos4[i] = r;
@@ -431,8 +441,9 @@ int mpsk_viscosity(mps_ctx* c) {
 int mpsk_predict(mps_ctx* c) {
   int n = (int)c->n;
   int cur = c->cur;
+  const bool skin = c->kc.stale && c->carry_rows && c->prm.rebin_every == 1;  // inside mps_step with a skin
   MPS_LAUNCH(c, MPS_T_PREDICT, k_predict, div_up(n, 256), 256, c->kc, c->pos4[cur], c->vel4[cur],
-             c->acc4, c->tp[cur]);
+             c->acc4, c->tp[cur], c->pos_ref, skin ? c->flags : nullptr);
   c->binned = false;
   c->carry_valid = false;
   c->ppe_ready = false;
@@ -484,8 +495,9 @@ int mpsk_gradient(mps_ctx* c) {
 int mpsk_correct(mps_ctx* c) {
   int n = (int)c->n;
   int cur = c->cur;
+  const bool skin = c->kc.stale && c->carry_rows && c->prm.rebin_every == 1;  // inside mps_step with a skin
   MPS_LAUNCH(c, MPS_T_CORRECT, k_correct, div_up(n, 256), 256, c->kc, c->pos4[cur], c->vel4[cur],
-             c->grad4, c->tp[cur], c->carry_rows ? c->flags : nullptr);
+             c->grad4, c->tp[cur], c->pos_ref, skin ? c->flags : nullptr);
   c->binned = false;
   c->carry_valid = false;  // mps_step sets it again once its own corrector has run
   c->ppe_ready = false;

@@ -72,7 +72,7 @@ static void free_all(mps_ctx* c) {
   }
   cudaFree(c->ent); cudaFree(c->key); cudaFree(c->key_tmp); cudaFree(c->rank); cudaFree(c->tmp_src);
   cudaFree(c->tmp_oid); cudaFree(c->cell_count); cudaFree(c->cell_start); cudaFree(c->scan_tmp);
-  cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co);
+  cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co); cudaFree(c->pos_ref);
   cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
   cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->rho_s[0]); cudaFree(c->rho_s[1]); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
   cudaFree(c->cg_x); cudaFree(c->cg_p); cudaFree(c->cg_s); cudaFree(c->cg_w); cudaFree(c->cg_part);
@@ -110,6 +110,7 @@ static int check_params(const mps_params* p, int64_t n) {
     return fail(nullptr, MPS_ERR_ARG, "ppe_operator 1 stores 24-bit column indices: n must be below 2^24 (use ppe_operator 0)");
   if (p->cg_warm_start < 0 || p->cg_warm_start > 1) return fail(nullptr, MPS_ERR_ARG, "cg_warm_start must be 0 or 1");
   if (p->kernel < 0 || p->kernel > 1) return fail(nullptr, MPS_ERR_ARG, "kernel must be 0 (Eq. 3) or 1 (Eq. 4)");
+  if (!(p->row_skin <= 1.0)) return fail(nullptr, MPS_ERR_ARG, "row_skin must be at most 1 (in units of l0); 0 = default, < 0 = off");
   if (p->kernel == 1 && (p->ppe_source != 0 || p->ppe_laplacian != 0))
     return fail(nullptr, MPS_ERR_ARG, "Eq. 15-18 are derived for the Eq. 3 kernel: kernel 1 needs ppe_source = ppe_laplacian = 0");
   if (p->grad_variant < 0 || p->grad_variant > 3) return fail(nullptr, MPS_ERR_ARG, "grad_variant must be 0..3");
@@ -205,14 +206,14 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   k.inv_h_dom = k.inv_h; k.nx_dom = k.nx; k.ny_dom = k.ny; k.nz_dom = k.nz;
   k.carry_d2 = 0.0;
   {
-    // mps_step's own bin (Q26): cells 1/256 larger than the contract's, rows built with a margin of 0.8 of
-    // that slack on both radii.  A 27-cell scan still finds every pair inside the enlarged radius, and
-    // the rows stay exact supersets at r^(k+1) as long as no particle moves by more than 0.45 margins in
-    // the corrector -- which k_correct checks.  GHOST decisions stay on the contract's grid.
+    // mps_step's own bins (Q26): cells of (max re + skin) / cell_div, rows built with both radii enlarged by
+    // the skin.  A scan of cell_div cells to each side still finds every pair inside the enlarged radius,
+    // and the rows stay exact supersets while no particle is further than 0.45 skins from where it was at
+    // the build -- which the predictor and the corrector check.  GHOST decisions stay on the contract's grid.
     KConst& s = c->kc_step;
     s = k;
-    const double hs = c->h * (1.0 + 1.0 / 256.0);
-    const double margin = 0.8 * (hs - c->h) * prm->cell_div;  // slack per radius: cell_div cells cover re_lap
+    const double skin = (prm->row_skin == 0.0 ? 0.2 : prm->row_skin) * prm->l0;
+    const double hs = (std::max(prm->re_n, prm->re_lap) + 1.001 * std::max(skin, 0.0)) / prm->cell_div;
     s.inv_h = 1.0 / hs;
     int64_t ncs = 1;
     int ns[3];
@@ -227,17 +228,16 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
       ncs = (int64_t)1 << (3 * bits);
     }
     s.ncells = (int)ncs;
-    s.re_lap2 = (prm->re_lap + margin) * (prm->re_lap + margin);
-    s.re_n2 = (prm->re_n + margin) * (prm->re_n + margin);
-    s.R_lap = std::max(1, (int)ceil((prm->re_lap + margin) * s.inv_h - 1e-9));
-    s.R_n = std::max(1, (int)ceil((prm->re_n + margin) * s.inv_h - 1e-9));
-    k.carry_d2 = s.carry_d2 = (0.45 * margin) * (0.45 * margin);
-    // one bin per step with rows carried across the corrector (off with list reuse, which has its own
-    // schedule, and for small scenes, where the per-step read-back of the validity flag costs more than
-    // the second bin: measured 0.166 vs 0.179 ms per step at 19k particles, 1.10 vs 1.01 at 89k;
-    // MPS_B200_CARRY=0 / 1 forces the two bins per step of reading Q7 as literally stated / the carry)
+    s.re_lap2 = (prm->re_lap + skin) * (prm->re_lap + skin);
+    s.re_n2 = (prm->re_n + skin) * (prm->re_n + skin);
+    s.R_lap = std::max(1, (int)ceil((prm->re_lap + skin) * s.inv_h - 1e-9));
+    s.R_n = std::max(1, (int)ceil((prm->re_n + skin) * s.inv_h - 1e-9));
+    k.carry_d2 = s.carry_d2 = (0.45 * skin) * (0.45 * skin);
+    // off with the paper's list reuse (rebin_every > 1 has its own schedule, Q24) and with row_skin < 0;
+    // MPS_B200_CARRY=0 forces the two bins per step of reading Q7 as literally stated
     const char* cr = getenv("MPS_B200_CARRY");
-    c->carry_rows = prm->rebin_every == 1 && ncs <= ncells && s.R_lap == k.R_lap && (cr ? atoi(cr) != 0 : n >= 32768);
+    c->carry_rows = prm->rebin_every == 1 && skin > 0.0 && ncs <= ncells && s.R_lap == k.R_lap &&
+                    !(cr && atoi(cr) == 0);
   }
 
   // every buffer any later call needs
@@ -252,6 +252,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->cell_count, (size_t)ncells + 2)); A(dalloc(&c->cell_start, (size_t)ncells + 2));
   A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
   A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
+  A(dalloc(&c->pos_ref, c->carry_rows ? N : 1));
   A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
   A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->dndt, N));
   A(dalloc(&c->keep2[0], N)); A(dalloc(&c->keep2[1], N));
@@ -365,7 +366,7 @@ static int read_flags(mps_ctx* c) {
     c->err = "a particle has more than max_neighbours neighbours";
   }
   c->stats.device_error = c->sticky_error;
-  c->stats.bins_total = c->bins_run;
+  c->stats.bins_total = c->bins_run + c->flags_host->bins;
   return c->sticky_error;
 }
 
@@ -530,6 +531,14 @@ int mps_bin(mps_ctx* c) {
     if (!(c)->binned) return fail((c), MPS_ERR_ORDER, "positions changed since the last mps_bin"); \
   } while (0)
 
+// Skin rows left by mps_step: valid for the current positions unless the last corrector raised need_k.
+static bool skin_rows_valid(mps_ctx* c) {
+  if (!c->carry_rows || !c->carry_valid) return false;
+  if (cudaMemcpyAsync(c->flags_host, c->flags, sizeof(DevFlags), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return false;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) return false;
+  return c->flags_host->need_k == 0;
+}
+
 int mps_density(mps_ctx* c) {
   MPS_RANGE();
   NEED_BIN(c);
@@ -612,6 +621,10 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     mpsk_bin(c);
     mpsk_smooth_density(c);
   }
+  // rows the route needs from a skin build: the explicit route takes the re_lap part for fluid rows only
+  // (viscosity); the PPE operator has rows for walls too, ECS needs n^k and (Dn/Dt)^k of every row
+  const bool skin = K == 1 && c->carry_rows;
+  const int skin_mode = route == MPS_ROUTE_EXPLICIT && !ecs ? ROWS_BACK_FLUID : 0;
   for (int s = 0; s < nsteps; ++s) {
     if (K > 1) {
       // list reuse (Q24): bin (all rows, both radii) once every K steps at r^k; every sweep of
@@ -623,22 +636,27 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       c->kc.stale = 1;
       ++c->reuse_count;
     }
-    // Rows carried over from the last step's bin at r* (margin rows, Q26)?  Only if that step's
-    // corrector left them exact supersets: one small read-back per step.
-    bool carried = false;
-    if (c->carry_rows && c->carry_valid) {
-      CK(cudaMemcpyAsync(&c->flags_host->carry_bad, &c->flags->carry_bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-      CK(cudaStreamSynchronize(c->stream));
-      carried = c->flags_host->carry_bad == 0;
+    if (skin && (!c->carry_valid || (c->rows_mode_built & ~skin_mode) != 0)) {
+      // no skin rows yet (first step, new particles, an API-level stage call in between), or rows that
+      // lack a part this route needs: make the predicated bin at r^k run
+      const int up[2] = {1, 0};  // need_k, need_star
+      CK(cudaMemcpyAsync(&c->flags->need_k, up, sizeof(up), cudaMemcpyHostToDevice, c->stream));
+      c->rows_mode_built = skin_mode;
+    } else if (skin) {
+      c->rows_mode_built |= skin_mode;  // a rebuild on the device during this step leaves out what this route skips
     }
-    const bool carry = c->carry_rows;
     // everything up to the pressure: one replayable segment (list reuse changes the sequence from
     // step to step and runs its launches directly)
     auto pre = [&]() {
-      if (K == 1) {
-        if (carried) c->kc.stale = 1;  // the rows are supersets: every sweep re-tests the distance (exact)
+      if (skin) {
+        // Q26: the rows are supersets, every sweep re-tests the distance (exact); the bin runs only if
+        // the last corrector found a particle further than 0.45 skins from its build position
+        c->kc.stale = 1;
+        mpsk_bin(c, skin_mode, &c->flags->need_k);
+      } else if (K == 1) {
         // viscosity and nu_t are computed for fluid i only; ECS also needs n^k and (Dn/Dt)^k of every row
-        else { c->kc.stale = 0; mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY); }
+        c->kc.stale = 0;
+        mpsk_bin(c, ecs ? 0 : ROWS_FLUID_ONLY);
       }
       if (ecs) {
         mpsk_density(c);
@@ -646,17 +664,9 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       }
       mpsk_viscosity(c);
       mpsk_predict(c);
-      if (K == 1) {
-        if (carry) {
-          // the step's one full bin: on the internal grid, with margin rows that the next step's first
-          // sweeps reuse; the explicit route needs the re_lap part for fluid rows only (next viscosity)
-          mpsk_bin(c, route == MPS_ROUTE_EXPLICIT && !ecs ? ROWS_BACK_FLUID : 0, /*step_grid=*/true);
-          c->kc.stale = 1;
-        } else {
-          // the explicit route needs only the re_n part at r* (density, p-hat, gradient)
-          mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
-        }
-      }
+      if (skin) mpsk_bin(c, skin_mode, &c->flags->need_star);  // runs only if the predictor said so
+      // without a skin the explicit route needs only the re_n part at r* (density, p-hat, gradient)
+      else if (K == 1) mpsk_bin(c, route == MPS_ROUTE_EXPLICIT ? ROWS_RN_ONLY : 0);
       mpsk_density(c);
       if (hs) mpsk_dndt(c, 0);
       if (route == MPS_ROUTE_EXPLICIT) mpsk_pressure_explicit(c);
@@ -665,14 +675,14 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       mpsk_gradient(c);
       mpsk_correct(c);
     };
-    if (K > 1) pre(); else run_segment(c, route, carried ? 2 : 0, pre);
+    if (K > 1) pre(); else run_segment(c, route, 0, pre);
     if (route == MPS_ROUTE_PPE) {
       // the solve is a cooperative launch of its own, between the two segments
       int rc = mpsk_pressure_ppe(c, /*sync=*/false);  // statistics are read once, after the last step
       if (rc == MPS_ERR_CUDA) return rc;
     }
     if (K > 1) post(); else run_segment(c, route, 1, post);
-    c->carry_valid = carry && K == 1;
+    c->carry_valid = skin;
     c->stats.steps_total++;
   }
   c->kc.stale = 0;  // API-level sweeps always run on exact rows (they need mps_bin first)
@@ -798,7 +808,10 @@ int mps_get_cell_start(mps_ctx* c, uint32_t* dst) {
 int mps_get_neighbours(mps_ctx* c, int32_t radius_id, uint32_t* counts, uint32_t* idx, int64_t cap,
                        int64_t* total) {
   MPS_RANGE();
-  NEED_BIN(c);
+  if (!c) return MPS_ERR_ARG;
+  if (!c->binned && !skin_rows_valid(c)) return fail(c, MPS_ERR_ORDER, "positions changed since the last mps_bin");
+  if (!c->binned && radius_id == MPS_RADIUS_LAP && (c->rows_mode_built & ROWS_BACK_FLUID))
+    return fail(c, MPS_ERR_ORDER, "the explicit route keeps the re_lap part of fluid rows only");
   if (!counts || (radius_id != MPS_RADIUS_N && radius_id != MPS_RADIUS_LAP)) return MPS_ERR_ARG;
   int rc = mpsk_get_neighbours(c, radius_id, counts, idx, cap, total);
   CK(cudaGetLastError());

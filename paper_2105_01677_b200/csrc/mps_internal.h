@@ -59,8 +59,13 @@ struct DevFlags {
   int nonfinite;      // NaN/Inf position or coincident pair
   int max_row;        // largest r_lap row
   int n_ghost;
-  int carry_bad;      // the last corrector moved a particle too far (or out of the domain) for the rows
-                      // of the step's bin to serve the next step's first sweeps: that step bins again
+  // mps_step with a skin (Q26): "the rows in nbr no longer cover the positions" -- raised by the corrector
+  // (need_k: read by the predicated bin at the start of the next step, cleared by the predictor) and by the
+  // predictor (need_star: read by the predicated bin at r*, cleared by the corrector) when a particle is
+  // further than 0.45 skins from its position at the last build, left the domain or is non-finite
+  int need_k;
+  int need_star;
+  int bins;           // predicated bins that actually ran
   int pad;
 };
 
@@ -83,7 +88,7 @@ struct KConst {  // by-value kernel parameter
   // equal to the fields above except in kc_step, whose cells are a little larger)
   double inv_h_dom;
   int nx_dom, ny_dom, nz_dom;
-  double carry_d2;  // (0.45 x row margin)^2: the corrector displacement up to which carried rows stay exact
+  double carry_d2;  // (0.45 x skin)^2: the distance from the build position up to which the rows stay exact supersets
   int R_lap;  // cells to each side for re_lap
   int R_n;    // ... and for re_n
   int key_mode;  // 0: key = c_x + n_x (c_y + n_y c_z); 1: Morton (3 x 10-bit interleave), ncells = 8^bits
@@ -111,9 +116,11 @@ struct StepSeg {
 struct mps_ctx {
   mps_params prm;
   KConst kc;
-  KConst kc_step;   // kc with the internal grid and the margin radii of mps_step's bin (mps_api.cu)
-  bool carry_rows = false;   // mps_step keeps one bin per step and carries its rows into the next step
-  bool carry_valid = false;  // the rows in nbr are margin rows built at the r* of the last step
+  KConst kc_step;   // kc with the internal grid and the skin radii of mps_step's bins (mps_api.cu)
+  bool carry_rows = false;   // mps_step builds rows with a skin and rebuilds them only when the device says so
+  bool carry_valid = false;  // the rows in nbr are skin rows and the device flags tell whether they still hold
+  int rows_mode_built = 0;   // rows_mode of the skin rows in nbr (a route change may need more of them)
+  double4* pos_ref = nullptr;  // positions at the last skin build, by slot
   int64_t n = 0;
   int64_t n_pad = 0;  // n rounded up to 32
   cudaStream_t stream = nullptr;
@@ -206,7 +213,7 @@ struct mps_ctx {
   int sm_count = 148;
   // mps_step replays its launch sequence from CUDA graphs (one per route, buffer parity and segment)
   // when the ctx has a capturable stream (not the legacy default stream) and timers are off
-  StepSeg seg[2][2][4];   // [route][buffer parity][segment: 0 pre (with first bin), 1 post, 2 pre (carried rows)]
+  StepSeg seg[2][2][4];   // [route][buffer parity][segment: 0 pre, 1 post]
   bool graphs_ok = true;
 };
 
@@ -233,11 +240,12 @@ static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); 
 #define ROWS_FLUID_ONLY 1
 #define ROWS_RN_ONLY 2
 #define ROWS_BACK_FLUID 4   // the re_n part of every row, the rest of the re_lap part for FLUID rows only
-// step_grid: bin on the ctx's internal grid of mps_step (cells 1/256 larger than the contract's) and build
-// rows with a margin (kc_step), so that they stay exact supersets across the corrector
-int mpsk_bin(mps_ctx* c, int rows_mode = 0, bool step_grid = false);
+// go != NULL: the bin of mps_step with a skin -- on the ctx's internal grid, rows with the skin radii
+// (kc_step), every kernel returns at once unless *go != 0 (a device flag), and the sorted arrays are
+// copied back into the current buffers, so the host state does not depend on whether it ran
+int mpsk_bin(mps_ctx* c, int rows_mode = 0, const int* go = nullptr);
 void mpsk_exclusive_scan(mps_ctx* c, int cat, const uint32_t* in, uint32_t* out, int64_t n,
-                         uint32_t* tmp);
+                         uint32_t* tmp, const int* go = nullptr);
 int mpsk_density(mps_ctx* c);
 int mpsk_dndt(mps_ctx* c, int keep);
 int mpsk_smooth_density(mps_ctx* c);

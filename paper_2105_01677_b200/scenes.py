@@ -92,6 +92,7 @@ def default_params(l0: float) -> Dict[str, object]:
         ppe_operator=1,      # CUDA path only: 0 matrix-free operator, 1 coefficients assembled once per solve
         cg_warm_start=0,     # 1: CG starts from the particle's previous pressure instead of 0
         key_mode=0,          # 0 linear x-fastest cell key, 1 Morton (3 x 10-bit interleave)
+        row_skin=0.0,        # CUDA path only: Verlet skin of mps_step's rows in units of l0 (0: default, < 0: off)
         clamp_negative_p=1,
         rho_pair_mean=0,
         nu_pair_mean=1,

@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(B):
 
 def test_struct_layout_matches_header(B):
     # 16 int32 then 28 doubles, no padding
-    assert C.sizeof(B.MpsParams) == 16 * 4 + 28 * 8
+    assert C.sizeof(B.MpsParams) == 16 * 4 + 29 * 8
     assert B.MpsParams.l0.offset == 64
     assert C.sizeof(B.MpsStats) == 96
     # field ids in the binding equal the header's enum

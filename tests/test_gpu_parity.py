@@ -752,35 +752,87 @@ def test_water_drop_trajectory_and_invariant(B, O):
     assert g.stats()["n_ghost"] == 0
 
 
-# ---- one bin per step: rows carried across the corrector (reading Q26) ----
+# ---- mps_step with a Verlet skin on its neighbour rows (reading Q26) ----
 @pytest.mark.parametrize("route", [0, 1])
-@pytest.mark.parametrize("carry", ["1", "0"])
-def test_row_carry_on_and_off_give_the_oracle_trajectory(B, O, route, carry, monkeypatch):
-    """MPS_B200_CARRY=1 forces the carry on a small scene (default: only from 32k particles), =0 the two
-    bins per step of Q7 as literally stated.  Both must follow the oracle; the bin count tells which ran."""
-    monkeypatch.setenv("MPS_B200_CARRY", carry)
+@pytest.mark.parametrize("skin", [0.0, 0.05, -1.0])   # library default (0.2 l0) / a thin skin / none
+def test_row_skin_on_and_off_give_the_oracle_trajectory(B, O, route, skin):
+    """row_skin > 0: rows are rebuilt only when the device finds a particle 0.45 skins from its build
+    position; row_skin < 0: the two bins per step of Q7 as literally stated.  Both must follow the
+    oracle; the bin count tells which ran."""
     s = scenes.small_tank(shuffle=True)
-    eL, el0, moved, g, o = _trajectory(B, O, s, 20, route, cs=0.12)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 20, route, cs=0.12, row_skin=skin)
     bins = g.stats()["bins_total"]
-    print(f"carry={carry} route={route}: max |dr|/L = {eL:.2e}, bins in 20 steps {bins}")
+    print(f"row_skin={skin} route={route}: max |dr|/L = {eL:.2e}, moved {moved:.3f} l0, bins in 20 steps {bins}")
     assert eL <= 1e-7
-    assert bins == (21 if carry == "1" else 40)     # 2 in the first step, then 1 per step | 2 per step
+    if skin < 0:
+        assert bins == 40
+    else:
+        assert 1 <= bins <= (6 if skin == 0.0 else 20)
     assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-6
 
 
+def test_env_switch_forces_two_bins_per_step(B, O, monkeypatch):
+    monkeypatch.setenv("MPS_B200_CARRY", "0")
+    s = scenes.small_tank(shuffle=True)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 6, 0)
+    assert eL <= 1e-7 and g.stats()["bins_total"] == 12
+
+
 @pytest.mark.parametrize("route", [0, 1])
-def test_row_carry_falls_back_when_the_corrector_moves_too_far(B, O, route, monkeypatch):
-    """A corrector displacement beyond the rows' margin (0.45 x 0.8 x re_lap / 256 = 0.0044 l0) must send
-    the next step back to a bin at r^k.  Random velocities of 0.4 m/s compress the small tank enough
-    (pressures of 5-13 kPa) that most steps fall back, and the trajectory still follows the oracle."""
-    monkeypatch.setenv("MPS_B200_CARRY", "1")
+def test_row_skin_rebuilds_when_particles_move_far(B, O, route):
+    """Random velocities of 0.4 m/s (0.02 l0 per step, pressures of 5-13 kPa) against a skin of 0.05 l0
+    (limit 0.0225 l0): almost every step must rebuild, some at r* and some at r^k, and the trajectory
+    still follows the oracle."""
     s = scenes.small_tank(shuffle=True)
     rng = np.random.default_rng(3)
     fl = s.type == scenes.FLUID
     for k in "uvw":
         getattr(s, k)[fl] = 0.4 * rng.standard_normal(fl.sum())
-    eL, el0, moved, g, o = _trajectory(B, O, s, 12, route)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 12, route, row_skin=0.05)
     bins = g.stats()["bins_total"]
-    print(f"carry with fallback, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0, bins in 12 steps {bins}")
+    print(f"skin 0.05 l0 with fast particles, route {route}: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0, bins in 12 steps {bins}")
     assert eL <= 1e-7 and moved > 0.3
-    assert 13 < bins <= 24                       # more than one per step: the fallback ran
+    assert 8 <= bins <= 24
+
+
+@pytest.mark.parametrize("rows", ["lean", "warp", "cell"])
+@pytest.mark.parametrize("skin", [0.0, 0.4])
+def test_row_skin_sets_stay_bit_exact(B, O, rows, skin, monkeypatch):
+    """The set a sweep of mps_step sees = the stored skin row filtered by the re-test at the current
+    positions.  After steps with and without rebuilds it must equal the oracle's set at the same
+    positions bit for bit, at both radii (PPE route: rows of every particle)."""
+    monkeypatch.setenv("MPS_B200_ROWS", rows)
+    s = scenes.small_tank(shuffle=True)
+    rng = np.random.default_rng(5)
+    fl = s.type == scenes.FLUID
+    for k in "uvw":
+        getattr(s, k)[fl] = 0.15 * rng.standard_normal(fl.sum())
+    g = B.Mps(s, row_skin=skin)
+    o = O.Oracle(s)
+    seen = set()
+    for nst in (1, 3, 2, 4):
+        g.step(nst, 1)
+        seen.add(g.stats()["bins_total"])
+        for k in "xyz":
+            o.set(k, g.get(k))
+        o.bin()
+        for rid, re in ((B.RADIUS_N, s.params["re_n"]), (B.RADIUS_LAP, s.params["re_lap"])):
+            co, io = o.neighbours(re)
+            cg, ig = g.neighbours(rid)
+            assert np.array_equal(cg, co)
+            assert np.array_equal(ig, io)
+    print(f"rows={rows} skin={skin}: bins after 1, 4, 6, 10 steps {sorted(seen)}")
+    assert max(seen) < 20        # fewer than two bins per step: rows were reused in between
+
+
+def test_row_skin_follows_a_route_change(B, O):
+    """Explicit steps keep the re_lap part of fluid rows only; a PPE step after them needs every row."""
+    s = scenes.small_tank(shuffle=True)
+    g = B.Mps(s)
+    o = O.Oracle(s)
+    for route in (0, 1, 0, 1):
+        g.step(3, route)
+        o.step(3, route)
+    L = max(hi - lo for lo, hi in zip(s.params["domain_min"], s.params["domain_max"]))
+    d = np.sqrt(sum((g.get(k) - o.get(k)) ** 2 for k in "xyz"))
+    assert d.max() / L <= 1e-7
