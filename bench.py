@@ -44,7 +44,7 @@ ROUTE_NAME = {0: "explicit", 1: "ppe"}
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50, help="timed steps (BASELINE.json configs[4]: 50 steps each)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=5, help="scene 1..5 (SURVEY.md 8(d)); default 5 = BASELINE configs[4], the throughput sweep; 6 = paper-shaped 2D dam break")
@@ -58,12 +58,13 @@ def parse_args():
     ap.add_argument("--warm-start", action="store_true", help="cg_warm_start = 1")
     ap.add_argument("--key-mode", type=int, default=None, choices=[0, 1], help="0 linear cell key, 1 Morton")
     ap.add_argument("--row-skin", type=float, default=None,
-                    help="Verlet skin of mps_step's rows in units of l0 (library default 0.2; < 0: two bins per step)")
+                    help="Verlet skin of mps_step's rows in units of l0 (library default 0.1; < 0: two bins per step)")
     ap.add_argument("--pre-steps", type=int, default=0,
                     help="untimed steps before the warm-up (0: the timed window starts W steps from rest, as BASELINE.json's "
                          "workloads do; e.g. 400 puts it in the developed dam-break flow)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-developed", action="store_true", help="skip the developed-flow leg (400 untimed steps, then K timed)")
     ap.add_argument("--no-replay", action="store_true", help="skip the instrumented per-kernel replay")
     return ap.parse_args()
 
@@ -283,7 +284,11 @@ def neighbour_statistics(np, B, g, scene, route):
         for dy in range(2 * R_ + 1):
             for dx in range(2 * R_ + 1):
                 cand += pad[dz:dz + nz_, dy:dy + ny_, dx:dx + nx_]
+    fl, fw = typ == 0, (typ == 0) | (typ == 1)
     return {"kl": float(cl.mean()), "kn": float(cn.mean()), "rows": rows,
+            "n_fluid": int(fl.sum()), "kl_fluid": float(cl[fl].mean()) if fl.any() else 0.0,
+            "kn_fluid": float(cn[fl].mean()) if fl.any() else 0.0,
+            "n_fw": int(fw.sum()), "kn_fw": float(cn[fw].mean()) if fw.any() else 0.0,
             "klr": float(cl[bc == 0].mean()) if rows else 0.0,
             "tests_all": float((cnt * cand).sum()), "tests_fluid": float((fl_cnt * cand).sum())}
 
@@ -301,7 +306,6 @@ def load_traffic():
 def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K, W, sample_clocks):
     """One route of one scene: the device-resident timed steps, then an instrumented replay of the
     same steps with per-kernel CUDA events, and the roofline of the dominant kernel."""
-    g = B.Mps(scene, device=str(dev))
     clocks = None
     if sample_clocks:
         try:
@@ -309,16 +313,20 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
         except Exception:
             gpu_id = str(dev.index)
         # the sampler runs over warm-up and timed steps: the timed region alone can be shorter than
-        # nvidia-smi's start-up, and both are the same load
+        # nvidia-smi's start-up, and both are the same load.  Until it reports, a scratch copy of the scene
+        # keeps the GPU under the same load, so that the measured ctx always times steps W .. W+K from rest
+        # (how often the skin rows are rebuilt depends on how far the flow has developed)
         sampler = ClockSampler(gpu_id)
         sampler.start()
+        g0 = B.Mps(scene, device=str(dev))
+        t_end = time.perf_counter() + 1.0
+        while time.perf_counter() < t_end and len(sampler.rows) < 3:
+            g0.step(1, route)
+        g0.close()
+    g = B.Mps(scene, device=str(dev))
     if getattr(args, "pre_steps", 0) > 0:
         g.step(int(args.pre_steps), route)
     g.step(max(W, 3), route)
-    if sample_clocks:
-        t_end = time.perf_counter() + 0.5
-        while time.perf_counter() < t_end and len(sampler.rows) < 3:
-            g.step(1, route)           # untimed: keep the GPU under load until the sampler reports
     l0 = g.launch_count()
     st0 = g.stats()
     ms_rank = timed_steps(torch, world, g, route, K, flush, stream)
@@ -427,6 +435,20 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
         roof.update({"per": "use", "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                      "traffic": traffic["dram_bytes_per_use"] if traffic else None, "uses": uses,
                      "us_per_use": 1e3 * ms_top / max(uses, 1), "launches": ln_top})
+        # the list-driven sweeps gather one 32-byte record (sector) per pair and array from the L1: by measurement
+        # (profiles/r01_ceilings_microbench.md: 31 SM-cycles per 32 records with the texture + LSU split) that, not
+        # HBM, binds them.  Sectors counted from the exact sets (the skin's extra pairs are not credited).
+        sectors = {"viscosity": ns["n_fluid"] * ns["kl_fluid"] * 2.0,                      # position + velocity record
+                   "density": N * kn,
+                   "gradient": ns["n_fw"] * ns["kn_fw"] + ns["n_fluid"] * ns["kn_fluid"]}.get(top)  # p-hat pass + sum
+        if sectors:
+            sm, ghz = 148, 1.965
+            per_clk = sectors * uses / (ms_top * 1e-3) / (sm * ghz * 1e9)
+            roof.update({"bound": "l1-gather (one 32-byte record per pair and array through the L1; the HBM fraction is "
+                                  "reported against the measured copy peak but is not what binds)",
+                         "l1_gather": {"achieved_sectors_per_sm_clk": per_clk, "ceiling": 32.0 / 31.0,
+                                       "frac": per_clk / (32.0 / 31.0),
+                                       "ceiling_source": "stand-alone gather of the same shape, texture + LSU split: 31 SM-cycles per 32 records"}})
     out.update({"kernels": kernels, "roofline": roof})
     return out
 
@@ -478,8 +500,22 @@ def run_b200(args):
     if world == 1 and not args.no_other_route and args.rebin_every == 1:
         r2 = 1 - route
         o = measure_route(torch, np, B, args, scene, r2, 1, dev, stream, flush, K, W, sample_clocks=False)
-        other = {ROUTE_NAME[r2]: {k: o[k] for k in ("value", "ms_per_step", "gpu_launches", "roofline", "kernels")
+        other = {ROUTE_NAME[r2]: {k: o[k] for k in ("value", "ms_per_step", "bins_per_step", "gpu_launches", "roofline", "kernels")
                                   if k in o} | ({"cg": o["cg"]} if "cg" in o else {})}
+
+    # the same scene once the flow has developed (the timed window of BASELINE.json's workloads starts from rest,
+    # where particles move little and the skin rows last for many steps): 400 untimed steps first, no replay
+    developed = None
+    if world == 1 and not args.no_developed and args.pre_steps == 0 and args.rebin_every == 1:
+        import copy
+        a2 = copy.copy(args)
+        a2.pre_steps, a2.no_replay = 400, True
+        developed = {"pre_steps": 400}
+        for r_ in ((route, 1 - route) if not args.no_other_route else (route,)):
+            o = measure_route(torch, np, B, a2, scene, r_, 1, dev, stream, flush, K, W, sample_clocks=False)
+            developed[ROUTE_NAME[r_]] = {k: o[k] for k in ("value", "ms_per_step", "bins_per_step", "gpu_launches")} | (
+                {"cg_iters_per_step": o["cg"]["iters_per_step"], "ps_per_row_per_iteration": o["cg"]["ps_per_row_per_iteration"]}
+                if "cg" in o else {})
 
     # ---- end to end: pinned host buffers in, one step, host buffers out, every step ----
     e2e = None
@@ -551,6 +587,8 @@ def run_b200(args):
             out["cg_iters_per_sec"] = main["cg"]["iters_per_sec"]
         if other:
             out["routes"] = other
+        if developed:
+            out["developed_flow"] = developed
         print(json.dumps(out))
     if world > 1:
         torch.distributed.destroy_process_group()

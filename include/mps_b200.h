@@ -134,7 +134,7 @@ typedef struct mps_params {
                                with both radii enlarged by row_skin * l0 and serve every sweep -- each re-tests
                                r2 < re^2 with the rounding of Q2, so the sets stay exact -- until some particle has
                                moved by more than 0.45 skins since the build (checked on the device by the predictor
-                               and the corrector).  0 => the library's default (0.2); < 0 => no skin: mps_step
+                               and the corrector).  0 => the library's default (0.1); < 0 => no skin: mps_step
                                bins at r^k and at r* in every step, as Q7 is literally stated */
 } mps_params;
 

@@ -3,6 +3,7 @@
 // cell, physical reorder, and the per-step neighbour rows.
 // Paper: section 4.1 (cell-linked list), P:288, P:273-274 (neigh[] rows).
 #include <algorithm>
+#include <string.h>
 
 #include "mps_internal.h"
 
@@ -268,6 +269,15 @@ __global__ void k_reorder(int n, int ncells, const uint32_t* __restrict__ key,
   // the neighbour-row entry that names this particle (flags of mps_internal.h)
   ent_out[f] = f | (ty == MPS_DUMMY ? NB_DUMMY : 0u) | (ty == MPS_WALL ? NB_WALL : 0u) |
                ((tj & 0x100) ? NB_PHASE1 : 0u);
+}
+
+// Inside a CUDA graph the skin bin is the body of a conditional node (cudaGraphCondTypeIf): this one-thread
+// kernel, placed just before the node, hands the device flag to the node, so a bin that is not needed costs
+// one graph node instead of eight launches that return at once.
+__global__ void k_set_cond(cudaGraphConditionalHandle h, const int* go, DevFlags* flags) {
+  const int on = *(const volatile int*)go != 0;
+  if (on) flags->cond_taken += 1;
+  cudaGraphSetConditional(h, on ? 1u : 0u);
 }
 
 // The bin of mps_step with a skin leaves the sorted particles in the buffers they came from (so that no
@@ -941,6 +951,47 @@ int mpsk_bin(mps_ctx* c, int rows_mode, const int* go) {
   const KConst& kg = go ? c->kc_step : c->kc;
   const int nc = kg.ncells;
   const int cur = c->cur, nxt = cur ^ 1;
+  // A skin bin captured into a graph becomes the body of an IF node keyed on the device flag
+  cudaStream_t outer = c->stream;
+  bool cond = false;
+  int64_t launches_before = 0, t_before[MPS_NUM_TIMERS];
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (go && c->aux_stream && c->stream && cudaStreamIsCapturing(c->stream, &cap) == cudaSuccess &&
+      cap == cudaStreamCaptureStatusActive) {
+    cudaGraph_t graph = nullptr, body = nullptr;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    unsigned long long id = 0;
+    cudaGraphConditionalHandle handle;
+    cudaGraphNode_t node;
+    cudaGraphNodeParams np = {};
+    bool ok = cudaStreamGetCaptureInfo_v2(outer, &cap, &id, &graph, &deps, &ndeps) == cudaSuccess &&
+              cudaGraphConditionalHandleCreate(&handle, graph, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+    if (ok) {
+      MPS_LAUNCH(c, MPS_T_BIN_SORT, k_set_cond, 1, 1, handle, go, c->flags);
+      np.type = cudaGraphNodeTypeConditional;
+      np.conditional.handle = handle;
+      np.conditional.type = cudaGraphCondTypeIf;
+      np.conditional.size = 1;
+      ok = cudaStreamGetCaptureInfo_v2(outer, &cap, &id, &graph, &deps, &ndeps) == cudaSuccess &&
+           cudaGraphAddNode(&node, graph, deps, ndeps, &np) == cudaSuccess &&
+           cudaStreamUpdateCaptureDependencies(outer, &node, 1, cudaStreamSetCaptureDependencies) == cudaSuccess;
+      if (ok) {
+        body = np.conditional.phGraph_out[0];
+        ok = cudaStreamBeginCaptureToGraph(c->aux_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+      }
+      if (ok) {
+        cond = true;
+        c->stream = c->aux_stream;  // the launches below go into the body
+        launches_before = c->launches;
+        for (int k = 0; k < MPS_NUM_TIMERS; ++k) t_before[k] = c->t_launches[k];
+      } else {
+        cudaGetLastError();  // the capture is broken: run_segment sees EndCapture fail and falls back to launches
+      }
+    } else {
+      cudaGetLastError();
+    }
+  }
   cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * (nc + 2), c->stream);
   if (!go) cudaMemsetAsync(&c->flags->max_row, 0, sizeof(int), c->stream);  // predicated: k_scatter does it
   MPS_LAUNCH(c, MPS_T_BIN_SORT, k_keys, div_up(n, TPB), TPB, kg, c->pos4[cur], c->tp[cur],
@@ -977,6 +1028,15 @@ int mpsk_bin(mps_ctx* c, int rows_mode, const int* go) {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, kg,
                c->pos4[at], c->tp[at], c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
+  }
+  if (cond) {
+    cudaGraph_t body_out = nullptr;
+    cudaStreamEndCapture(c->aux_stream, &body_out);
+    c->stream = outer;
+    // the body's launches happen only when the bin runs: mps_launch_count adds them from the device counter
+    c->cond_launches_per_bin = (int)(c->launches - launches_before);
+    c->launches = launches_before;
+    for (int k = 0; k < MPS_NUM_TIMERS; ++k) c->t_launches[k] = t_before[k];
   }
   if (!go) {
     c->binned = true;

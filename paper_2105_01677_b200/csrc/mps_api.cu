@@ -80,6 +80,7 @@ static void free_all(mps_ctx* c) {
   cudaFree(c->mat_val); cudaFree(c->mat_col); cudaFree(c->mat_cnt); cudaFree(c->mat_dex); cudaFree(c->mat_scale); cudaFree(c->rowmap);
   cudaFree(c->cg_rc); cudaFree(c->cg_xc);
   if (c->bar_host) cudaFreeHost(c->bar_host);
+  if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
   cudaFree(c->cg); cudaFree(c->flags); cudaFree(c->io_tmp);
   if (c->cg_host) cudaFreeHost(c->cg_host);
   if (c->flags_host) cudaFreeHost(c->flags_host);
@@ -212,7 +213,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     // the build -- which the predictor and the corrector check.  GHOST decisions stay on the contract's grid.
     KConst& s = c->kc_step;
     s = k;
-    const double skin = (prm->row_skin == 0.0 ? 0.2 : prm->row_skin) * prm->l0;
+    const double skin = (prm->row_skin == 0.0 ? 0.1 : prm->row_skin) * prm->l0;
     const double hs = (std::max(prm->re_n, prm->re_lap) + 1.001 * std::max(skin, 0.0)) / prm->cell_div;
     s.inv_h = 1.0 / hs;
     int64_t ncs = 1;
@@ -253,6 +254,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
   A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
   A(dalloc(&c->pos_ref, c->carry_rows ? N : 1));
+  if (c->carry_rows) A(cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
   A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
   A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->dndt, N));
   A(dalloc(&c->keep2[0], N)); A(dalloc(&c->keep2[1], N));
@@ -867,6 +869,10 @@ int mps_timers_read(mps_ctx* c, double* ms, int64_t* launches) {
   }
   return MPS_OK;
 }
-int64_t mps_launch_count(mps_ctx* c) { return c ? c->launches : 0; }
+int64_t mps_launch_count(mps_ctx* c) {
+  // launches issued by the host, plus those of the skin bins that ran as conditional graph bodies (counted on the
+  // device; as of the last read of the device flags: mps_step, mps_sync and mps_get_stats read them)
+  return c ? c->launches + (int64_t)c->flags_host->cond_taken * c->cond_launches_per_bin : 0;
+}
 
 }  // extern "C"

@@ -66,7 +66,7 @@ struct DevFlags {
   int need_k;
   int need_star;
   int bins;           // predicated bins that actually ran
-  int pad;
+  int cond_taken;     // ... of which as the body of a conditional graph node (their launches are counted from this)
 };
 
 struct KConst {  // by-value kernel parameter
@@ -121,6 +121,8 @@ struct mps_ctx {
   bool carry_valid = false;  // the rows in nbr are skin rows and the device flags tell whether they still hold
   int rows_mode_built = 0;   // rows_mode of the skin rows in nbr (a route change may need more of them)
   double4* pos_ref = nullptr;  // positions at the last skin build, by slot
+  cudaStream_t aux_stream = nullptr;  // captures the body of the conditional graph node that holds a skin bin
+  int cond_launches_per_bin = 0;      // kernel launches inside such a body (they happen only when the bin runs)
   int64_t n = 0;
   int64_t n_pad = 0;  // n rounded up to 32
   cudaStream_t stream = nullptr;

@@ -754,7 +754,7 @@ def test_water_drop_trajectory_and_invariant(B, O):
 
 # ---- mps_step with a Verlet skin on its neighbour rows (reading Q26) ----
 @pytest.mark.parametrize("route", [0, 1])
-@pytest.mark.parametrize("skin", [0.0, 0.05, -1.0])   # library default (0.2 l0) / a thin skin / none
+@pytest.mark.parametrize("skin", [0.0, 0.05, -1.0])   # library default (0.1 l0) / a thin skin / none
 def test_row_skin_on_and_off_give_the_oracle_trajectory(B, O, route, skin):
     """row_skin > 0: rows are rebuilt only when the device finds a particle 0.45 skins from its build
     position; row_skin < 0: the two bins per step of Q7 as literally stated.  Both must follow the
