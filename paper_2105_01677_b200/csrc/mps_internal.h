@@ -174,7 +174,7 @@ struct mps_ctx {
   uint32_t* cg_rows = nullptr;   // compacted slot indices of the PPE unknowns (bc == 0)
   // ppe_operator 1: the assembled operator over the compacted rows g = 0..n_rows-1 (ELL, row g at
   // g * kc.stride) and the CG vectors in the same compact numbering
-  double* mat_val = nullptr;     // one 64-bit word per stored pair: column (24 bits) | coefficient (40-bit fraction
+  double* mat_val = nullptr;     // one 64-bit word per stored pair: column (high 24 bits) | coefficient (low 40 bits: fraction
                                  // of the row's largest); holds plain fp64 coefficients while a row is assembled
   uint32_t* mat_col = nullptr;   // assembly scratch: the columns before packing
   double* mat_scale = nullptr;   // row's largest coefficient / (2^40 - 1)
