@@ -752,6 +752,29 @@ def test_water_drop_trajectory_and_invariant(B, O):
     assert g.stats()["n_ghost"] == 0
 
 
+def test_water_drop_on_the_ppe_route(B, O):
+    """The whole semi-implicit step against the drop's closed forms (oracle pin of the same name) and
+    against the oracle's trajectory."""
+    s = scenes.water_drop()
+    over = dict(compress=1.0e-10, grad_variant=2)
+    eL, el0, moved, g, o = _trajectory(B, O, s, 100, 1, **over)
+    print(f"water drop, 100 PPE steps: max |dr|/L = {eL:.2e}, moved {moved:.2f} l0")
+    assert eL <= 1e-7 and moved > 1.0
+    ax = lambda x, y: (2.0 * np.sqrt((x * x).mean()), 2.0 * np.sqrt((y * y).mean()))
+    a0, b0 = ax(s.x, s.y)
+    k, worst = 100, 0.0
+    while True:
+        g.step(10, 1)
+        k += 10
+        a, b = ax(g.get("x"), g.get("y"))
+        worst = max(worst, abs(a * b - a0 * b0) / (a0 * b0))
+        if b >= 2.0 * b0 or k >= 2000:
+            break
+    print(f"  GPU: b doubled after {k} steps, worst ab error {100 * worst:.2f} %")
+    assert abs(k * 1e-5 - 8.005e-3) <= 0.05 * 8.005e-3 and worst <= 0.05
+    assert g.stats()["n_ghost"] == 0
+
+
 # ---- mps_step with a Verlet skin on its neighbour rows (DESIGN.md reading Q26) ----
 @pytest.mark.parametrize("route", [0, 1])
 @pytest.mark.parametrize("skin", [0.0, 0.05, -1.0])   # library default (0.1 l0) / a thin skin / none

@@ -1100,3 +1100,29 @@ def test_water_drop_ab_invariant_and_doubling_time():
     y, v = o.get("y"), o.get("v")
     A_fit = float((y * v).sum() / (y * y).sum())
     assert A_fit == pytest.approx(100.0 * 2.0 * math.sqrt(2.0 / 17.0), rel=0.08)
+
+
+def test_water_drop_on_the_ppe_route():
+    # The same closed forms pin a WHOLE semi-implicit step (flags, source, solve, gradient, corrector, in
+    # this order and with these signs): an incompressible drop keeps a b = R^2 and doubles b at t2.  The
+    # paper does not state the configuration behind its 0.26 %; Listing 2's compressibility
+    # term 1e-7 / dt^2 is sized for its dam-break step (dt ~ 1e-3), at dt = 1e-5 it would swamp
+    # the Laplacian (the solve then takes 3 iterations and the drop's area grows by 19 %), so the pin
+    # scales it with dt^2 (compress = 1e-10) and takes the momentum-conserving gradient (variant 2).
+    # Measured: b doubles after 820 steps (8.20e-3 s, theory 8.005e-3), a b within 3.5 %.
+    s = scenes.water_drop()
+    o = O.Oracle(s, compress=1.0e-10, grad_variant=2)
+    a0, b0 = _drop_axes(s.x, s.y)
+    k, worst = 0, 0.0
+    while True:
+        o.step(10, 1)
+        k += 10
+        a, b = _drop_axes(o.get("x"), o.get("y"))
+        worst = max(worst, abs(a * b - a0 * b0) / (a0 * b0))
+        if b >= 2.0 * b0 or k >= 2000:
+            break
+    print(f"water drop, PPE route: b doubled after {k} steps, worst ab error {100 * worst:.2f} %, "
+          f"cg iterations in the last step {o.stats()['cg_iters']}")
+    assert o.stats()["n_ghost"] == 0 and o.stats()["cg_iters"] > 5
+    assert abs(k * s.params["dt"] - 8.005e-3) <= 0.05 * 8.005e-3
+    assert worst <= 0.05
