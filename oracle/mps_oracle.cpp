@@ -24,8 +24,12 @@
 // rho*g*h; NEXT rows: Dn/Dt (dilation closed form, brute force, finite difference of the density),
 // HS/ECS worked example, HL shell sum and dense solve, 2D constants and closed forms, Eq. 4 shell
 // sums, list reuse against brute force on the stored sets, smoothed density at a flat interface and
-// the multi-density term by brute force.  Whole-step trajectories in a moving fluid: the paper prints no
-// values => "parity unpinned" against the paper for those (pinned on the parts).
+// the multi-density term by brute force; pair viscosity at a two-viscosity interface (hand shell sum, brute
+// force with walls), p-hat and gradient variants 0-2 by brute force with dummies carrying a pressure, the Morton
+// key table, preconditioned CG against the dense solve, and -- whole steps -- the paper's water drop on both
+// pressure routes (a b = R^2 and the analytic doubling time; Table 1).  The VALUES of PPE pressures
+// in a moving fluid: the paper prints none => "parity unpinned" against the paper for those (pinned on the
+// parts and through the water drop).
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
