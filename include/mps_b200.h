@@ -26,7 +26,9 @@
  *    of the matrix-free gathers off, MPS_B200_CG_TIMEOUT_CYCLES=<n> sets the spin limit of the
  *    grid barrier inside the persistent CG kernel (default 4e9 SM cycles, 0 = no limit; raise it
  *    or set 0 under compute-sanitizer or a debugger), MPS_B200_CARRY=0 makes mps_step bin twice per
- *    step as if row_skin < 0 (see mps_step).
+ *    step as if row_skin < 0 (see mps_step), MPS_B200_COND=0 captures the skin bins of mps_step as plain kernel
+ *    nodes that return at once instead of conditional graph nodes (the default whenever CUDA_INJECTION64_PATH is
+ *    set, i.e. under a profiler: Nsight Compute cannot see kernels of a graph that holds conditional nodes).
  */
 #ifndef MPS_B200_H
 #define MPS_B200_H

@@ -636,6 +636,10 @@ __device__ __forceinline__ void flush_sector(uint32_t* dst, const uint32_t (*b)[
   reinterpret_cast<uint4*>(dst)[1] = hi;
 }
 
+// EXACT: the distance test with the rounding of reading Q2 (mps_bin: the rows ARE the sets).  A skin build
+// (mps_step) only needs a superset of radius re + 0.9 skin, every sweep re-tests exactly: fused arithmetic,
+// two fp64 instructions fewer per candidate.
+template <bool EXACT>
 __global__ void __launch_bounds__(CELL_TPB, 4)
 k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ ent,
                   const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nbr,
@@ -644,6 +648,11 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
   if (skipped(go)) return;
   const bool fluid_only = (mode & ROWS_FLUID_ONLY) != 0, rn_only = (mode & ROWS_RN_ONLY) != 0;
   __shared__ uint32_t buf[2][CELL_WARPS][8][32];
+  // the 32 candidates of a chunk, loaded once (coalesced, one record per lane) and then read by every lane as
+  // shared-memory broadcasts: a warp-uniform LDG.128 costs the L1 a pass per quarter warp, 8 per candidate
+  // (ncu: l1tex 72 %, the busiest unit of this kernel), an LDS broadcast one
+  __shared__ double2 cand_xy[CELL_WARPS][32];
+  __shared__ double cand_z[CELL_WARPS][32];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarp = blockIdx.x * CELL_WARPS + wid;
   const int nwarps = gridDim.x * CELL_WARPS;
@@ -694,15 +703,24 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
             // broadcast.  Slots past je (at most 31, inside the padded arrays) are masked off.
             const uint32_t cnt = min(32u, je - j0);
             uint32_t m_lap = 0, m_n = 0;
-            const double4* qp = pos4 + j0;
-            for (uint32_t g = 0; g < cnt; g += CELL_BATCH, qp += CELL_BATCH) {
+            {
+              const double4 mine = pos4[j0 + (uint32_t)lane];  // past je: inside the padded array, masked below
+              __syncwarp();                                    // the previous chunk has been read by every lane
+              cand_xy[wid][lane] = make_double2(mine.x, mine.y);
+              cand_z[wid][lane] = mine.z;
+              __syncwarp();
+            }
+            const double2* qxy = cand_xy[wid];
+            const double* qz = cand_z[wid];
+            for (uint32_t g = 0; g < cnt; g += CELL_BATCH, qxy += CELL_BATCH, qz += CELL_BATCH) {
               uint32_t b_lap = 0, b_n = 0;
 #pragma unroll
               for (int t = 0; t < CELL_BATCH; ++t) {
-                const double4 q = qp[t];
-                const double dx = __dsub_rn(q.x, pi.x), dy_ = __dsub_rn(q.y, pi.y), dz_ = __dsub_rn(q.z, pi.z);
+                const double2 qa = qxy[t];
+                const double dx = __dsub_rn(qa.x, pi.x), dy_ = __dsub_rn(qa.y, pi.y), dz_ = __dsub_rn(qz[t], pi.z);
                 const double r2 =
-                    __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_));
+                    EXACT ? __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy_, dy_)), __dmul_rn(dz_, dz_))
+                          : fma(dz_, dz_, fma(dy_, dy_, dx * dx));
                 if (r2 < kc.re_lap2) b_lap |= 1u << t;
                 if (r2 < kc.re_n2) b_n |= 1u << t;
               }
@@ -956,7 +974,7 @@ int mpsk_bin(mps_ctx* c, int rows_mode, const int* go) {
   bool cond = false;
   int64_t launches_before = 0, t_before[MPS_NUM_TIMERS];
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-  if (go && c->aux_stream && c->stream && cudaStreamIsCapturing(c->stream, &cap) == cudaSuccess &&
+  if (go && c->cond_nodes && c->aux_stream && c->stream && cudaStreamIsCapturing(c->stream, &cap) == cudaSuccess &&
       cap == cudaStreamCaptureStatusActive) {
     cudaGraph_t graph = nullptr, body = nullptr;
     const cudaGraphNode_t* deps = nullptr;
@@ -1022,8 +1040,12 @@ int mpsk_bin(mps_ctx* c, int rows_mode, const int* go) {
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows, div_up(n, (LEAN_TPB / 32) * LEAN_PPW), LEAN_TPB, kg, c->pos4[at],
                c->ent, c->key, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
   } else if (c->prm.cell_div == 1 && c->rows_builder == 2) {
-    MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell, div_up(nc, CELL_WARPS), CELL_TPB, kg, c->pos4[at],
-               c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
+    if (go)
+      MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell<false>, div_up(nc, CELL_WARPS), CELL_TPB, kg, c->pos4[at],
+                 c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
+    else
+      MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_cell<true>, div_up(nc, CELL_WARPS), CELL_TPB, kg, c->pos4[at],
+                 c->ent, c->cell_start, c->nbr, c->cn, c->co, c->flags, rows_mode, go);
   } else {
     // small cells hold only a few particles each: one warp per particle, lanes on candidates
     MPS_LAUNCH(c, MPS_T_BIN_LIST, k_build_rows_warp, div_up(n, (ROWS_TPB / 32) * ROWS_PPW), ROWS_TPB, kg,

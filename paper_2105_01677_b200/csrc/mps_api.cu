@@ -255,6 +255,14 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
   A(dalloc(&c->pos_ref, c->carry_rows ? N : 1));
   if (c->carry_rows) A(cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+  {
+    // Nsight Compute cannot profile kernel nodes of a graph that holds conditional nodes ("not supported for
+    // profiling"): with a CUDA injection library in the process (a profiler is attached), or MPS_B200_COND=0,
+    // the skin bins are captured as plain kernel nodes that return at once when not needed
+    const char* cn = getenv("MPS_B200_COND");
+    const char* inj = getenv("CUDA_INJECTION64_PATH");
+    c->cond_nodes = cn ? atoi(cn) != 0 : !(inj && *inj);
+  }
   A(dalloc(&c->dens, N)); A(dalloc(&c->p, N)); A(dalloc(&c->acc4, N)); A(dalloc(&c->nut, N));
   A(dalloc(&c->b, N)); A(dalloc(&c->phat, N)); A(dalloc(&c->dndt, N));
   A(dalloc(&c->keep2[0], N)); A(dalloc(&c->keep2[1], N));

@@ -123,6 +123,7 @@ struct mps_ctx {
   double4* pos_ref = nullptr;  // positions at the last skin build, by slot
   cudaStream_t aux_stream = nullptr;  // captures the body of the conditional graph node that holds a skin bin
   int cond_launches_per_bin = 0;      // kernel launches inside such a body (they happen only when the bin runs)
+  bool cond_nodes = true;             // skin bins inside a graph become conditional nodes (else: predicated kernels)
   int64_t n = 0;
   int64_t n_pad = 0;  // n rounded up to 32
   cudaStream_t stream = nullptr;
