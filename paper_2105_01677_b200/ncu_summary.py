@@ -70,6 +70,33 @@ def read_report(path):
     return out
 
 
+def hot_lines(path, launches, rx, top=14):
+    """SASS lines by warp-stall samples (`ncu --page source --csv`) of the longest launch whose name matches rx."""
+    idx = [k for k, l in enumerate(launches) if re.search(rx, l["full"])]
+    if not idx:
+        return [f"`{rx}`: no launch in the report"]
+    best = max(idx, key=lambda k: launches[k]["gpu__time_duration.sum"] or 0.0)
+    skip = idx.index(best)
+    txt = subprocess.run(["ncu", "-i", path, "--page", "source", "--csv", "--kernel-name", "regex:" + rx],
+                         capture_output=True, text=True).stdout
+    # one block of rows per matching launch, each opened by a "Kernel Name" row: keep the block of the launch wanted
+    blocks = []
+    for r in csv.reader(io.StringIO(txt)):
+        if r and r[0] == "Kernel Name":
+            blocks.append([])
+        elif blocks:
+            blocks[-1].append(r)
+    body = [r for r in (blocks[skip] if skip < len(blocks) else []) if len(r) > 5 and r[2].isdigit() and r[5].isdigit()]
+    if not body:
+        return [f"`{rx}`: no source page in the report"]
+    tot, toti = sum(int(r[2]) for r in body), sum(int(r[5]) for r in body)
+    out = [f"Hottest SASS lines of `{launches[best]['name']}` ({launches[best]['gpu__time_duration.sum']:.1f} us; {toti} warp "
+           f"instructions, {tot} stall samples; `ncu --page source --csv`, sorted by samples):", "", "```"]
+    for r in sorted(body, key=lambda r: -int(r[2]))[:top]:
+        out.append(f"{100 * int(r[2]) / max(tot, 1):5.1f}% samples {100 * int(r[5]) / max(toti, 1):5.2f}% instr        {r[1].strip()}")
+    return out + ["```"]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("report")
@@ -78,6 +105,8 @@ def main():
     ap.add_argument("--out", required=True)
     ap.add_argument("--traffic", action="append", default=[], help="KEY=KERNEL_REGEX:DIVISOR")
     ap.add_argument("--note", action="append", default=[])
+    ap.add_argument("--hot", action="append", default=[],
+                    help="KERNEL_REGEX: append the SASS lines with the most warp-stall samples of the longest launch that matches")
     ap.add_argument("--traffic-file", default=TRAFFIC, help="where the traffic table lives (default profiles/r02_traffic.json)")
     ap.add_argument("--source-name", default=None, help="path recorded as the entry's source (default: --out)")
     a = ap.parse_args()
@@ -85,6 +114,17 @@ def main():
     groups = {}
     for l in launches:
         groups.setdefault(l["name"], []).append(l)
+    # mps_step launches the kernels of its two skin bins in every step and those of a bin that is not needed
+    # return at once: keep them apart from the launches that ran
+    split = {}
+    for name, ls in groups.items():
+        tmax = max((l["gpu__time_duration.sum"] or 0.0) for l in ls)
+        ran = [l for l in ls if (l["gpu__time_duration.sum"] or 0.0) >= 0.05 * tmax]
+        idle = [l for l in ls if l not in ran]
+        split[name] = ran
+        if idle:
+            split[name + " (bin not needed: returned at once)"] = idle
+    groups = split
     lines = [f"# {a.title}", "", "Command (one B200 under `gpurun`, after the same command exited 0 without ncu):", "",
              "    " + a.command, "",
              f"Summary written by `python -m paper_2105_01677_b200.ncu_summary {os.path.basename(a.report)} ...` "
@@ -108,6 +148,8 @@ def main():
         lines.append(f"| {name} | {len(ls)} | {ls[0]['grid']} x {ls[0]['block']} | " + " | ".join(cells) + " |")
     for n in a.note:
         lines += ["", n]
+    for rx in a.hot:
+        lines += ["", *hot_lines(a.report, launches, rx)]
     if a.traffic:
         try:
             with open(a.traffic_file) as f:

@@ -1,9 +1,11 @@
 """Run W warm-up steps, then ONE step between cudaProfilerStart / cudaProfilerStop.
 
     ncu --profile-from-start off --set full ... python -m paper_2105_01677_b200.profile_step \
-        --config 5 --sweep-index 3 --route ppe [--warmup 3] [--steps 1] [--ppe-operator 1] [--key-mode 0]
+        --config 5 --sweep-index 3 --route ppe [--warmup 3] [--steps 1] [--ppe-operator 1] [--key-mode 0] [--row-skin S]
 
-so that an Nsight Compute capture holds exactly the kernels of the profiled step(s).  Measurement
+so that an Nsight Compute capture holds exactly the kernels of the profiled step(s).  --warmup 0 profiles the
+first step, the one that bins (with the default skin the later steps of a scene at rest skip their bins).  Run
+it with MPS_B200_COND=0: Nsight Compute cannot see kernels of a graph that holds conditional nodes.  Measurement
 tooling: argument marshalling only, every kernel is the library's.
 """
 from __future__ import annotations
@@ -26,6 +28,7 @@ def main():
     ap.add_argument("--steps", type=int, default=1)
     ap.add_argument("--ppe-operator", type=int, default=None)
     ap.add_argument("--key-mode", type=int, default=None)
+    ap.add_argument("--row-skin", type=float, default=None)
     a = ap.parse_args()
     import torch
     import __graft_entry__ as ge
@@ -36,6 +39,8 @@ def main():
         s.params["ppe_operator"] = a.ppe_operator
     if a.key_mode is not None:
         s.params["key_mode"] = a.key_mode
+    if a.row_skin is not None:
+        s.params["row_skin"] = a.row_skin
     route = 1 if a.route == "ppe" else 0
     g = B.Mps(s)
     g.step(a.warmup, route)
