@@ -107,9 +107,10 @@ typedef struct mps_params {
   int32_t ppe_operator;     /* (1) how the CG applies A of Listing 2.  0: matrix-free -- rows hold
                                neighbour indices only and every application recomputes c_ij from the positions;
                                1: assembled -- the coefficients of the rows bc = 0 are computed once per solve
-                               (positions are fixed during a solve) into a compact ELL matrix (fp64 value +
-                               uint32 column, the paper's poiss[] of P:272-282 without its N x 300 stride over all
-                               particles) and every application streams it.  Same operator, same parity bars. */
+                               (positions are fixed during a solve) into a compact ELL matrix over the unknowns
+                               (one 64-bit word per pair: 24-bit column + 40-bit fixed-point coefficient, Q28; the
+                               paper's poiss[] of P:272-282 without its N x 300 stride over all particles) and
+                               every application streams it.  Same operator, same parity bars; needs n < 2^24. */
   int32_t cg_warm_start;    /* (0) 1: CG starts from the previous step's pressure of the particle (x0 = p^k on
                                the rows bc = 0) instead of x0 = 0 (Q15); one extra operator application per solve */
   double l0;                /* initial particle spacing */

@@ -240,9 +240,13 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 // whose j is an unknown too as (value, compact column), in the row's order, at the start of
 // ELL row g; neighbours on the free surface (p = 0) only add to the diagonal term.
 // Every lane of the warp must come through here with a warp-uniform trip count m_max.
-template <bool TWO_PHASE>
+// The word needs the row's scale before its first coefficient is known.  EXACT = false: one pass with a
+// provisional scale -- the coefficient of a pair at 0.5 l0 (kc.asm_wmax), within a bit or two of the true
+// largest one of a row -- packing as it goes; if some pair of the row is closer than that (redo), the caller
+// runs the row again with EXACT = true: coefficients to scratch, their true maximum, then the packing pass.
+template <bool TWO_PHASE, bool EXACT>
 __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs& a, int g, int i, int sub,
-                                                 int grp, bool live, uint32_t m_max) {
+                                                 int grp, bool live, uint32_t m_max, bool& redo) {
   const double4 pi = a.pos4[i];
   const uint32_t* row = row_ptr(a.nbr, kc.stride, i);
   const uint32_t nf = live ? a.cn[i] : 0u;
@@ -253,6 +257,9 @@ __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs
   const double scale = (hl ? kc.hl_c : kc.A_lap) * (TWO_PHASE ? 1.0 : 1.0 / kc.rho[0]);
   double* vrow = a.mval + (size_t)g * (size_t)kc.stride;
   uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
+  unsigned long long* prow = reinterpret_cast<unsigned long long*>(vrow);
+  const double cprov = scale * kc.asm_wmax * (TWO_PHASE ? fmax(inv_rij0, inv_rij1) : 1.0);
+  const double invp = PACK_QMAX / cprov;
   const uint32_t lt = (1u << sub) - 1u;
   uint32_t cnt = 0;
   double dex = 0.0, cmax = 0.0;
@@ -284,8 +291,12 @@ __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs
       const uint32_t m8 = (__ballot_sync(0xffffffffu, off) >> (grp * L)) & ((1u << L) - 1u);
       if (off) {
         const uint32_t at = cnt + (uint32_t)__popc(m8 & lt);
-        vrow[at] = c;
-        crow[at] = rm[u];
+        if (EXACT) {
+          vrow[at] = c;
+          crow[at] = rm[u];
+        } else {
+          prow[at] = ((unsigned long long)rm[u] << 40) | __double2ull_rn(fmin(c, cprov) * invp);
+        }
         cmax = fmax(cmax, c);
       }
       cnt += (uint32_t)__popc(m8);
@@ -293,18 +304,20 @@ __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs
   }
   dex = group_sum<L>(dex);
   cmax = group_max<L>(cmax);
-  // second pass over the row just written (L1 / L2 hot): pack (coefficient, column) into one word
-  __syncwarp();
-  const double inv = cmax > 0.0 ? PACK_QMAX / cmax : 0.0;
-  unsigned long long* prow = reinterpret_cast<unsigned long long*>(vrow);
-  for (uint32_t k = sub; k < cnt; k += L) {
-    const unsigned long long q = __double2ull_rn(vrow[k] * inv);
-    prow[k] = ((unsigned long long)crow[k] << 40) | q;
+  redo = !EXACT && cmax > cprov;
+  if (EXACT) {
+    // second pass over the row just written (L1 / L2 hot): pack (coefficient, column) into one word
+    __syncwarp();
+    const double inv = cmax > 0.0 ? PACK_QMAX / cmax : 0.0;
+    for (uint32_t k = sub; k < cnt; k += L) {
+      const unsigned long long q = __double2ull_rn(vrow[k] * inv);
+      prow[k] = ((unsigned long long)crow[k] << 40) | q;
+    }
   }
   if (live && sub == 0) {
     a.mcnt[g] = cnt;
     a.mdex[g] = dex + kc.compress_dt2;
-    a.mscale[g] = cmax / PACK_QMAX;
+    a.mscale[g] = (EXACT ? cmax : cprov) / PACK_QMAX;
   }
   return cnt;
 }
@@ -489,7 +502,10 @@ k_ppe_cg(KConst kc, PpeArgs a) {
       const int i = live ? (int)a.rows[g] : 0;
       uint32_t m = live ? a.cn[i] + a.co[i] : 0u;
       m = __reduce_max_sync(0xffffffffu, m);
-      const uint32_t cnt = assemble_row<TWO_PHASE>(kc, a, live ? g : 0, i, sub, grp, live, m);
+      bool redo;
+      uint32_t cnt = assemble_row<TWO_PHASE, false>(kc, a, live ? g : 0, i, sub, grp, live, m, redo);
+      if (__any_sync(0xffffffffu, redo))  // a pair closer than 0.5 l0 in one of the warp's rows: the two-pass form
+        cnt = assemble_row<TWO_PHASE, true>(kc, a, live ? g : 0, i, sub, grp, live, m, redo);
       if (live && sub == 0) {
         nnz += cnt;
         a.xc[g] = a.x[i];

@@ -72,6 +72,7 @@ static void free_all(mps_ctx* c) {
   }
   cudaFree(c->ent); cudaFree(c->key); cudaFree(c->key_tmp); cudaFree(c->rank); cudaFree(c->tmp_src);
   cudaFree(c->tmp_oid); cudaFree(c->cell_count); cudaFree(c->cell_start); cudaFree(c->scan_tmp);
+  cudaFree(c->gbit); cudaFree(c->gcnt); cudaFree(c->gpre);
   cudaFree(c->nbr); cudaFree(c->cn); cudaFree(c->co); cudaFree(c->pos_ref);
   cudaFree(c->dens); cudaFree(c->p); cudaFree(c->acc4); cudaFree(c->nut); cudaFree(c->b);
   cudaFree(c->phat); cudaFree(c->dndt); cudaFree(c->rho_s[0]); cudaFree(c->rho_s[1]); cudaFree(c->keep2[0]); cudaFree(c->keep2[1]); cudaFree(c->grad4); cudaFree(c->bc);
@@ -172,6 +173,10 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     }
   k.relax = prm->ppe_relax;
   k.hl_c = 2.0 * prm->re_lap / k.n0_lap;
+  {
+    const double r0 = 0.5 * prm->l0;
+    k.asm_wmax = prm->ppe_laplacian == 1 ? 1.0 / (r0 * r0 * r0) : prm->kernel == 1 ? 1.0 : prm->re_lap / r0 - 1.0;
+  }
   k.ppe_source = prm->ppe_source; k.ppe_laplacian = prm->ppe_laplacian;
   k.kernel = prm->kernel; k.inv_re_n = 1.0 / prm->re_n; k.inv_re_lap = 1.0 / prm->re_lap;
   c->h = std::max(prm->re_n, prm->re_lap) / prm->cell_div;
@@ -252,6 +257,7 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
   A(dalloc(&c->tmp_src, N + 1)); A(dalloc(&c->tmp_oid, N));
   A(dalloc(&c->cell_count, (size_t)ncells + 2)); A(dalloc(&c->cell_start, (size_t)ncells + 2));
   A(dalloc(&c->scan_tmp, std::max<size_t>((size_t)ncells + 2, N) / 2048 + 2));
+  A(dalloc(&c->gbit, N / 32 + 2)); A(dalloc(&c->gcnt, N / 32 + 2)); A(dalloc(&c->gpre, N / 32 + 2));
   A(dalloc(&c->nbr, N * (size_t)k.stride)); A(dalloc(&c->cn, N)); A(dalloc(&c->co, N));
   A(dalloc(&c->pos_ref, c->carry_rows ? N : 1));
   if (c->carry_rows) A(cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));

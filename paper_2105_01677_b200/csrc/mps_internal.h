@@ -78,6 +78,7 @@ struct KConst {  // by-value kernel parameter
   double cs_l0_sq, d_over_n0;
   double inv_rho_pair[2][2];  // 1 / rho_ij by the phases of i and j (arithmetic or harmonic mean, Q6)
   double relax, hl_c;  // ppe_relax; 2 re_lap / n0_lap (Eq. 16)
+  double asm_wmax;     // pair weight of the PPE operator at r = 0.5 l0: provisional row scale of the assembly
   int ppe_source, ppe_laplacian;
   int kernel;          // 0: Eq. 3, 1: Eq. 4
   int stale;           // 1 while mps_step walks reused rows: every pair is re-tested (Q24)
@@ -149,6 +150,9 @@ struct mps_ctx {
   uint32_t* cell_count = nullptr;  // ncells + 2
   uint32_t* cell_start = nullptr;  // ncells + 2
   uint32_t* scan_tmp = nullptr;
+  uint32_t* gbit = nullptr;        // ghosts by original index: bitmap, ones per word, their exclusive scan
+  uint32_t* gcnt = nullptr;
+  uint32_t* gpre = nullptr;
   // neighbour rows
   uint32_t* nbr = nullptr;
   uint32_t* cn = nullptr;

@@ -79,6 +79,31 @@ def test_bin_is_bit_exact(B, O, scene, cell_div, key_mode):
     assert np.array_equal(g.perm(), perm) and np.array_equal(g.cell_start(), cs)
 
 
+def test_bin_with_many_ghosts_is_bit_exact(B, O):
+    """A third of config 1 outside the domain (what a tank looks like after the fluid has been thrown out):
+    the ghosts sit behind the last cell in ascending original index, ranked from a bitmap (no loop over
+    the ghost pseudo-cell); a second bin of the sorted state and a step leave the order as the oracle's."""
+    s = scenes.make_scene(1, shuffle=True)
+    rng = np.random.default_rng(11)
+    out = rng.random(s.n) < 0.33
+    s.z[out] = 5.0 + rng.random(int(out.sum()))
+    o = O.Oracle(s)
+    key, perm, cs = o.bin()
+    g = B.Mps(s)
+    g.bin()
+    assert np.array_equal(g.get("key"), key) and np.array_equal(g.perm(), perm)
+    assert np.array_equal(g.cell_start(), cs)
+    assert g.stats()["n_ghost"] == int(out.sum()) == o.stats()["n_ghost"]
+    assert (np.diff(perm[-int(out.sum()):]) > 0).all()          # ascending original index
+    g.bin()
+    assert np.array_equal(g.perm(), perm)
+    g.step(2, 0); o.step(2, 0)
+    assert np.array_equal(g.get("type"), o.get("type"))
+    L = max(hi - lo for lo, hi in zip(s.params["domain_min"], s.params["domain_max"]))
+    live = o.get("type") != 3
+    assert max(np.abs(g.get(k) - o.get(k))[live].max() for k in "xyz") <= 1e-7 * L
+
+
 def test_bin_after_motion_matches_oracle(B, O):
     s = scenes.small_tank(shuffle=True)
     o = moved_state(O, s, 3)
@@ -273,6 +298,34 @@ def test_ppe_flags_rhs_operator_and_solution(B, O, over, op):
     # pressures (after the clamp) against the oracle's own solve at the same tolerance
     o.pressure_ppe()
     assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-8 * kappa_est
+
+
+def test_assembled_operator_with_a_close_pair(B, O):
+    """The assembly packs with a provisional row scale (the coefficient of a pair at 0.5 l0) and falls back to
+    the two-pass form for a row that holds a closer pair.  Two interior fluid particles at 0.3 l0: operator
+    parity on a random vector and the solve's true residual, as for any other row."""
+    s = scenes.small_tank(shuffle=False)
+    l0 = s.params["l0"]
+    fl = np.flatnonzero(s.type == scenes.FLUID)
+    c = np.array([s.x[fl].mean(), s.y[fl].mean(), s.z[fl].mean()])
+    d2 = (s.x[fl] - c[0]) ** 2 + (s.y[fl] - c[1]) ** 2 + (s.z[fl] - c[2]) ** 2
+    i, j = fl[np.argsort(d2)[:2]]
+    s.x[j], s.y[j], s.z[j] = s.x[i] + 0.3 * l0, s.y[i], s.z[i]
+    g, o = B.Mps(s, ppe_operator=1), O.Oracle(s)     # at rest: a step would blow the pair apart
+    g.bin(); o.bin()
+    g.density(); o.density()
+    g.set("n", np.minimum(o.get("n"), 1.2 * o.constants()["n0_n"]))   # the pair's own n is huge: keep both unknowns
+    o.set("n", np.minimum(o.get("n"), 1.2 * o.constants()["n0_n"]))
+    it_g, relres_g = g.pressure_ppe()
+    o.ppe_flags(); o.ppe_rhs()
+    bc = o.get("bc")
+    assert np.array_equal(g.get("bc"), bc) and bc[i] == 0 and bc[j] == 0
+    rows = bc == 0
+    v = np.where(rows, np.random.default_rng(1).standard_normal(s.n), 0.0)
+    Ao = o.ppe_apply(v)
+    assert relerr(g.ppe_apply(v), Ao, 1e-30) <= TOL
+    x, b = g.get("xcg"), o.get("b")
+    assert np.linalg.norm(b - o.ppe_apply(x)) / np.linalg.norm(b) <= 2e-8
 
 
 @pytest.mark.parametrize("op", [0, 1])
