@@ -901,6 +901,30 @@ def test_row_skin_sets_stay_bit_exact(B, O, rows, skin, monkeypatch):
     assert max(seen) < 20        # fewer than two bins per step: rows were reused in between
 
 
+@pytest.mark.parametrize("route", [0, 1])
+def test_row_skin_particles_leaving_the_domain_become_ghosts(B, O, route):
+    """The top fluid layer is thrown upwards through the open top over the next steps: the predictor / corrector
+    must notice on the device that a particle left the domain, the bin that follows makes it a GHOST exactly when
+    the oracle's BIN does, and the rest of the fluid follows the oracle."""
+    s = scenes.small_tank(shuffle=True)
+    zmax = s.params["domain_max"][2]
+    top = (s.type == scenes.FLUID) & (s.z > s.z[s.type == scenes.FLUID].max() - 0.5 * s.params["l0"])
+    rng = np.random.default_rng(2)
+    # speeds that carry the particles out at different steps (2.5 to 12 steps away)
+    s.w[top] = (zmax - s.z[top]) / (s.params["dt"] * rng.uniform(2.5, 12.0, int(top.sum())))
+    g, o = B.Mps(s), O.Oracle(s)
+    seen = []
+    for _ in range(7):
+        g.step(2, route); o.step(2, route)
+        assert np.array_equal(g.get("type"), o.get("type"))
+        seen.append(int((o.get("type") == 3).sum()))
+    assert 0 < seen[2] < seen[-1] <= int(top.sum()) and seen[-1] == g.stats()["n_ghost"]   # they leave a few at a time
+    live = o.get("type") != 3
+    L = max(hi - lo for lo, hi in zip(s.params["domain_min"], s.params["domain_max"]))
+    assert max(np.abs(g.get(k) - o.get(k))[live].max() for k in "xyz") <= 1e-7 * L
+    print(f"route {route}: ghosts after 2, 4, ... steps {seen}, bins {g.stats()['bins_total']}")
+
+
 def test_row_skin_follows_a_route_change(B, O):
     """Explicit steps keep the re_lap part of fluid rows only; a PPE step after them needs every row."""
     s = scenes.small_tank(shuffle=True)
