@@ -312,7 +312,10 @@ enum {
 };
 int mps_timers_enable(mps_ctx* ctx, int32_t mask);
 int mps_timers_read(mps_ctx* ctx, double* ms, int64_t* launches);
-/* Kernels launched by this ctx so far (every __global__ launch is counted). */
+/* Kernels launched by this ctx so far: every __global__ launch issued by the host, plus the kernels of the skin
+ * bins that ran as bodies of conditional graph nodes (counted on the device; as of the last mps_step / mps_sync /
+ * mps_get_stats, which read the counter).  A bin that did not run is not counted.  While timers are on
+ * (mps_timers_enable) mps_step reads the device flag before each of its bins and leaves out the ones not needed. */
 int64_t mps_launch_count(mps_ctx* ctx);
 /* Message of the last error of this ctx (owned by the ctx; valid until the
  * next call).  ctx == NULL returns the message of the last failed mps_init. */

@@ -301,7 +301,7 @@ k_phat(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__
 // --------------------------------------------------------------- S10 gradient ---
 // G_i = (d/n0) sum coef / r^2 (r_j - r_i) w(r) over non-dummy j in N(i, re_n):
 // coef = p_j - phat_i (0) | (p_i + p_j) - (phat_i + phat_j) (1, Eq. 14) | p_i + p_j (2).
-// Variants 0 and 2 find phat_i in a first pass over the same row (no pre-pass
+// Variants 0 and 2 find phat_i in the same pass over the row as the sum (no pre-pass
 // kernel); variant 1 needs phat_j of the neighbours, so k_phat runs first.
 template <int VARIANT>
 __global__ void __launch_bounds__(TPB)
@@ -314,33 +314,23 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
   const bool wall = row_live && ty == MPS_WALL;
   const double4 pi = pos4[ii];  // .w = p_i
   const uint32_t* row = row_ptr(nbr, kc.stride, ii);
-  const uint32_t m = (fluid || wall) ? cn[ii] : 0u;
+  // variants 0 and 2 also produce p-hat, which wall rows have too; the sum itself is for fluid rows
+  const uint32_t m = ((VARIANT == 0 || VARIANT == 2) ? (fluid || wall) : fluid) ? cn[ii] : 0u;
   double phi = 0.0;
-  if (VARIANT == 3) {
-    // pi.w = beta_i; phat carries <rho> (see mpsk_gradient): nothing to pre-compute
-  } else if (VARIANT == 1) {
-    phi = phat[ii];
-  } else {
-    double mn = pi.w;
-    for (uint32_t k = sub; k < m; k += L) {
-      const uint32_t e = row[k];
-      if (e & NB_DUMMY) continue;
-      const double4 q = gather_rec(kc.pos_tex, pos4, e & NB_INDEX);
-      if (kc.stale && !(pair_r2(q.x - pi.x, q.y - pi.y, q.z - pi.z, 1) < kc.re_n2)) continue;
-      mn = fmin(mn, q.w);
-    }
-    phi = group_min<L>(mn);
-    if (row_live && sub == 0) phat[i] = (fluid || wall) ? phi : 0.0;
-  }
+  if (VARIANT == 1) phi = phat[ii];
   double inv_rsi = 0.0, ai = 0.0, scale = kc.d_over_n0;
   if (VARIANT == 3) {
+    // pi.w = beta_i; phat carries <rho> (see mpsk_gradient): nothing to pre-compute
     inv_rsi = 1.0 / phat[ii];     // phat points at <rho> for this variant
     ai = pi.w * inv_rsi;          // alpha_i = beta_i / <rho>_i
     scale *= kc.rho[(tp[ii] >> 8) & 1];  // stored as rho_i x Eq. 11: the corrector divides by rho_i
   }
-  double sx = 0.0, sy = 0.0, sz = 0.0;
-  const uint32_t mg = fluid ? m : 0u;
-  for (uint32_t k = sub; k < mg; k += L) {
+  // ONE pass over the row.  Variant 0 is linear in phat_i: sum (p_j - phat_i) c x_ij = sum p_j c x_ij -
+  // phat_i sum c x_ij, so the minimum and both sums come out of the same gathers (the two-pass form gathered
+  // every record twice); the difference to the oracle's order of operations is rounding (a few 1e-14 relative).
+  double sx = 0.0, sy = 0.0, sz = 0.0, bx = 0.0, by = 0.0, bz = 0.0;
+  double mn = pi.w;
+  for (uint32_t k = sub; k < m; k += L) {
     const uint32_t e = row[k];
     if (e & NB_DUMMY) continue;
     const uint32_t j = e & NB_INDEX;
@@ -348,17 +338,34 @@ k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ pha
     const double dx = q.x - pi.x, dy = q.y - pi.y, dz = q.z - pi.z;
     const double r2 = pair_r2(dx, dy, dz, kc.stale);
     if (kc.stale && !(r2 < kc.re_n2)) continue;
+    if (VARIANT == 0 || VARIANT == 2) mn = fmin(mn, q.w);
     const double ir = rsqrt_f64(r2);
+    const double c = kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, ir) * ir * ir;
     double coef;
-    if (VARIANT == 0) coef = q.w - phi;
+    if (VARIANT == 0) coef = q.w;
     else if (VARIANT == 1) coef = (pi.w + q.w) - (phi + phat[j]);
     else if (VARIANT == 2) coef = pi.w + q.w;
     else coef = fma(q.w, inv_rsi, -ai);  // (<rho>_j / <rho>_i) alpha_j - alpha_i, Eq. 11
-    const double c = coef * kernel_w(kc.kernel, kc.re_n, kc.inv_re_n, r2, ir) * ir * ir;
-    sx += c * dx;
-    sy += c * dy;
-    sz += c * dz;
+    const double cc = coef * c;
+    sx += cc * dx;
+    sy += cc * dy;
+    sz += cc * dz;
+    if (VARIANT == 0) {
+      bx += c * dx;
+      by += c * dy;
+      bz += c * dz;
+    }
   }
+  if (VARIANT == 0 || VARIANT == 2) {
+    phi = group_min<L>(mn);
+    if (row_live && sub == 0) phat[i] = (fluid || wall) ? phi : 0.0;
+  }
+  if (VARIANT == 0) {
+    sx = fma(-phi, bx, sx);
+    sy = fma(-phi, by, sy);
+    sz = fma(-phi, bz, sz);
+  }
+  if (!fluid) sx = sy = sz = 0.0;  // wall rows only wanted their p-hat
   sx = group_sum<L>(sx);
   sy = group_sum<L>(sy);
   sz = group_sum<L>(sz);
