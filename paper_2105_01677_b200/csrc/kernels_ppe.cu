@@ -40,6 +40,12 @@ constexpr int PPE_ILP = 4;   // independent neighbour gathers in flight per lane
 // (measured at 1.44M rows: 315 ps per row per iteration with 4, 265 with 8; two blocks per SM at 32
 // registers spill and are slower, 303-330)
 constexpr int ASM_ILP = 8;
+#ifndef MPS_ASM_L
+#define MPS_ASM_L 8
+#endif
+// lanes per row in the CG loop's operator application (assembled form); measured at 1.44M rows: 4 lanes 229 ps
+// per row per iteration, 8 lanes 216, 16 lanes 243 (260k rows: 259 / 221 / 239)
+constexpr int ASM_L = MPS_ASM_L;
 constexpr double PACK_QMAX = 1099511627775.0;  // 2^40 - 1: a stored coefficient is q / QMAX of the row's largest
 constexpr int CG_TPB = 1024;
 constexpr int L = 8;         // lanes per row
@@ -331,17 +337,18 @@ __device__ __forceinline__ uint32_t assemble_row(const KConst& kc, const PpeArgs
 __device__ __forceinline__ double word_coef(uint32_t hi, uint32_t lo) {
   return __hiloint2double((int)((hi & 0xffu) | 0x43300000u), (int)lo) - 4503599627370496.0;
 }
+template <int LL = L>
 __device__ __forceinline__ double asm_row(const KConst& kc, const PpeArgs& a, const double* __restrict__ v,
                                           int g, int sub, bool live, double& vg) {
   vg = v[g];
   const uint32_t n = live ? a.mcnt[g] : 0u;
   const unsigned long long* prow = reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g * (size_t)kc.stride;
   double s0 = 0.0, s1 = 0.0;
-  for (uint32_t k = sub; k < n; k += ASM_ILP * L) {
+  for (uint32_t k = sub; k < n; k += ASM_ILP * LL) {
     unsigned long long w[ASM_ILP];
 #pragma unroll
     for (int u = 0; u < ASM_ILP; ++u) {
-      const uint32_t kk = k + (uint32_t)(u * L);
+      const uint32_t kk = k + (uint32_t)(u * LL);
       w[u] = kk < n ? __ldcs(prow + kk) : ((unsigned long long)(uint32_t)g << 40);  // q = 0, column g
     }
     double vj[ASM_ILP];
@@ -355,7 +362,7 @@ __device__ __forceinline__ double asm_row(const KConst& kc, const PpeArgs& a, co
       s1 = fma(c1, vg - vj[u + 1], s1);
     }
   }
-  const double s = group_sum<L>(s0 + s1);
+  const double s = group_sum<LL>(s0 + s1);
   return live ? fma(a.mdex[g], vg, a.mscale[g] * s) : 0.0;
 }
 
@@ -555,33 +562,43 @@ k_ppe_cg(KConst kc, PpeArgs a) {
       // assembled operator: the loop is bound by HBM latency x bytes in flight, so each group asks
       // the L2 for the words of its NEXT row (one 128-byte line per lane, as many as that row has)
       // while it works on this one; the row counts run one more row ahead
-      uint32_t n_ahead = 0;
       if (ASM) {
-        const int g1 = (sc_first + sc_step) * (SCW * GPW) + g_in_sc;
-        n_ahead = g1 < n_rows ? a.mcnt[g1] : 0u;
-      }
-      for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
-        const int g = sc * (SCW * GPW) + g_in_sc;
-        const bool live = g < n_rows;
-        double ri, wi;
-        if (ASM) {
-          const int g1 = g + sc_step * (SCW * GPW), g2 = g1 + sc_step * (SCW * GPW);
-          if ((uint32_t)(sub * 16) < n_ahead)
-            prefetch_l2(reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g1 * (size_t)kc.stride + sub * 16);
-          if (sub == 0 && n_ahead > 128u)  // a row longer than 128 pairs: its second kilobyte
-            for (uint32_t k = 128; k < n_ahead; k += 16)
-              prefetch_l2(reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g1 * (size_t)kc.stride + k);
-          n_ahead = g2 < n_rows ? a.mcnt[g2] : 0u;
-          wi = asm_row(kc, a, a.rc, live ? g : 0, sub, live, ri);
-          if (live && sub == 0) a.wv[g] = wi;
-        } else {
-          const int i = live ? (int)a.rows[g] : 0;
-          wi = ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
-          if (live && sub == 0) a.wv[i] = wi;
+        // LA lanes per row: a batch of ASM_ILP words per lane covers 8 LA entries of the row
+        constexpr int LA = ASM_L, GPWA = 32 / LA;
+        const int subA = lane & (LA - 1);
+        const int g_in_scA = (wid % SCW) * GPWA + lane / LA;
+        uint32_t n_ahead = 0;
+        {
+          const int g1 = (sc_first + sc_step) * (SCW * GPWA) + g_in_scA;
+          n_ahead = g1 < n_rows ? a.mcnt[g1] : 0u;
         }
-        if (live && sub == 0) {
-          g_part = fma(ri, ri, g_part);
-          d_part = fma(ri, wi, d_part);
+        for (int sc = sc_first; sc * (SCW * GPWA) < n_rows; sc += sc_step) {
+          const int g = sc * (SCW * GPWA) + g_in_scA;
+          const bool live = g < n_rows;
+          double ri;
+          const int g1 = g + sc_step * (SCW * GPWA), g2 = g1 + sc_step * (SCW * GPWA);
+          for (uint32_t k = (uint32_t)subA * 16u; k < n_ahead; k += 16u * LA)
+            prefetch_l2(reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g1 * (size_t)kc.stride + k);
+          n_ahead = g2 < n_rows ? a.mcnt[g2] : 0u;
+          const double wi = asm_row<LA>(kc, a, a.rc, live ? g : 0, subA, live, ri);
+          if (live && subA == 0) {
+            a.wv[g] = wi;
+            g_part = fma(ri, ri, g_part);
+            d_part = fma(ri, wi, d_part);
+          }
+        }
+      } else {
+        for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
+          const int g = sc * (SCW * GPW) + g_in_sc;
+          const bool live = g < n_rows;
+          double ri;
+          const int i = live ? (int)a.rows[g] : 0;
+          const double wi = ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+          if (live && sub == 0) {
+            a.wv[i] = wi;
+            g_part = fma(ri, ri, g_part);
+            d_part = fma(ri, wi, d_part);
+          }
         }
       }
       block_sum2<CG_TPB>(g_part, d_part);
