@@ -46,6 +46,10 @@ constexpr int ASM_ILP = 8;
 // lanes per row in the CG loop's operator application (assembled form); measured at 1.44M rows: 4 lanes 229 ps
 // per row per iteration, 8 lanes 216, 16 lanes 243 (260k rows: 259 / 221 / 239)
 constexpr int ASM_L = MPS_ASM_L;
+#ifndef MPS_ASM_RUN_LOG2
+#define MPS_ASM_RUN_LOG2 3
+#endif
+constexpr int ASM_RUN_LOG2 = MPS_ASM_RUN_LOG2;  // log2 of the consecutive super-chunks a warp group works through before it jumps
 constexpr double PACK_QMAX = 1099511627775.0;  // 2^40 - 1: a stored coefficient is q / QMAX of the row's largest
 constexpr int CG_TPB = 1024;
 constexpr int L = 8;         // lanes per row
@@ -567,16 +571,25 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         constexpr int LA = ASM_L, GPWA = 32 / LA;
         const int subA = lane & (LA - 1);
         const int g_in_scA = (wid % SCW) * GPWA + lane / LA;
+        // super-chunks are dealt in runs of ASM_RUN consecutive ones (round-robin over the grid between runs): the
+        // next trip of a warp then works on the rows next to the ones it just did, whose neighbours it has just
+        // gathered into this SM's L1
+        // (runs of 2^ASM_RUN_LOG2 super-chunks; single ones when a warp group would get fewer than eight runs --
+        // load balance: 260k rows measured 221 ps per row per iteration with single super-chunks, 227 with runs of 8)
+        constexpr int RPS = SCW * GPWA;  // rows per super-chunk
+        const int rs = n_rows >= RPS * sc_step * 8 * (1 << ASM_RUN_LOG2) ? ASM_RUN_LOG2 : 0;
+        auto row_of = [&](int t) { return ((((sc_first + (t >> rs) * sc_step) << rs) + (t & ((1 << rs) - 1))) * RPS) + g_in_scA; };
+        auto trips_left = [&](int t) { return ((sc_first + (t >> rs) * sc_step) << rs) * RPS < n_rows; };
         uint32_t n_ahead = 0;
         {
-          const int g1 = (sc_first + sc_step) * (SCW * GPWA) + g_in_scA;
+          const int g1 = row_of(1);
           n_ahead = g1 < n_rows ? a.mcnt[g1] : 0u;
         }
-        for (int sc = sc_first; sc * (SCW * GPWA) < n_rows; sc += sc_step) {
-          const int g = sc * (SCW * GPWA) + g_in_scA;
+        for (int t = 0; trips_left(t); ++t) {
+          const int g = row_of(t);
           const bool live = g < n_rows;
           double ri;
-          const int g1 = g + sc_step * (SCW * GPWA), g2 = g1 + sc_step * (SCW * GPWA);
+          const int g1 = row_of(t + 1), g2 = row_of(t + 2);
           for (uint32_t k = (uint32_t)subA * 16u; k < n_ahead; k += 16u * LA)
             prefetch_l2(reinterpret_cast<const unsigned long long*>(a.mval) + (size_t)g1 * (size_t)kc.stride + k);
           n_ahead = g2 < n_rows ? a.mcnt[g2] : 0u;
