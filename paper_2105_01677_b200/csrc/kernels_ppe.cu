@@ -54,8 +54,11 @@ constexpr double PACK_QMAX = 1099511627775.0;  // 2^40 - 1: a stored coefficient
 constexpr int CG_TPB = 1024;
 constexpr int L = 8;         // lanes per row
 constexpr int GPW = 32 / L;  // row groups per warp
-constexpr int SCW = 8;       // warps per super-chunk of consecutive rows
-static_assert(CG_TPB % (32 * SCW) == 0, "phase A deals rows in super-chunks of 8 warps");
+#ifndef MPS_SCW
+#define MPS_SCW 32
+#endif
+constexpr int SCW = MPS_SCW;  // warps per super-chunk of consecutive rows (measured 8 vs 32: 219 vs 215 ps at 260k rows, 207 vs 205 at 5.8M)
+static_assert(CG_TPB % (32 * SCW) == 0, "phase A deals rows in super-chunks of SCW warps");
 
 struct PpeArgs {
   double4* pos4;  // matrix-free: .w is the CG residual r during the solve; pressure at exit
@@ -496,7 +499,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
   const int gtid = bid * CG_TPB + tid;
   const int sub = tid & (L - 1);
   const int grp = lane / L;
-  // Rows are dealt to the blocks in super-chunks of 8 warps (8 * 32 / L consecutive rows, so
+  // Rows are dealt to the blocks in super-chunks of SCW warps (SCW * 32 / L consecutive rows, so
   // the warps that share an SM's L1 work on neighbouring rows) round-robin over the grid:
   // every block gets an even sample of cheap (wall) and expensive (fluid) rows and at most
   // one super-chunk more than any other.  The trip count is warp-uniform.
