@@ -303,6 +303,13 @@ def load_traffic():
         return {}
 
 
+def pre_steps(g, route, n):
+    """n untimed steps in calls of 16: the library looks at its row skin between mps_step calls."""
+    while n > 0:
+        g.step(min(n, 16), route)
+        n -= 16
+
+
 def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K, W, sample_clocks):
     """One route of one scene: the device-resident timed steps, then an instrumented replay of the
     same steps with per-kernel CUDA events, and the roofline of the dominant kernel."""
@@ -324,8 +331,7 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
             g0.step(1, route)
         g0.close()
     g = B.Mps(scene, device=str(dev))
-    if getattr(args, "pre_steps", 0) > 0:
-        g.step(int(args.pre_steps), route)
+    pre_steps(g, route, int(getattr(args, "pre_steps", 0)))
     g.step(max(W, 3), route)
     l0 = g.launch_count()
     st0 = g.stats()
@@ -370,7 +376,8 @@ def measure_route(torch, np, B, args, scene, route, world, dev, stream, flush, K
 
     # ---- instrumented replay of the same steps: per-kernel CUDA-event times ------------------
     g = B.Mps(scene, device=str(dev))
-    g.step(W + int(getattr(args, "pre_steps", 0)), route)
+    pre_steps(g, route, int(getattr(args, "pre_steps", 0)))
+    g.step(W, route)
     bins0 = g.stats()["bins_total"]
     g.timers_enable((1 << len(B.TIMERS)) - 1)
     ms_replay = timed_steps(torch, 1, g, route, K, flush, stream)

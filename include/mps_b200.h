@@ -137,7 +137,10 @@ typedef struct mps_params {
                                with both radii enlarged by row_skin * l0 and serve every sweep -- each re-tests
                                r2 < re^2 with the rounding of Q2, so the sets stay exact -- until some particle has
                                moved by more than 0.45 skins since the build (checked on the device by the predictor
-                               and the corrector).  0 => the library's default (0.1); < 0 => no skin: mps_step
+                               and the corrector).  0 => the library chooses: 0.1, and 0.3 while a flow needs more
+                               than 0.4 bins per step with 0.1 (looked at between mps_step calls, over windows of
+                               at least 16 steps; back to 0.1 below 0.06 bins per step, and above 0.8, where neither
+                               skin saves a bin and the thin one has the shorter sweeps); < 0 => no skin: mps_step
                                bins at r^k and at r* in every step, as Q7 is literally stated */
 } mps_params;
 
@@ -160,6 +163,7 @@ typedef struct mps_stats {
   int64_t cg_nnz;           /* ppe_operator 1: off-diagonal entries of the matrix assembled by the last solve */
   int64_t bins_total;       /* bins (sort + neighbour rows) run over the life of the ctx: two per step of mps_step
                                without a skin; with one (row_skin), only when a particle has moved 0.45 skins */
+  double row_skin_now;      /* the skin mps_step currently builds its rows with, in units of l0 (-1: none) */
 } mps_stats;
 
 /* mps_init: create a ctx and copy n particles in (device pointers, caller's

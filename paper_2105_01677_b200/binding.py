@@ -66,7 +66,7 @@ class MpsStats(C.Structure):
         ("n_rows", C.c_int32), ("cg_iters_total", C.c_int64), ("steps_total", C.c_int64),
         ("device_error", C.c_int32), ("cg_noconv_total", C.c_int32),
         ("cg_setup_ms", C.c_double), ("cg_loop_ms", C.c_double), ("cg_loop_ms_total", C.c_double),
-        ("cg_nnz", C.c_int64), ("bins_total", C.c_int64),
+        ("cg_nnz", C.c_int64), ("bins_total", C.c_int64), ("row_skin_now", C.c_double),
     ]
 
     def as_dict(self) -> Dict[str, float]:

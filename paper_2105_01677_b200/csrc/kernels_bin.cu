@@ -983,7 +983,7 @@ int mpsk_load_particles(mps_ctx* c, const double* x, const double* y, const doub
 
 int mpsk_bin(mps_ctx* c, int rows_mode, const int* go) {
   const int n = (int)c->n;
-  const KConst& kg = go ? c->kc_step : c->kc;
+  const KConst& kg = go ? c->kc_step[c->skin_level] : c->kc;
   const int nc = kg.ncells;
   const int cur = c->cur, nxt = cur ^ 1;
   if (go && c->timer_mask != 0) {

@@ -49,6 +49,9 @@ constexpr int ASM_L = MPS_ASM_L;
 #ifndef MPS_ASM_RUN_LOG2
 #define MPS_ASM_RUN_LOG2 3
 #endif
+#ifndef MPS_ASM_MINRUNS
+#define MPS_ASM_MINRUNS 8
+#endif
 constexpr int ASM_RUN_LOG2 = MPS_ASM_RUN_LOG2;  // log2 of the consecutive super-chunks a warp group works through before it jumps
 constexpr double PACK_QMAX = 1099511627775.0;  // 2^40 - 1: a stored coefficient is q / QMAX of the row's largest
 constexpr int CG_TPB = 1024;
@@ -580,7 +583,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         // (runs of 2^ASM_RUN_LOG2 super-chunks; single ones when a warp group would get fewer than eight runs --
         // load balance: 260k rows measured 221 ps per row per iteration with single super-chunks, 227 with runs of 8)
         constexpr int RPS = SCW * GPWA;  // rows per super-chunk
-        const int rs = n_rows >= RPS * sc_step * 8 * (1 << ASM_RUN_LOG2) ? ASM_RUN_LOG2 : 0;
+        const int rs = n_rows >= RPS * sc_step * MPS_ASM_MINRUNS * (1 << ASM_RUN_LOG2) ? ASM_RUN_LOG2 : 0;
         auto row_of = [&](int t) { return ((((sc_first + (t >> rs) * sc_step) << rs) + (t & ((1 << rs) - 1))) * RPS) + g_in_scA; };
         auto trips_left = [&](int t) { return ((sc_first + (t >> rs) * sc_step) << rs) * RPS < n_rows; };
         uint32_t n_ahead = 0;

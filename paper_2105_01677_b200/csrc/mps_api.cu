@@ -86,7 +86,7 @@ static void free_all(mps_ctx* c) {
   if (c->cg_host) cudaFreeHost(c->cg_host);
   if (c->flags_host) cudaFreeHost(c->flags_host);
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
-  for (auto& r : c->seg) for (auto& p : r) for (auto& g : p) if (g.exec) cudaGraphExecDestroy(g.exec);
+  for (auto& l : c->seg) for (auto& r : l) for (auto& p : r) for (auto& g : p) if (g.exec) cudaGraphExecDestroy(g.exec);
 }
 
 static int check_params(const mps_params* p, int64_t n) {
@@ -216,34 +216,42 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     // the skin.  A scan of cell_div cells to each side still finds every pair inside the enlarged radius,
     // and the rows stay exact supersets while no particle is further than 0.45 skins from where it was at
     // the build -- which the predictor and the corrector check.  GHOST decisions stay on the contract's grid.
-    KConst& s = c->kc_step;
-    s = k;
-    const double skin = (prm->row_skin == 0.0 ? 0.1 : prm->row_skin) * prm->l0;
-    const double hs = (std::max(prm->re_n, prm->re_lap) + 1.001 * std::max(skin, 0.0)) / prm->cell_div;
-    s.inv_h = 1.0 / hs;
-    int64_t ncs = 1;
-    int ns[3];
-    for (int a = 0; a < 3; ++a) {
-      ns[a] = std::max(1, (int)ceil(nc[a] * c->h * s.inv_h));  // covers the contract grid's extent
-      ncs *= ns[a];
-    }
-    s.nx = ns[0]; s.ny = ns[1]; s.nz = ns[2];
-    if (prm->key_mode == 1) {
-      int bits = 0;
-      while ((1 << bits) < std::max(ns[0], std::max(ns[1], ns[2]))) ++bits;
-      ncs = (int64_t)1 << (3 * bits);
-    }
-    s.ncells = (int)ncs;
-    s.re_lap2 = (prm->re_lap + skin) * (prm->re_lap + skin);
-    s.re_n2 = (prm->re_n + skin) * (prm->re_n + skin);
-    s.R_lap = std::max(1, (int)ceil((prm->re_lap + skin) * s.inv_h - 1e-9));
-    s.R_n = std::max(1, (int)ceil((prm->re_n + skin) * s.inv_h - 1e-9));
-    k.carry_d2 = s.carry_d2 = (0.45 * skin) * (0.45 * skin);
-    // off with the paper's list reuse (rebin_every > 1 has its own schedule, Q24) and with row_skin < 0;
-    // MPS_B200_CARRY=0 forces the two bins per step of reading Q7 as literally stated
+    // Two skins when the caller leaves the choice to the library (row_skin = 0): 0.1 l0, and 0.3 l0 for a flow
+    // that needs more than 0.4 bins per step with the thin one (mps_step switches between calls, see there).
     const char* cr = getenv("MPS_B200_CARRY");
-    c->carry_rows = prm->rebin_every == 1 && skin > 0.0 && ncs <= ncells && s.R_lap == k.R_lap &&
-                    !(cr && atoi(cr) == 0);
+    c->skin_auto = prm->row_skin == 0.0;
+    c->carry_rows = prm->rebin_every == 1 && !(prm->row_skin < 0.0) && !(cr && atoi(cr) == 0);
+    for (int lv = 0; lv < 2; ++lv) {
+      KConst& s = c->kc_step[lv];
+      s = k;
+      const double skin_l0 = c->skin_auto ? (lv == 0 ? 0.1 : 0.3) : prm->row_skin;
+      const double skin = skin_l0 * prm->l0;
+      c->skin_l0[lv] = skin_l0;
+      const double hs = (std::max(prm->re_n, prm->re_lap) + 1.001 * std::max(skin, 0.0)) / prm->cell_div;
+      s.inv_h = 1.0 / hs;
+      int64_t ncs = 1;
+      int ns[3];
+      for (int a = 0; a < 3; ++a) {
+        ns[a] = std::max(1, (int)ceil(nc[a] * c->h * s.inv_h));  // covers the contract grid's extent
+        ncs *= ns[a];
+      }
+      s.nx = ns[0]; s.ny = ns[1]; s.nz = ns[2];
+      if (prm->key_mode == 1) {
+        int bits = 0;
+        while ((1 << bits) < std::max(ns[0], std::max(ns[1], ns[2]))) ++bits;
+        ncs = (int64_t)1 << (3 * bits);
+      }
+      s.ncells = (int)ncs;
+      s.re_lap2 = (prm->re_lap + skin) * (prm->re_lap + skin);
+      s.re_n2 = (prm->re_n + skin) * (prm->re_n + skin);
+      s.R_lap = std::max(1, (int)ceil((prm->re_lap + skin) * s.inv_h - 1e-9));
+      s.R_n = std::max(1, (int)ceil((prm->re_n + skin) * s.inv_h - 1e-9));
+      s.carry_d2 = (0.45 * skin) * (0.45 * skin);
+      // off with the paper's list reuse (rebin_every > 1 has its own schedule, Q24) and with row_skin < 0;
+      // MPS_B200_CARRY=0 forces the two bins per step of reading Q7 as literally stated
+      c->carry_rows = c->carry_rows && skin > 0.0 && ncs <= ncells && s.R_lap == k.R_lap;
+    }
+    k.carry_d2 = c->kc_step[0].carry_d2;
   }
 
   // every buffer any later call needs
@@ -383,6 +391,7 @@ static int read_flags(mps_ctx* c) {
   }
   c->stats.device_error = c->sticky_error;
   c->stats.bins_total = c->bins_run + c->flags_host->bins;
+  c->stats.row_skin_now = c->carry_rows ? c->skin_l0[c->skin_level] : -1.0;
   return c->sticky_error;
 }
 
@@ -430,7 +439,7 @@ static void restore_state(mps_ctx* c, const HostState& h) {
 template <class F>
 static void run_segment(mps_ctx* c, int route, int which, F&& body) {
   if (!c->graphs_ok || c->timer_mask != 0 || c->stream == nullptr) { body(); return; }
-  StepSeg& g = c->seg[route][c->cur][which];
+  StepSeg& g = c->seg[c->skin_level][route][c->cur][which];
   if (!g.exec) {
     const HostState before = save_state(c);
     if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
@@ -658,6 +667,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
       const int up[2] = {1, 0};  // need_k, need_star
       CK(cudaMemcpyAsync(&c->flags->need_k, up, sizeof(up), cudaMemcpyHostToDevice, c->stream));
       c->rows_mode_built = skin_mode;
+      ++c->win_forced;
     } else if (skin) {
       c->rows_mode_built |= skin_mode;  // a rebuild on the device during this step leaves out what this route skips
     }
@@ -709,6 +719,34 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     if (rc) first_err = rc;
   }
   int fl = read_flags(c);
+  if (skin && c->skin_auto && nsteps > 0) {
+    // the skin for the NEXT call, from the bins the last sixteen or more steps needed (those forced by new particles
+    // or a change of route do not count).  Thin skin and more than 0.4 bins per step: rows of 0.3 l0 last three times
+    // as long and their longer sweeps cost less than the bins saved (measured at 2M in the developed dam break:
+    // 5.2 -> 4.4 ms per explicit step); thick skin and fewer than 0.06: back (from rest 2.46 vs 2.6 ms).
+    const int64_t bins_now = c->flags_host->bins;
+    c->win_bins += bins_now - c->bins_seen - c->win_forced;
+    c->bins_seen = bins_now;
+    c->win_forced = 0;
+    c->win_steps += nsteps;
+    if (c->win_steps >= 16) {
+      const double rate = (double)c->win_bins / (double)c->win_steps;
+      int lv = c->skin_level;
+      if (lv == 0 && rate >= 0.4 && c->skin_hold == 0) lv = 1;
+      else if (lv == 1 && rate <= 0.06) lv = 0;
+      else if (lv == 1 && rate >= 0.8) {  // too fast even for the thick skin (one bin per step either way): the thin
+        lv = 0;                           // one has the shorter sweeps; do not try again for eight windows
+        c->skin_hold = 8;
+      } else if (c->skin_hold > 0) --c->skin_hold;
+      if (lv != c->skin_level) {
+        c->skin_level = lv;
+        c->kc.carry_d2 = c->kc_step[lv].carry_d2;
+        c->carry_valid = false;  // rows of the other skin: the next step rebuilds (not counted as needed)
+      }
+      c->win_steps = c->win_bins = 0;
+    }
+    c->stats.row_skin_now = c->skin_l0[c->skin_level];
+  }
   if (fl) return fl;
   return first_err;
 }

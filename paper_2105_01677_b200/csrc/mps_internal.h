@@ -117,7 +117,12 @@ struct StepSeg {
 struct mps_ctx {
   mps_params prm;
   KConst kc;
-  KConst kc_step;   // kc with the internal grid and the skin radii of mps_step's bins (mps_api.cu)
+  KConst kc_step[2];  // kc with the internal grid and the skin radii of mps_step's bins, per skin level (mps_api.cu)
+  double skin_l0[2] = {0, 0};  // the two skins in units of l0 (equal when the caller fixed row_skin)
+  bool skin_auto = false;      // row_skin = 0: mps_step picks the level from the bins it needed lately
+  int skin_level = 0;
+  int skin_hold = 0;           // windows during which the thick skin is not tried again
+  int64_t win_steps = 0, win_bins = 0, bins_seen = 0, win_forced = 0;  // steps and bins since the level was last looked at
   bool carry_rows = false;   // mps_step builds rows with a skin and rebuilds them only when the device says so
   bool carry_valid = false;  // the rows in nbr are skin rows and the device flags tell whether they still hold
   int rows_mode_built = 0;   // rows_mode of the skin rows in nbr (a route change may need more of them)
@@ -220,7 +225,7 @@ struct mps_ctx {
   int sm_count = 148;
   // mps_step replays its launch sequence from CUDA graphs (one per route, buffer parity and segment)
   // when the ctx has a capturable stream (not the legacy default stream) and timers are off
-  StepSeg seg[2][2][4];   // [route][buffer parity][segment: 0 pre, 1 post]
+  StepSeg seg[2][2][2][4];   // [skin level][route][buffer parity][segment: 0 pre, 1 post]
   bool graphs_ok = true;
 };
 

@@ -37,7 +37,7 @@ def test_struct_layout_matches_header(B):
     # 16 int32 then 28 doubles, no padding
     assert C.sizeof(B.MpsParams) == 16 * 4 + 29 * 8
     assert B.MpsParams.l0.offset == 64
-    assert C.sizeof(B.MpsStats) == 96
+    assert C.sizeof(B.MpsStats) == 104
     # field ids in the binding equal the header's enum
     src = open(os.path.join(ROOT, "include", "mps_b200.h")).read()
     for name, fid in B.FIELDS.items():

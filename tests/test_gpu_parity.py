@@ -925,6 +925,34 @@ def test_row_skin_particles_leaving_the_domain_become_ghosts(B, O, route):
     print(f"route {route}: ghosts after 2, 4, ... steps {seen}, bins {g.stats()['bins_total']}")
 
 
+@pytest.mark.parametrize("route", [0, 1])
+def test_row_skin_level_follows_the_flow(B, O, route):
+    """row_skin = 0 lets the library choose: 0.1 l0, and 0.3 l0 once a window of 16 steps needed more than 0.4 bins
+    per step (random velocities of 0.4 m/s move particles 0.02 l0 per step against a limit of 0.045 l0).  The
+    switch happens between mps_step calls, rebuilds the rows, and the trajectory still follows the oracle."""
+    s = scenes.small_tank(shuffle=True)
+    rng = np.random.default_rng(3)
+    fl = s.type == scenes.FLUID
+    for k in "uvw":
+        getattr(s, k)[fl] = 0.4 * rng.standard_normal(fl.sum())
+    g, o = B.Mps(s), O.Oracle(s)
+    skins, bins = [], []
+    for _ in range(12):
+        g.step(4, route); o.step(4, route)
+        st = g.stats()
+        skins.append(round(st["row_skin_now"], 3)); bins.append(st["bins_total"])
+    print(f"route {route}: skin after every 4 steps {skins}, bins {bins}")
+    assert skins[0] == 0.1 and 0.3 in skins
+    L = max(hi - lo for lo, hi in zip(s.params["domain_min"], s.params["domain_max"]))
+    assert np.array_equal(g.get("type"), o.get("type"))
+    live = o.get("type") != 3
+    assert max(np.abs(g.get(k) - o.get(k))[live].max() for k in "xyz") <= 1e-7 * L
+    # a fixed skin stays what the caller asked for
+    g2 = B.Mps(s, row_skin=0.05)
+    g2.step(20, route)
+    assert round(g2.stats()["row_skin_now"], 3) == 0.05
+
+
 def test_row_skin_follows_a_route_change(B, O):
     """Explicit steps keep the re_lap part of fluid rows only; a PPE step after them needs every row."""
     s = scenes.small_tank(shuffle=True)
