@@ -1074,7 +1074,15 @@ def test_water_drop_ab_invariant_and_doubling_time():
     # (no surface or collision treatment, Q11; explicit route with Eq. 4 and c0 = 2000 m/s, Mach 0.09)
     # the measured figures are ab within 2.7 % and t2 = 8.3e-3 s.
     s = scenes.water_drop()
-    assert s.n == 1257
+    T1 = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "water_drop_table1.txt")) as f:
+        for line in f:
+            w = line.split("#")[0].split()
+            if len(w) == 2:
+                T1[w[0]] = float(w[1])
+    assert s.n == T1["particles"] == 1257
+    assert s.x.max() == pytest.approx(T1["b_start"], rel=1e-12) and -s.u[0] / s.x[0] == pytest.approx(T1["rate"])
+    assert T1["ab_start"] == pytest.approx(T1["b_start"] ** 2, abs=5e-4)    # the table's ab(0) is b(0)^2: a disc
     sN = np.linspace(1.0, 2.0, 20001)
     f = np.sqrt(1.0 + sN ** 4) / sN ** 2
     t2 = float(((f[1:] + f[:-1]) * 0.5 * np.diff(sN)).sum()) / (100.0 * math.sqrt(2.0))
