@@ -29,6 +29,7 @@ def main():
     ap.add_argument("--ppe-operator", type=int, default=None)
     ap.add_argument("--key-mode", type=int, default=None)
     ap.add_argument("--row-skin", type=float, default=None)
+    ap.add_argument("--param", action="append", default=[], help="KEY=VALUE: any other scene parameter (e.g. ppe_source=2)")
     a = ap.parse_args()
     import torch
     import __graft_entry__ as ge
@@ -41,6 +42,9 @@ def main():
         s.params["key_mode"] = a.key_mode
     if a.row_skin is not None:
         s.params["row_skin"] = a.row_skin
+    for kv in a.param:
+        k, v = kv.split("=", 1)
+        s.params[k] = type(s.params[k])(float(v)) if k in s.params and not isinstance(s.params[k], tuple) else float(v)
     route = 1 if a.route == "ppe" else 0
     g = B.Mps(s)
     g.step(a.warmup, route)
