@@ -160,8 +160,9 @@ k_nu_eff(KConst kc, int with_sps, const double4* __restrict__ pos4, double4* __r
 // a_i = A_lap sum_{j in N(i, re_lap)} nu_ij (u_j - u_i) w(r) + g, fluid i
 // (Eq. 10, Eq. 2; Q9).  SPS = false: nu_j comes from the entry's
 // phase / wall / dummy bits (no pre-pass); SPS = true: nu_j = vel4[j].w.
+// (five blocks per SM: 48 registers with a 16-byte spill beat four blocks at 60 -- 1.398 -> 1.350 ms at 2M -- and six at 40)
 template <bool SPS>
-__global__ void __launch_bounds__(TPB)
+__global__ void __launch_bounds__(TPB, 5)
 k_viscosity(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ vel4,
             const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
             const uint32_t* __restrict__ cn, const uint32_t* __restrict__ co,
@@ -304,7 +305,7 @@ k_phat(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__
 // Variants 0 and 2 find phat_i in the same pass over the row as the sum (no pre-pass
 // kernel); variant 1 needs phat_j of the neighbours, so k_phat runs first.
 template <int VARIANT>
-__global__ void __launch_bounds__(TPB)
+__global__ void __launch_bounds__(TPB, 6)
 k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ phat,
            const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
            const uint32_t* __restrict__ cn, double4* __restrict__ grad4) {
