@@ -8,7 +8,10 @@
 namespace {
 
 constexpr int TPB = 256;
-constexpr int L = 8;  // lanes per row; TPB / L rows per block
+// L lanes per row (a template parameter of every row kernel; TPB / L rows per block): 4 from 50,000 particles up,
+// 8 below, where four lanes per row leave an SM short of threads (measured at 2M: viscosity 1.35 -> 1.31 ms, density
+// 0.234 -> 0.212, gradient 0.353 -> 0.279; 16 lanes: 1.59 / 0.366 / 0.522; 2 lanes: 1.66 / 0.234 / 0.271; at 19k
+// particles the explicit step takes 0.105 ms with 8 lanes and 0.125 with 4)
 
 // group -> particle; sub = lane within the group
 #define ROW_GROUP(i, sub)                                              \
@@ -19,6 +22,7 @@ constexpr int L = 8;  // lanes per row; TPB / L rows per block
 
 // ---------------------------------------------------------------- S4 density ---
 // n_i = sum_{j in N(i, re_n)} (re_n / r_ij - 1), all non-ghost i and j (Eq. 5).
+template <int L>
 __global__ void __launch_bounds__(TPB)
 k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ nbr,
           const uint32_t* __restrict__ cn, double* __restrict__ dens) {
@@ -41,6 +45,7 @@ k_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restric
 // ------------------------------------ NEXT-2: smoothed density of the multi-density model ---
 // <rho>_i = sum_j rho_j w(r_ij) / sum_j w(r_ij) over N(i, re_n), every non-ghost i; rho_j comes
 // from the phase bit of the row entry (Q25).  No neighbour: the particle's own density.
+template <int L>
 __global__ void __launch_bounds__(TPB)
 k_smooth_density(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
                  const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn,
@@ -75,6 +80,7 @@ __global__ void k_stage_beta(KConst kc, const double* __restrict__ p, const doub
 // Dn/Dt_i = d/dt sum_j (re_n / r_ij - 1) = -sum_{j in N(i, re_n)} re_n / r^3 (x_ij . u_ij),
 // x_ij = x_j - x_i, u_ij = u_j - u_i; walls and dummies hold u = 0 in vel4 (P:224-228
 // Eq. 15; sign: Q22).  keep: also store (n_i, Dn/Dt_i) as the start-of-step pair of Eq. 17.
+template <int L>
 __global__ void __launch_bounds__(TPB)
 k_dndt(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ vel4,
        const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn,
@@ -107,6 +113,7 @@ k_dndt(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ 
 // G_ab = (d/n0) sum (u_b,j - u_b,i)(x_a,j - x_a,i) / r^2 w(r) over N(i, re_n);
 // S = (G + G^T)/2; nu_t = (Cs l0)^2 sqrt(2 S:S) (Eq. 13; Q10).
 // Writes nut and vel4.w = nu_eff (fluid: nu[phase] + nu_t; wall/dummy/ghost: -1).
+template <int L>
 __global__ void __launch_bounds__(TPB)
 k_nu_eff(KConst kc, int with_sps, const double4* __restrict__ pos4, double4* __restrict__ vel4,
          const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
@@ -161,7 +168,7 @@ k_nu_eff(KConst kc, int with_sps, const double4* __restrict__ pos4, double4* __r
 // (Eq. 10, Eq. 2; Q9).  SPS = false: nu_j comes from the entry's
 // phase / wall / dummy bits (no pre-pass); SPS = true: nu_j = vel4[j].w.
 // (five blocks per SM: 48 registers with a 16-byte spill beat four blocks at 60 -- 1.398 -> 1.350 ms at 2M -- and six at 40)
-template <bool SPS>
+template <bool SPS, int L>
 __global__ void __launch_bounds__(TPB, 5)
 k_viscosity(KConst kc, const double4* __restrict__ pos4, const double4* __restrict__ vel4,
             const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
@@ -278,6 +285,7 @@ __global__ void k_stage_p(int n, const double* __restrict__ p, double4* __restri
 // ------------------------------------------------------------------ S9 p-hat ---
 // phat_i = min(p_i, min over non-dummy j in N(i, re_n) of p_j), fluid and wall i
 // (Q12).  p_j is read from pos4.w.
+template <int L>
 __global__ void __launch_bounds__(TPB)
 k_phat(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__ tp,
        const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ cn, double* __restrict__ phat) {
@@ -304,7 +312,7 @@ k_phat(KConst kc, const double4* __restrict__ pos4, const uint32_t* __restrict__
 // coef = p_j - phat_i (0) | (p_i + p_j) - (phat_i + phat_j) (1, Eq. 14) | p_i + p_j (2).
 // Variants 0 and 2 find phat_i in the same pass over the row as the sum (no pre-pass
 // kernel); variant 1 needs phat_j of the neighbours, so k_phat runs first.
-template <int VARIANT>
+template <int VARIANT, int L>
 __global__ void __launch_bounds__(TPB, 6)
 k_gradient(KConst kc, const double4* __restrict__ pos4, double* __restrict__ phat,
            const uint32_t* __restrict__ tp, const uint32_t* __restrict__ nbr,
@@ -405,11 +413,23 @@ __global__ void k_correct(KConst kc, double4* __restrict__ pos4, double4* __rest
 }  // namespace
 
 // ============================================================ host launchers ===
-static inline int group_grid(int n) { return div_up((int64_t)n * L, TPB); }
+static inline int group_grid(int n, int lanes) { return div_up((int64_t)n * lanes, TPB); }
+static inline int sweep_lanes(const mps_ctx* c) { return c->n >= 50000 ? 4 : 8; }
+// launch a row kernel with the lanes per row that suit the scene: KERN<4> or KERN<8> (PRE: leading template arguments)
+#define LAUNCH_ROWS(c, cat, KERN, n, ...)                                                                   \
+  do {                                                                                                      \
+    if (sweep_lanes(c) == 4) MPS_LAUNCH(c, cat, (KERN<4>), group_grid(n, 4), TPB, __VA_ARGS__);             \
+    else MPS_LAUNCH(c, cat, (KERN<8>), group_grid(n, 8), TPB, __VA_ARGS__);                                 \
+  } while (0)
+#define LAUNCH_ROWS2(c, cat, KERN, PRE, n, ...)                                                             \
+  do {                                                                                                      \
+    if (sweep_lanes(c) == 4) MPS_LAUNCH(c, cat, (KERN<PRE, 4>), group_grid(n, 4), TPB, __VA_ARGS__);        \
+    else MPS_LAUNCH(c, cat, (KERN<PRE, 8>), group_grid(n, 8), TPB, __VA_ARGS__);                            \
+  } while (0)
 
 int mpsk_density(mps_ctx* c) {
   int n = (int)c->n;
-  MPS_LAUNCH(c, MPS_T_DENSITY, k_density, group_grid(n), TPB, c->kc, c->pos4[c->cur], c->nbr, c->cn,
+  LAUNCH_ROWS(c, MPS_T_DENSITY, k_density, n, c->kc, c->pos4[c->cur], c->nbr, c->cn,
              c->dens);
   return MPS_OK;
 }
@@ -417,7 +437,7 @@ int mpsk_density(mps_ctx* c) {
 int mpsk_smooth_density(mps_ctx* c) {
   int n = (int)c->n;
   int cur = c->cur;
-  MPS_LAUNCH(c, MPS_T_DENSITY, k_smooth_density, group_grid(n), TPB, c->kc, c->pos4[cur], c->tp[cur],
+  LAUNCH_ROWS(c, MPS_T_DENSITY, k_smooth_density, n, c->kc, c->pos4[cur], c->tp[cur],
              c->nbr, c->cn, c->rho_s[cur]);
   c->rho_s_ready = true;
   return MPS_OK;
@@ -426,7 +446,7 @@ int mpsk_smooth_density(mps_ctx* c) {
 int mpsk_dndt(mps_ctx* c, int keep) {
   int n = (int)c->n;
   int cur = c->cur;
-  MPS_LAUNCH(c, MPS_T_DENSITY, k_dndt, group_grid(n), TPB, c->kc, c->pos4[cur], c->vel4[cur], c->nbr,
+  LAUNCH_ROWS(c, MPS_T_DENSITY, k_dndt, n, c->kc, c->pos4[cur], c->vel4[cur], c->nbr,
              c->cn, c->dens, c->dndt, keep ? c->keep2[cur] : nullptr);
   return MPS_OK;
 }
@@ -435,12 +455,12 @@ int mpsk_viscosity(mps_ctx* c) {
   int n = (int)c->n;
   int cur = c->cur;
   if (c->prm.cs > 0.0) {
-    MPS_LAUNCH(c, MPS_T_VISCOSITY, k_nu_eff, group_grid(n), TPB, c->kc, 1, c->pos4[cur], c->vel4[cur],
+    LAUNCH_ROWS(c, MPS_T_VISCOSITY, k_nu_eff, n, c->kc, 1, c->pos4[cur], c->vel4[cur],
                c->tp[cur], c->nbr, c->cn, c->nut);
-    MPS_LAUNCH(c, MPS_T_VISCOSITY, k_viscosity<true>, group_grid(n), TPB, c->kc, c->pos4[cur],
+    LAUNCH_ROWS2(c, MPS_T_VISCOSITY, k_viscosity, true, n, c->kc, c->pos4[cur],
                c->vel4[cur], c->tp[cur], c->nbr, c->cn, c->co, c->acc4);
   } else {
-    MPS_LAUNCH(c, MPS_T_VISCOSITY, k_viscosity<false>, group_grid(n), TPB, c->kc, c->pos4[cur],
+    LAUNCH_ROWS2(c, MPS_T_VISCOSITY, k_viscosity, false, n, c->kc, c->pos4[cur],
                c->vel4[cur], c->tp[cur], c->nbr, c->cn, c->co, c->acc4);
   }
   return MPS_OK;
@@ -473,7 +493,7 @@ int mpsk_gradient(mps_ctx* c) {
     MPS_LAUNCH(c, MPS_T_GRADIENT, k_stage_beta, div_up(n, 256), 256, c->kc, c->p, c->rho_s[cur], c->tp[cur],
                c->pos4[cur]);
     c->posw_is_p = false;
-    MPS_LAUNCH(c, MPS_T_GRADIENT, k_gradient<3>, group_grid(n), TPB, c->kc, c->pos4[cur], c->rho_s[cur],
+    LAUNCH_ROWS2(c, MPS_T_GRADIENT, k_gradient, 3, n, c->kc, c->pos4[cur], c->rho_s[cur],
                c->tp[cur], c->nbr, c->cn, c->grad4);
     return MPS_OK;
   }
@@ -483,17 +503,17 @@ int mpsk_gradient(mps_ctx* c) {
   }
   switch (c->prm.grad_variant) {
     case 0:
-      MPS_LAUNCH(c, MPS_T_GRADIENT, k_gradient<0>, group_grid(n), TPB, c->kc, c->pos4[cur], c->phat,
+      LAUNCH_ROWS2(c, MPS_T_GRADIENT, k_gradient, 0, n, c->kc, c->pos4[cur], c->phat,
                  c->tp[cur], c->nbr, c->cn, c->grad4);
       break;
     case 1:
-      MPS_LAUNCH(c, MPS_T_GRADIENT, k_phat, group_grid(n), TPB, c->kc, c->pos4[cur], c->tp[cur], c->nbr,
+      LAUNCH_ROWS(c, MPS_T_GRADIENT, k_phat, n, c->kc, c->pos4[cur], c->tp[cur], c->nbr,
                  c->cn, c->phat);
-      MPS_LAUNCH(c, MPS_T_GRADIENT, k_gradient<1>, group_grid(n), TPB, c->kc, c->pos4[cur], c->phat,
+      LAUNCH_ROWS2(c, MPS_T_GRADIENT, k_gradient, 1, n, c->kc, c->pos4[cur], c->phat,
                  c->tp[cur], c->nbr, c->cn, c->grad4);
       break;
     default:
-      MPS_LAUNCH(c, MPS_T_GRADIENT, k_gradient<2>, group_grid(n), TPB, c->kc, c->pos4[cur], c->phat,
+      LAUNCH_ROWS2(c, MPS_T_GRADIENT, k_gradient, 2, n, c->kc, c->pos4[cur], c->phat,
                  c->tp[cur], c->nbr, c->cn, c->grad4);
       break;
   }
