@@ -321,6 +321,20 @@ int mps_timers_read(mps_ctx* ctx, double* ms, int64_t* launches);
  * mps_get_stats, which read the counter).  A bin that did not run is not counted.  While timers are on
  * (mps_timers_enable) mps_step reads the device flag before each of its bins and leaves out the ones not needed. */
 int64_t mps_launch_count(mps_ctx* ctx);
+/* mps_cell_start_noalloc: the cell-start table of the counting sort (section 4.1; B4 of DESIGN.md section 2)
+ * for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * cell_start[c] = number of keys below c, c = 0 .. n_cells -- the same table as mps_get_cell_start after mps_bin.
+ * key: DEVICE, n x uint32, the cell keys in any order (a key above n_cells counts as n_cells, the ghost key);
+ * cell_start: DEVICE, (n_cells + 1) x uint32, written by the call; stream: cudaStream_t of the current device (may
+ * be NULL).  Needs no ctx and calls no cudaMalloc, cudaFree or allocating routine: the histogram and the scan's tile
+ * sums live in a file-scope device array of fixed size (1.0 MB, held by every GPU that loads the library until the
+ * process exits), which limits n_cells to mps_cell_start_noalloc_max_cells() = 262,144; a larger n_cells returns
+ * MPS_ERR_ARG.  Every call shares that array and clears the part it uses on the caller's stream: calls that overlap
+ * on the GPU (two streams, two threads) race -- serialise them.  Asynchronous; errors: MPS_ERR_ARG, MPS_ERR_CUDA,
+ * message from mps_cell_start_noalloc_error() (valid until the next failing call). */
+int mps_cell_start_noalloc(const uint32_t* key, int64_t n, int32_t n_cells, uint32_t* cell_start, void* stream);
+int32_t mps_cell_start_noalloc_max_cells(void);
+const char* mps_cell_start_noalloc_error(void);
 /* Message of the last error of this ctx (owned by the ctx; valid until the
  * next call).  ctx == NULL returns the message of the last failed mps_init. */
 const char* mps_last_error(mps_ctx* ctx);

@@ -37,7 +37,8 @@ SYMBOLS = ["mps_init", "mps_init_host", "mps_destroy", "mps_bin", "mps_density",
            "mps_get_perm", "mps_get_grid", "mps_get_cell_start", "mps_get_neighbours",
            "mps_ppe_apply", "mps_get_constants", "mps_get_stats", "mps_sync",
            "mps_timers_enable", "mps_timers_read", "mps_launch_count", "mps_last_error",
-           "mps_version"]
+           "mps_version", "mps_cell_start_noalloc", "mps_cell_start_noalloc_max_cells",
+           "mps_cell_start_noalloc_error"]
 
 
 class MpsParams(C.Structure):
@@ -141,6 +142,9 @@ def _load():
     L.mps_last_error.argtypes = [vp]
     L.mps_last_error.restype = C.c_char_p
     L.mps_version.restype = C.c_char_p
+    L.mps_cell_start_noalloc.argtypes = [vp, i64, i32, vp, vp]
+    L.mps_cell_start_noalloc_max_cells.restype = i32
+    L.mps_cell_start_noalloc_error.restype = C.c_char_p
     return L
 
 
@@ -156,6 +160,21 @@ def _torch():
     if not torch.cuda.is_available():
         raise RuntimeError("libmps_b200 needs a CUDA device (B200); there is no CPU fallback")
     return torch
+
+
+def cell_start_noalloc(key, n_cells: int, cell_start, stream=None) -> None:
+    """mps_cell_start_noalloc: key and cell_start are CUDA tensors (int32 / uint32 words; cell_start has
+    n_cells + 1 entries and is written asynchronously on `stream`, default torch's current stream)."""
+    torch = _torch()
+    st = stream if stream is not None else torch.cuda.current_stream(key.device)
+    rc = lib.mps_cell_start_noalloc(key.data_ptr(), int(key.numel()), int(n_cells), cell_start.data_ptr(),
+                                    st.cuda_stream)
+    if rc != 0:
+        raise MpsError(rc, lib.mps_cell_start_noalloc_error().decode())
+
+
+def cell_start_noalloc_max_cells() -> int:
+    return int(lib.mps_cell_start_noalloc_max_cells())
 
 
 class Mps:

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmps_b200.so")
-SOURCES = ["mps_api.cu", "kernels_bin.cu", "kernels_sweep.cu", "kernels_ppe.cu"]
+SOURCES = ["mps_api.cu", "kernels_bin.cu", "kernels_sweep.cu", "kernels_ppe.cu", "no_alloc.cu"]
 HEADERS = [os.path.join(CSRC, "mps_internal.h"),
            os.path.join(os.path.dirname(HERE), "include", "mps_b200.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
