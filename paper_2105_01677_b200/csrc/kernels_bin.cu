@@ -670,6 +670,7 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
   // (ncu: l1tex 72 %, the busiest unit of this kernel), an LDS broadcast one
   __shared__ double2 cand_xy[CELL_WARPS][32];
   __shared__ double cand_z[CELL_WARPS][32];
+  __shared__ uint32_t cand_e[CELL_WARPS][32];  // and their row entries
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int gwarp = blockIdx.x * CELL_WARPS + wid;
   const int nwarps = gridDim.x * CELL_WARPS;
@@ -725,6 +726,7 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
               __syncwarp();                                    // the previous chunk has been read by every lane
               cand_xy[wid][lane] = make_double2(mine.x, mine.y);
               cand_z[wid][lane] = mine.z;
+              cand_e[wid][lane] = ent[j0 + (uint32_t)lane];
               __syncwarp();
             }
             const double2* qxy = cand_xy[wid];
@@ -755,28 +757,23 @@ k_build_rows_cell(KConst kc, const double4* __restrict__ pos4, const uint32_t* _
             }
             m_n &= m_lap;
             uint32_t m_o = m_lap & ~m_n;
-            // the chunk's row entries, one per lane
-            const uint32_t eb = ent[j0 + (uint32_t)lane];
-            // phase 2: every lane appends its hits in ascending j (warp-convergent loops)
-            while (__any_sync(0xffffffffu, m_n != 0u)) {
+            // phase 2: every lane appends its own hits in ascending j.  The entries come from shared memory (word
+            // `bit`: distinct bits are distinct banks, equal bits a broadcast), so the loops need no vote and no
+            // shuffle and each lane simply runs as long as it has hits
+            const uint32_t* ce = cand_e[wid];
+            while (m_n) {
               const int bit = __ffs((int)m_n) - 1;
-              const uint32_t e = __shfl_sync(0xffffffffu, eb, bit & 31);
-              if (m_n) {
-                m_n &= m_n - 1u;
-                bn[nf & 7u][lane] = e;
-                ++nf;
-                if ((nf & 7u) == 0u) flush_sector(row + (nf - 8u), bn, lane);
-              }
+              m_n &= m_n - 1u;
+              bn[nf & 7u][lane] = ce[bit];
+              ++nf;
+              if ((nf & 7u) == 0u) flush_sector(row + (nf - 8u), bn, lane);
             }
-            while (__any_sync(0xffffffffu, m_o != 0u)) {
+            while (m_o) {
               const int bit = __ffs((int)m_o) - 1;
-              const uint32_t e = __shfl_sync(0xffffffffu, eb, bit & 31);
-              if (m_o) {
-                m_o &= m_o - 1u;
-                bo[nb & 7u][lane] = e;
-                ++nb;
-                if ((nb & 7u) == 0u) flush_sector(row + ((uint32_t)S - nb), bo, lane);
-              }
+              m_o &= m_o - 1u;
+              bo[nb & 7u][lane] = ce[bit];
+              ++nb;
+              if ((nb & 7u) == 0u) flush_sector(row + ((uint32_t)S - nb), bo, lane);
             }
           }
         }
