@@ -641,7 +641,8 @@ k_build_rows(KConst kc, const double4* __restrict__ pos4, const uint32_t* __rest
 // at 438k, no change at 2M), and a tests-only kernel writing hit masks followed by a warp-per-row
 // expansion (1.7 + 1.8 ms per bin at 2M against 2.5 ms: the tests alone take 1.7 ms at 58 % of the
 // fp64 pipe, so the appends cost about a third of this kernel, not the half their instruction
-// count suggests).
+// count suggests).  Round 2, later: one loop over both parts of a row with the target chosen per hit (3.67 vs
+// 3.51 ms for the two exact bins of a step at 2M: the select costs more than the second loop's overhead).
 constexpr int CELL_TPB = 256;
 constexpr int CELL_WARPS = CELL_TPB / 32;
 constexpr int CELL_BATCH = 8;  // candidates tested per lane before the hits are appended
