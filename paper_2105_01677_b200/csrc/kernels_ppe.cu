@@ -586,6 +586,8 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         const int rs = n_rows >= RPS * sc_step * MPS_ASM_MINRUNS * (1 << ASM_RUN_LOG2) ? ASM_RUN_LOG2 : 0;
         auto row_of = [&](int t) { return ((((sc_first + (t >> rs) * sc_step) << rs) + (t & ((1 << rs) - 1))) * RPS) + g_in_scA; };
         auto trips_left = [&](int t) { return ((sc_first + (t >> rs) * sc_step) << rs) * RPS < n_rows; };
+        // (prefetch distance 1 / 2 / 3 trips measured: 208 / 210 / 215 ps per row per iteration at 1.44M rows,
+        // 216 / 227 / 240 at 260k)
         uint32_t n_ahead = 0;
         {
           const int g1 = row_of(1);
