@@ -541,12 +541,13 @@ def test_full_size_sampled_config3(B, O):
     assert (np.diff(perm.astype(np.int64))[same] > 0).all()
 
 
-@pytest.mark.parametrize("cfg,idx,op", [(3, 0, 1), (3, 0, 0), (4, 0, 1), (4, 0, 0), (5, 2, 1)])
+@pytest.mark.parametrize("cfg,idx,op", [(3, 0, 1), (3, 0, 0), (4, 0, 1), (4, 0, 0), (5, 2, 1), (5, 3, 1)])
 def test_full_size_ppe_residual_under_oracle_operator(B, O, cfg, idx, op):
-    """Configs 3 (N = 438,208), 4 (two-phase, Smagorinsky, N = 634,808) and 5[2] (N = 1,011,096)
-    in the launch configuration bench.py times (warp-per-cell row builder, 148 x 1024 persistent
-    CG): density, flags, right-hand side and operator against the oracle on identical positions,
-    and the GPU's CG solution checked by its true residual under the ORACLE's operator."""
+    """Configs 3 (N = 438,208), 4 (two-phase, Smagorinsky, N = 634,808), 5[2] (N = 1,011,096) and 5[3]
+    (N = 1,994,776: bench.py's default workload, and the size from which the CG loop deals its rows in
+    runs of eight super-chunks) in the launch configuration bench.py times (warp-per-cell row builder,
+    148 x 1024 persistent CG): density, flags, right-hand side and operator against the oracle on identical
+    positions, and the GPU's CG solution checked by its true residual under the ORACLE's operator."""
     s = scenes.make_scene(cfg, sweep_index=idx)
     s.params["ppe_operator"] = op
     g = B.Mps(s)
