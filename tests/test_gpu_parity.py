@@ -460,6 +460,19 @@ def test_config5_250k_explicit_10_steps(B, O):
     assert eL <= 1e-7 and moved > 0.005
 
 
+@pytest.mark.parametrize("route,nsteps", [(0, 3), (1, 3)])
+def test_config5_2m_trajectory_of_the_bench_workload(B, O, route, nsteps):
+    """Scene 5[3] (N = 1,994,776), the workload bench.py times, stepped as bench.py steps it (mps_step from CUDA
+    graphs, skin rows, persistent CG with run-dealt rows) against the oracle stepping on its own from the same
+    initial scene."""
+    s = scenes.make_scene(5, sweep_index=3)
+    eL, el0, moved, g, o = _trajectory(B, O, s, nsteps, route)
+    print(f"config 5[3] (N={s.n}), {nsteps} steps of route {route}: max |dr|/L = {eL:.2e}, /l0 = {el0:.2e}, "
+          f"moved {moved:.4f} l0; cg iters {g.stats()['cg_iters']} vs {o.stats()['cg_iters']}")
+    assert eL <= 1e-7 and moved > (0.0005 if route == 0 else 0.0002)
+    assert relerr(g.get("p"), o.get("p"), 1.0) <= 1e-6
+
+
 def test_step_host_equals_ctx_path(B, O):
     s = scenes.small_tank(shuffle=True)
     g = B.Mps(s)
