@@ -138,8 +138,8 @@ typedef struct mps_params {
                                r2 < re^2 with the rounding of Q2, so the sets stay exact -- until some particle has
                                moved by more than 0.45 skins since the build (checked on the device by the predictor
                                and the corrector).  0 => the library chooses: 0.1, and 0.3 while a flow needs more
-                               than 0.4 bins per step with 0.1 (looked at between mps_step calls, over windows of
-                               at least 16 steps; back to 0.1 below 0.06 bins per step, and above 0.8, where neither
+                               than 0.4 bins per step with 0.1 (looked at over windows of at least 16 steps, between
+                               mps_step calls and, with one 4-byte read-back, inside long ones; back to 0.1 below 0.06 bins per step, and above 0.8, where neither
                                skin saves a bin and the thin one has the shorter sweeps); < 0 => no skin: mps_step
                                bins at r^k and at r* in every step, as Q7 is literally stated */
 } mps_params;

@@ -476,6 +476,36 @@ static void run_segment(mps_ctx* c, int route, int which, F&& body) {
   cudaGraphLaunch(g.exec, c->stream);
 }
 
+// The automatic skin (row_skin = 0): looked at after windows of sixteen or more steps, from the bins those steps
+// needed (c->flags_host->bins must be fresh; bins forced by new particles or a change of route do not count).  Thin
+// skin and more than 0.4 bins per step: rows of 0.3 l0 last three times as long and their longer sweeps cost less
+// than the bins saved (measured at 2M in the developed dam break: 5.0 -> 4.1 ms per explicit step); thick skin and
+// fewer than 0.06: back (from rest 2.26 vs 2.4 ms).
+static void skin_policy(mps_ctx* c, int64_t steps) {
+  const int64_t bins_now = c->flags_host->bins;
+  c->win_bins += bins_now - c->bins_seen - c->win_forced;
+  c->bins_seen = bins_now;
+  c->win_forced = 0;
+  c->win_steps += steps;
+  if (c->win_steps >= 16) {
+    const double rate = (double)c->win_bins / (double)c->win_steps;
+    int lv = c->skin_level;
+    if (lv == 0 && rate >= 0.4 && c->skin_hold == 0) lv = 1;
+    else if (lv == 1 && rate <= 0.06) lv = 0;
+    else if (lv == 1 && rate >= 0.8) {  // too fast even for the thick skin (one bin per step either way): the thin
+      lv = 0;                           // one has the shorter sweeps; do not try again for eight windows
+      c->skin_hold = 8;
+    } else if (c->skin_hold > 0) --c->skin_hold;
+    if (lv != c->skin_level) {
+      c->skin_level = lv;
+      c->kc.carry_d2 = c->kc_step[lv].carry_d2;
+      c->carry_valid = false;  // rows of the other skin: the next step rebuilds (not counted as needed)
+    }
+    c->win_steps = c->win_bins = 0;
+  }
+  c->stats.row_skin_now = c->skin_l0[c->skin_level];
+}
+
 extern "C" {
 
 const char* mps_version(void) { return "mps_b200 0.1 (sm_100a)"; }
@@ -650,6 +680,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
   // (viscosity); the PPE operator has rows for walls too, ECS needs n^k and (Dn/Dt)^k of every row
   const bool skin = K == 1 && c->carry_rows;
   const int skin_mode = route == MPS_ROUTE_EXPLICIT && !ecs ? ROWS_BACK_FLUID : 0;
+  int64_t since_look = 0;  // steps of this call the skin policy has not seen yet
   for (int s = 0; s < nsteps; ++s) {
     if (K > 1) {
       // list reuse (Q24): bin (all rows, both radii) once every K steps at r^k; every sweep of
@@ -710,6 +741,14 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     if (K > 1) post(); else run_segment(c, route, 1, post);
     c->carry_valid = skin;
     c->stats.steps_total++;
+    ++since_look;
+    if (skin && c->skin_auto && c->win_steps + since_look >= 16 && s + 1 < nsteps) {
+      // inside a long call too: one 4-byte read-back per sixteen steps
+      CK(cudaMemcpyAsync(&c->flags_host->bins, &c->flags->bins, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+      CK(cudaStreamSynchronize(c->stream));
+      skin_policy(c, since_look);
+      since_look = 0;
+    }
   }
   c->kc.stale = 0;  // API-level sweeps always run on exact rows (they need mps_bin first)
   CK(cudaGetLastError());
@@ -719,34 +758,7 @@ int mps_step(mps_ctx* c, int32_t nsteps, int32_t route) {
     if (rc) first_err = rc;
   }
   int fl = read_flags(c);
-  if (skin && c->skin_auto && nsteps > 0) {
-    // the skin for the NEXT call, from the bins the last sixteen or more steps needed (those forced by new particles
-    // or a change of route do not count).  Thin skin and more than 0.4 bins per step: rows of 0.3 l0 last three times
-    // as long and their longer sweeps cost less than the bins saved (measured at 2M in the developed dam break:
-    // 5.2 -> 4.4 ms per explicit step); thick skin and fewer than 0.06: back (from rest 2.46 vs 2.6 ms).
-    const int64_t bins_now = c->flags_host->bins;
-    c->win_bins += bins_now - c->bins_seen - c->win_forced;
-    c->bins_seen = bins_now;
-    c->win_forced = 0;
-    c->win_steps += nsteps;
-    if (c->win_steps >= 16) {
-      const double rate = (double)c->win_bins / (double)c->win_steps;
-      int lv = c->skin_level;
-      if (lv == 0 && rate >= 0.4 && c->skin_hold == 0) lv = 1;
-      else if (lv == 1 && rate <= 0.06) lv = 0;
-      else if (lv == 1 && rate >= 0.8) {  // too fast even for the thick skin (one bin per step either way): the thin
-        lv = 0;                           // one has the shorter sweeps; do not try again for eight windows
-        c->skin_hold = 8;
-      } else if (c->skin_hold > 0) --c->skin_hold;
-      if (lv != c->skin_level) {
-        c->skin_level = lv;
-        c->kc.carry_d2 = c->kc_step[lv].carry_d2;
-        c->carry_valid = false;  // rows of the other skin: the next step rebuilds (not counted as needed)
-      }
-      c->win_steps = c->win_bins = 0;
-    }
-    c->stats.row_skin_now = c->skin_l0[c->skin_level];
-  }
+  if (skin && c->skin_auto && since_look > 0) skin_policy(c, since_look);
   if (fl) return fl;
   return first_err;
 }

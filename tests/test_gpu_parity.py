@@ -961,6 +961,12 @@ def test_row_skin_level_follows_the_flow(B, O, route):
     assert np.array_equal(g.get("type"), o.get("type"))
     live = o.get("type") != 3
     assert max(np.abs(g.get(k) - o.get(k))[live].max() for k in "xyz") <= 1e-7 * L
+    # one long call adapts too (a look every sixteen steps inside mps_step)
+    g3, o3 = B.Mps(s), O.Oracle(s)
+    g3.step(40, route); o3.step(40, route)
+    assert round(g3.stats()["row_skin_now"], 3) == 0.3
+    live = o3.get("type") != 3
+    assert max(np.abs(g3.get(k) - o3.get(k))[live].max() for k in "xyz") <= 1e-7 * L
     # a fixed skin stays what the caller asked for
     g2 = B.Mps(s, row_skin=0.05)
     g2.step(20, route)
