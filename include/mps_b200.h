@@ -105,7 +105,8 @@ typedef struct mps_params {
                                list reuse: mps_step bins once every K steps, at r^k, and every
                                sweep keeps the stored pairs whose current distance is below the radius; Q24 */
   int32_t ppe_operator;     /* (1) how the CG applies A of Listing 2.  0: matrix-free -- rows hold
-                               neighbour indices only and every application recomputes c_ij from the positions;
+                               neighbour indices only and every application recomputes c_ij from the positions
+                               (inside mps_step with a skin: from an exact index list filtered once per solve);
                                1: assembled -- the coefficients of the rows bc = 0 are computed once per solve
                                (positions are fixed during a solve) into a compact ELL matrix over the unknowns
                                (one 64-bit word per pair: 24-bit column + 40-bit fixed-point coefficient, Q28; the

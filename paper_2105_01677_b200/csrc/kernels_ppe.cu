@@ -98,6 +98,7 @@ struct PpeArgs {
   long long timeout_cycles;
   int maxit;
   int warm;
+  int compact;  // matrix-free on skin rows: walk the exact lists built once per solve (compact_row)
 };
 
 __device__ __forceinline__ void prefetch_l2(const void* p) {
@@ -196,18 +197,16 @@ __device__ __forceinline__ double pair_coef(const KConst& kc, bool hl, double r2
 // c_ij = A_lap w(r_ij) / rho_ij (Listing 2; Q5, Q6).  r_j is read from
 // pos4.w, which is 0 on free-surface slots (Dirichlet p = 0).  The L lanes of the
 // group each take every L-th entry; the result is valid in every lane.
+// row / nf / m: the entries to walk (a neighbour row with its front and back parts, or -- nf = m -- a plain list);
+// stale: re-test every pair against re_lap (skin rows, reused lists).
 template <bool TWO_PHASE, bool TEX>
-__device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4, cudaTextureObject_t tex,
-                                          const uint32_t* tp,
-                                          const uint32_t* nbr, const uint32_t* cn, const uint32_t* co,
-                                          int i, int sub, bool live, double& ri) {
+__device__ __forceinline__ double ppe_row_core(const KConst& kc, const double4* pos4, cudaTextureObject_t tex,
+                                               const uint32_t* tp, const uint32_t* row, uint32_t nf, uint32_t m,
+                                               int stale, int i, int sub, double& ri) {
   // every lane of the warp must come through here (full-mask shuffles below): a
-  // group without a row passes live = false and any valid i
+  // group without a row passes m = 0 and any valid i
   const double4 pi = pos4[i];
   ri = pi.w;
-  const uint32_t* row = row_ptr(nbr, kc.stride, i);
-  const uint32_t nf = live ? cn[i] : 0u;
-  const uint32_t m = live ? nf + co[i] : 0u;
   // 1 / rho_ij for a neighbour of phase 0 and of phase 1 (Q6): two values per row, no division per pair
   const int ph_i = TWO_PHASE ? (int)((tp[i] >> 8) & 1) : 0;
   const double inv_rij0 = kc.inv_rho_pair[ph_i][0], inv_rij1 = kc.inv_rho_pair[ph_i][1];
@@ -240,15 +239,61 @@ __device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4,
 #pragma unroll
     for (int u = 0; u < PPE_ILP; ++u) {
       const double dx = q[u].x - pi.x, dy = q[u].y - pi.y, dz = q[u].z - pi.z;
-      const double r2 = pair_r2(dx, dy, dz, kc.stale);
+      const double r2 = pair_r2(dx, dy, dz, stale);
       double w = pair_coef<TWO_PHASE>(kc, hl, r2, e[u], inv_rij0, inv_rij1);
-      if ((e[u] & NB_DUMMY) || (kc.stale && !(r2 < kc.re_lap2))) w = 0.0;  // dummy, empty slot, or left the radius
+      if ((e[u] & NB_DUMMY) || (stale && !(r2 < kc.re_lap2))) w = 0.0;  // dummy, empty slot, or left the radius
       s = fma(w, pi.w - q[u].w, s);
     }
   }
   s = group_sum<L>(s);
   if (!TWO_PHASE) s *= 1.0 / kc.rho[0];
   return fma(hl ? kc.hl_c : kc.A_lap, s, kc.compress_dt2 * pi.w);
+}
+template <bool TWO_PHASE, bool TEX>
+__device__ __forceinline__ double ppe_row(const KConst& kc, const double4* pos4, cudaTextureObject_t tex,
+                                          const uint32_t* tp,
+                                          const uint32_t* nbr, const uint32_t* cn, const uint32_t* co,
+                                          int i, int sub, bool live, double& ri) {
+  const uint32_t nf = live ? cn[i] : 0u;
+  const uint32_t m = live ? nf + co[i] : 0u;
+  return ppe_row_core<TWO_PHASE, TEX>(kc, pos4, tex, tp, row_ptr(nbr, kc.stride, i), nf, m, kc.stale, i, sub, ri);
+}
+
+// ---- matrix-free solve on skin rows: the exact list of row g, once per solve -----------------------------
+// Positions are fixed during a solve, so the re-test of a skin row (and the skipping of its dummies) need not be
+// repeated in every application: the entries that pass go to a plain list (a.mcol row g, count a.mcnt[g]) in the
+// row's order, and the CG loop walks that (10 % fewer gathers, no test).  Every lane of the warp comes through
+// here with a warp-uniform trip count m_max.
+__device__ __forceinline__ void compact_row(const KConst& kc, const PpeArgs& a, int g, int i, int sub, int grp,
+                                            bool live, uint32_t m_max) {
+  const double4 pi = a.pos4[i];
+  const uint32_t* row = row_ptr(a.nbr, kc.stride, i);
+  const uint32_t nf = live ? a.cn[i] : 0u;
+  const uint32_t m = live ? nf + a.co[i] : 0u;
+  uint32_t* crow = a.mcol + (size_t)g * (size_t)kc.stride;
+  const uint32_t lt = (1u << sub) - 1u;
+  uint32_t cnt = 0;
+  for (uint32_t k0 = 0; k0 < m_max; k0 += PPE_ILP * L) {
+    uint32_t e[PPE_ILP];
+    double4 q[PPE_ILP];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const uint32_t kk = k0 + (uint32_t)(u * L + sub);
+      e[u] = kk < m ? row_entry(row, kc.stride, nf, kk) : NB_DUMMY;
+    }
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u)
+      q[u] = (e[u] & NB_DUMMY) ? make_double4(pi.x + 2.0 * kc.re_lap, pi.y, pi.z, 0.0) : a.pos4[e[u] & NB_INDEX];
+#pragma unroll
+    for (int u = 0; u < PPE_ILP; ++u) {
+      const double r2 = pair_r2(q[u].x - pi.x, q[u].y - pi.y, q[u].z - pi.z, 1);
+      const bool keep = !(e[u] & NB_DUMMY) && r2 < kc.re_lap2;
+      const uint32_t m8 = (__ballot_sync(0xffffffffu, keep) >> (grp * L)) & ((1u << L) - 1u);
+      if (keep) crow[cnt + (uint32_t)__popc(m8 & lt)] = e[u];
+      cnt += (uint32_t)__popc(m8);
+    }
+  }
+  if (live && sub == 0) a.mcnt[g] = cnt;
 }
 
 // ---- assembly of one row (ppe_operator 1) ----------------------------------------------
@@ -535,6 +580,26 @@ k_ppe_cg(KConst kc, PpeArgs a) {
     if (lane == 0 && nnz) atomicAdd(&a.cg->nnz, (unsigned long long)nnz);
     if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
   }
+  // -- matrix-free on skin rows: the exact list of every unknown row, once ------------------------------
+  if (!ASM && a.compact) {
+    for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
+      const int g = sc * (SCW * GPW) + g_in_sc;
+      const bool live = g < n_rows;
+      const int i = live ? (int)a.rows[g] : 0;
+      uint32_t m = live ? a.cn[i] + a.co[i] : 0u;
+      m = __reduce_max_sync(0xffffffffu, m);
+      compact_row(kc, a, live ? g : 0, i, sub, grp, live, m);
+    }
+    if (!grid_barrier(a.bar, gen, a.timeout_cycles)) return;
+  }
+  // one row of the matrix-free operator, from the exact list when there is one
+  auto mf_row = [&](int g, int i, bool live, double& ri) {
+    if (a.compact) {
+      const uint32_t m = live ? a.mcnt[g] : 0u;
+      return ppe_row_core<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.mcol + (size_t)g * (size_t)kc.stride, m, m, 0, i, sub, ri);
+    }
+    return ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+  };
   // -- warm start: r0 = b - A x0 ---------------------------------------------------------------
   if (a.warm) {
     for (int sc = sc_first; sc * (SCW * GPW) < n_rows; sc += sc_step) {
@@ -546,7 +611,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
         if (live && sub == 0) a.rc[g] = a.rc[g] - t;
       } else {
         const int i = live ? (int)a.rows[g] : 0;
-        const double t = ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, xi);
+        const double t = mf_row(live ? g : 0, i, live, xi);
         if (live && sub == 0) a.wv[i] = t;
       }
     }
@@ -614,7 +679,7 @@ k_ppe_cg(KConst kc, PpeArgs a) {
           const bool live = g < n_rows;
           double ri;
           const int i = live ? (int)a.rows[g] : 0;
-          const double wi = ppe_row<TWO_PHASE, TEX>(kc, a.pos4, a.tex, a.tp, a.nbr, a.cn, a.co, i, sub, live, ri);
+          const double wi = mf_row(live ? g : 0, i, live, ri);
           if (live && sub == 0) {
             a.wv[i] = wi;
             g_part = fma(ri, ri, g_part);
@@ -792,6 +857,7 @@ PpeArgs make_args(mps_ctx* c) {
   a.timeout_cycles = c->cg_timeout_cycles;
   a.maxit = c->prm.cg_maxit;
   a.warm = c->prm.cg_warm_start ? 1 : 0;
+  a.compact = (c->prm.ppe_operator == 0 && c->kc.stale && c->mat_col && c->mat_cnt) ? 1 : 0;
   return a;
 }
 

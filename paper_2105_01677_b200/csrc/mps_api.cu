@@ -289,6 +289,8 @@ static int create_ctx(mps_ctx** out, const mps_params* prm, int64_t n, void* str
     A(dalloc(&c->mat_val, N * (size_t)k.stride)); A(dalloc(&c->mat_col, N * (size_t)k.stride));
     A(dalloc(&c->mat_cnt, N)); A(dalloc(&c->mat_dex, N)); A(dalloc(&c->mat_scale, N)); A(dalloc(&c->rowmap, N));
     A(dalloc(&c->cg_rc, N)); A(dalloc(&c->cg_xc, N));
+  } else if (c->carry_rows) {  // matrix-free on skin rows: the exact list of every unknown row, built once per solve
+    A(dalloc(&c->mat_col, N * (size_t)k.stride)); A(dalloc(&c->mat_cnt, N));
   }
   A(cudaMallocHost((void**)&c->bar_host, sizeof(GridBar)));
   A(dalloc(&c->cg, 1)); A(dalloc(&c->flags, 1)); A(dalloc(&c->io_tmp, N));
